@@ -1,0 +1,144 @@
+/*
+ * ssm.h -- C ABI of libssm.so: ensemble time-stepping of Uneyama's single-chain
+ * slip-spring model (arxiv 1106.2899) on one NVIDIA B200 (sm_100a).
+ *
+ * P:Lnnn = PAPER.md line nnn.  Units b = kT = zeta = 1.
+ *
+ * The library advances M independent chains of N beads through the three substeps of
+ * P:L292-L347 (section 3.1): explicit Euler for beads and anchors (eqs 44, 45), Glauber
+ * hop of every slip-spring (eqs 22-24, 48, 49), construction / destruction at the chain
+ * ends (eqs 50-53); it records the ensemble means (eq 54) of the stress tensor
+ * (eq 16) and of the virtual stress (eq 76) and feeds a per-chain
+ * multi-tau correlator for the relaxation modulus G(t) (eq 43).
+ *
+ * Conventions
+ *  - No torch types, no exceptions, no global state.  Every function returns 0 on
+ *    success or a negative SSM_E* code; ssm_last_error() gives the text.
+ *  - OWNERSHIP: the caller owns every device byte.  It allocates ONE device workspace of
+ *    ssm_workspace_bytes() bytes (256-byte aligned) and passes it with a CUDA stream
+ *    handle (cudaStream_t cast to void*; NULL = legacy default stream).  The library owns
+ *    only the small host-side ssm_ctx.  The workspace must outlive the ctx.
+ *  - All work is enqueued on that stream.  Calls that return data to HOST pointers
+ *    synchronise the stream before returning; ssm_step() is asynchronous.
+ *  - Pointers are marked (host) or (device); "device" means device memory of the GPU the
+ *    workspace lives on.
+ *  - There is no CPU fallback: without a CUDA device every call fails with SSM_ECUDA.
+ *
+ * External state layout ("SoA, chain index fastest", used by get/set state):
+ *    R[c][i][k]  float32  c = axis 0..2, i = bead 0..N-1, k = chain 0..M-1   -> R[(c*N+i)*M+k]
+ *    A[c][j][k]  float32  j = slip-spring slot 0..zmax-1                     -> A[(c*zmax+j)*M+k]
+ *    S[j][k]     uint8    bead index 1..N of slip-spring j, 0 = empty slot   -> S[j*M+k]
+ *  The occupied slots of a chain are always the first Z_k ones (the paper's "indices run
+ *  from 1 to Z"); zmax = N (the paper's Z <= N).
+ */
+#ifndef SSM_H
+#define SSM_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    SSM_OK      = 0,
+    SSM_EINVAL  = -1,   /* bad parameter / unsupported N                         */
+    SSM_ENOMEM  = -2,   /* workspace too small or misaligned                     */
+    SSM_ECUDA   = -3,   /* CUDA runtime / launch error (text in ssm_last_error)  */
+    SSM_ESTATE  = -4,   /* call out of order                                     */
+    SSM_ERANGE  = -5    /* sample range not recorded / capacity exceeded         */
+};
+
+typedef struct ssm_ctx ssm_ctx;   /* opaque, host side */
+
+/* Parameters of the model as the paper states them plus bookkeeping. */
+typedef struct {
+    int32_t  n_beads;         /* N: 8, 16, 32, 64 or 128 (4 beads per lane, N/4 lanes per chain)  */
+    int64_t  n_chains;        /* M >= 1                                                           */
+    double   n_s;             /* slip-spring strength N_s (eq 1)                           */
+    double   n_0;             /* beads per slip-spring N_0 (eq 10); <= 0 or inf: no slip-  */
+                              /* springs (Rouse limit)                                    */
+    double   zeta_s;          /* slip-spring friction zeta_s (eqs 23, 24)                         */
+    double   dt;              /* time step Delta t                                                */
+    uint64_t seed;            /* Philox4x32-10 key                                                */
+    uint64_t chain_offset;    /* global index of local chain 0 (Philox is keyed by the global     */
+                              /* chain index, so a shard reproduces its part of the full run)     */
+    int32_t  stress_every;    /* record the ensemble stress after every k-th step; 0 = never      */
+    int64_t  stress_capacity; /* number of stress samples the workspace can hold                  */
+    int32_t  sample_every;    /* feed the G(t) correlator after every k-th step; 0 = off          */
+    int32_t  corr_levels;     /* multi-tau levels (16); averaging factor m = 2 fixed              */
+    int32_t  corr_bins;       /* bins per level (16), even, <= 32                                 */
+    int32_t  corr_groups;     /* chain groups for the standard error (32); group = chain % groups */
+} ssm_params;
+
+/* Bytes of device workspace ssm_init() needs for these parameters (0 on bad parameters). */
+size_t ssm_workspace_bytes(const ssm_params *p);
+
+/* Create a context on (device) workspace and sample the equilibrium ensemble on the GPU
+ * (eq 13: Gaussian bonds eq 6, Z ~ Poisson(N/N0) eq 12 clamped at zmax,
+ * S uniform eq 14, anchors Gaussian eq 15).  Global step counter = 0, accumulators clear. */
+int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, size_t workspace_bytes,
+             void *cuda_stream);
+
+/* Advance every chain n_steps time steps with kappa_xy = shear_rate (simple shear, eq 60
+ * P:L410; 0 = no flow).  Asynchronous.  The global step counter (Philox's step coordinate)
+ * only increases: step(a); step(b) == step(a+b) bit for bit.  Stress samples are appended
+ * after every step whose (1-based) global index is a multiple of stress_every; correlator
+ * samples likewise with sample_every.  SSM_ERANGE if the stress buffer would overflow. */
+int ssm_step(ssm_ctx *ctx, int64_t n_steps, double shear_rate);
+
+/* Number of stress samples recorded since init / the last reset. */
+int64_t ssm_stress_count(const ssm_ctx *ctx);
+
+/* Ensemble means (eq 54) of sigma (eq 16) and sigma^(v) (eq 76) for samples
+ * [first_sample, first_sample + n_samples): h_out (host) [n_samples][12] =
+ * sigma xx,yy,zz,xy,yz,zx then sigma_v xx,yy,zz,xy,yz,zx.  Means are over the LOCAL
+ * chains; ssm_stress_sums gives the exact integer sums a multi-GPU run all-reduces. */
+int ssm_stress(ssm_ctx *ctx, int64_t first_sample, int64_t n_samples, double *h_out);
+
+/* Raw fixed-point sums behind ssm_stress: h_out (host) [n_samples][12] int64, value =
+ * sum over local chains of (component + delta_ab) * 2^24 rounded per warp. */
+int ssm_stress_sums(ssm_ctx *ctx, int64_t first_sample, int64_t n_samples, int64_t *h_out);
+
+/* Per-chain stresses of the CURRENT state: out [12][M] float32 (component-major, chain
+ * fastest), host or device. */
+int ssm_chain_stress(ssm_ctx *ctx, float *out, int pointers_are_device);
+
+/* Relaxation modulus from the multi-tau correlator (eq 43; per-chain estimator):
+ * on entry *n_lags = capacity of the arrays, on exit the number of lags written.
+ * h_lag_time[i] in tau0, h_G[i] = G(t_i)/(rho0 kT), h_se[i] (may be NULL) = standard
+ * error over chain groups.  All (host). */
+int ssm_gt(ssm_ctx *ctx, int32_t *n_lags, double *h_lag_time, double *h_G, double *h_se);
+
+/* Raw correlator sums for multi-GPU reduction: h_sum (host) [groups][levels][bins] double,
+ * h_count (host) [groups][levels][bins] int64. */
+int ssm_gt_sums(ssm_ctx *ctx, double *h_sum, int64_t *h_count);
+
+/* Checkpoint: copy the state out / in, in the external SoA layout above.  Buffers are
+ * caller-owned; pointers_are_device selects device or host pointers for R, A and S.
+ * global_step (host) may be NULL on get.  State + global_step = exact resume. */
+int ssm_get_state(ssm_ctx *ctx, float *R, float *A, uint8_t *S, int64_t *global_step,
+                  int pointers_are_device);
+int ssm_set_state(ssm_ctx *ctx, const float *R, const float *A, const uint8_t *S,
+                  int64_t global_step, int pointers_are_device);
+
+/* Clear the stress samples and the correlator; keep the chains and the step counter. */
+int ssm_reset_accumulators(ssm_ctx *ctx);
+
+/* Kernel launches issued so far by this ctx (all kernels of this library). */
+int64_t ssm_launch_count(const ssm_ctx *ctx);
+
+/* Set the number of time steps fused per kernel launch (1..128; default 64).  Results do
+ * not depend on it. */
+int ssm_set_fusion(ssm_ctx *ctx, int32_t steps_per_launch);
+
+void ssm_destroy(ssm_ctx *ctx);
+
+/* Text of the last error on this ctx (valid until the next call on it); ctx may be NULL
+ * for errors of ssm_init / ssm_workspace_bytes. */
+const char *ssm_last_error(const ssm_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SSM_H */

@@ -1,0 +1,201 @@
+"""paper_1106_2899_b200 -- Python binding of libssm.so (include/ssm.h).
+
+Argument marshalling only: every step of the method runs in the CUDA kernels behind the
+C ABI.  PyTorch is used for device memory (the workspace, state buffers) and streams.
+There is no CPU fallback: importing works without a GPU (so that the library can be built
+and its symbols checked), but creating an Ensemble without CUDA raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+SSM_OK, SSM_EINVAL, SSM_ENOMEM, SSM_ECUDA, SSM_ESTATE, SSM_ERANGE = 0, -1, -2, -3, -4, -5
+
+EXPORTS = ["ssm_workspace_bytes", "ssm_init", "ssm_step", "ssm_stress_count", "ssm_stress", "ssm_stress_sums",
+           "ssm_chain_stress", "ssm_gt", "ssm_gt_sums", "ssm_get_state", "ssm_set_state",
+           "ssm_reset_accumulators", "ssm_launch_count", "ssm_set_fusion", "ssm_destroy", "ssm_last_error"]
+
+
+class Params(C.Structure):
+    """ssm_params of include/ssm.h."""
+    _fields_ = [("n_beads", C.c_int32), ("n_chains", C.c_int64), ("n_s", C.c_double), ("n_0", C.c_double),
+                ("zeta_s", C.c_double), ("dt", C.c_double), ("seed", C.c_uint64), ("chain_offset", C.c_uint64),
+                ("stress_every", C.c_int32), ("stress_capacity", C.c_int64), ("sample_every", C.c_int32),
+                ("corr_levels", C.c_int32), ("corr_bins", C.c_int32), ("corr_groups", C.c_int32)]
+
+
+class SsmError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__("libssm error %d: %s" % (code, text))
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load libssm.so (building it with nvcc if missing or stale) and declare prototypes."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    L = C.CDLL(path)
+    PP, vp, dp, fp = C.POINTER(Params), C.c_void_p, C.POINTER(C.c_double), C.c_void_p
+    L.ssm_workspace_bytes.argtypes = [PP]; L.ssm_workspace_bytes.restype = C.c_size_t
+    L.ssm_init.argtypes = [C.POINTER(vp), PP, vp, C.c_size_t, vp]; L.ssm_init.restype = C.c_int
+    L.ssm_step.argtypes = [vp, C.c_int64, C.c_double]; L.ssm_step.restype = C.c_int
+    L.ssm_stress_count.argtypes = [vp]; L.ssm_stress_count.restype = C.c_int64
+    L.ssm_stress.argtypes = [vp, C.c_int64, C.c_int64, dp]; L.ssm_stress.restype = C.c_int
+    L.ssm_stress_sums.argtypes = [vp, C.c_int64, C.c_int64, C.POINTER(C.c_int64)]; L.ssm_stress_sums.restype = C.c_int
+    L.ssm_chain_stress.argtypes = [vp, fp, C.c_int]; L.ssm_chain_stress.restype = C.c_int
+    L.ssm_gt.argtypes = [vp, C.POINTER(C.c_int32), dp, dp, dp]; L.ssm_gt.restype = C.c_int
+    L.ssm_gt_sums.argtypes = [vp, dp, C.POINTER(C.c_int64)]; L.ssm_gt_sums.restype = C.c_int
+    L.ssm_get_state.argtypes = [vp, fp, fp, vp, C.POINTER(C.c_int64), C.c_int]; L.ssm_get_state.restype = C.c_int
+    L.ssm_set_state.argtypes = [vp, fp, fp, vp, C.c_int64, C.c_int]; L.ssm_set_state.restype = C.c_int
+    L.ssm_reset_accumulators.argtypes = [vp]; L.ssm_reset_accumulators.restype = C.c_int
+    L.ssm_launch_count.argtypes = [vp]; L.ssm_launch_count.restype = C.c_int64
+    L.ssm_set_fusion.argtypes = [vp, C.c_int32]; L.ssm_set_fusion.restype = C.c_int
+    L.ssm_destroy.argtypes = [vp]; L.ssm_destroy.restype = None
+    L.ssm_last_error.argtypes = [vp]; L.ssm_last_error.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def library_path():
+    return _build.LIB
+
+
+def workspace_bytes(params):
+    return lib().ssm_workspace_bytes(C.byref(params))
+
+
+class Ensemble:
+    """M chains on one GPU.  Thin wrapper: each method is one C-ABI call of the same name."""
+
+    def __init__(self, n_beads, n_chains, n_s=0.5, n_0=4.0, zeta_s=0.1, dt=0.01, seed=1, chain_offset=0,
+                 stress_every=0, stress_capacity=0, sample_every=0, corr_levels=16, corr_bins=16,
+                 corr_groups=32, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise SsmError(SSM_ECUDA, "no CUDA device: libssm has no CPU fallback")
+        self._torch = torch
+        self.device = torch.device(device)
+        self.p = Params(n_beads, n_chains, n_s, n_0, zeta_s, dt, seed, chain_offset, stress_every,
+                        stress_capacity, sample_every, corr_levels, corr_bins, corr_groups)
+        self.N, self.M = n_beads, n_chains
+        L = lib()
+        nbytes = L.ssm_workspace_bytes(C.byref(self.p))
+        if nbytes == 0:
+            raise SsmError(SSM_EINVAL, L.ssm_last_error(None).decode())
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = (self.workspace.data_ptr() + 255) // 256 * 256
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            h = C.c_void_p()
+            rc = L.ssm_init(C.byref(h), C.byref(self.p), C.c_void_p(base), nbytes, C.c_void_p(self.stream.cuda_stream))
+        if rc != SSM_OK:
+            raise SsmError(rc, L.ssm_last_error(None).decode())
+        self.h = h
+
+    def _ck(self, rc):
+        if rc != SSM_OK:
+            raise SsmError(rc, lib().ssm_last_error(self.h).decode())
+
+    def step(self, n_steps, shear_rate=0.0):
+        with self._torch.cuda.device(self.device):
+            self._ck(lib().ssm_step(self.h, n_steps, shear_rate))
+
+    def stress_count(self):
+        return lib().ssm_stress_count(self.h)
+
+    def stress(self, first=0, n=None):
+        n = self.stress_count() - first if n is None else n
+        out = np.zeros((max(n, 1), 12))
+        self._ck(lib().ssm_stress(self.h, first, n, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out[:n]
+
+    def stress_sums(self, first=0, n=None):
+        n = self.stress_count() - first if n is None else n
+        out = np.zeros((max(n, 1), 12), dtype=np.int64)
+        self._ck(lib().ssm_stress_sums(self.h, first, n, out.ctypes.data_as(C.POINTER(C.c_int64))))
+        return out[:n]
+
+    def chain_stress(self, out=None):
+        """[12][M] float32: numpy (host) by default, or fill a given CUDA tensor."""
+        if out is None:
+            a = np.zeros((12, self.M), dtype=np.float32)
+            self._ck(lib().ssm_chain_stress(self.h, C.c_void_p(a.ctypes.data), 0))
+            return a
+        self._ck(lib().ssm_chain_stress(self.h, C.c_void_p(out.data_ptr()), 1))
+        return out
+
+    def gt(self):
+        cap = self.p.corr_levels * self.p.corr_bins
+        n = C.c_int32(cap)
+        t = np.zeros(cap); G = np.zeros(cap); se = np.zeros(cap)
+        d = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+        self._ck(lib().ssm_gt(self.h, C.byref(n), d(t), d(G), d(se)))
+        return t[:n.value].copy(), G[:n.value].copy(), se[:n.value].copy()
+
+    def gt_sums(self):
+        shape = (self.p.corr_groups, self.p.corr_levels, self.p.corr_bins)
+        s = np.zeros(shape); c = np.zeros(shape, dtype=np.int64)
+        self._ck(lib().ssm_gt_sums(self.h, s.ctypes.data_as(C.POINTER(C.c_double)),
+                                   c.ctypes.data_as(C.POINTER(C.c_int64))))
+        return s, c
+
+    def get_state(self, R=None, A=None, S=None):
+        """External SoA layout: R[3][N][M], A[3][N][M] float32, S[N][M] uint8.  Host numpy
+        arrays by default; pass CUDA tensors (all three) to stay on the device."""
+        step = C.c_int64()
+        if R is None:
+            R = np.zeros((3, self.N, self.M), dtype=np.float32); A = np.zeros((3, self.N, self.M), dtype=np.float32)
+            S = np.zeros((self.N, self.M), dtype=np.uint8)
+            self._ck(lib().ssm_get_state(self.h, C.c_void_p(R.ctypes.data), C.c_void_p(A.ctypes.data),
+                                         C.c_void_p(S.ctypes.data), C.byref(step), 0))
+        elif isinstance(R, np.ndarray):
+            self._ck(lib().ssm_get_state(self.h, C.c_void_p(R.ctypes.data), C.c_void_p(A.ctypes.data),
+                                         C.c_void_p(S.ctypes.data), C.byref(step), 0))
+        else:
+            dev = 1 if R.is_cuda else 0
+            self._ck(lib().ssm_get_state(self.h, C.c_void_p(R.data_ptr()), C.c_void_p(A.data_ptr()),
+                                         C.c_void_p(S.data_ptr()), C.byref(step), dev))
+        return R, A, S, step.value
+
+    def set_state(self, R, A, S, global_step):
+        if isinstance(R, np.ndarray):
+            assert R.dtype == np.float32 and A.dtype == np.float32 and S.dtype == np.uint8
+            assert R.flags.c_contiguous and A.flags.c_contiguous and S.flags.c_contiguous
+            assert R.shape == (3, self.N, self.M) and A.shape == (3, self.N, self.M) and S.shape == (self.N, self.M)
+            self._ck(lib().ssm_set_state(self.h, C.c_void_p(R.ctypes.data), C.c_void_p(A.ctypes.data),
+                                         C.c_void_p(S.ctypes.data), global_step, 0))
+        else:
+            dev = 1 if R.is_cuda else 0
+            self._ck(lib().ssm_set_state(self.h, C.c_void_p(R.data_ptr()), C.c_void_p(A.data_ptr()),
+                                         C.c_void_p(S.data_ptr()), global_step, dev))
+
+    def reset_accumulators(self):
+        self._ck(lib().ssm_reset_accumulators(self.h))
+
+    def launch_count(self):
+        return lib().ssm_launch_count(self.h)
+
+    def set_fusion(self, steps_per_launch):
+        self._ck(lib().ssm_set_fusion(self.h, steps_per_launch))
+
+    def synchronize(self):
+        self.stream.synchronize()
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib().ssm_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,468 @@
+// ssm_api.cu -- the C ABI of libssm.so (include/ssm.h): argument checking, workspace
+// carve-up, host-side tables and launch sequencing.  Every step of the method runs in the
+// kernels of ssm_step.cu / ssm_aux.cu; nothing here computes on chains.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/ssm.h"
+#include "ssm_common.h"
+
+namespace ssm {
+cudaError_t step_occupancy(int n_beads, int *blocks_per_sm);
+cudaError_t launch_step(int n_beads, const StepParams &p, int grid, cudaStream_t st);
+cudaError_t launch_init(const InitParams &p, cudaStream_t st);
+cudaError_t launch_xfer(bool do_export, unsigned char *state, float *R, float *A, unsigned char *S, int N,
+                        long long k0, long long nk, long long pitch, cudaStream_t st);
+cudaError_t launch_chain_stress(const unsigned char *state, float *out, int N, long long M, float cs, cudaStream_t st);
+cudaError_t launch_corr(const CorrParams &c, cudaStream_t st);
+}  // namespace ssm
+
+using namespace ssm;
+
+static thread_local std::string g_err;   // errors without a ctx
+
+struct Layout {
+    size_t state, stress, samples, ring, accf, accg, csum, stage, total;
+    long long n_tiles, stage_chains;
+};
+
+struct ssm_ctx {
+    ssm_params p;
+    Layout lay;
+    unsigned char *ws;
+    cudaStream_t st;
+    long long step;          // global step counter
+    long long n_records;     // stress samples recorded since the last reset
+    int fuse, grid;
+    long long launches;
+    bool springs_on;
+    StepParams sp;           // constant part filled at init
+    // correlator schedule (identical for all chains) and product counts, host side
+    unsigned char cpos[kCorrMaxLevels], cfil[kCorrMaxLevels], cpar[kCorrMaxLevels];
+    std::vector<long long> ccount;      // [L][P] insertions with a product at (level, bin)
+    std::string err;
+};
+
+static int fail(ssm_ctx *c, int code, const std::string &msg)
+{
+    if (c) c->err = msg; else g_err = msg;
+    return code;
+}
+static int cuda_fail(ssm_ctx *c, cudaError_t e, const char *what)
+{
+    return fail(c, SSM_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CK(c, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail((c), e_, #call); } while (0)
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+static bool check_params(const ssm_params *p, std::string &why)
+{
+    if (!p) { why = "params is NULL"; return false; }
+    const int N = p->n_beads;
+    if (!(N == 8 || N == 16 || N == 32 || N == 64 || N == 128)) { why = "n_beads must be 8, 16, 32, 64 or 128"; return false; }
+    if (p->n_chains < 1) { why = "n_chains must be >= 1"; return false; }
+    if (p->chain_offset + (uint64_t)p->n_chains + 16 > 0xFFFFFFFFull) { why = "global chain index must fit 32 bits"; return false; }
+    if (!(p->dt > 0.0) || !(p->dt < 1.0 / 6.0)) { why = "dt must be in (0, 1/6): the Euler map needs 12 dt < 2"; return false; }
+    if (!(p->n_s > 0.0)) { why = "n_s must be > 0"; return false; }
+    if (!(p->zeta_s > 0.0)) { why = "zeta_s must be > 0"; return false; }
+    if (p->stress_every < 0 || p->sample_every < 0 || p->stress_capacity < 0) { why = "negative sampling parameter"; return false; }
+    if (p->stress_every > 0 && p->stress_capacity < 1) { why = "stress_capacity must be >= 1 when stress_every > 0"; return false; }
+    if (p->sample_every > 0) {
+        if (p->corr_levels < 1 || p->corr_levels > kCorrMaxLevels) { why = "corr_levels must be 1..32"; return false; }
+        if (p->corr_bins < 2 || p->corr_bins > 32 || (p->corr_bins & 1)) { why = "corr_bins must be even, 2..32"; return false; }
+        if (p->corr_groups < 1 || p->corr_groups > 1024) { why = "corr_groups must be 1..1024"; return false; }
+    }
+    return true;
+}
+
+static Layout make_layout(const ssm_params *p)
+{
+    Layout L{};
+    const int cpw = 128 / p->n_beads;
+    L.n_tiles = (p->n_chains + cpw - 1) / cpw;
+    size_t o = 0;
+    L.state = o; o = align_up(o + (size_t)L.n_tiles * kTileBytes, 256);
+    L.stress = o; o = align_up(o + (size_t)p->stress_capacity * 12 * 8, 256);
+    const bool corr = p->sample_every > 0;
+    const size_t M = (size_t)p->n_chains;
+    L.samples = o; if (corr) o = align_up(o + (size_t)kMaxFuse * M * 8, 256);
+    L.ring = o; if (corr) o = align_up(o + (size_t)p->corr_levels * p->corr_bins * M * 4, 256);
+    L.accf = o; if (corr) o = align_up(o + (size_t)p->corr_levels * M * 4, 256);
+    L.accg = o; if (corr) o = align_up(o + (size_t)p->corr_levels * M * 4, 256);
+    L.csum = o; if (corr) o = align_up(o + (size_t)p->corr_groups * p->corr_levels * p->corr_bins * 8, 256);
+    // staging for host-pointer get/set state and chain stress: chunks of <= 65536 chains
+    L.stage_chains = p->n_chains < 65536 ? p->n_chains : 65536;
+    L.stage = o; o = align_up(o + (size_t)L.stage_chains * (size_t)(25 * p->n_beads > 48 ? 25 * p->n_beads : 48), 256);
+    L.total = o;
+    return L;
+}
+
+// "u < p" with u = (k + 1/2) 2^-23  <=>  k < T(p) = ceil(p 2^23 - 1/2)
+static unsigned threshold23(double p)
+{
+    double t = std::ceil(p * 8388608.0 - 0.5);
+    if (t < 0.0) t = 0.0;
+    if (t > 8388608.0) t = 8388608.0;
+    return (unsigned)t;
+}
+
+extern "C" size_t ssm_workspace_bytes(const ssm_params *p)
+{
+    std::string why;
+    if (!check_params(p, why)) { g_err = why; return 0; }
+    return make_layout(p).total;
+}
+
+static void corr_clear(ssm_ctx *c)
+{
+    std::memset(c->cpos, 0, sizeof c->cpos); std::memset(c->cfil, 0, sizeof c->cfil); std::memset(c->cpar, 0, sizeof c->cpar);
+    c->ccount.assign((size_t)kCorrMaxLevels * 32, 0);
+}
+
+static int clear_accumulators(ssm_ctx *c)
+{
+    const ssm_params &p = c->p;
+    if (p.stress_capacity > 0)
+        CK(c, cudaMemsetAsync(c->ws + c->lay.stress, 0, (size_t)p.stress_capacity * 12 * 8, c->st));
+    if (p.sample_every > 0) {
+        CK(c, cudaMemsetAsync(c->ws + c->lay.ring, 0, c->lay.stage - c->lay.ring, c->st));
+        corr_clear(c);
+    }
+    c->n_records = 0;
+    return SSM_OK;
+}
+
+extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!out) return fail(nullptr, SSM_EINVAL, "out is NULL");
+    *out = nullptr;
+    std::string why;
+    if (!check_params(p, why)) return fail(nullptr, SSM_EINVAL, why);
+    const Layout lay = make_layout(p);
+    if (!d_workspace || workspace_bytes < lay.total) return fail(nullptr, SSM_ENOMEM, "workspace too small");
+    if (((uintptr_t)d_workspace & 255u) != 0) return fail(nullptr, SSM_ENOMEM, "workspace must be 256-byte aligned");
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev < 1) return fail(nullptr, SSM_ECUDA, "no CUDA device (there is no CPU fallback)");
+
+    ssm_ctx *c = new (std::nothrow) ssm_ctx();
+    if (!c) return fail(nullptr, SSM_ENOMEM, "host allocation failed");
+    c->p = *p; c->lay = lay; c->ws = (unsigned char *)d_workspace; c->st = (cudaStream_t)cuda_stream;
+    c->step = 0; c->n_records = 0; c->fuse = kMaxFuse; c->launches = 0;
+    c->springs_on = p->n_0 > 0.0 && std::isfinite(p->n_0);
+    corr_clear(c);
+
+    int dev = 0, n_sm = 0, bps = 0;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess || (e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess
+        || (e = step_occupancy(p->n_beads, &bps)) != cudaSuccess) {
+        int rc = cuda_fail(nullptr, e, "device query"); delete c; return rc;
+    }
+    if (bps < 1) { delete c; return fail(nullptr, SSM_ECUDA, "step kernel does not fit on an SM"); }
+    const long long want = (lay.n_tiles + kWarpsPerBlock - 1) / kWarpsPerBlock;
+    const long long cap = (long long)n_sm * bps;
+    c->grid = (int)(want < cap ? want : cap);
+
+    // constant launch parameters and integer decision thresholds (fp64 on the host)
+    const double h = p->dt / p->zeta_s;
+    StepParams &sp = c->sp;
+    std::memset(&sp, 0, sizeof sp);
+    sp.state = c->ws + lay.state;
+    sp.n_chains = p->n_chains; sp.chain_offset = p->chain_offset; sp.n_tiles = (int)lay.n_tiles;
+    sp.stress_every = p->stress_every; sp.sample_every = p->sample_every;
+    sp.key0 = (unsigned)(p->seed & 0xFFFFFFFFull); sp.key1 = (unsigned)(p->seed >> 32);
+    sp.springs_on = c->springs_on ? 1 : 0;
+    sp.dt3 = (float)(3.0 * p->dt);
+    sp.sq2dt = (float)std::sqrt(2.0 * p->dt);
+    sp.fx_scale = (float)(p->dt * (3.0 / p->n_s) * (double)(1 << kFxShift));
+    sp.q2l = (float)(2.0 * (3.0 / (4.0 * p->n_s)) * 1.4426950408889634);
+    sp.h2 = (float)(2.0 * h);
+    sp.cs = (float)(3.0 / p->n_s);
+    sp.sq_ns3 = (float)std::sqrt(p->n_s / 3.0);
+    sp.t_destroy = threshold23(std::fmin(h, 1.0));
+    for (int K = 1; K <= 128; ++K) {
+        const double pc = c->springs_on ? std::fmin(h / (p->n_0 * (double)K), 0.5) : 0.0;
+        sp.t_c1[K] = threshold23(pc); sp.t_c2[K] = threshold23(2.0 * pc);
+    }
+
+    InitParams ip;
+    std::memset(&ip, 0, sizeof ip);
+    ip.state = c->ws + lay.state;
+    ip.n_chains_padded = lay.n_tiles * (128 / p->n_beads);
+    ip.chain_offset = p->chain_offset; ip.key0 = sp.key0; ip.key1 = sp.key1;
+    ip.n_beads = p->n_beads; ip.springs_on = sp.springs_on;
+    ip.sq13 = (float)std::sqrt(1.0 / 3.0); ip.sq_ns3 = sp.sq_ns3;
+    if (c->springs_on) {       // Poisson(N/N0) CDF (eq 12) as integer thresholds
+        const double lam = (double)p->n_beads / p->n_0;
+        double pmf = std::exp(-lam), cdf = 0.0;
+        for (int z = 0; z < p->n_beads; ++z) {
+            if (z > 0) pmf = pmf * lam / (double)z;
+            cdf += pmf;
+            ip.t_cdf[z] = threshold23(cdf);
+        }
+    }
+    if ((e = cudaMemsetAsync(c->ws + lay.state, 0, (size_t)lay.n_tiles * kTileBytes, c->st)) != cudaSuccess
+        || (e = launch_init(ip, c->st)) != cudaSuccess) {
+        int rc = cuda_fail(nullptr, e, "ssm_init launch"); delete c; return rc;
+    }
+    c->launches += 1;
+    int rc = clear_accumulators(c);
+    if (rc != SSM_OK) { g_err = c->err; delete c; return rc; }
+    *out = c;
+    return SSM_OK;
+}
+
+// advance the host copy of the correlator schedule by one sample, counting products
+static void corr_schedule_sample(ssm_ctx *c)
+{
+    const int L = c->p.corr_levels, Pb = c->p.corr_bins;
+    for (int lev = 0; lev < L; ++lev) {
+        if (c->cfil[lev] < Pb) ++c->cfil[lev];
+        const int kmin = lev == 0 ? 0 : Pb / 2;
+        for (int q = kmin; q < c->cfil[lev]; ++q) c->ccount[(size_t)lev * 32 + q] += 1;
+        c->cpos[lev] = (unsigned char)((c->cpos[lev] + 1) % Pb);
+        if (c->cpar[lev] == 0) { c->cpar[lev] = 1; break; }
+        c->cpar[lev] = 0;
+    }
+}
+
+extern "C" int ssm_step(ssm_ctx *c, int64_t n_steps, double shear_rate)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (n_steps < 0) return fail(c, SSM_EINVAL, "n_steps < 0");
+    if (!std::isfinite(shear_rate)) return fail(c, SSM_EINVAL, "shear_rate is not finite");
+    const ssm_params &p = c->p;
+    if (p.stress_every > 0) {
+        const long long need = (c->step + n_steps) / p.stress_every - c->step / p.stress_every;
+        if (c->n_records + need > p.stress_capacity) return fail(c, SSM_ERANGE, "stress buffer would overflow (stress_capacity)");
+    }
+    StepParams sp = c->sp;
+    sp.gdt = (float)(shear_rate * p.dt);
+    long long left = n_steps;
+    while (left > 0) {
+        const int T = (int)(left < c->fuse ? left : c->fuse);
+        sp.step0 = (unsigned long long)c->step; sp.n_fuse = T;
+        long long nrec = 0, nsmp = 0;
+        if (p.stress_every > 0) nrec = (c->step + T) / p.stress_every - c->step / p.stress_every;
+        if (p.sample_every > 0) nsmp = (c->step + T) / p.sample_every - c->step / p.sample_every;
+        sp.stress = reinterpret_cast<long long *>(c->ws + c->lay.stress) + c->n_records * 12;
+        sp.samples = nsmp > 0 ? reinterpret_cast<float2 *>(c->ws + c->lay.samples) : nullptr;
+        CK(c, launch_step(p.n_beads, sp, c->grid, c->st));
+        c->launches += 1;
+        if (nsmp > 0) {
+            CorrParams cp;
+            std::memset(&cp, 0, sizeof cp);
+            cp.samples = sp.samples;
+            cp.ring = reinterpret_cast<float *>(c->ws + c->lay.ring);
+            cp.acc_f = reinterpret_cast<float *>(c->ws + c->lay.accf);
+            cp.acc_g = reinterpret_cast<float *>(c->ws + c->lay.accg);
+            cp.sum = reinterpret_cast<long long *>(c->ws + c->lay.csum);
+            cp.M = p.n_chains; cp.chain_offset = p.chain_offset;
+            cp.n_samples = (int)nsmp; cp.L = p.corr_levels; cp.Pb = p.corr_bins; cp.groups = p.corr_groups;
+            std::memcpy(cp.pos, c->cpos, sizeof cp.pos); std::memcpy(cp.filled, c->cfil, sizeof cp.filled);
+            std::memcpy(cp.parity, c->cpar, sizeof cp.parity);
+            CK(c, launch_corr(cp, c->st));
+            c->launches += 1;
+            for (long long s = 0; s < nsmp; ++s) corr_schedule_sample(c);
+        }
+        c->n_records += nrec;
+        c->step += T;
+        left -= T;
+    }
+    return SSM_OK;
+}
+
+extern "C" int64_t ssm_stress_count(const ssm_ctx *c) { return c ? c->n_records : 0; }
+extern "C" int64_t ssm_launch_count(const ssm_ctx *c) { return c ? c->launches : 0; }
+
+extern "C" int ssm_stress_sums(ssm_ctx *c, int64_t first, int64_t n, int64_t *h_out)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (first < 0 || n < 0 || first + n > c->n_records) return fail(c, SSM_ERANGE, "stress samples not recorded");
+    if (n == 0) return SSM_OK;
+    if (!h_out) return fail(c, SSM_EINVAL, "h_out is NULL");
+    CK(c, cudaMemcpyAsync(h_out, c->ws + c->lay.stress + (size_t)first * 96, (size_t)n * 96, cudaMemcpyDeviceToHost, c->st));
+    CK(c, cudaStreamSynchronize(c->st));
+    return SSM_OK;
+}
+
+extern "C" int ssm_stress(ssm_ctx *c, int64_t first, int64_t n, double *h_out)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (n > 0 && !h_out) return fail(c, SSM_EINVAL, "h_out is NULL");
+    std::vector<int64_t> raw((size_t)(n > 0 ? n : 0) * 12);
+    int rc = ssm_stress_sums(c, first, n, raw.data());
+    if (rc != SSM_OK) return rc;
+    // sums hold sum_bonds (3 b_a b_b - delta_ab) and sum_j ((3/N_s) d_a d_b - delta_ab):
+    // sigma_aa = 3 sum b_a^2 - N needs one more -1 per chain (eq 16); sigma^(v) needs none (eq 76)
+    const double scale = 1.0 / ((double)(1 << kStressShift) * (double)c->p.n_chains);
+    for (int64_t i = 0; i < n; ++i)
+        for (int t = 0; t < 12; ++t)
+            h_out[i * 12 + t] = (double)raw[(size_t)i * 12 + t] * scale - (t < 3 ? 1.0 : 0.0);
+    return SSM_OK;
+}
+
+extern "C" int ssm_chain_stress(ssm_ctx *c, float *out, int dev)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (!out) return fail(c, SSM_EINVAL, "out is NULL");
+    const long long M = c->p.n_chains;
+    if (dev) {
+        CK(c, launch_chain_stress(c->ws + c->lay.state, out, c->p.n_beads, M, c->sp.cs, c->st));
+        c->launches += 1;
+        return SSM_OK;
+    }
+    // host pointer: stage the whole [12][M] array if it fits the staging area, else fail
+    if ((size_t)M * 48 > c->lay.total - c->lay.stage) return fail(c, SSM_ENOMEM, "staging area too small for host chain stress");
+    float *d = reinterpret_cast<float *>(c->ws + c->lay.stage);
+    CK(c, launch_chain_stress(c->ws + c->lay.state, d, c->p.n_beads, M, c->sp.cs, c->st));
+    c->launches += 1;
+    CK(c, cudaMemcpyAsync(out, d, (size_t)M * 48, cudaMemcpyDeviceToHost, c->st));
+    CK(c, cudaStreamSynchronize(c->st));
+    return SSM_OK;
+}
+
+static int xfer_state(ssm_ctx *c, bool do_export, float *R, float *A, uint8_t *S, int dev)
+{
+    const int N = c->p.n_beads; const long long M = c->p.n_chains;
+    unsigned char *state = c->ws + c->lay.state;
+    if (dev) {
+        CK(c, launch_xfer(do_export, state, R, A, S, N, 0, M, M, c->st));
+        c->launches += do_export ? 1 : 2;
+        return SSM_OK;
+    }
+    const long long chunk = c->lay.stage_chains;
+    float *dR = reinterpret_cast<float *>(c->ws + c->lay.stage);
+    float *dA = dR + (size_t)3 * N * chunk;
+    unsigned char *dS = reinterpret_cast<unsigned char *>(dA + (size_t)3 * N * chunk);
+    for (long long k0 = 0; k0 < M; k0 += chunk) {
+        const long long nk = M - k0 < chunk ? M - k0 : chunk;
+        if (do_export) {
+            CK(c, launch_xfer(true, state, dR, dA, dS, N, k0, nk, chunk, c->st));
+            CK(c, cudaMemcpy2DAsync(R + k0, (size_t)M * 4, dR, (size_t)chunk * 4, (size_t)nk * 4, (size_t)3 * N, cudaMemcpyDeviceToHost, c->st));
+            CK(c, cudaMemcpy2DAsync(A + k0, (size_t)M * 4, dA, (size_t)chunk * 4, (size_t)nk * 4, (size_t)3 * N, cudaMemcpyDeviceToHost, c->st));
+            CK(c, cudaMemcpy2DAsync(S + k0, (size_t)M, dS, (size_t)chunk, (size_t)nk, (size_t)N, cudaMemcpyDeviceToHost, c->st));
+            c->launches += 1;
+        } else {
+            CK(c, cudaMemcpy2DAsync(dR, (size_t)chunk * 4, R + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)3 * N, cudaMemcpyHostToDevice, c->st));
+            CK(c, cudaMemcpy2DAsync(dA, (size_t)chunk * 4, A + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)3 * N, cudaMemcpyHostToDevice, c->st));
+            CK(c, cudaMemcpy2DAsync(dS, (size_t)chunk, S + k0, (size_t)M, (size_t)nk, (size_t)N, cudaMemcpyHostToDevice, c->st));
+            CK(c, launch_xfer(false, state, dR, dA, dS, N, k0, nk, chunk, c->st));
+            c->launches += 2;
+        }
+    }
+    CK(c, cudaStreamSynchronize(c->st));
+    return SSM_OK;
+}
+
+extern "C" int ssm_get_state(ssm_ctx *c, float *R, float *A, uint8_t *S, int64_t *global_step, int dev)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (!R || !A || !S) return fail(c, SSM_EINVAL, "NULL state pointer");
+    if (global_step) *global_step = c->step;
+    return xfer_state(c, true, R, A, S, dev);
+}
+
+extern "C" int ssm_set_state(ssm_ctx *c, const float *R, const float *A, const uint8_t *S, int64_t global_step, int dev)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (!R || !A || !S) return fail(c, SSM_EINVAL, "NULL state pointer");
+    if (global_step < 0) return fail(c, SSM_EINVAL, "global_step < 0");
+    int rc = xfer_state(c, false, const_cast<float *>(R), const_cast<float *>(A), const_cast<uint8_t *>(S), dev);
+    if (rc == SSM_OK) c->step = global_step;
+    return rc;
+}
+
+extern "C" int ssm_reset_accumulators(ssm_ctx *c)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    return clear_accumulators(c);
+}
+
+extern "C" int ssm_set_fusion(ssm_ctx *c, int32_t t)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (t < 1 || t > kMaxFuse) return fail(c, SSM_EINVAL, "steps_per_launch out of range");
+    c->fuse = t;
+    return SSM_OK;
+}
+
+extern "C" int ssm_gt_sums(ssm_ctx *c, double *h_sum, int64_t *h_count)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    const ssm_params &p = c->p;
+    if (p.sample_every <= 0) return fail(c, SSM_ESTATE, "correlator is off (sample_every = 0)");
+    if (!h_sum || !h_count) return fail(c, SSM_EINVAL, "NULL output");
+    const size_t n = (size_t)p.corr_groups * p.corr_levels * p.corr_bins;
+    std::vector<long long> raw(n);
+    CK(c, cudaMemcpyAsync(raw.data(), c->ws + c->lay.csum, n * 8, cudaMemcpyDeviceToHost, c->st));
+    CK(c, cudaStreamSynchronize(c->st));
+    for (int g = 0; g < p.corr_groups; ++g) {
+        // chains of this group among the local ones: global index = chain_offset + k, group = index % groups
+        const unsigned long long first = (p.chain_offset % (unsigned)p.corr_groups);
+        long long ng = 0;
+        {   // count k in [0, M) with (first + k) % groups == g
+            const long long G = p.corr_groups, M = p.n_chains;
+            const long long r = ((long long)g - (long long)first % G + G) % G;
+            ng = r < M ? (M - 1 - r) / G + 1 : 0;
+        }
+        for (int lev = 0; lev < p.corr_levels; ++lev)
+            for (int q = 0; q < p.corr_bins; ++q) {
+                const size_t i = ((size_t)g * p.corr_levels + lev) * p.corr_bins + q;
+                h_sum[i] = (double)raw[i] / 65536.0;
+                h_count[i] = c->ccount[(size_t)lev * 32 + q] * ng;
+            }
+    }
+    return SSM_OK;
+}
+
+extern "C" int ssm_gt(ssm_ctx *c, int32_t *n_lags, double *h_t, double *h_G, double *h_se)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (!n_lags || !h_t || !h_G) return fail(c, SSM_EINVAL, "NULL output");
+    const ssm_params &p = c->p;
+    if (p.sample_every <= 0) return fail(c, SSM_ESTATE, "correlator is off (sample_every = 0)");
+    const int L = p.corr_levels, Pb = p.corr_bins, Gn = p.corr_groups;
+    std::vector<double> sum((size_t)Gn * L * Pb); std::vector<int64_t> cnt((size_t)Gn * L * Pb);
+    int rc = ssm_gt_sums(c, sum.data(), cnt.data());
+    if (rc != SSM_OK) return rc;
+    const double base = p.dt * p.sample_every, N = (double)p.n_beads;
+    int n = 0;
+    for (int lev = 0; lev < L; ++lev)
+        for (int q = (lev == 0 ? 0 : Pb / 2); q < Pb; ++q) {
+            double s = 0.0; int64_t cn = 0;
+            for (int g = 0; g < Gn; ++g) { s += sum[((size_t)g * L + lev) * Pb + q]; cn += cnt[((size_t)g * L + lev) * Pb + q]; }
+            if (cn == 0) continue;
+            if (n >= *n_lags) return fail(c, SSM_ERANGE, "n_lags capacity too small");
+            h_t[n] = (double)q * std::ldexp(1.0, lev) * base;
+            h_G[n] = s / ((double)cn * N);            // G/(rho0 kT) = <.>/N  (c0 = rho0/N)
+            if (h_se) {
+                double mean = 0.0, var = 0.0; int used = 0;
+                for (int g = 0; g < Gn; ++g) {
+                    const int64_t cg = cnt[((size_t)g * L + lev) * Pb + q];
+                    if (cg > 0) { mean += sum[((size_t)g * L + lev) * Pb + q] / ((double)cg * N); ++used; }
+                }
+                if (used > 1) {
+                    mean /= used;
+                    for (int g = 0; g < Gn; ++g) {
+                        const int64_t cg = cnt[((size_t)g * L + lev) * Pb + q];
+                        if (cg > 0) { const double v = sum[((size_t)g * L + lev) * Pb + q] / ((double)cg * N) - mean; var += v * v; }
+                    }
+                    h_se[n] = std::sqrt(var / (used - 1) / used);
+                } else h_se[n] = NAN;
+            }
+            ++n;
+        }
+    *n_lags = n;
+    return SSM_OK;
+}
+
+extern "C" void ssm_destroy(ssm_ctx *c) { delete c; }
+
+extern "C" const char *ssm_last_error(const ssm_ctx *c) { return c ? c->err.c_str() : g_err.c_str(); }

@@ -1,0 +1,207 @@
+// ssm_aux.cu -- the kernels around the fused step kernel: equilibrium sampler (ssm_init),
+// state import / export (ssm_set_state / ssm_get_state), per-chain stress, and the
+// per-chain multi-tau correlator that turns (sigma_xy, sigma_xy + sigma^(v)_xy) samples
+// into the sums behind G(t) (eq 43).
+#include <cuda_runtime.h>
+
+#include "ssm_common.h"
+#include "ssm_rng.cuh"
+
+namespace ssm {
+
+// ---------------------------------------------------------------------------------------
+// Equilibrium sampler, PAPER.md lines 351-355 (eq 13): one thread per chain.
+//   1. Gaussian bonds, variance b^2/3 per axis (eq 6); R_1 = 0
+//   2. Z ~ Poisson(N/N0) (eq 12) by inversion against integer CDF thresholds, clamped at zmax
+//   3. S_j uniform on 1..N (eq 14), A_j Gaussian about R_{S_j}, variance N_s/3 per axis (eq 15)
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) ssm_init_kernel(const __grid_constant__ InitParams P)
+{
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= P.n_chains_padded) return;
+    const int N = P.n_beads, zmax = N;
+    const uint32_t chain = (uint32_t)(P.chain_offset + (unsigned long long)k);
+    const StreamKey sk = make_stream(P.key0, P.key1, 0ull);
+    unsigned char *st = P.state;
+
+    float R[128 * 3];
+    R[0] = R[1] = R[2] = 0.0f;
+    float z4[4] = {0.f, 0.f, 0.f, 0.f};
+    for (int m = 0; m < 3 * (N - 1); ++m) {               // normal m = 3*bond + axis
+        if ((m & 3) == 0) normal_call(sk, DOM_INIT_BOND, chain, (uint32_t)(m >> 2), z4);
+        R[m + 3] = fmaf(P.sq13, z4[m & 3], R[m]);
+    }
+    for (int i = 0; i < N; ++i)
+        for (int c = 0; c < 3; ++c) *reinterpret_cast<float *>(st + off_R(k, N, i, c)) = R[3 * i + c];
+
+    int Z = 0;
+    if (P.springs_on) {
+        uint32_t w[4];
+        stream_call(sk, DOM_INIT_Z, chain, 0u, w);
+        const uint32_t code = code23(w[0]);
+        while (Z < zmax && code >= P.t_cdf[Z]) ++Z;
+    }
+    *reinterpret_cast<int *>(st + off_Z(k, N)) = Z;
+    for (int j = 0; j < zmax; ++j) {
+        int s = 0; float a[3] = {0.f, 0.f, 0.f};
+        if (j < Z) {
+            uint32_t w[4];
+            stream_call(sk, DOM_INIT_SLOT, chain, (uint32_t)j, w);
+            s = 1 + (int)__umulhi(w[0], (uint32_t)N);
+            normal_call(sk, DOM_INIT_ANCHOR, chain, (uint32_t)j, z4);
+            for (int c = 0; c < 3; ++c) a[c] = fmaf(P.sq_ns3, z4[c], R[3 * (s - 1) + c]);
+        }
+        st[off_S(k, N, j)] = (unsigned char)s;
+        for (int c = 0; c < 3; ++c) *reinterpret_cast<float *>(st + off_A(k, N, j, c)) = a[c];
+    }
+}
+
+cudaError_t launch_init(const InitParams &p, cudaStream_t st)
+{
+    const int threads = 128;
+    const long long blocks = (p.n_chains_padded + threads - 1) / threads;
+    ssm_init_kernel<<<(unsigned)blocks, threads, 0, st>>>(p);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------
+// State export / import between the tiled image and the external SoA layout of ssm.h.
+// rows 0..3N-1 of R, then 3N rows of A, then N rows of S; chains [k0, k0+nk), external
+// element (row, k) at row*pitch + (k - k0).
+// ---------------------------------------------------------------------------------------
+template <bool EXPORT>
+__global__ void __launch_bounds__(256) ssm_xfer_kernel(unsigned char *state, float *R, float *A, unsigned char *S,
+                                                       int N, long long k0, long long nk, long long pitch)
+{
+    const long long kk = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (kk >= nk) return;
+    const long long k = k0 + kk;
+    const int row = blockIdx.y;                         // 0 .. 7N-1
+    if (row < 3 * N) {
+        const int c = row / N, i = row % N;
+        float *p = reinterpret_cast<float *>(state + off_R(k, N, i, c));
+        if (EXPORT) R[(long long)row * pitch + kk] = *p; else *p = R[(long long)row * pitch + kk];
+    } else if (row < 6 * N) {
+        const int rr = row - 3 * N, c = rr / N, j = rr % N;
+        float *p = reinterpret_cast<float *>(state + off_A(k, N, j, c));
+        if (EXPORT) A[(long long)rr * pitch + kk] = *p; else *p = A[(long long)rr * pitch + kk];
+    } else {
+        const int j = row - 6 * N;
+        unsigned char *p = state + off_S(k, N, j);
+        if (EXPORT) S[(long long)j * pitch + kk] = *p; else *p = S[(long long)j * pitch + kk];
+    }
+}
+
+// after an import: Z_k = number of occupied slots (they must be the leading ones)
+__global__ void __launch_bounds__(256) ssm_count_z_kernel(unsigned char *state, int N, long long k0, long long nk)
+{
+    const long long kk = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (kk >= nk) return;
+    const long long k = k0 + kk;
+    int Z = 0;
+    while (Z < N && state[off_S(k, N, Z)] != 0) ++Z;
+    *reinterpret_cast<int *>(state + off_Z(k, N)) = Z;
+}
+
+cudaError_t launch_xfer(bool do_export, unsigned char *state, float *R, float *A, unsigned char *S, int N,
+                        long long k0, long long nk, long long pitch, cudaStream_t st)
+{
+    dim3 grid((unsigned)((nk + 255) / 256), (unsigned)(7 * N));
+    if (do_export) ssm_xfer_kernel<true><<<grid, 256, 0, st>>>(state, R, A, S, N, k0, nk, pitch);
+    else {
+        ssm_xfer_kernel<false><<<grid, 256, 0, st>>>(state, R, A, S, N, k0, nk, pitch);
+        ssm_count_z_kernel<<<(unsigned)((nk + 255) / 256), 256, 0, st>>>(state, N, k0, nk);
+    }
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------
+// Per-chain stress of the current state (eqs 16 and 76): out[t][k], t = 0..11.
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) ssm_chain_stress_kernel(const unsigned char *state, float *out, int N,
+                                                               long long M, float cs)
+{
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= M) return;
+    float sg[6] = {0, 0, 0, 0, 0, 0}, sv[6] = {0, 0, 0, 0, 0, 0};
+    float p[3], q[3];
+    for (int c = 0; c < 3; ++c) p[c] = *reinterpret_cast<const float *>(state + off_R(k, N, 0, c));
+    for (int i = 1; i < N; ++i) {
+        float b[3];
+        for (int c = 0; c < 3; ++c) { q[c] = *reinterpret_cast<const float *>(state + off_R(k, N, i, c)); b[c] = q[c] - p[c]; p[c] = q[c]; }
+        sg[0] += fmaf(3.f * b[0], b[0], -1.f); sg[1] += fmaf(3.f * b[1], b[1], -1.f); sg[2] += fmaf(3.f * b[2], b[2], -1.f);
+        sg[3] = fmaf(3.f * b[0], b[1], sg[3]); sg[4] = fmaf(3.f * b[1], b[2], sg[4]); sg[5] = fmaf(3.f * b[2], b[0], sg[5]);
+    }
+    sg[0] -= 1.f; sg[1] -= 1.f; sg[2] -= 1.f;                 // 3 sum b^2 - N = sum (3 b^2 - 1) - 1
+    const int Z = *reinterpret_cast<const int *>(state + off_Z(k, N));
+    for (int j = 0; j < Z; ++j) {
+        const int s = state[off_S(k, N, j)] - 1;
+        float d[3];
+        for (int c = 0; c < 3; ++c)
+            d[c] = *reinterpret_cast<const float *>(state + off_R(k, N, s, c)) - *reinterpret_cast<const float *>(state + off_A(k, N, j, c));
+        sv[0] += fmaf(cs * d[0], d[0], -1.f); sv[1] += fmaf(cs * d[1], d[1], -1.f); sv[2] += fmaf(cs * d[2], d[2], -1.f);
+        sv[3] = fmaf(cs * d[0], d[1], sv[3]); sv[4] = fmaf(cs * d[1], d[2], sv[4]); sv[5] = fmaf(cs * d[2], d[0], sv[5]);
+    }
+    for (int t = 0; t < 6; ++t) { out[(long long)t * M + k] = sg[t]; out[(long long)(6 + t) * M + k] = sv[t]; }
+}
+
+cudaError_t launch_chain_stress(const unsigned char *state, float *out, int N, long long M, float cs, cudaStream_t st)
+{
+    ssm_chain_stress_kernel<<<(unsigned)((M + 127) / 128), 128, 0, st>>>(state, out, N, M, cs);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------
+// Multi-tau correlator (BASELINE.json config 2).  One thread per chain.
+// Level l holds the last P values of g block-averaged over 2^l samples; inserting (f, g)
+// at level l adds f * g_(k entries ago) to sum[group][l][k] for k = kmin .. filled-1
+// (kmin = 0 on level 0, P/2 above), then feeds the running pair; every second insertion
+// pushes the pair's mean to level l+1.  Every chain receives the same number of samples,
+// so ring positions, fill counts and pair parities are the same for all chains: they live
+// on the host (which also keeps the product counts) and are replayed here from their
+// values at the start of the launch.  Sums are int64 fixed point (2^-16) so that the
+// result does not depend on the order of the atomics.
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) ssm_corr_kernel(const __grid_constant__ CorrParams C)
+{
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= C.M) return;
+    const int L = C.L, Pb = C.Pb;
+    const int group = (int)((C.chain_offset + (unsigned long long)k) % (unsigned)C.groups);
+    long long *gsum = C.sum + (long long)group * L * Pb;
+    unsigned char pos[kCorrMaxLevels], fil[kCorrMaxLevels], par[kCorrMaxLevels];
+    for (int lev = 0; lev < L; ++lev) { pos[lev] = C.pos[lev]; fil[lev] = C.filled[lev]; par[lev] = C.parity[lev]; }
+    for (int s = 0; s < C.n_samples; ++s) {
+        const float2 fg = C.samples[(long long)s * C.M + k];
+        float f = fg.x, g = fg.y;
+        for (int lev = 0; lev < L; ++lev) {
+            const long long lm = (long long)lev * C.M + k;
+            float *ring = C.ring + (long long)lev * Pb * C.M + k;
+            const int p0 = pos[lev];
+            ring[(long long)p0 * C.M] = g;
+            if (fil[lev] < Pb) ++fil[lev];
+            const int kmin = lev == 0 ? 0 : Pb / 2;
+            for (int q = kmin; q < fil[lev]; ++q) {
+                int idx = p0 - q; if (idx < 0) idx += Pb;
+                const float prod = f * ring[(long long)idx * C.M];
+                atomicAdd(reinterpret_cast<unsigned long long *>(gsum + lev * Pb + q),
+                          (unsigned long long)__double2ll_rn((double)prod * 65536.0));
+            }
+            pos[lev] = (unsigned char)((p0 + 1) % Pb);
+            if (par[lev] == 0) {
+                C.acc_f[lm] = f; C.acc_g[lm] = g; par[lev] = 1;
+                break;
+            }
+            f = 0.5f * (C.acc_f[lm] + f); g = 0.5f * (C.acc_g[lm] + g);
+            par[lev] = 0;
+        }
+    }
+}
+
+cudaError_t launch_corr(const CorrParams &c, cudaStream_t st)
+{
+    ssm_corr_kernel<<<(unsigned)((c.M + 255) / 256), 256, 0, st>>>(c);
+    return cudaGetLastError();
+}
+
+}  // namespace ssm

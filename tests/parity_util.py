@@ -1,0 +1,57 @@
+"""Helpers of the GPU parity tests: move a state between the oracle's arrays (fp64,
+[M][N][3]) and the library's external SoA layout (fp32, [3][N][M]), and the acceptance
+rules of DESIGN.md section 8.  No arithmetic of the method lives here."""
+import numpy as np
+
+TOL = 1e-5          # BASELINE.json north_star: positions and stress within 1e-5 relative (fp32 GPU vs fp64 oracle)
+GUARD = 1e-5        # a hop decision with |u - threshold| < GUARD is "fragile" (fp32 may decide differently)
+
+
+def to_external(e):
+    """oracle.Ensemble -> (R[3][N][M] f32, A[3][N][M] f32, S[N][M] u8)."""
+    assert e.zmax == e.N
+    R = np.ascontiguousarray(e.R.transpose(2, 1, 0)).astype(np.float32)
+    A = np.ascontiguousarray(e.A.transpose(2, 1, 0)).astype(np.float32)
+    S = np.ascontiguousarray(e.S.T).astype(np.uint8)
+    return R, A, S
+
+
+def from_external(R, A, S):
+    """-> (R[M][N][3], A[M][N][3], S[M][N] int32, Z[M]) as fp64 / int arrays."""
+    Ro = np.ascontiguousarray(R.transpose(2, 1, 0)).astype(np.float64)
+    Ao = np.ascontiguousarray(A.transpose(2, 1, 0)).astype(np.float64)
+    So = np.ascontiguousarray(S.T).astype(np.int32)
+    return Ro, Ao, So, (So > 0).sum(1).astype(np.int32)
+
+
+def upload(e, g):
+    """Reading R19: both sides start from the oracle's state rounded to fp32."""
+    e.round_to_fp32()
+    R, A, S = to_external(e)
+    g.set_state(R, A, S, e.step)
+
+
+def close(a, b, tol=TOL):
+    """|a - b| <= tol * max(1, |b|) element-wise; returns (ok, worst ratio)."""
+    a = np.asarray(a, dtype=np.float64); b = np.asarray(b, dtype=np.float64)
+    ratio = np.abs(a - b) / np.maximum(1.0, np.abs(b))
+    worst = float(ratio.max()) if ratio.size else 0.0
+    return worst <= tol, worst
+
+
+def compare_state(e, g, upto_step=None):
+    """Compare the GPU state with the oracle's on every chain whose first fragile hop
+    decision (if any) lies at or after the current step: S and Z bit-exact, R and A within
+    TOL.  Returns (number of chains compared, worst position ratio)."""
+    R, A, S, step = g.get_state()
+    assert step == e.step
+    Rg, Ag, Sg, Zg = from_external(R, A, S)
+    ok = (e.first_fragile < 0) | (e.first_fragile >= e.step)
+    assert np.array_equal(Sg[ok], e.S[ok]), "slip-spring indices differ on a non-fragile chain"
+    assert np.array_equal(Zg[ok], e.Z[ok])
+    good, worst = close(Rg[ok], e.R[ok])
+    assert good, "bead positions off by %.3g (tolerance %.1g)" % (worst, TOL)
+    occ = e.S[ok] > 0
+    good, worst_a = close(Ag[ok][occ], e.A[ok][occ])
+    assert good, "anchors off by %.3g" % worst_a
+    return int(ok.sum()), max(worst, worst_a)

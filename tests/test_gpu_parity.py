@@ -1,0 +1,163 @@
+"""GPU parity: the CUDA path (through the C ABI of include/ssm.h) against the fp64 oracle on
+the same seeded inputs.  Acceptance (BASELINE.json north_star):
+slip-spring indices, counts and accept/reject decisions bit-exact on every chain up to its
+first fragile hop decision; bead positions, anchors and stresses within 1e-5 relative."""
+import numpy as np
+import pytest
+
+import oracle
+from parity_util import GUARD, TOL, close, compare_state, from_external, to_external, upload
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ssm():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_1106_2899_b200 as m
+    m.lib()
+    return m
+
+
+def _pair(ssm, N, M, steps, seed=1, n_0=4.0, dt=0.01, stress_every=1, **kw):
+    e = oracle.Ensemble(N, M, n_0=n_0, dt=dt, seed=seed)
+    g = ssm.Ensemble(N, M, n_0=n_0, dt=dt, seed=seed, stress_every=stress_every,
+                     stress_capacity=steps // max(stress_every, 1) + 1, **kw)
+    upload(e, g)
+    return e, g
+
+
+def test_set_get_state_roundtrip_is_bit_exact(ssm):
+    e = oracle.Ensemble(32, 37, seed=5)            # 37 chains: ragged last warp tile (4 chains per warp)
+    e.round_to_fp32()
+    R, A, S = to_external(e)
+    g = ssm.Ensemble(32, 37, seed=5)
+    g.set_state(R, A, S, 123)
+    R2, A2, S2, step = g.get_state()
+    assert step == 123
+    assert np.array_equal(R, R2) and np.array_equal(A, A2) and np.array_equal(S, S2)
+
+
+def test_device_init_matches_oracle_init(ssm):
+    """a0: Z and S bit-exact (integer-domain sampling), R and A to fp32 rounding."""
+    for N, M in ((8, 300), (32, 130), (128, 20)):
+        e = oracle.Ensemble(N, M, seed=9)
+        g = ssm.Ensemble(N, M, seed=9)
+        Rg, Ag, Sg, Zg = from_external(*g.get_state()[:3])
+        assert np.array_equal(Sg, e.S) and np.array_equal(Zg, e.Z)
+        assert close(Rg, e.R, 2e-6)[0]
+        assert close(Ag, e.A, 2e-6)[0]
+
+
+def test_rouse_limit_positions_and_ensemble_stress_1000_steps(ssm):
+    """Slip-springs off: no discrete decisions, so all chains and the ensemble
+    stress of every step must match.  M = 70 leaves a ragged tile."""
+    N, M, steps = 32, 70, 1000
+    e, g = _pair(ssm, N, M, steps, seed=3, n_0=0.0)
+    want = e.run(steps, stress_every=1)
+    g.step(steps)
+    n, worst = compare_state(e, g)
+    assert n == M
+    got = g.stress()
+    ok, w = close(got, want)
+    assert ok, "ensemble stress off by %.3g" % w
+    assert np.all(got[:, 6:] == 0.0)
+
+
+def test_c1_tiny_equilibrium_ensemble(ssm):
+    """BASELINE.json config 1: 256 chains, N = 8, 2000 steps, dumps at 1, 10, 100, 1000, 2000."""
+    N, M = 8, 256
+    e, g = _pair(ssm, N, M, 2000, seed=1)
+    done, wants = 0, []
+    for upto in (1, 10, 100, 1000, 2000):
+        wants.append(e.run(upto - done, stress_every=1, guard=GUARD))
+        g.step(upto - done)
+        done = upto
+        n, worst = compare_state(e, g)
+        # expected cut-short chains ~ hop decisions x 2 x 2 GUARD ~ 20 per 1000 steps; more is a bug
+        assert n >= M - (3 + upto // 20), (upto, n)
+    want = np.concatenate(wants)
+    got = g.stress()
+    first = e.first_fragile[e.first_fragile >= 0]
+    clean = int(first.min()) if first.size else 2000        # steps before any chain could have forked
+    assert clean >= 5
+    ok, w = close(got[:clean], want[:clean])
+    assert ok, "ensemble stress off by %.3g over the first %d steps" % (w, clean)
+    # after forks the ensemble means differ by O(forked chains / M) only
+    assert np.abs(got - want).max() < 0.5
+
+
+@pytest.mark.parametrize("N,M,steps", [(16, 200, 300), (32, 100, 1000), (64, 33, 200), (128, 19, 200)])
+def test_slipspring_chains_all_sizes(ssm, N, M, steps):
+    e, g = _pair(ssm, N, M, steps, seed=7)
+    e.run(steps, guard=GUARD)
+    g.step(steps)
+    n, worst = compare_state(e, g)
+    assert n >= 0.8 * M
+    # per-chain stresses of the final state on the chains that cannot have forked
+    cs = g.chain_stress()
+    ok = (e.first_fragile < 0)
+    want = np.array([np.concatenate(e.chain_stress(k)) for k in np.nonzero(ok)[0]])
+    good, w = close(cs.T[ok], want, 2e-5)
+    assert good, w
+
+
+def test_shear_flow(ssm):
+    """eq 44/45 with kappa_xy = gamma_dot (eq 60): beads and anchors are advected."""
+    N, M, steps = 32, 64, 400
+    e, g = _pair(ssm, N, M, steps, seed=11)
+    want = e.run(steps, shear_rate=0.1, stress_every=1, guard=GUARD)
+    g.step(steps, shear_rate=0.1)
+    n, worst = compare_state(e, g)
+    assert n >= 0.8 * M
+    first = e.first_fragile[e.first_fragile >= 0]
+    clean = int(first.min()) if first.size else steps
+    ok, w = close(g.stress()[:clean], want[:clean])
+    assert ok, w
+
+
+def test_split_runs_fusion_depth_and_ensemble_size_do_not_change_results(ssm):
+    """P8: step(a); step(b) == step(a+b); results do not depend on the fusion depth nor on M
+    (Philox is keyed by the global chain index and step)."""
+    N = 32
+    ref = ssm.Ensemble(N, 256, seed=21, stress_every=1, stress_capacity=100)
+    ref.step(90)
+    R0, A0, S0, _ = ref.get_state()
+    a = ssm.Ensemble(N, 256, seed=21, stress_every=1, stress_capacity=100)
+    for n in (1, 7, 32, 33, 17):
+        a.step(n)
+    b = ssm.Ensemble(N, 256, seed=21, stress_every=1, stress_capacity=100)
+    b.set_fusion(5)
+    b.step(90)
+    for x in (a, b):
+        R, A, S, step = x.get_state()
+        assert step == 90
+        assert np.array_equal(R, R0) and np.array_equal(A, A0) and np.array_equal(S, S0)
+        assert np.array_equal(x.stress_sums(), ref.stress_sums())
+    small = ssm.Ensemble(N, 64, seed=21)
+    small.step(90)
+    R, A, S, _ = small.get_state()
+    assert np.array_equal(R, R0[:, :, :64]) and np.array_equal(S, S0[:, :64]) and np.array_equal(A, A0[:, :, :64])
+    # a shard with chain_offset reproduces its part of the full run (multi-GPU partition)
+    shard = ssm.Ensemble(N, 64, seed=21, chain_offset=128)
+    shard.step(90)
+    R, A, S, _ = shard.get_state()
+    assert np.array_equal(R, R0[:, :, 128:192]) and np.array_equal(S, S0[:, 128:192])
+
+
+def test_correlator_matches_oracle_on_identical_trajectories(ssm):
+    """Rouse limit (no forks): GPU multi-tau sums against the oracle's correlator fed by
+    the oracle's own stresses of the same trajectories."""
+    N, M, steps = 8, 512, 2000
+    e = oracle.Ensemble(N, M, n_0=0.0, seed=13)
+    g = ssm.Ensemble(N, M, n_0=0.0, seed=13, sample_every=10, corr_levels=6, corr_bins=16, corr_groups=32)
+    upload(e, g)
+    corr = oracle.Correlator(M, levels=6, bins=16, groups=32)
+    e.run(steps, sample_every=10, corr=corr)
+    g.step(steps)
+    t0, G0, se0 = corr.result(N, 0.1)
+    t1, G1, se1 = g.gt()
+    assert np.allclose(t0, t1)
+    assert np.allclose(G1, G0, rtol=0, atol=2e-4 * np.abs(G0).max())
+    assert np.allclose(se1, se0, rtol=0.02, atol=1e-6)
