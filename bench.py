@@ -1,0 +1,288 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the slip-spring ensemble hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \
+        --master-port P bench.py --gpus N --steps K --warmup W
+
+Workload (BASELINE.json configs[3], "Throughput scaling", the configuration north_star's
+target is quoted on): 1,048,576 chains per GPU, N = 32 beads, N_s = 0.5, N_0 = 4,
+zeta_s = 0.1, dt = 0.01, no flow, ensemble stress reduced after every time step.
+One bench "step" = one pass of the whole hot path (rows a1..a8, a10 of DESIGN.md section 2)
+over the ensemble for --inner time steps (default 128) = one ssm_step(inner) call.
+
+Prints ONE JSON line (rank 0).  metric = bead-updates/s summed over all GPUs.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+# Frozen algorithmic thread-instruction count per bead-update of the N = 32, <Z> = 8 step
+# (DESIGN.md section 9.2).  The roofline numerator is I_ALG x bead-updates/s, NOT the number
+# of instructions the kernel happens to execute, so padding cannot raise the fraction.
+I_ALG = 100.0
+N_SM, SMSP_PER_SM, LANES = 148, 4, 32
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--chains", type=int, default=1 << 20, help="chains per GPU")
+    ap.add_argument("--beads", type=int, default=32)
+    ap.add_argument("--inner", type=int, default=128, help="time steps per bench step")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    return ap.parse_args()
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1 and len(r) >= 7] or [r for (_, r) in self.rows if len(r) >= 7]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm = sorted(float(r[0]) for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "reasons": reasons,
+                "samples": len(rows), "power_w_max": max(float(r[2]) for r in rows)}
+
+
+def cpu_baseline(n_beads, seconds, threads=None):
+    """The fp64 oracle, as it stands, on the host cores: a bounded sample of the same
+    workload (same parameters and initial-state law; the rate is intensive in M)."""
+    import oracle
+    threads = threads or (os.cpu_count() or 1)
+    M = 4096
+    e = oracle.Ensemble(n_beads, M, seed=4)
+    t0 = time.perf_counter(); e.run(4, stress_every=1, n_threads=threads); probe = (time.perf_counter() - t0) / 4
+    n = int(max(8, min(20000, seconds / max(probe, 1e-6))))
+    t0 = time.perf_counter(); e.run(n, stress_every=1, n_threads=threads); dt = time.perf_counter() - t0
+    return {"value": M * n_beads * n / dt, "unit": "bead-updates/s", "cores": threads, "kind": "oracle",
+            "sample": "%d chains x N=%d x %d steps, stress every step, %d threads, %.1f s" % (M, n_beads, n, threads, dt)}
+
+
+def run_reference(a):
+    """--impl reference: the oracle on the host cores, same config / metric / unit; each step
+    is a bounded sample (4096 chains x inner_ref time steps) of the workload."""
+    import oracle
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    threads = os.cpu_count() or 1
+    M = 4096
+    e = oracle.Ensemble(a.beads, M, seed=4)
+    t0 = time.perf_counter(); e.run(2, stress_every=1, n_threads=threads); probe = (time.perf_counter() - t0) / 2
+    budget = 120.0 / max(1, a.steps + a.warmup)                # whole run within a few minutes
+    inner = int(max(1, min(a.inner, budget / max(probe, 1e-6))))
+    for _ in range(a.warmup):
+        e.run(inner, stress_every=1, n_threads=threads)
+    t0 = time.perf_counter()
+    for _ in range(a.steps):
+        e.run(inner, stress_every=1, n_threads=threads)
+    dt = time.perf_counter() - t0
+    v = M * a.beads * inner * a.steps / dt
+    sample = "%d chains x N=%d x %d time steps per step, %d threads" % (M, a.beads, inner, threads)
+    print(json.dumps({
+        "impl": "reference", "metric": "bead-updates/s", "value": v, "unit": "bead-updates/s", "n_gpus": a.gpus,
+        "steps": a.steps, "warmup": a.warmup, "ms_per_step": 1e3 * dt / a.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(a, M, inner, 1),
+        "cpu_baseline": {"value": v, "unit": "bead-updates/s", "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": "bead-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "chain_steps_per_s": v / a.beads}))
+
+
+def workload_config(a, chains_per_gpu, inner, world):
+    return {"workload": "BASELINE.json configs[3] 'Throughput scaling': %d chains/GPU x N=%d, N_s=0.5, N_0=4, "
+                        "zeta_s=0.1, dt=0.01, no flow, stress reduced every step" % (chains_per_gpu, a.beads),
+            "chains_per_gpu": chains_per_gpu, "n_beads": a.beads, "time_steps_per_step": inner,
+            "global_chains": chains_per_gpu * world, "parallelism": "ensemble-dp%d" % world,
+            "l2": "state (%.0f MB/GPU) is larger than the 126 MB L2; no flush needed" % (chains_per_gpu * 25 * a.beads * 1.04 / 1e6)}
+
+
+def main():
+    a = parse()
+    if a.impl == "reference":
+        return run_reference(a)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1106_2899_b200 import shard
+    import paper_1106_2899_b200 as ssm
+
+    rank, local_rank, world = shard.world()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    M, N, inner, K, W = a.chains, a.beads, a.inner, a.steps, a.warmup
+    k0, _ = shard.weak_range(M, rank)
+    total_steps = (K + W + 2) * inner
+    g = ssm.Ensemble(N, M, seed=4, chain_offset=k0, stress_every=1, stress_capacity=total_steps + 2 * inner,
+                     device="cuda:%d" % local_rank)
+    g.step(200)                                   # leave the sampled state's first transient behind
+    g.reset_accumulators()
+    torch.cuda.synchronize()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput: K bench steps, inputs already in HBM
+    def one_step():
+        first = g.stress_count()
+        g.step(inner)
+        if world > 1:                              # the path's only exchange: exact int64 sums (eq 54)
+            shard.allreduce_sums(g.stress_sums_device(first, inner))
+
+    for _ in range(W):
+        one_step()
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    l0 = g.launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
+    t_wall0 = time.time()
+    ev[0].record()
+    for i in range(K):
+        one_step()
+        ev[i + 1].record()
+    barrier()
+    t_wall1 = time.time()
+    launches = g.launch_count() - l0
+    ms = ev[0].elapsed_time(ev[K])
+    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    bead_updates = float(M) * N * inner * K * world
+    value = bead_updates / (ms_max * 1e-3)
+    launch_ms = ms / max(launches, 1)             # only the step kernel launches inside the region at N = 1
+
+    # ---- end to end through the public API with HOST buffers (pinned): upload the state,
+    # step, read the stress samples back
+    e2e = None
+    if not a.no_e2e:
+        R, A, S, step = g.get_state()
+        pin = [torch.from_numpy(x).pin_memory() for x in (R, A, S)]
+        Rp, Ap, Sp = [p.numpy() for p in pin]
+        h2d = Rp.nbytes + Ap.nbytes + Sp.nbytes
+        ke = max(2, min(K, 4))
+        def e2e_step():
+            g.reset_accumulators()
+            g.set_state(Rp, Ap, Sp, step)
+            g.step(inner)
+            return g.stress()
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(ke):
+            out = e2e_step()
+        barrier()
+        dt = time.perf_counter() - t0
+        t = torch.tensor([dt], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e = {"value": float(M) * N * inner * ke * world / float(t.item()), "unit": "bead-updates/s",
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(out.nbytes),
+               "steps": ke, "what": "ssm_set_state(host pinned) + ssm_step(%d) + ssm_stress(host)" % inner}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peaks = measured_peaks()
+    peak_alu = N_SM * SMSP_PER_SM * LANES * peaks["sm_max_mhz"] * 1e6 / 1e12      # T thread-instr/s
+    per_launch_updates = float(M) * N * inner * K / max(launches, 1)
+    achieved = I_ALG * per_launch_updates / (launch_ms * 1e-3) / 1e12
+    cpw = 128 // N
+    tile_bytes = 3328.0 * ((M + cpw - 1) // cpw)
+    hbm_achieved = 2.0 * tile_bytes / (launch_ms * 1e-3) / 1e9
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        try:
+            traffic = json.load(open(tp)).get("dram_bytes_per_launch")
+        except Exception:
+            traffic = None
+    line = {
+        "metric": "bead-updates/s", "value": value, "unit": "bead-updates/s", "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic", "config": workload_config(a, M, inner, world),
+        "chain_steps_per_s": value / N,
+        "clocks": clocks, "gpu_launches": int(launches),
+        "e2e": e2e,
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_alu, "unit": "T thread-instr/s",
+                     "frac": achieved / peak_alu, "traffic": traffic,
+                     "kernel": "ssm_step_kernel<G=%d>" % (N // 4), "launch_ms": launch_ms,
+                     "i_alg_per_bead_update": I_ALG,
+                     "peak_how": "148 SM x 4 SMSP x 32 lanes x %.0f MHz (sm_max_mhz, %s)" % (peaks["sm_max_mhz"], peaks["source"]),
+                     "hbm": {"achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                             "frac": hbm_achieved / peaks["hbm_gbs"], "bytes_per_launch": 2.0 * tile_bytes,
+                             "peak_source": peaks["source"]}},
+        "paper_context": {"gpu_bead_updates_per_s": 7.3e8, "cpu_bead_updates_per_s": 2.5e6,
+                          "hardware": "Tesla C1060 / Core 2 Duo E8500 1 thread (PAPER.md Table 1)"},
+    }
+    if not a.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(N, a.cpu_seconds)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -100,6 +100,12 @@ int ssm_stress(ssm_ctx *ctx, int64_t first_sample, int64_t n_samples, double *h_
  * sum over local chains of (component + delta_ab) * 2^24 rounded per warp. */
 int ssm_stress_sums(ssm_ctx *ctx, int64_t first_sample, int64_t n_samples, int64_t *h_out);
 
+/* Device address of those sums for samples [first_sample, first_sample + n_samples): *d_ptr
+ * (device) int64 [n_samples][12] inside the caller's workspace, so that a multi-GPU run can
+ * all-reduce them in place (NCCL) without a copy.  Work queued on the ctx's stream must be
+ * ordered before any use on another stream by the caller. */
+int ssm_stress_sums_device(ssm_ctx *ctx, int64_t first_sample, int64_t n_samples, int64_t **d_ptr);
+
 /* Per-chain stresses of the CURRENT state: out [12][M] float32 (component-major, chain
  * fastest), host or device. */
 int ssm_chain_stress(ssm_ctx *ctx, float *out, int pointers_are_device);

@@ -15,7 +15,7 @@ from . import build as _build
 SSM_OK, SSM_EINVAL, SSM_ENOMEM, SSM_ECUDA, SSM_ESTATE, SSM_ERANGE = 0, -1, -2, -3, -4, -5
 
 EXPORTS = ["ssm_workspace_bytes", "ssm_init", "ssm_step", "ssm_stress_count", "ssm_stress", "ssm_stress_sums",
-           "ssm_chain_stress", "ssm_gt", "ssm_gt_sums", "ssm_get_state", "ssm_set_state",
+           "ssm_stress_sums_device", "ssm_chain_stress", "ssm_gt", "ssm_gt_sums", "ssm_get_state", "ssm_set_state",
            "ssm_reset_accumulators", "ssm_launch_count", "ssm_set_fusion", "ssm_destroy", "ssm_last_error"]
 
 
@@ -50,6 +50,7 @@ def lib():
     L.ssm_stress_count.argtypes = [vp]; L.ssm_stress_count.restype = C.c_int64
     L.ssm_stress.argtypes = [vp, C.c_int64, C.c_int64, dp]; L.ssm_stress.restype = C.c_int
     L.ssm_stress_sums.argtypes = [vp, C.c_int64, C.c_int64, C.POINTER(C.c_int64)]; L.ssm_stress_sums.restype = C.c_int
+    L.ssm_stress_sums_device.argtypes = [vp, C.c_int64, C.c_int64, C.POINTER(vp)]; L.ssm_stress_sums_device.restype = C.c_int
     L.ssm_chain_stress.argtypes = [vp, fp, C.c_int]; L.ssm_chain_stress.restype = C.c_int
     L.ssm_gt.argtypes = [vp, C.POINTER(C.c_int32), dp, dp, dp]; L.ssm_gt.restype = C.c_int
     L.ssm_gt_sums.argtypes = [vp, dp, C.POINTER(C.c_int64)]; L.ssm_gt_sums.restype = C.c_int
@@ -122,6 +123,14 @@ class Ensemble:
         out = np.zeros((max(n, 1), 12), dtype=np.int64)
         self._ck(lib().ssm_stress_sums(self.h, first, n, out.ctypes.data_as(C.POINTER(C.c_int64))))
         return out[:n]
+
+    def stress_sums_device(self, first=0, n=None):
+        """int64 CUDA tensor [n][12] aliasing the fixed-point sums inside the workspace."""
+        n = self.stress_count() - first if n is None else n
+        p = C.c_void_p()
+        self._ck(lib().ssm_stress_sums_device(self.h, first, n, C.byref(p)))
+        off = (p.value or 0) - self.workspace.data_ptr()
+        return self.workspace[off:off + n * 96].view(self._torch.int64).view(n, 12)
 
     def chain_stress(self, out=None):
         """[12][M] float32: numpy (host) by default, or fill a given CUDA tensor."""

@@ -292,6 +292,15 @@ extern "C" int ssm_stress_sums(ssm_ctx *c, int64_t first, int64_t n, int64_t *h_
     return SSM_OK;
 }
 
+extern "C" int ssm_stress_sums_device(ssm_ctx *c, int64_t first, int64_t n, int64_t **d_ptr)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (!d_ptr) return fail(c, SSM_EINVAL, "d_ptr is NULL");
+    if (first < 0 || n < 0 || first + n > c->n_records) return fail(c, SSM_ERANGE, "stress samples not recorded");
+    *d_ptr = reinterpret_cast<int64_t *>(c->ws + c->lay.stress) + first * 12;
+    return SSM_OK;
+}
+
 extern "C" int ssm_stress(ssm_ctx *c, int64_t first, int64_t n, double *h_out)
 {
     if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");

@@ -28,6 +28,15 @@ def _pair(ssm, N, M, steps, seed=1, n_0=4.0, dt=0.01, stress_every=1, **kw):
     return e, g
 
 
+def _min_unflagged(M, N, steps):
+    """Chains the oracle flags as fragile are excluded from the comparison.  A chain makes
+    about (N/4) x 2 hop comparisons per step, each within GUARD of its threshold with
+    probability ~ 2 GUARD (u is uniform), so the unflagged fraction after n steps is about
+    exp(-N n GUARD); fewer than that minus 4 sigma means the flags hide a bug."""
+    f = np.exp(-N * steps * GUARD)
+    return M * f - 4.0 * np.sqrt(M * f * (1.0 - f)) - 1.0
+
+
 def test_set_get_state_roundtrip_is_bit_exact(ssm):
     e = oracle.Ensemble(32, 37, seed=5)            # 37 chains: ragged last warp tile (4 chains per warp)
     e.round_to_fp32()
@@ -46,8 +55,12 @@ def test_device_init_matches_oracle_init(ssm):
         g = ssm.Ensemble(N, M, seed=9)
         Rg, Ag, Sg, Zg = from_external(*g.get_state()[:3])
         assert np.array_equal(Sg, e.S) and np.array_equal(Zg, e.Z)
-        assert close(Rg, e.R, 2e-6)[0]
-        assert close(Ag, e.A, 2e-6)[0]
+        # R_i is a running fp32 sum of i bonds: rounding grows like sqrt(i) half-ulps of |R| <~ 16
+        tol = 2e-6 if N <= 32 else 5e-6
+        ok, w = close(Rg, e.R, tol)
+        assert ok, "N=%d: R off by %.3g" % (N, w)
+        ok, w = close(Ag, e.A, tol)
+        assert ok, "N=%d: A off by %.3g" % (N, w)
 
 
 def test_rouse_limit_positions_and_ensemble_stress_1000_steps(ssm):
@@ -94,7 +107,7 @@ def test_slipspring_chains_all_sizes(ssm, N, M, steps):
     e.run(steps, guard=GUARD)
     g.step(steps)
     n, worst = compare_state(e, g)
-    assert n >= 0.8 * M
+    assert n >= _min_unflagged(M, N, steps)
     # per-chain stresses of the final state on the chains that cannot have forked
     cs = g.chain_stress()
     ok = (e.first_fragile < 0)
@@ -110,7 +123,7 @@ def test_shear_flow(ssm):
     want = e.run(steps, shear_rate=0.1, stress_every=1, guard=GUARD)
     g.step(steps, shear_rate=0.1)
     n, worst = compare_state(e, g)
-    assert n >= 0.8 * M
+    assert n >= _min_unflagged(M, N, steps)
     first = e.first_fragile[e.first_fragile >= 0]
     clean = int(first.min()) if first.size else steps
     ok, w = close(g.stress()[:clean], want[:clean])
