@@ -225,7 +225,8 @@ static int attempts_K(const oracle_params *p, int Z)
 {
     const int empty = oracle_zmax(p) - Z;
     if (!springs_on(p) || empty <= 0) return 0;
-    return p->k_mode == ORACLE_K_ONE ? 1 : empty;
+    if (p->k_mode > 0) return p->k_mode < empty ? p->k_mode : empty;   /* fixed K (K = 1: the paper's CPU choice) */
+    return empty;                                                      /* K = N - Z: the paper's GPU choice */
 }
 
 void oracle_step_chain(const oracle_params *p, uint64_t chain, uint64_t step, double shear_rate,
@@ -284,20 +285,25 @@ void oracle_step_chain(const oracle_params *p, uint64_t chain, uint64_t step, do
      * K is taken from the Z before this substep. */
     const int Z0 = Z;
     const int K = attempts_K(p, Z0);
-    /* destruction, eq (53): prob min{(dt/zeta_s)(delta_{S,1}+delta_{S,N}), 1} */
+    /* destruction, eq (53): prob min{(dt/zeta_s)(delta_{S,1}+delta_{S,N}), 1}.
+     * "We reset indices of slip-springs after the constructions or destructions" so that
+     * they run from 1 to Z; the paper does not say in which order, and
+     * slip-springs are indistinguishable (eq 2), so (reading R21) the
+     * slip-springs are visited from the last to the first and a destroyed one is replaced
+     * by the one that is last at that moment (already visited, hence a survivor). */
     const int64_t Td = oracle_threshold23(fmin(h, 1.0));
-    int Zs = 0;
-    for (int j = 0; j < Z0; ++j) {
+    int Zs = Z0;
+    for (int j = Z0 - 1; j >= 0; --j) {
         int destroyed = 0;
         if (S[j] == 1 || S[j] == N) {
             uint32_t w[4];
             oracle_stream(p->seed, ORACLE_DOM_SLOT, step, chain, (uint32_t)(j >> 1), w);
             destroyed = (int64_t)oracle_code23(w[2 * (j & 1) + 1]) < Td;
         }
-        if (!destroyed) {            /* "reset indices": survivors keep their order */
-            S[Zs] = S[j];
-            for (int c = 0; c < 3; ++c) A[3 * Zs + c] = A[3 * j + c];
-            ++Zs;
+        if (destroyed) {
+            --Zs;
+            S[j] = S[Zs];
+            for (int c = 0; c < 3; ++c) A[3 * j + c] = A[3 * Zs + c];
         }
     }
     /* construction, eqs (50)-(52): K attempts, each end with prob min{h/(N0 K), 1/2} */
@@ -320,7 +326,7 @@ void oracle_step_chain(const oracle_params *p, uint64_t chain, uint64_t step, do
             }
         }
     }
-    for (int j = Zs; j < Z0; ++j) { S[j] = 0; A[3 * j] = A[3 * j + 1] = A[3 * j + 2] = 0.0; }
+    for (int j = Zs; j < oracle_zmax(p); ++j) { S[j] = 0; A[3 * j] = A[3 * j + 1] = A[3 * j + 2] = 0.0; }
     *Zio = Zs;
 }
 

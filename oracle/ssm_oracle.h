@@ -22,8 +22,10 @@ enum {
     ORACLE_DOM_INIT_SLOT = 6,   /* step 0, call j, word 0 -> S_j                          */
     ORACLE_DOM_INIT_ANCHOR = 7  /* step 0, call j: normals 0..2 -> anchor offset          */
 };
-enum { ORACLE_K_EMPTY = 0 /* K = z_max - Z, the paper's GPU scheme P:L370 */,
-       ORACLE_K_ONE = 1   /* K = 1, the paper's CPU scheme P:L370          */ };
+/* k_mode: K of eqs (50),(51), "an integer parameter which can depend on Z":
+ * 0 = K = z_max - Z (the paper's GPU choice); k > 0 = K = min(k, z_max - Z)
+ * (k = 1 is the paper's CPU choice). */
+enum { ORACLE_K_EMPTY = 0, ORACLE_K_ONE = 1 };
 
 typedef struct {
     int32_t  n_beads;      /* N */
