@@ -26,7 +26,11 @@
  *
  * External state layout ("SoA, chain index fastest", used by get/set state):
  *    R[c][i][k]  float32  c = axis 0..2, i = bead 0..N-1, k = chain 0..M-1   -> R[(c*N+i)*M+k]
- *    A[c][j][k]  float32  j = slip-spring slot 0..zmax-1                     -> A[(c*zmax+j)*M+k]
+ *    A[c][j][k]  float32  c = 0..3: x, y, z and the low part of x; j = slip-spring slot 0..zmax-1
+ *                                                                            -> A[(c*zmax+j)*M+k]
+ *                         The anchor's x is A[0] + A[3]: under shear the library advects it as a
+ *                         compensated sum (eq 45 adds the same increment every step, which a plain
+ *                         fp32 sum would round the same way every step).  A[3] = 0 is a valid input.
  *    S[j][k]     uint8    bead index 1..N of slip-spring j, 0 = empty slot   -> S[j*M+k]
  *  The occupied slots of a chain are always the first Z_k ones (the paper's "indices run
  *  from 1 to Z"); zmax = N (the paper's Z <= N).
@@ -53,7 +57,7 @@ typedef struct ssm_ctx ssm_ctx;   /* opaque, host side */
 
 /* Parameters of the model as the paper states them plus bookkeeping. */
 typedef struct {
-    int32_t  n_beads;         /* N: 8, 16, 32, 64 or 128 (4 beads per lane, N/4 lanes per chain)  */
+    int32_t  n_beads;         /* N: 8, 16, 32, 64 or 128 (8 beads per lane, N/8 lanes per chain)  */
     int64_t  n_chains;        /* M >= 1                                                           */
     double   n_s;             /* slip-spring strength N_s (eq 1)                           */
     double   n_0;             /* beads per slip-spring N_0 (eq 10); <= 0 or inf: no slip-  */
@@ -69,6 +73,9 @@ typedef struct {
     int32_t  corr_levels;     /* multi-tau levels (16); averaging factor m = 2 fixed              */
     int32_t  corr_bins;       /* bins per level (16), even, <= 32                                 */
     int32_t  corr_groups;     /* chain groups for the standard error (32); group = chain % groups */
+    int32_t  k_attempts;      /* K of eqs (50), (51), "an integer parameter which can depend on Z"    */
+                              /* (P:L328): 0 = K = N - Z (the paper's GPU choice);           */
+                              /* k > 0 = K = min(k, N - Z) (k = 1 is the paper's CPU choice)         */
 } ssm_params;
 
 /* Bytes of device workspace ssm_init() needs for these parameters (0 on bad parameters). */
@@ -97,7 +104,7 @@ int64_t ssm_stress_count(const ssm_ctx *ctx);
 int ssm_stress(ssm_ctx *ctx, int64_t first_sample, int64_t n_samples, double *h_out);
 
 /* Raw fixed-point sums behind ssm_stress: h_out (host) [n_samples][12] int64, value =
- * sum over local chains of (component + delta_ab) * 2^24 rounded per warp. */
+ * sum over local chains of (component + delta_ab) * 2^18 rounded per lane. */
 int ssm_stress_sums(ssm_ctx *ctx, int64_t first_sample, int64_t n_samples, int64_t *h_out);
 
 /* Device address of those sums for samples [first_sample, first_sample + n_samples): *d_ptr

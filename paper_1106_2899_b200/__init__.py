@@ -24,7 +24,8 @@ class Params(C.Structure):
     _fields_ = [("n_beads", C.c_int32), ("n_chains", C.c_int64), ("n_s", C.c_double), ("n_0", C.c_double),
                 ("zeta_s", C.c_double), ("dt", C.c_double), ("seed", C.c_uint64), ("chain_offset", C.c_uint64),
                 ("stress_every", C.c_int32), ("stress_capacity", C.c_int64), ("sample_every", C.c_int32),
-                ("corr_levels", C.c_int32), ("corr_bins", C.c_int32), ("corr_groups", C.c_int32)]
+                ("corr_levels", C.c_int32), ("corr_bins", C.c_int32), ("corr_groups", C.c_int32),
+                ("k_attempts", C.c_int32)]
 
 
 class SsmError(RuntimeError):
@@ -78,14 +79,14 @@ class Ensemble:
 
     def __init__(self, n_beads, n_chains, n_s=0.5, n_0=4.0, zeta_s=0.1, dt=0.01, seed=1, chain_offset=0,
                  stress_every=0, stress_capacity=0, sample_every=0, corr_levels=16, corr_bins=16,
-                 corr_groups=32, device="cuda:0", stream=None):
+                 corr_groups=32, k_attempts=0, device="cuda:0", stream=None):
         import torch
         if not torch.cuda.is_available():
             raise SsmError(SSM_ECUDA, "no CUDA device: libssm has no CPU fallback")
         self._torch = torch
         self.device = torch.device(device)
         self.p = Params(n_beads, n_chains, n_s, n_0, zeta_s, dt, seed, chain_offset, stress_every,
-                        stress_capacity, sample_every, corr_levels, corr_bins, corr_groups)
+                        stress_capacity, sample_every, corr_levels, corr_bins, corr_groups, k_attempts)
         self.N, self.M = n_beads, n_chains
         L = lib()
         nbytes = L.ssm_workspace_bytes(C.byref(self.p))
@@ -157,11 +158,11 @@ class Ensemble:
         return s, c
 
     def get_state(self, R=None, A=None, S=None):
-        """External SoA layout: R[3][N][M], A[3][N][M] float32, S[N][M] uint8.  Host numpy
+        """External SoA layout: R[3][N][M], A[4][N][M] float32 (x, y, z, low part of x), S[N][M] uint8.  Host numpy
         arrays by default; pass CUDA tensors (all three) to stay on the device."""
         step = C.c_int64()
         if R is None:
-            R = np.zeros((3, self.N, self.M), dtype=np.float32); A = np.zeros((3, self.N, self.M), dtype=np.float32)
+            R = np.zeros((3, self.N, self.M), dtype=np.float32); A = np.zeros((4, self.N, self.M), dtype=np.float32)
             S = np.zeros((self.N, self.M), dtype=np.uint8)
             self._ck(lib().ssm_get_state(self.h, C.c_void_p(R.ctypes.data), C.c_void_p(A.ctypes.data),
                                          C.c_void_p(S.ctypes.data), C.byref(step), 0))
@@ -178,7 +179,7 @@ class Ensemble:
         if isinstance(R, np.ndarray):
             assert R.dtype == np.float32 and A.dtype == np.float32 and S.dtype == np.uint8
             assert R.flags.c_contiguous and A.flags.c_contiguous and S.flags.c_contiguous
-            assert R.shape == (3, self.N, self.M) and A.shape == (3, self.N, self.M) and S.shape == (self.N, self.M)
+            assert R.shape == (3, self.N, self.M) and A.shape == (4, self.N, self.M) and S.shape == (self.N, self.M)
             self._ck(lib().ssm_set_state(self.h, C.c_void_p(R.ctypes.data), C.c_void_p(A.ctypes.data),
                                          C.c_void_p(S.ctypes.data), global_step, 0))
         else:

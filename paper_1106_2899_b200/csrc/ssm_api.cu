@@ -12,6 +12,7 @@
 
 #include "../../include/ssm.h"
 #include "ssm_common.h"
+#include "ssm_rng.cuh"
 
 namespace ssm {
 cudaError_t step_occupancy(int n_beads, int *blocks_per_sm);
@@ -72,6 +73,7 @@ static bool check_params(const ssm_params *p, std::string &why)
     if (!(p->dt > 0.0) || !(p->dt < 1.0 / 6.0)) { why = "dt must be in (0, 1/6): the Euler map needs 12 dt < 2"; return false; }
     if (!(p->n_s > 0.0)) { why = "n_s must be > 0"; return false; }
     if (!(p->zeta_s > 0.0)) { why = "zeta_s must be > 0"; return false; }
+    if (p->k_attempts < 0) { why = "k_attempts must be >= 0"; return false; }
     if (p->stress_every < 0 || p->sample_every < 0 || p->stress_capacity < 0) { why = "negative sampling parameter"; return false; }
     if (p->stress_every > 0 && p->stress_capacity < 1) { why = "stress_capacity must be >= 1 when stress_every > 0"; return false; }
     if (p->sample_every > 0) {
@@ -85,7 +87,7 @@ static bool check_params(const ssm_params *p, std::string &why)
 static Layout make_layout(const ssm_params *p)
 {
     Layout L{};
-    const int cpw = 128 / p->n_beads;
+    const int cpw = chains_per_warp(p->n_beads);
     L.n_tiles = (p->n_chains + cpw - 1) / cpw;
     size_t o = 0;
     L.state = o; o = align_up(o + (size_t)L.n_tiles * kTileBytes, 256);
@@ -99,7 +101,7 @@ static Layout make_layout(const ssm_params *p)
     L.csum = o; if (corr) o = align_up(o + (size_t)p->corr_groups * p->corr_levels * p->corr_bins * 8, 256);
     // staging for host-pointer get/set state and chain stress: chunks of <= 65536 chains
     L.stage_chains = p->n_chains < 65536 ? p->n_chains : 65536;
-    L.stage = o; o = align_up(o + (size_t)L.stage_chains * (size_t)(25 * p->n_beads > 48 ? 25 * p->n_beads : 48), 256);
+    L.stage = o; o = align_up(o + (size_t)L.stage_chains * (size_t)(29 * p->n_beads > 48 ? 29 * p->n_beads : 48), 256);
     L.total = o;
     return L;
 }
@@ -175,16 +177,17 @@ extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, s
     std::memset(&sp, 0, sizeof sp);
     sp.state = c->ws + lay.state;
     sp.n_chains = p->n_chains; sp.chain_offset = p->chain_offset; sp.n_tiles = (int)lay.n_tiles;
-    sp.stress_every = p->stress_every; sp.sample_every = p->sample_every;
-    sp.key0 = (unsigned)(p->seed & 0xFFFFFFFFull); sp.key1 = (unsigned)(p->seed >> 32);
+    philox_round_keys((unsigned)(p->seed & 0xFFFFFFFFull), (unsigned)(p->seed >> 32), sp.rk);
     sp.springs_on = c->springs_on ? 1 : 0;
+    sp.k_attempts = p->k_attempts;
     sp.dt3 = (float)(3.0 * p->dt);
-    sp.sq2dt = (float)std::sqrt(2.0 * p->dt);
+    const double m2ln2 = -2.0 * 0.6931471805599453;        // r^2 = -2 ln u = (-2 ln 2) log2 u
+    sp.bm_noise = (float)(m2ln2 * 2.0 * p->dt);
+    sp.bm_anchor = (float)(m2ln2 * p->n_s / 3.0);
     sp.fx_scale = (float)(p->dt * (3.0 / p->n_s) * (double)(1 << kFxShift));
     sp.q2l = (float)(2.0 * (3.0 / (4.0 * p->n_s)) * 1.4426950408889634);
     sp.h2 = (float)(2.0 * h);
     sp.cs = (float)(3.0 / p->n_s);
-    sp.sq_ns3 = (float)std::sqrt(p->n_s / 3.0);
     sp.t_destroy = threshold23(std::fmin(h, 1.0));
     for (int K = 1; K <= 128; ++K) {
         const double pc = c->springs_on ? std::fmin(h / (p->n_0 * (double)K), 0.5) : 0.0;
@@ -194,10 +197,10 @@ extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, s
     InitParams ip;
     std::memset(&ip, 0, sizeof ip);
     ip.state = c->ws + lay.state;
-    ip.n_chains_padded = lay.n_tiles * (128 / p->n_beads);
-    ip.chain_offset = p->chain_offset; ip.key0 = sp.key0; ip.key1 = sp.key1;
+    ip.n_chains_padded = lay.n_tiles * chains_per_warp(p->n_beads);
+    ip.chain_offset = p->chain_offset; std::memcpy(ip.rk, sp.rk, sizeof ip.rk);
     ip.n_beads = p->n_beads; ip.springs_on = sp.springs_on;
-    ip.sq13 = (float)std::sqrt(1.0 / 3.0); ip.sq_ns3 = sp.sq_ns3;
+    ip.bm_bond = (float)(m2ln2 / 3.0); ip.bm_anchor = sp.bm_anchor;
     if (c->springs_on) {       // Poisson(N/N0) CDF (eq 12) as integer thresholds
         const double lam = (double)p->n_beads / p->n_0;
         double pmf = std::exp(-lam), cdf = 0.0;
@@ -251,6 +254,12 @@ extern "C" int ssm_step(ssm_ctx *c, int64_t n_steps, double shear_rate)
         long long nrec = 0, nsmp = 0;
         if (p.stress_every > 0) nrec = (c->step + T) / p.stress_every - c->step / p.stress_every;
         if (p.sample_every > 0) nsmp = (c->step + T) / p.sample_every - c->step / p.sample_every;
+        sp.rec_mask = 0u; sp.smp_mask = 0u;
+        for (int n = 0; n < T; ++n) {
+            if (p.stress_every > 0 && (c->step + n + 1) % p.stress_every == 0) sp.rec_mask |= 1u << n;
+            if (p.sample_every > 0 && (c->step + n + 1) % p.sample_every == 0) sp.smp_mask |= 1u << n;
+        }
+        sp.n_rec = (int)nrec;
         sp.stress = reinterpret_cast<long long *>(c->ws + c->lay.stress) + c->n_records * 12;
         sp.samples = nsmp > 0 ? reinterpret_cast<float2 *>(c->ws + c->lay.samples) : nullptr;
         CK(c, launch_step(p.n_beads, sp, c->grid, c->st));
@@ -349,18 +358,18 @@ static int xfer_state(ssm_ctx *c, bool do_export, float *R, float *A, uint8_t *S
     const long long chunk = c->lay.stage_chains;
     float *dR = reinterpret_cast<float *>(c->ws + c->lay.stage);
     float *dA = dR + (size_t)3 * N * chunk;
-    unsigned char *dS = reinterpret_cast<unsigned char *>(dA + (size_t)3 * N * chunk);
+    unsigned char *dS = reinterpret_cast<unsigned char *>(dA + (size_t)4 * N * chunk);
     for (long long k0 = 0; k0 < M; k0 += chunk) {
         const long long nk = M - k0 < chunk ? M - k0 : chunk;
         if (do_export) {
             CK(c, launch_xfer(true, state, dR, dA, dS, N, k0, nk, chunk, c->st));
             CK(c, cudaMemcpy2DAsync(R + k0, (size_t)M * 4, dR, (size_t)chunk * 4, (size_t)nk * 4, (size_t)3 * N, cudaMemcpyDeviceToHost, c->st));
-            CK(c, cudaMemcpy2DAsync(A + k0, (size_t)M * 4, dA, (size_t)chunk * 4, (size_t)nk * 4, (size_t)3 * N, cudaMemcpyDeviceToHost, c->st));
+            CK(c, cudaMemcpy2DAsync(A + k0, (size_t)M * 4, dA, (size_t)chunk * 4, (size_t)nk * 4, (size_t)4 * N, cudaMemcpyDeviceToHost, c->st));
             CK(c, cudaMemcpy2DAsync(S + k0, (size_t)M, dS, (size_t)chunk, (size_t)nk, (size_t)N, cudaMemcpyDeviceToHost, c->st));
             c->launches += 1;
         } else {
             CK(c, cudaMemcpy2DAsync(dR, (size_t)chunk * 4, R + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)3 * N, cudaMemcpyHostToDevice, c->st));
-            CK(c, cudaMemcpy2DAsync(dA, (size_t)chunk * 4, A + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)3 * N, cudaMemcpyHostToDevice, c->st));
+            CK(c, cudaMemcpy2DAsync(dA, (size_t)chunk * 4, A + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)4 * N, cudaMemcpyHostToDevice, c->st));
             CK(c, cudaMemcpy2DAsync(dS, (size_t)chunk, S + k0, (size_t)M, (size_t)nk, (size_t)N, cudaMemcpyHostToDevice, c->st));
             CK(c, launch_xfer(false, state, dR, dA, dS, N, k0, nk, chunk, c->st));
             c->launches += 2;

@@ -21,15 +21,15 @@ __global__ void __launch_bounds__(128) ssm_init_kernel(const __grid_constant__ I
     if (k >= P.n_chains_padded) return;
     const int N = P.n_beads, zmax = N;
     const uint32_t chain = (uint32_t)(P.chain_offset + (unsigned long long)k);
-    const StreamKey sk = make_stream(P.key0, P.key1, 0ull);
+    const StreamKey sk = make_stream(0ull);
     unsigned char *st = P.state;
 
     float R[128 * 3];
     R[0] = R[1] = R[2] = 0.0f;
     float z4[4] = {0.f, 0.f, 0.f, 0.f};
     for (int m = 0; m < 3 * (N - 1); ++m) {               // normal m = 3*bond + axis
-        if ((m & 3) == 0) normal_call(sk, DOM_INIT_BOND, chain, (uint32_t)(m >> 2), z4);
-        R[m + 3] = fmaf(P.sq13, z4[m & 3], R[m]);
+        if ((m & 3) == 0) normal_call(sk, P.rk, DOM_INIT_BOND, chain, (uint32_t)(m >> 2), P.bm_bond, z4);
+        R[m + 3] = R[m] + z4[m & 3];
     }
     for (int i = 0; i < N; ++i)
         for (int c = 0; c < 3; ++c) *reinterpret_cast<float *>(st + off_R(k, N, i, c)) = R[3 * i + c];
@@ -37,22 +37,22 @@ __global__ void __launch_bounds__(128) ssm_init_kernel(const __grid_constant__ I
     int Z = 0;
     if (P.springs_on) {
         uint32_t w[4];
-        stream_call(sk, DOM_INIT_Z, chain, 0u, w);
+        stream_call(sk, P.rk, DOM_INIT_Z, chain, 0u, w);
         const uint32_t code = code23(w[0]);
         while (Z < zmax && code >= P.t_cdf[Z]) ++Z;
     }
     *reinterpret_cast<int *>(st + off_Z(k, N)) = Z;
     for (int j = 0; j < zmax; ++j) {
-        int s = 0; float a[3] = {0.f, 0.f, 0.f};
+        int s = 0; float a[4] = {0.f, 0.f, 0.f, 0.f};
         if (j < Z) {
             uint32_t w[4];
-            stream_call(sk, DOM_INIT_SLOT, chain, (uint32_t)j, w);
+            stream_call(sk, P.rk, DOM_INIT_SLOT, chain, (uint32_t)j, w);
             s = 1 + (int)__umulhi(w[0], (uint32_t)N);
-            normal_call(sk, DOM_INIT_ANCHOR, chain, (uint32_t)j, z4);
-            for (int c = 0; c < 3; ++c) a[c] = fmaf(P.sq_ns3, z4[c], R[3 * (s - 1) + c]);
+            normal_call(sk, P.rk, DOM_INIT_ANCHOR, chain, (uint32_t)j, P.bm_anchor, z4);
+            for (int c = 0; c < 3; ++c) a[c] = R[3 * (s - 1) + c] + z4[c];
         }
         st[off_S(k, N, j)] = (unsigned char)s;
-        for (int c = 0; c < 3; ++c) *reinterpret_cast<float *>(st + off_A(k, N, j, c)) = a[c];
+        for (int c = 0; c < 4; ++c) *reinterpret_cast<float *>(st + off_A(k, N, j, c)) = a[c];
     }
 }
 
@@ -66,8 +66,8 @@ cudaError_t launch_init(const InitParams &p, cudaStream_t st)
 
 // ---------------------------------------------------------------------------------------
 // State export / import between the tiled image and the external SoA layout of ssm.h.
-// rows 0..3N-1 of R, then 3N rows of A, then N rows of S; chains [k0, k0+nk), external
-// element (row, k) at row*pitch + (k - k0).
+// rows 0..3N-1 of R, then 4N rows of A (x, y, z, low part of x), then N rows of S; chains
+// [k0, k0+nk), external element (row, k) at row*pitch + (k - k0).
 // ---------------------------------------------------------------------------------------
 template <bool EXPORT>
 __global__ void __launch_bounds__(256) ssm_xfer_kernel(unsigned char *state, float *R, float *A, unsigned char *S,
@@ -76,17 +76,17 @@ __global__ void __launch_bounds__(256) ssm_xfer_kernel(unsigned char *state, flo
     const long long kk = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (kk >= nk) return;
     const long long k = k0 + kk;
-    const int row = blockIdx.y;                         // 0 .. 7N-1
+    const int row = blockIdx.y;                         // 0 .. 8N-1
     if (row < 3 * N) {
         const int c = row / N, i = row % N;
         float *p = reinterpret_cast<float *>(state + off_R(k, N, i, c));
         if (EXPORT) R[(long long)row * pitch + kk] = *p; else *p = R[(long long)row * pitch + kk];
-    } else if (row < 6 * N) {
+    } else if (row < 7 * N) {
         const int rr = row - 3 * N, c = rr / N, j = rr % N;
         float *p = reinterpret_cast<float *>(state + off_A(k, N, j, c));
         if (EXPORT) A[(long long)rr * pitch + kk] = *p; else *p = A[(long long)rr * pitch + kk];
     } else {
-        const int j = row - 6 * N;
+        const int j = row - 7 * N;
         unsigned char *p = state + off_S(k, N, j);
         if (EXPORT) S[(long long)j * pitch + kk] = *p; else *p = S[(long long)j * pitch + kk];
     }
@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(256) ssm_count_z_kernel(unsigned char *state, 
 cudaError_t launch_xfer(bool do_export, unsigned char *state, float *R, float *A, unsigned char *S, int N,
                         long long k0, long long nk, long long pitch, cudaStream_t st)
 {
-    dim3 grid((unsigned)((nk + 255) / 256), (unsigned)(7 * N));
+    dim3 grid((unsigned)((nk + 255) / 256), (unsigned)(8 * N));
     if (do_export) ssm_xfer_kernel<true><<<grid, 256, 0, st>>>(state, R, A, S, N, k0, nk, pitch);
     else {
         ssm_xfer_kernel<false><<<grid, 256, 0, st>>>(state, R, A, S, N, k0, nk, pitch);

@@ -1,40 +1,50 @@
 // ssm_common.h -- internal layout and launch-parameter structs of libssm (host + device).
 //
-// Mapping: a chain of N = 4G beads is owned by G consecutive lanes of
-// one warp (G = 2, 4, 8, 16, 32), 4 consecutive beads per lane, so a warp owns CPW = 32/G
-// chains and never talks to another warp.  The unit of state in HBM is therefore the
-// "warp tile": the register / shared-memory image of one warp's chains, stored so that a
-// warp loads and stores it with fully coalesced 16-byte accesses:
+// Mapping: a chain of N = 8G beads is owned by G consecutive lanes of
+// one warp (G = 1, 2, 4, 8, 16), 8 consecutive beads per lane, so a warp owns CPW = 32/G
+// = 256/N chains (256 beads, up to 256 slip-spring slots) and never talks to another warp.
+// The unit of state in HBM is the "warp tile": the register / shared-memory image of one
+// warp's chains, laid out so that a warp loads and stores it with coalesced 16-byte accesses:
 //
-//   bytes [   0,1536)  R image : 3 x float4 per lane, element [v][lane], float f = 4v+e of
+//   bytes [   0,3072)  R image : 6 x float4 per lane, element [v][lane]; float f = 4v+e of a
 //                                lane = coordinate (f%3) of the lane's bead f/3
-//   bytes [1536,3072)  A image : [chain in warp][slot 0..zmax-1][3] float   (zmax = N)
-//   bytes [3072,3200)  S image : [chain in warp][slot] uint8, 0 = empty, 1..N
-//   bytes [3200,3264)  Z       : [chain in warp] int32 (16 entries, CPW used)
-//   bytes [3264,3328)  pad
+//   bytes [3072,7168)  A image : [chain in warp][slot 0..N-1] float4 = (A_x, A_y, A_z, A_x low part);
+//                                A_x + low part is the anchor's x, kept as a compensated sum so
+//                                that the affine advection of eq (45) does not drift in fp32
+//   bytes [7168,7424)  S image : [chain in warp][slot] uint8, 0 = empty, 1..N
+//   bytes [7424,7552)  Z       : [chain in warp] int32 (32 entries, CPW used)
 #pragma once
 #include <cstdint>
 
 namespace ssm {
 
-constexpr int kTileBytes = 3328;
-constexpr int kTileR = 0, kTileA = 1536, kTileS = 3072, kTileZ = 3200;
+constexpr int kBPL = 8;                      // beads per lane
+constexpr int kTileBytes = 7552;
+constexpr int kTileR = 0, kTileA = 3072, kTileS = 7168, kTileZ = 7424;
 constexpr int kWarpsPerBlock = 8;
 constexpr int kBlockThreads = 32 * kWarpsPerBlock;
 constexpr int kMaxFuse = 32;                 // time steps fused per launch (stress accumulators in smem)
 constexpr int kFxShift = 26;                 // slip-spring displacement fixed point: 2^-26 b
-constexpr int kStressShift = 24;             // ensemble stress fixed point: 2^-24 kT
+constexpr int kStressShift = 18;             // ensemble stress fixed point: 2^-18 kT per lane share
+constexpr int kSampleShift = 20;             // per-chain slip-spring virial (correlator samples): 2^-20
 
-// per-warp shared memory of the step kernel
-constexpr int kSmRm = 0;        // float[384]  bead positions mirror [chain][bead][3]
-constexpr int kSmFx = 1536;     // int  [384]  fixed-point slip-spring displacement per bead coordinate
-constexpr int kSmA = 3072;      // float[384]  anchors [chain][slot][3]
-constexpr int kSmS = 4608;      // uint8[128]  bead index per slot
-constexpr int kSmZ = 4736;      // int  [16]   Z per chain
-constexpr int kSmAtt = 4800;    // uint8[128]  result of construction attempt k (0, 1 or N)
-constexpr int kSmWarp = 4928;
-constexpr int kSmAcc = kWarpsPerBlock * kSmWarp;                          // int64 [8][kMaxFuse][12]
-constexpr int kSmStep = kSmAcc + kWarpsPerBlock * kMaxFuse * 12 * 8;      // 63,744 B + 0
+// per-warp shared memory of the step kernel.  Two arrays are padded so that the bead lanes'
+// 16-byte accesses (one per lane, consecutive lanes) fall into distinct banks:
+//   bead b of the warp (0..255) sits at float4 index  b + (b >> 3)      (9 float4 per lane)
+//   its coordinate c at int index  (b >> 3) * 28 + (b & 7) * 3 + c      (28 ints per lane)
+constexpr int kSmRm = 0;         // float4[288] bead positions mirror (x, y, z, -), padded
+constexpr int kSmA = 4608;       // float4[256] anchors [chain][slot] (x, y, z, x low part)
+constexpr int kSmFx = 8704;      // int  [896]  fixed-point slip-spring displacement per bead coordinate, padded
+constexpr int kSmS = 12288;      // uint8[256]  bead index per slot (0xFF = destroyed in this step)
+constexpr int kSmZ = 12544;      // int  [32]   Z per chain
+constexpr int kSmX = 12672;      // int  [33]   exclusive prefix of Z over the warp's chains (+ total), padded to 36
+constexpr int kSmEv = 12816;     // uint [64]   creation masks: created at bead 1 / at bead N, [2][chain][word]
+constexpr int kSmSamp = 13072;   // int  [32]   per-chain fixed-point sum of d_x d_y over slip-springs (sample steps)
+constexpr int kSmWarp = 13200;
+constexpr int kSmAcc = kWarpsPerBlock * kSmWarp;                          // int64 [kMaxFuse][12] per CTA
+constexpr int kSmStep = kSmAcc + kMaxFuse * 12 * 8;                       // 108,672 B: 2 CTAs per SM
+__host__ __device__ constexpr int rm_index(int bead_in_warp) { return bead_in_warp + (bead_in_warp >> 3); }
+__host__ __device__ constexpr int fx_index(int bead_in_warp) { return (bead_in_warp >> 3) * 28 + (bead_in_warp & 7) * 3; }
 
 struct StepParams {
     unsigned char *state;             // warp tiles
@@ -45,18 +55,20 @@ struct StepParams {
     unsigned long long step0;         // global index of the first step of this launch
     int            n_tiles;
     int            n_fuse;            // steps in this launch (<= kMaxFuse)
-    int            stress_every;      // 0 = never
-    int            sample_every;      // 0 = never
-    unsigned       key0, key1;        // Philox key
+    unsigned       rec_mask;          // bit n: the ensemble stress is recorded after step n of this launch
+    unsigned       smp_mask;          // bit n: the correlator is fed after step n of this launch
+    int            n_rec;             // popcount(rec_mask)
     int            springs_on;
+    int            k_attempts;        // 0: K = N - Z (GPU); k > 0: K = min(k, N - Z)
+    unsigned rk[20];  // Philox round keys: (k0 + r W0, k1 + r W1), r = 0..9
     float dt3;        // 3 dt                 (Rouse spring constant 3kT/b^2, eq 1)
-    float sq2dt;      // sqrt(2 dt)           (eq 44)
+    float bm_noise;   // -2 ln2 * 2 dt: r^2 = bm * log2(u) gives sqrt(2 dt) * N(0,1)  (eqs 44, 46, 47)
+    float bm_anchor;  // -2 ln2 * N_s/3: anchor offsets of new slip-springs (eq 52)
     float gdt;        // shear_rate * dt      (eq 44, 45 with kappa_xy of eq 60)
     float fx_scale;   // dt * (3/N_s) * 2^kFxShift
     float q2l;        // 2 * (3/(4 N_s)) * log2(e): exponent scale of 1 - tanh(x) = 2/(1+e^{2x})
     float h2;         // 2 dt/zeta_s
     float cs;         // 3/N_s                (eq 76)
-    float sq_ns3;     // sqrt(N_s/3)          (eq 52)
     unsigned t_destroy;               // T(min{dt/zeta_s, 1})                 (eq 53)
     unsigned t_c1[129], t_c2[129];    // T(p_c(K)), T(2 p_c(K)), K = 1..128   (eqs 50, 51)
 };
@@ -65,11 +77,11 @@ struct InitParams {
     unsigned char *state;
     long long      n_chains_padded;   // n_tiles * CPW
     unsigned long long chain_offset;
-    unsigned       key0, key1;
+    unsigned       rk[20];            // Philox round keys
     int            n_beads;
     int            springs_on;
-    float          sq13;              // sqrt(1/3)   (eq 6)
-    float          sq_ns3;            // sqrt(N_s/3) (eq 15)
+    float          bm_bond;           // -2 ln2 / 3:     bond components N(0, 1/3)    (eq 6)
+    float          bm_anchor;         // -2 ln2 N_s / 3: anchor offsets N(0, N_s/3)  (eq 15)
     unsigned       t_cdf[128];        // T(P(Z <= z)), z = 0..zmax-1  (eq 12)
 };
 
@@ -86,27 +98,27 @@ struct CorrParams {
 };
 
 // address of bead coordinate / slot entry inside the tiled state (host and device)
-__host__ __device__ inline long long tile_of(long long chain, int n_beads) { return chain / (128 / n_beads); }
+__host__ __device__ inline int chains_per_warp(int n_beads) { return 256 / n_beads; }
 __host__ __device__ inline long long off_R(long long chain, int n_beads, int bead, int c)
 {
-    const int G = n_beads / 4, cpw = 32 / G;
+    const int G = n_beads / kBPL, cpw = 32 / G;
     const long long tile = chain / cpw; const int cw = (int)(chain % cpw);
-    const int lane = cw * G + bead / 4, f = (bead % 4) * 3 + c;
+    const int lane = cw * G + bead / kBPL, f = (bead % kBPL) * 3 + c;
     return tile * kTileBytes + kTileR + (((f >> 2) * 32 + lane) * 4 + (f & 3)) * 4;
 }
-__host__ __device__ inline long long off_A(long long chain, int n_beads, int slot, int c)
+__host__ __device__ inline long long off_A(long long chain, int n_beads, int slot, int c /* 0..3 */)
 {
-    const int cpw = 128 / n_beads;
-    return (chain / cpw) * kTileBytes + kTileA + (((int)(chain % cpw) * n_beads + slot) * 3 + c) * 4;
+    const int cpw = 256 / n_beads;
+    return (chain / cpw) * kTileBytes + kTileA + (((int)(chain % cpw) * n_beads + slot) * 4 + c) * 4;
 }
 __host__ __device__ inline long long off_S(long long chain, int n_beads, int slot)
 {
-    const int cpw = 128 / n_beads;
+    const int cpw = 256 / n_beads;
     return (chain / cpw) * kTileBytes + kTileS + (int)(chain % cpw) * n_beads + slot;
 }
 __host__ __device__ inline long long off_Z(long long chain, int n_beads)
 {
-    const int cpw = 128 / n_beads;
+    const int cpw = 256 / n_beads;
     return (chain / cpw) * kTileBytes + kTileZ + (int)(chain % cpw) * 4;
 }
 

@@ -24,37 +24,45 @@ enum : uint32_t {
 
 // Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11): ten rounds of
 //   (c0,c1,c2,c3) <- (hi(M1*c2)^c1^k0, lo(M1*c2), hi(M0*c0)^c3^k1, lo(M0*c0)),
-// the key bumped by the Weyl constants between rounds.
-__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
-                                              uint32_t k0, uint32_t k1, uint32_t (&out)[4])
+// the key bumped by the Weyl constants between rounds.  RK holds the 20 round keys
+// (k0 + r W0, k1 + r W1): the host computes them once so that the kernel reads them from
+// the constant bank instead of spending 20 additions per call.
+struct RoundKeys { const unsigned *rk; };
+
+__host__ __device__ inline void philox_round_keys(uint32_t k0, uint32_t k1, unsigned (&rk)[20])
 {
-    constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+    for (int r = 0; r < 10; ++r) { rk[2 * r] = k0 + (uint32_t)r * 0x9E3779B9u; rk[2 * r + 1] = k1 + (uint32_t)r * 0xBB67AE85u; }
+}
+
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              const unsigned (&rk)[20], uint32_t (&out)[4])
+{
+    constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
         const uint64_t p0 = (uint64_t)M0 * c0;
         const uint64_t p1 = (uint64_t)M1 * c2;
-        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ (k0 + (uint32_t)r * W0);
-        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ (k1 + (uint32_t)r * W1);
-        c1 = (uint32_t)p1; c3 = (uint32_t)p0; c0 = n0; c2 = n2;
+        c0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk[2 * r];
+        c2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk[2 * r + 1];
+        c1 = (uint32_t)p1; c3 = (uint32_t)p0;
     }
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
 // counter = (step low 32, domain<<28 | step bits 32..59, global chain index, item)
 struct StreamKey {
-    uint32_t k0, k1;        // seed low / high
     uint32_t c0, c1hi;      // step low 32 bits, step bits 32..59
 };
-__device__ __forceinline__ StreamKey make_stream(uint32_t k0, uint32_t k1, unsigned long long step)
+__device__ __forceinline__ StreamKey make_stream(unsigned long long step)
 {
-    StreamKey s; s.k0 = k0; s.k1 = k1; s.c0 = (uint32_t)step;
+    StreamKey s; s.c0 = (uint32_t)step;
     s.c1hi = (uint32_t)(step >> 32) & 0x0FFFFFFFu;
     return s;
 }
-__device__ __forceinline__ void stream_call(const StreamKey& s, uint32_t domain, uint32_t chain,
-                                            uint32_t item, uint32_t (&w)[4])
+__device__ __forceinline__ void stream_call(const StreamKey& s, const unsigned (&rk)[20], uint32_t domain,
+                                            uint32_t chain, uint32_t item, uint32_t (&w)[4])
 {
-    philox4x32_10(s.c0, (domain << 28) | s.c1hi, chain, item, s.k0, s.k1, w);
+    philox4x32_10(s.c0, (domain << 28) | s.c1hi, chain, item, rk, w);
 }
 
 // 23-bit code k = w >> 9 and the uniform u = (k + 1/2) 2^-23 in (0,1); exact in fp32:
@@ -65,27 +73,35 @@ __device__ __forceinline__ float u23(uint32_t w)
     return __uint_as_float(0x3F800000u | (w >> 9)) - 0.99999994f;
 }
 
-// Box-Muller: r = sqrt(-2 ln u_a), theta = 2 pi (u_b - 1/2) = pi t with
-// t = 2 u_b - 1 = (2k+1) 2^-23 - 1 formed exactly; (z0, z1) = (r cos theta, r sin theta).
-__device__ __forceinline__ void box_muller(uint32_t wa, uint32_t wb, float& z0, float& z1)
+__device__ __forceinline__ float mufu_sqrt(float x)
+{
+    float y;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// Box-Muller: r = sigma sqrt(-2 ln u_a), theta = 2 pi (u_b - 1/2);
+// (z0, z1) = (r cos theta, r sin theta) are two N(0, sigma^2) numbers.
+// bm = -2 ln2 sigma^2, so that r^2 = bm log2(u_a).  The special-function unit evaluates
+// log2, sqrt, sin and cos (absolute error <= 2^-21.4 each in the ranges used here, DESIGN.md
+// section 8.2); theta = 2 pi x + pi 2^-23 with x = k 2^-23 - 1/2 formed exactly.
+__device__ __forceinline__ void box_muller(uint32_t wa, uint32_t wb, float bm, float& z0, float& z1)
 {
     const float ua = u23(wa);
-    const float x = __uint_as_float(0x3F800000u | (wb >> 9)) - 1.5f;   // k 2^-23 - 1/2, exact
-    const float t = fmaf(2.0f, x, 1.1920929e-07f);                     // + 2^-23, exact
-    const float r = sqrtf(-2.0f * logf(ua));
-    float sn, cs;
-    sincospif(t, &sn, &cs);
-    z0 = r * cs; z1 = r * sn;
+    const float x = __uint_as_float(0x3F800000u | (wb >> 9)) - 1.5f;          // k 2^-23 - 1/2, exact
+    const float th = fmaf(6.283185307179586f, x, 3.7450704e-07f);             // + pi 2^-23
+    const float r = mufu_sqrt(bm * __log2f(ua));
+    z0 = r * __cosf(th); z1 = r * __sinf(th);
 }
 
 // the four normals of one call: (0,1) from words (0,1), (2,3) from words (2,3)
-__device__ __forceinline__ void normal_call(const StreamKey& s, uint32_t domain, uint32_t chain,
-                                            uint32_t call, float (&z)[4])
+__device__ __forceinline__ void normal_call(const StreamKey& s, const unsigned (&rk)[20], uint32_t domain,
+                                            uint32_t chain, uint32_t call, float bm, float (&z)[4])
 {
     uint32_t w[4];
-    stream_call(s, domain, chain, call, w);
-    box_muller(w[0], w[1], z[0], z[1]);
-    box_muller(w[2], w[3], z[2], z[3]);
+    stream_call(s, rk, domain, chain, call, w);
+    box_muller(w[0], w[1], bm, z[0], z[1]);
+    box_muller(w[2], w[3], bm, z[2], z[3]);
 }
 
 }  // namespace ssm

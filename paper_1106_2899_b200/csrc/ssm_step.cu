@@ -2,13 +2,14 @@
 //
 // One launch advances every chain n_fuse time steps through the three substeps of
 // PAPER.md lines 292-347 (section 3.1) with the chain state resident on chip:
-//   bead phase  (all lanes, 4 beads each): noise w_i (eqs 46, 47), Rouse bond force and
+//   bead phase  (every lane, 8 beads each): noise w_i (eqs 46, 47), Rouse bond force and
 //               slip-spring force (eq 1), explicit Euler (eq 44), bond virial (eq 16);
-//   slot phase  (lanes own slip-spring pairs): anchor advection (eq 45), Glauber hop
-//               (eqs 23, 24, 48, 49), construction / destruction at the ends (eqs 50-53),
+//   slot phase  (the warp's slip-springs, dealt one per lane over all its chains): anchor
+//               advection (eq 45), Glauber hop (eqs 23, 24, 48, 49), destruction (eq 53),
 //               virtual stress (eq 76) and the force scatter for the next step;
-//   reduction   per recorded step, a fixed-tree warp sum of the 12 stress components into
-//               warp-private int64 fixed-point accumulators (eq 54), flushed once per CTA.
+//               construction attempts (eqs 50-52) are drawn by the chain's bead lanes;
+//   reduction   per recorded step, one warp-wide integer add (redux) per stress component
+//               into CTA-wide int64 fixed-point accumulators (eq 54), flushed once per CTA.
 // Mapping and layouts: ssm_common.h and DESIGN.md section 6.
 #include <cuda_runtime.h>
 
@@ -18,349 +19,404 @@
 namespace ssm {
 
 template <int G> struct Log2;
+template <> struct Log2<1> { static constexpr int v = 0; };
 template <> struct Log2<2> { static constexpr int v = 1; };
 template <> struct Log2<4> { static constexpr int v = 2; };
 template <> struct Log2<8> { static constexpr int v = 3; };
 template <> struct Log2<16> { static constexpr int v = 4; };
-template <> struct Log2<32> { static constexpr int v = 5; };
 
-// Sum 12 per-lane values over the warp with a fixed tree (recursive halving): on return
-// lane L holds in v[0] the warp total of component L>>1 (components 12..15 are padding).
-__device__ __forceinline__ void warp_reduce_scatter16(float (&v)[16], int lane)
+__device__ __forceinline__ float mufu_ex2(float x)
 {
-#pragma unroll
-    for (int h = 8; h >= 1; h >>= 1) {
-        const bool up = (lane & (2 * h)) != 0;
-#pragma unroll
-        for (int i = 0; i < h; ++i) {
-            const float send = up ? v[i] : v[i + h];
-            const float keep = up ? v[i + h] : v[i];
-            v[i] = keep + __shfl_xor_sync(0xffffffffu, send, 2 * h);
-        }
-    }
-    v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
 }
 
+constexpr unsigned kFull = 0xffffffffu;
+constexpr int kEvStride = 32;     // words per event-mask type
+
 template <int G>
-__global__ void __launch_bounds__(kBlockThreads, 3) ssm_step_kernel(const __grid_constant__ StepParams P)
+__global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid_constant__ StepParams P)
 {
-    constexpr int N = 4 * G, ZMAX = N, CPW = 32 / G;
-    constexpr unsigned GMASK = (G == 32) ? 0xffffffffu : ((1u << G) - 1u);
+    constexpr int N = kBPL * G, CPW = 32 / G, LG = Log2<G>::v, LN = LG + 3, WPC = (N + 31) / 32;
     extern __shared__ __align__(16) unsigned char smem[];
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int l = lane & (G - 1), cw = lane >> Log2<G>::v, lane0 = lane - l;
+    const int l = lane & (G - 1), cw = lane >> LG;
     unsigned char *wb = smem + warp * kSmWarp;
-    float *Rl = reinterpret_cast<float *>(wb + kSmRm) + lane * 12;     // this lane's 4 beads
-    int *Fl = reinterpret_cast<int *>(wb + kSmFx) + lane * 12;
-    float *Rc = reinterpret_cast<float *>(wb + kSmRm) + lane0 * 12;    // this lane's chain
-    int *Fc = reinterpret_cast<int *>(wb + kSmFx) + lane0 * 12;
-    float *Ac = reinterpret_cast<float *>(wb + kSmA) + cw * ZMAX * 3;
-    unsigned char *Sc = wb + kSmS + cw * ZMAX;
-    int *Zw = reinterpret_cast<int *>(wb + kSmZ);
-    unsigned char *attc = wb + kSmAtt + cw * ZMAX;
-    long long *acc = reinterpret_cast<long long *>(smem + kSmAcc) + warp * (kMaxFuse * 12);
+    float4 *Rm = reinterpret_cast<float4 *>(wb + kSmRm);
+    float4 *A4 = reinterpret_cast<float4 *>(wb + kSmA);
+    int *Fx = reinterpret_cast<int *>(wb + kSmFx);
+    int4 *Fx4 = reinterpret_cast<int4 *>(wb + kSmFx);
+    unsigned char *Sb = wb + kSmS;
+    int *Zs = reinterpret_cast<int *>(wb + kSmZ);
+    int *Xp = reinterpret_cast<int *>(wb + kSmX);
+    unsigned *Ev = reinterpret_cast<unsigned *>(wb + kSmEv);
+    int *Samp = reinterpret_cast<int *>(wb + kSmSamp);
+    unsigned long long *acc = reinterpret_cast<unsigned long long *>(smem + kSmAcc);
 
-    for (int i = lane; i < kMaxFuse * 12; i += 32) acc[i] = 0;
-    reinterpret_cast<unsigned *>(wb + kSmAtt)[lane] = 0u;
-    __syncwarp();
+    for (int i = threadIdx.x; i < kMaxFuse * 12; i += kBlockThreads) acc[i] = 0ull;
+    for (int i = lane; i < 2 * kEvStride; i += 32) Ev[i] = 0u;
+    Samp[lane] = 0;
+    __syncthreads();
+
+    // exclusive prefix of Z over the warp's chains: slip-spring f of the warp (0 <= f < Tz)
+    // belongs to the chain c with Xp[c] <= f < Xp[c+1] and is its slot f - Xp[c]
+    auto rescan = [&]() {
+        const int z = lane < CPW ? Zs[lane] : 0;
+        int incl = z;
+#pragma unroll
+        for (int o = 1; o < CPW; o <<= 1) {
+            const int t = __shfl_up_sync(kFull, incl, o);
+            if (lane >= o) incl += t;
+        }
+        if (lane < CPW) Xp[lane + 1] = incl;
+        if (lane == 0) Xp[0] = 0;
+    };
+    auto locate = [&](int f, int &c, int &j) {
+        c = 0;
+#pragma unroll
+        for (int st = CPW / 2; st >= 1; st >>= 1)
+            if (f >= Xp[c + st]) c += st;
+        j = f - Xp[c];
+    };
 
     const int nwarps = gridDim.x * kWarpsPerBlock;
     for (int tile = blockIdx.x * kWarpsPerBlock + warp; tile < P.n_tiles; tile += nwarps) {
         unsigned char *tp = P.state + (long long)tile * kTileBytes;
         const long long chain_local = (long long)tile * CPW + cw;
-        const uint32_t chain = (uint32_t)(P.chain_offset + (unsigned long long)chain_local);
-        const float valid = chain_local < P.n_chains ? 1.0f : 0.0f;
+        const uint32_t chain0 = (uint32_t)(P.chain_offset + (unsigned long long)tile * CPW);
+        const uint32_t chain = chain0 + (uint32_t)cw;
+        const bool valid = chain_local < P.n_chains;
 
         // ---- load the warp tile: R into registers (+ mirror), A, S, Z into shared memory
-        float r[12];
+        float r[24];
         {
             const float4 *gR = reinterpret_cast<const float4 *>(tp + kTileR);
 #pragma unroll
-            for (int v = 0; v < 3; ++v) {
+            for (int v = 0; v < 6; ++v) {
                 const float4 t = gR[v * 32 + lane];
                 r[4 * v] = t.x; r[4 * v + 1] = t.y; r[4 * v + 2] = t.z; r[4 * v + 3] = t.w;
-                reinterpret_cast<float4 *>(Rl)[v] = t;
-                reinterpret_cast<int4 *>(Fl)[v] = make_int4(0, 0, 0, 0);
             }
+#pragma unroll
+            for (int v = 0; v < 7; ++v) Fx4[v * 32 + lane] = make_int4(0, 0, 0, 0);
             const float4 *gA = reinterpret_cast<const float4 *>(tp + kTileA);
-            float4 *sA = reinterpret_cast<float4 *>(wb + kSmA);
 #pragma unroll
-            for (int v = 0; v < 3; ++v) sA[v * 32 + lane] = gA[v * 32 + lane];
-            reinterpret_cast<unsigned *>(wb + kSmS)[lane] = reinterpret_cast<const unsigned *>(tp + kTileS)[lane];
-            if (lane < 16) Zw[lane] = reinterpret_cast<const int *>(tp + kTileZ)[lane];
+            for (int v = 0; v < 8; ++v) A4[v * 32 + lane] = gA[v * 32 + lane];
+            reinterpret_cast<uint2 *>(Sb)[lane] = reinterpret_cast<const uint2 *>(tp + kTileS)[lane];
+            Zs[lane] = reinterpret_cast<const int *>(tp + kTileZ)[lane];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) Rm[lane * 9 + k] = make_float4(r[3 * k], r[3 * k + 1], r[3 * k + 2], 0.0f);
         }
         __syncwarp();
-        int Zc = Zw[cw];
+        rescan();
+        __syncwarp();
+        int Tz = Xp[CPW];
 
-        // neighbours across the lane boundary: bead 4l-1 and bead 4l+4 (own end bead at the
-        // chain ends, so that the missing bond contributes zero: free ends, eq 1)
-        float left[3], right[3];
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            const float up = __shfl_up_sync(0xffffffffu, r[9 + c], 1, G);
-            const float dn = __shfl_down_sync(0xffffffffu, r[c], 1, G);
-            left[c] = (l == 0) ? r[c] : up;
-            right[c] = (l == G - 1) ? r[9 + c] : dn;
-        }
-
-        float sv[6];   // virtual-stress partial of this lane's slip-springs (eq 76)
-
-        // slip-spring bookkeeping shared by the prologue and by every step: for the lane's
-        // own slots, d = R_S - A; scatter -dt (3/N_s) d into the fixed-point force
-        // accumulators of bead S (used by the NEXT bead phase) and sum the virial.
-        auto scatter_and_virial = [&]() {
-#pragma unroll
-            for (int t = 0; t < 6; ++t) sv[t] = 0.0f;
-            for (int j0 = 2 * l; j0 < Zc; j0 += 2 * G) {
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const int j = j0 + e;
-                    if (j < Zc) {
-                        const int s = Sc[j] - 1;
-                        float d[3];
-#pragma unroll
-                        for (int c = 0; c < 3; ++c) {
-                            d[c] = Rc[3 * s + c] - Ac[3 * j + c];
-                            atomicAdd(&Fc[3 * s + c], __float2int_rn(-P.fx_scale * d[c]));
-                        }
-                        sv[0] += fmaf(P.cs * d[0], d[0], -1.0f);
-                        sv[1] += fmaf(P.cs * d[1], d[1], -1.0f);
-                        sv[2] += fmaf(P.cs * d[2], d[2], -1.0f);
-                        sv[3] = fmaf(P.cs * d[0], d[1], sv[3]);
-                        sv[4] = fmaf(P.cs * d[1], d[2], sv[4]);
-                        sv[5] = fmaf(P.cs * d[2], d[0], sv[5]);
-                    }
-                }
+        // forces of the loaded state: scatter -dt (3/N_s) (R_S - A) of every slip-spring into
+        // the fixed-point accumulators of bead S (eq 1; used by the first bead phase)
+        if (P.springs_on) {
+            for (int f = lane; f < Tz; f += 32) {
+                int c, j;
+                locate(f, c, j);
+                const int base = c << LN, sidx = base + j;
+                const int s = Sb[sidx];
+                const float4 a = A4[sidx], rb = Rm[rm_index(base + s - 1)];
+                int *fp = Fx + fx_index(base + s - 1);
+                atomicAdd(fp, __float2int_rn(-P.fx_scale * (rb.x - a.x)));
+                atomicAdd(fp + 1, __float2int_rn(-P.fx_scale * (rb.y - a.y)));
+                atomicAdd(fp + 2, __float2int_rn(-P.fx_scale * (rb.z - a.z)));
             }
-        };
-        if (P.springs_on) scatter_and_virial();
+        }
         __syncwarp();
 
-        int rec = 0, smp = 0;   // records / correlator samples taken so far in this launch
-        for (int n = 0; n < P.n_fuse; ++n) {
-            const unsigned long long step = P.step0 + (unsigned long long)n;
-            const StreamKey sk = make_stream(P.key0, P.key1, step);
-
-            // ================= bead phase: substep 1 (eq 44) =================
-            float z[12];
-#pragma unroll
-            for (int q = 0; q < 3; ++q) {
-                float z4[4];
-                normal_call(sk, DOM_NOISE, chain, (uint32_t)(3 * l + q), z4);
-                z[4 * q] = z4[0]; z[4 * q + 1] = z4[1]; z[4 * q + 2] = z4[2]; z[4 * q + 3] = z4[3];
-            }
-            int fx[12];
-#pragma unroll
-            for (int v = 0; v < 3; ++v) {
-                const int4 t = reinterpret_cast<int4 *>(Fl)[v];
-                fx[4 * v] = t.x; fx[4 * v + 1] = t.y; fx[4 * v + 2] = t.z; fx[4 * v + 3] = t.w;
-                reinterpret_cast<int4 *>(Fl)[v] = make_int4(0, 0, 0, 0);
-            }
-            float rn[12];
-#pragma unroll
-            for (int b = 0; b < 4; ++b)
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    const float x = r[3 * b + c];
-                    const float prev = (b == 0) ? left[c] : r[3 * (b - 1) + c];
-                    const float next = (b == 3) ? right[c] : r[3 * (b + 1) + c];
-                    float inc = fmaf(P.dt3, (next - x) - (x - prev), P.sq2dt * z[3 * b + c]);
-                    inc = fmaf((float)fx[3 * b + c], 1.0f / (float)(1 << kFxShift), inc);
-                    if (c == 0) inc = fmaf(P.gdt, r[3 * b + 1], inc);
-                    rn[3 * b + c] = x + inc;
-                }
-#pragma unroll
-            for (int i = 0; i < 12; ++i) r[i] = rn[i];
-#pragma unroll
-            for (int v = 0; v < 3; ++v)
-                reinterpret_cast<float4 *>(Rl)[v] = make_float4(r[4 * v], r[4 * v + 1], r[4 * v + 2], r[4 * v + 3]);
+        int rec = 0, smp = 0;           // records / correlator samples taken so far in this launch
+        bool rec_prev = false, smp_prev = false;
+        float sv[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, cnt = 0.f;   // sum d_a d_b and number of this lane's slip-springs
+        for (int n = 0;; ++n) {
+            // neighbours across the lane boundary: bead 8l-1 and bead 8l+8 (own end bead at the
+            // chain ends, so that the missing bond is zero: free ends, eq 1)
+            float bl[3], b[24];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                const float up = __shfl_up_sync(0xffffffffu, r[9 + c], 1, G);
-                const float dn = __shfl_down_sync(0xffffffffu, r[c], 1, G);
-                left[c] = (l == 0) ? r[c] : up;
-                right[c] = (l == G - 1) ? r[9 + c] : dn;
-            }
-            __syncwarp();
-
-            const unsigned long long done = step + 1ull;
-            const bool record = P.stress_every > 0 && done % (unsigned)P.stress_every == 0;
-            const bool sample = P.sample_every > 0 && done % (unsigned)P.sample_every == 0;
-
-            // ================= slot phase: substeps 2 and 3 =================
-            if (P.springs_on) {
-                const int Z0 = Zc;
-                bool event = false;
-                for (int j0 = 2 * l; j0 < Z0; j0 += 2 * G) {
-                    uint32_t w[4];
-                    stream_call(sk, DOM_SLOT, chain, (uint32_t)(j0 >> 1), w);
-#pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        const int j = j0 + e;
-                        if (j < Z0) {
-                            int s = Sc[j];                                   // 1..N
-                            float a[3] = {Ac[3 * j], Ac[3 * j + 1], Ac[3 * j + 2]};
-                            if (P.gdt != 0.0f) {                             // eq 45, kappa_xy only
-                                a[0] = fmaf(P.gdt, a[1], a[0]);
-                                Ac[3 * j] = a[0];
-                            }
-                            // Glauber hop (eqs 23, 24 with the cap of eqs 48, 49):
-                            // p+- = min{ h [1 - tanh x+-], 1/2 } = min{ 2h / (1 + e^{2 x+-}), 1/2 },
-                            // x+- = (3/4N_s)(|R_{s+-1}-A|^2 - |R_s-A|^2)
-                            //     = (3/4N_s)(R_{s+-1}-R_s).(R_{s+-1}+R_s-2A)   (no cancellation)
-                            const int sp = s < N ? s : s - 1, sm = s > 1 ? s - 2 : s - 1;   // 0-based, clamped
-                            float dp = 0.0f, dm = 0.0f;
-#pragma unroll
-                            for (int c = 0; c < 3; ++c) {
-                                const float r0 = Rc[3 * (s - 1) + c], rp = Rc[3 * sp + c], rm = Rc[3 * sm + c];
-                                const float two_a = 2.0f * a[c];
-                                dp = fmaf(rp - r0, (rp + r0) - two_a, dp);
-                                dm = fmaf(rm - r0, (rm + r0) - two_a, dm);
-                            }
-                            float pp = fminf(__fdividef(P.h2, 1.0f + exp2f(P.q2l * dp)), 0.5f);
-                            float pm = fminf(__fdividef(P.h2, 1.0f + exp2f(P.q2l * dm)), 0.5f);
-                            if (s == N) pp = 0.0f;
-                            if (s == 1) pm = 0.0f;
-                            const float u = u23(w[2 * e]);
-                            if (u < pp) s += 1;
-                            else if (u < pp + pm) s -= 1;
-                            // destruction at the ends (eq 53), integer-domain comparison
-                            const bool destroyed = (s == 1 || s == N) && code23(w[2 * e + 1]) < P.t_destroy;
-                            Sc[j] = (unsigned char)(destroyed ? 0xFF : s);     // 0xFF = destroyed marker (N <= 128)
-                            event |= destroyed;
-                        }
-                    }
+                float lf = r[c], rt = r[21 + c];
+                if (G > 1) {
+                    const float up = __shfl_up_sync(kFull, r[21 + c], 1, G);
+                    const float dn = __shfl_down_sync(kFull, r[c], 1, G);
+                    if (l != 0) lf = up;
+                    if (l != G - 1) rt = dn;
                 }
-                // construction attempts (eqs 50, 51): K = number of empty slots, attempt k
-                // uses word k&3 of call k>>2
-                const int K = ZMAX - Z0;
-                if (4 * l < K) {
-                    uint32_t w[4];
-                    stream_call(sk, DOM_ATTEMPT, chain, (uint32_t)l, w);
-                    const unsigned t1 = P.t_c1[K], t2 = P.t_c2[K];
+                bl[c] = r[c] - lf;
 #pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        const int k = 4 * l + e;
-                        const unsigned code = code23(w[e]);
-                        if (k < K && code < t2) {
-                            attc[k] = (unsigned char)(code < t1 ? 1 : N);
-                            event = true;
-                        }
-                    }
-                }
-                const unsigned ev = __ballot_sync(0xffffffffu, event);
-                __syncwarp();
-                if (((ev >> lane0) & GMASK) != 0u && l == 0) {
-                    // rare path: re-index the chain's slip-springs as the paper does:
-                    // survivors keep their order, new ones are appended in attempt order
-                    int Zs = 0;
-                    for (int j = 0; j < Z0; ++j) {
-                        const int s = Sc[j];
-                        if (s != 0xFF) {
-                            if (Zs != j) {
-                                Sc[Zs] = (unsigned char)s;
-                                Ac[3 * Zs] = Ac[3 * j]; Ac[3 * Zs + 1] = Ac[3 * j + 1]; Ac[3 * Zs + 2] = Ac[3 * j + 2];
-                            }
-                            ++Zs;
-                        }
-                    }
-                    for (int k = 0; k < K; ++k) {
-                        const int snew = attc[k];
-                        if (snew) {
-                            attc[k] = 0;
-                            float z4[4];
-                            normal_call(sk, DOM_ANCHOR, chain, (uint32_t)k, z4);   // eq 52
-                            Sc[Zs] = (unsigned char)snew;
-#pragma unroll
-                            for (int c = 0; c < 3; ++c) Ac[3 * Zs + c] = fmaf(P.sq_ns3, z4[c], Rc[3 * (snew - 1) + c]);
-                            ++Zs;
-                        }
-                    }
-                    for (int j = Zs; j < Z0; ++j) { Sc[j] = 0; Ac[3 * j] = 0.0f; Ac[3 * j + 1] = 0.0f; Ac[3 * j + 2] = 0.0f; }
-                    Zw[cw] = Zs;
-                }
-                __syncwarp();
-                Zc = Zw[cw];
-                scatter_and_virial();
-                __syncwarp();
+                for (int k = 0; k < 8; ++k) b[3 * k + c] = (k == 7 ? rt : r[3 * (k + 1) + c]) - r[3 * k + c];
             }
 
-            // ================= observables (eqs 16, 76) and ensemble sums (eq 54) =================
-            if (record || sample) {
-                float v[16];
+            // ---- observables of the state after step n-1 (eqs 16, 76) and ensemble sums (eq 54)
+            if (rec_prev || smp_prev) {
+                float v[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-                for (int t = 0; t < 6; ++t) v[t] = 0.0f;
-#pragma unroll
-                for (int b = 0; b < 4; ++b) {
-                    float bd[3];
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) bd[c] = ((b == 3) ? right[c] : r[3 * (b + 1) + c]) - r[3 * b + c];
-                    v[0] = fmaf(3.0f * bd[0], bd[0], v[0]);
-                    v[1] = fmaf(3.0f * bd[1], bd[1], v[1]);
-                    v[2] = fmaf(3.0f * bd[2], bd[2], v[2]);
-                    v[3] = fmaf(3.0f * bd[0], bd[1], v[3]);
-                    v[4] = fmaf(3.0f * bd[1], bd[2], v[4]);
-                    v[5] = fmaf(3.0f * bd[2], bd[0], v[5]);
+                for (int k = 0; k < 8; ++k) {
+                    v[0] = fmaf(b[3 * k], b[3 * k], v[0]);
+                    v[1] = fmaf(b[3 * k + 1], b[3 * k + 1], v[1]);
+                    v[2] = fmaf(b[3 * k + 2], b[3 * k + 2], v[2]);
+                    v[3] = fmaf(b[3 * k], b[3 * k + 1], v[3]);
+                    v[4] = fmaf(b[3 * k + 1], b[3 * k + 2], v[4]);
+                    v[5] = fmaf(b[3 * k + 2], b[3 * k], v[5]);
                 }
-                const float nb = (l == G - 1) ? 3.0f : 4.0f;       // real bonds of this lane: -1 each (eq 16: -N kT 1, +1 on host)
-                v[0] -= nb; v[1] -= nb; v[2] -= nb;
-#pragma unroll
-                for (int t = 0; t < 6; ++t) v[6 + t] = P.springs_on ? sv[t] : 0.0f;
-                if (sample) {
+                if (smp_prev) {
                     // per-chain f = sigma_xy, g = sigma_xy + sigma^(v)_xy for the correlator (eq 43)
-                    float f = v[3], g = v[3] + v[9];
+                    float f = 3.0f * v[3];
 #pragma unroll
-                    for (int o = G / 2; o >= 1; o >>= 1) {
-                        f += __shfl_xor_sync(0xffffffffu, f, o);
-                        g += __shfl_xor_sync(0xffffffffu, g, o);
+                    for (int o = G / 2; o >= 1; o >>= 1) f += __shfl_xor_sync(kFull, f, o);
+                    if (l == 0) {
+                        const int sx = Samp[cw];
+                        Samp[cw] = 0;
+                        const float g = fmaf(P.cs * (1.0f / (float)(1 << kSampleShift)), (float)sx, f);
+                        if (valid && P.samples) P.samples[(long long)smp * P.n_chains + chain_local] = make_float2(f, g);
                     }
-                    if (l == 0 && valid != 0.0f && P.samples)
-                        P.samples[(long long)smp * P.n_chains + chain_local] = make_float2(f, g);
                     ++smp;
                 }
-                if (record) {
+                if (rec_prev) {
+                    // this lane's share: sum over its bonds of (3 b_a b_b - delta_ab) and over the
+                    // slip-springs it handled of ((3/N_s) d_a d_b - delta_ab)
+                    const float s3 = valid ? 3.0f : 0.0f;
+                    const float nb = valid ? ((l == G - 1) ? 7.0f : 8.0f) : 0.0f;
+                    float t[12];
+                    t[0] = fmaf(s3, v[0], -nb); t[1] = fmaf(s3, v[1], -nb); t[2] = fmaf(s3, v[2], -nb);
+                    t[3] = s3 * v[3]; t[4] = s3 * v[4]; t[5] = s3 * v[5];
+                    t[6] = fmaf(P.cs, sv[0], -cnt); t[7] = fmaf(P.cs, sv[1], -cnt); t[8] = fmaf(P.cs, sv[2], -cnt);
+                    t[9] = P.cs * sv[3]; t[10] = P.cs * sv[4]; t[11] = P.cs * sv[5];
+                    // |off-diagonal| <= half the sum of two diagonals, so the two traces bound all
+                    // 12 shares by 256, and a 32-lane sum of shares * 2^18 fits 32 bits
+                    const bool big = !(3.0f * (v[0] + v[1] + v[2]) < 240.0f && P.cs * (sv[0] + sv[1] + sv[2]) < 240.0f);
+                    const float scale = (float)(1 << kStressShift);
+                    long long mine = 0;
+                    if (__any_sync(kFull, big)) {
+                        // rare (strongly stretched chains): sum the shares as two 32-bit halves
 #pragma unroll
-                    for (int t = 0; t < 12; ++t) v[t] *= valid;
-                    v[12] = v[13] = v[14] = v[15] = 0.0f;
-                    warp_reduce_scatter16(v, lane);
-                    if ((lane & 1) == 0 && lane < 24)
-                        acc[rec * 12 + (lane >> 1)] += __float2ll_rn(v[0] * (float)(1 << kStressShift));
+                        for (int i = 0; i < 12; ++i) {
+                            const long long q = __float2ll_rn(t[i] * scale);
+                            const int hi = __reduce_add_sync(kFull, (int)(q >> 16));
+                            const int lo = __reduce_add_sync(kFull, (int)(q & 0xFFFF));
+                            if (lane == i) mine = ((long long)hi << 16) + (long long)lo;
+                        }
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 12; ++i) {
+                            const int tot = __reduce_add_sync(kFull, __float2int_rn(t[i] * scale));
+                            if (lane == i) mine = (long long)tot;
+                        }
+                    }
+                    if (lane < 12) atomicAdd(acc + rec * 12 + lane, (unsigned long long)mine);
                     ++rec;
                 }
             }
+            if (n == P.n_fuse) break;
+
+            const unsigned long long step = P.step0 + (unsigned long long)n;
+            const StreamKey sk = make_stream(step);
+            const bool record = (P.rec_mask >> n) & 1u;
+            const bool sample = (P.smp_mask >> n) & 1u;
+            const int Z0 = Zs[cw];
+
+            // ================= bead phase: substep 1 (eq 44) =================
+#pragma unroll
+            for (int q = 0; q < 6; ++q) {
+                const int4 fx = Fx4[lane * 7 + q];
+                Fx4[lane * 7 + q] = make_int4(0, 0, 0, 0);
+                float z4[4];
+                normal_call(sk, P.rk, DOM_NOISE, chain, (uint32_t)(6 * l + q), P.bm_noise, z4);
+                const int fxa[4] = {fx.x, fx.y, fx.z, fx.w};
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int f = 4 * q + e, k = f / 3, c = f % 3;
+                    const float lap = b[f] - (k == 0 ? bl[c] : b[f - 3]);
+                    float inc = fmaf(P.dt3, lap, z4[e]);
+                    inc = fmaf((float)fxa[e], 1.0f / (float)(1 << kFxShift), inc);
+                    if (c == 0) inc = fmaf(P.gdt, r[f + 1], inc);
+                    r[f] += inc;
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < 8; ++k) Rm[lane * 9 + k] = make_float4(r[3 * k], r[3 * k + 1], r[3 * k + 2], 0.0f);
+            __syncwarp();
+
+            // ================= slot phase: substeps 2 and 3 =================
+#pragma unroll
+            for (int t = 0; t < 6; ++t) sv[t] = 0.0f;
+            cnt = 0.0f;
+            if (P.springs_on) {
+                bool event = false;
+                for (int f = lane; f < Tz; f += 32) {
+                    int c, j;
+                    locate(f, c, j);
+                    const int base = c << LN, sidx = base + j;
+                    uint32_t w[4];
+                    stream_call(sk, P.rk, DOM_SLOT, chain0 + (uint32_t)c, (uint32_t)(j >> 1), w);
+                    const uint32_t w_hop = (j & 1) ? w[2] : w[0], w_end = (j & 1) ? w[3] : w[1];
+                    const int s = Sb[sidx];                                   // 1..N
+                    float4 a = A4[sidx];
+                    if (P.gdt != 0.0f) {
+                        // eq 45 with kappa_xy only: A_x += dt gamma_dot A_y, as a compensated
+                        // (two-sum) update of (A_x, low part): the increment is the same every
+                        // step, so a plain fp32 sum would drift linearly instead of randomly
+                        const float t = fmaf(P.gdt, a.y, a.w);
+                        const float sum = a.x + t;
+                        const float bb = sum - a.x;
+                        a.w = (a.x - (sum - bb)) + (t - bb);
+                        a.x = sum;
+                        A4[sidx] = a;
+                    }
+                    // Glauber hop (eqs 23, 24 with the cap of eqs 48, 49):
+                    // p+- = min{ h [1 - tanh x+-], 1/2 } = min{ 2h / (1 + e^{2 x+-}), 1/2 },
+                    // x+- = (3/4N_s)(|R_{s+-1}-A|^2 - |R_s-A|^2)
+                    //     = (3/4N_s)(R_{s+-1}-R_s).(R_{s+-1}+R_s-2A)   (no cancellation)
+                    const float4 r0 = Rm[rm_index(base + s - 1)];
+                    const float4 rp = Rm[rm_index(base + (s < N ? s : N - 1))];
+                    const float4 rm = Rm[rm_index(base + (s > 1 ? s - 2 : 0))];
+                    const float ax2 = 2.0f * a.x, ay2 = 2.0f * a.y, az2 = 2.0f * a.z;
+                    float dp = (rp.x - r0.x) * ((rp.x + r0.x) - ax2);
+                    dp = fmaf(rp.y - r0.y, (rp.y + r0.y) - ay2, dp);
+                    dp = fmaf(rp.z - r0.z, (rp.z + r0.z) - az2, dp);
+                    float dm = (rm.x - r0.x) * ((rm.x + r0.x) - ax2);
+                    dm = fmaf(rm.y - r0.y, (rm.y + r0.y) - ay2, dm);
+                    dm = fmaf(rm.z - r0.z, (rm.z + r0.z) - az2, dm);
+                    float pp = fminf(__fdividef(P.h2, 1.0f + mufu_ex2(P.q2l * dp)), 0.5f);
+                    float pm = fminf(__fdividef(P.h2, 1.0f + mufu_ex2(P.q2l * dm)), 0.5f);
+                    if (s == N) pp = 0.0f;
+                    if (s == 1) pm = 0.0f;
+                    const float u = u23(w_hop);
+                    int sn = s;
+                    float4 rn = r0;
+                    if (u < pp) { sn = s + 1; rn = rp; }
+                    else if (u < pp + pm) { sn = s - 1; rn = rm; }
+                    // destruction at the ends (eq 53), integer-domain comparison
+                    const bool destroyed = (sn == 1 || sn == N) && code23(w_end) < P.t_destroy;
+                    event |= destroyed;
+                    if (destroyed || sn != s) Sb[sidx] = (unsigned char)(destroyed ? 0xFF : sn);   // 0xFF: removed in the rare path
+                    // a destroyed slip-spring exerts no force and has no virial: zero displacement
+                    const float dx = destroyed ? 0.0f : rn.x - a.x, dy = destroyed ? 0.0f : rn.y - a.y,
+                                dz = destroyed ? 0.0f : rn.z - a.z;
+                    int *fp = Fx + fx_index(base + sn - 1);
+                    atomicAdd(fp, __float2int_rn(-P.fx_scale * dx));
+                    atomicAdd(fp + 1, __float2int_rn(-P.fx_scale * dy));
+                    atomicAdd(fp + 2, __float2int_rn(-P.fx_scale * dz));
+                    if (record) {
+                        sv[0] = fmaf(dx, dx, sv[0]); sv[1] = fmaf(dy, dy, sv[1]); sv[2] = fmaf(dz, dz, sv[2]);
+                        sv[3] = fmaf(dx, dy, sv[3]); sv[4] = fmaf(dy, dz, sv[4]); sv[5] = fmaf(dz, dx, sv[5]);
+                        cnt += destroyed ? 0.0f : 1.0f;
+                    }
+                    if (sample) atomicAdd(Samp + c, __float2int_rn(dx * dy * (float)(1 << kSampleShift)));
+                }
+                // construction attempts (eqs 50, 51), drawn by the chain's own lanes: attempt k
+                // uses word k&3 of call k>>2; K = N - Z or a fixed K
+                {
+                    const int empty = N - Z0;
+                    int K = P.k_attempts > 0 ? (P.k_attempts < empty ? P.k_attempts : empty) : empty;
+                    if (!valid) K = 0;
+                    if (4 * l < K) {
+                        const unsigned t1 = P.t_c1[K], t2 = P.t_c2[K];
+                        for (int q = l; 4 * q < K; q += G) {
+                            uint32_t w[4];
+                            stream_call(sk, P.rk, DOM_ATTEMPT, chain, (uint32_t)q, w);
+#pragma unroll
+                            for (int e = 0; e < 4; ++e) {
+                                const int k = 4 * q + e;
+                                const unsigned code = code23(w[e]);
+                                if (k < K && code < t2) {
+                                    atomicOr(Ev + (code < t1 ? 0 : 1) * kEvStride + cw * WPC + (k >> 5), 1u << (k & 31));
+                                    event = true;
+                                }
+                            }
+                        }
+                    }
+                }
+                if (__any_sync(kFull, event)) {
+                    __syncwarp();
+                    if (l == 0) {
+                        // rare path, one lane per chain: re-index the chain's slip-springs so that
+                        // they occupy slots 0..Z-1.  Destroyed ones are visited from the
+                        // last to the first and replaced by the last one; new ones are appended in
+                        // attempt order (reading R21).
+                        const int base = cw << LN;
+                        int Zn = Z0;
+                        bool changed = false;
+                        for (int wd = (Z0 - 1) >> 2; wd >= 0; --wd) {
+                            unsigned m = __vcmpeq4(reinterpret_cast<const unsigned *>(Sb + base)[wd], 0xFFFFFFFFu);
+                            while (m) {
+                                const int bit = 31 - __clz(m);            // highest marked byte first
+                                m &= ~(0xFFu << (bit & 24));
+                                const int j = 4 * wd + (bit >> 3);
+                                --Zn;
+                                if (j != Zn) { Sb[base + j] = Sb[base + Zn]; A4[base + j] = A4[base + Zn]; }
+                                Sb[base + Zn] = 0;
+                                A4[base + Zn] = make_float4(0.f, 0.f, 0.f, 0.f);
+                                changed = true;
+                            }
+                        }
+#pragma unroll
+                        for (int wd = 0; wd < WPC; ++wd) {
+                            const unsigned m1 = Ev[cw * WPC + wd];
+                            unsigned m = m1 | Ev[kEvStride + cw * WPC + wd];
+                            if (m) { Ev[cw * WPC + wd] = 0u; Ev[kEvStride + cw * WPC + wd] = 0u; changed = true; }
+                            while (m) {
+                                const int bit = __ffs(m) - 1;
+                                m &= m - 1u;
+                                const int k = 32 * wd + bit;
+                                const int snew = ((m1 >> bit) & 1u) ? 1 : N;
+                                float z4[4];
+                                normal_call(sk, P.rk, DOM_ANCHOR, chain, (uint32_t)k, P.bm_anchor, z4);   // eq 52
+                                const float4 rb = Rm[rm_index(base + snew - 1)];
+                                const float4 a = make_float4(rb.x + z4[0], rb.y + z4[1], rb.z + z4[2], 0.0f);
+                                Sb[base + Zn] = (unsigned char)snew;
+                                A4[base + Zn] = a;
+                                ++Zn;
+                                const float dx = rb.x - a.x, dy = rb.y - a.y, dz = rb.z - a.z;
+                                int *fp = Fx + fx_index(base + snew - 1);
+                                atomicAdd(fp, __float2int_rn(-P.fx_scale * dx));
+                                atomicAdd(fp + 1, __float2int_rn(-P.fx_scale * dy));
+                                atomicAdd(fp + 2, __float2int_rn(-P.fx_scale * dz));
+                                if (record) {
+                                    sv[0] = fmaf(dx, dx, sv[0]); sv[1] = fmaf(dy, dy, sv[1]); sv[2] = fmaf(dz, dz, sv[2]);
+                                    sv[3] = fmaf(dx, dy, sv[3]); sv[4] = fmaf(dy, dz, sv[4]); sv[5] = fmaf(dz, dx, sv[5]);
+                                    cnt += 1.0f;
+                                }
+                                if (sample) atomicAdd(Samp + cw, __float2int_rn(dx * dy * (float)(1 << kSampleShift)));
+                            }
+                        }
+                        if (changed) Zs[cw] = Zn;
+                    }
+                    __syncwarp();
+                    rescan();
+                    __syncwarp();
+                    Tz = Xp[CPW];
+                }
+            }
+            __syncwarp();
+            rec_prev = record; smp_prev = sample;
         }
 
         // ---- store the warp tile
         {
             float4 *gR = reinterpret_cast<float4 *>(tp + kTileR);
 #pragma unroll
-            for (int v = 0; v < 3; ++v) gR[v * 32 + lane] = make_float4(r[4 * v], r[4 * v + 1], r[4 * v + 2], r[4 * v + 3]);
+            for (int v = 0; v < 6; ++v) gR[v * 32 + lane] = make_float4(r[4 * v], r[4 * v + 1], r[4 * v + 2], r[4 * v + 3]);
             float4 *gA = reinterpret_cast<float4 *>(tp + kTileA);
-            const float4 *sA = reinterpret_cast<const float4 *>(wb + kSmA);
 #pragma unroll
-            for (int v = 0; v < 3; ++v) gA[v * 32 + lane] = sA[v * 32 + lane];
-            reinterpret_cast<unsigned *>(tp + kTileS)[lane] = reinterpret_cast<const unsigned *>(wb + kSmS)[lane];
-            if (lane < 16) reinterpret_cast<int *>(tp + kTileZ)[lane] = Zw[lane];
+            for (int v = 0; v < 8; ++v) gA[v * 32 + lane] = A4[v * 32 + lane];
+            reinterpret_cast<uint2 *>(tp + kTileS)[lane] = reinterpret_cast<const uint2 *>(Sb)[lane];
+            reinterpret_cast<int *>(tp + kTileZ)[lane] = Zs[lane];
         }
         __syncwarp();
     }
 
-    // ---- flush: sum the 8 warps' accumulators in fixed order, one 64-bit reduction per
-    // (record, component) per CTA; integer addition is exact, so the result does not depend
-    // on the order in which CTAs arrive (deterministic ensemble sums)
+    // ---- flush: one 64-bit reduction per (record, component) per CTA; integer addition is
+    // exact, so the result does not depend on the order in which warps and CTAs arrive
+    // (deterministic ensemble sums)
     __syncthreads();
-    if (P.stress_every > 0) {
-        const unsigned long long first = P.step0 / (unsigned)P.stress_every;
-        const unsigned long long last = (P.step0 + (unsigned long long)P.n_fuse) / (unsigned)P.stress_every;
-        const int nrec = (int)(last - first);
-        const long long *a0 = reinterpret_cast<const long long *>(smem + kSmAcc);
-        for (int i = threadIdx.x; i < nrec * 12; i += kBlockThreads) {
-            long long s = 0;
-#pragma unroll
-            for (int w = 0; w < kWarpsPerBlock; ++w) s += a0[w * (kMaxFuse * 12) + i];
-            if (s != 0) atomicAdd(reinterpret_cast<unsigned long long *>(P.stress) + i, (unsigned long long)s);
-        }
+    for (int i = threadIdx.x; i < P.n_rec * 12; i += kBlockThreads) {
+        const unsigned long long s = acc[i];
+        if (s != 0ull) atomicAdd(reinterpret_cast<unsigned long long *>(P.stress) + i, s);
     }
 }
 
@@ -391,11 +447,11 @@ static cudaError_t occupancy_g(int *blocks_per_sm)
 cudaError_t step_occupancy(int n_beads, int *blocks_per_sm)
 {
     switch (n_beads) {
-        case 8: return occupancy_g<2>(blocks_per_sm);
-        case 16: return occupancy_g<4>(blocks_per_sm);
-        case 32: return occupancy_g<8>(blocks_per_sm);
-        case 64: return occupancy_g<16>(blocks_per_sm);
-        case 128: return occupancy_g<32>(blocks_per_sm);
+        case 8: return occupancy_g<1>(blocks_per_sm);
+        case 16: return occupancy_g<2>(blocks_per_sm);
+        case 32: return occupancy_g<4>(blocks_per_sm);
+        case 64: return occupancy_g<8>(blocks_per_sm);
+        case 128: return occupancy_g<16>(blocks_per_sm);
     }
     return cudaErrorInvalidValue;
 }
@@ -403,11 +459,11 @@ cudaError_t step_occupancy(int n_beads, int *blocks_per_sm)
 cudaError_t launch_step(int n_beads, const StepParams &p, int grid, cudaStream_t st)
 {
     switch (n_beads) {
-        case 8: return launch_g<2>(p, grid, st);
-        case 16: return launch_g<4>(p, grid, st);
-        case 32: return launch_g<8>(p, grid, st);
-        case 64: return launch_g<16>(p, grid, st);
-        case 128: return launch_g<32>(p, grid, st);
+        case 8: return launch_g<1>(p, grid, st);
+        case 16: return launch_g<2>(p, grid, st);
+        case 32: return launch_g<4>(p, grid, st);
+        case 64: return launch_g<8>(p, grid, st);
+        case 128: return launch_g<16>(p, grid, st);
     }
     return cudaErrorInvalidValue;
 }

@@ -42,7 +42,7 @@ def allreduce_sums(t, group=None):
     return t
 
 
-def stress_means(sums, n_chains_total, shift=24):
+def stress_means(sums, n_chains_total, shift=18):
     """Ensemble means (eq 54) from the all-reduced fixed-point sums [n][12]: value =
     sum / (2^shift M) and the remaining -1 of the three diagonal bond-stress components
     (eq 16: -N kT 1, of which N-1 are folded into the sums; see ssm_stress in ssm.h)."""

@@ -8,10 +8,12 @@ GUARD = 1e-5        # a hop decision with |u - threshold| < GUARD is "fragile" (
 
 
 def to_external(e):
-    """oracle.Ensemble -> (R[3][N][M] f32, A[3][N][M] f32, S[N][M] u8)."""
+    """oracle.Ensemble -> (R[3][N][M] f32, A[4][N][M] f32, S[N][M] u8); A[3], the low part of
+    the anchor's x (include/ssm.h), starts at zero."""
     assert e.zmax == e.N
     R = np.ascontiguousarray(e.R.transpose(2, 1, 0)).astype(np.float32)
-    A = np.ascontiguousarray(e.A.transpose(2, 1, 0)).astype(np.float32)
+    A = np.zeros((4, e.N, e.M), dtype=np.float32)
+    A[:3] = e.A.transpose(2, 1, 0)
     S = np.ascontiguousarray(e.S.T).astype(np.uint8)
     return R, A, S
 
@@ -19,7 +21,9 @@ def to_external(e):
 def from_external(R, A, S):
     """-> (R[M][N][3], A[M][N][3], S[M][N] int32, Z[M]) as fp64 / int arrays."""
     Ro = np.ascontiguousarray(R.transpose(2, 1, 0)).astype(np.float64)
-    Ao = np.ascontiguousarray(A.transpose(2, 1, 0)).astype(np.float64)
+    A3 = A[:3].astype(np.float64)
+    A3[0] += A[3].astype(np.float64)              # anchor x = A[0] + A[3] (compensated sum)
+    Ao = np.ascontiguousarray(A3.transpose(2, 1, 0))
     So = np.ascontiguousarray(S.T).astype(np.int32)
     return Ro, Ao, So, (So > 0).sum(1).astype(np.int32)
 

@@ -55,8 +55,9 @@ def test_device_init_matches_oracle_init(ssm):
         g = ssm.Ensemble(N, M, seed=9)
         Rg, Ag, Sg, Zg = from_external(*g.get_state()[:3])
         assert np.array_equal(Sg, e.S) and np.array_equal(Zg, e.Z)
-        # R_i is a running fp32 sum of i bonds: rounding grows like sqrt(i) half-ulps of |R| <~ 16
-        tol = 2e-6 if N <= 32 else 5e-6
+        # R_i is a running fp32 sum of i bonds, each a special-function-unit normal (absolute error
+        # <= 2^-21.4 in log2, sin, cos): the error grows like sqrt(i)
+        tol = 3e-6 if N <= 32 else 8e-6
         ok, w = close(Rg, e.R, tol)
         assert ok, "N=%d: R off by %.3g" % (N, w)
         ok, w = close(Ag, e.A, tol)
@@ -65,8 +66,11 @@ def test_device_init_matches_oracle_init(ssm):
 
 def test_rouse_limit_positions_and_ensemble_stress_1000_steps(ssm):
     """Slip-springs off: no discrete decisions, so all chains and the ensemble
-    stress of every step must match.  M = 70 leaves a ragged tile."""
-    N, M, steps = 32, 70, 1000
+    stress of every step must match.  M = 1030 leaves a ragged tile.  (The ensemble stress is a
+    mean over M chains of sums of 3 b_a b_b over N-1 bonds; the bonds carry the fp32 rounding of
+    the absolute coordinates, ~2e-6 after 1000 steps, so the mean is good to about
+    6 |b| 2e-6 sqrt(N-1)/sqrt(M): 1e-5 needs M of several hundred at N = 32.)"""
+    N, M, steps = 32, 1030, 1000
     e, g = _pair(ssm, N, M, steps, seed=3, n_0=0.0)
     want = e.run(steps, stress_every=1)
     g.step(steps)
@@ -112,7 +116,8 @@ def test_slipspring_chains_all_sizes(ssm, N, M, steps):
     cs = g.chain_stress()
     ok = (e.first_fragile < 0)
     want = np.array([np.concatenate(e.chain_stress(k)) for k in np.nonzero(ok)[0]])
-    good, w = close(cs.T[ok], want, 2e-5)
+    # one chain, no averaging: 6 |b| delta_b sqrt(N-1) with delta_b ~ 3e-6
+    good, w = close(cs.T[ok], want, 2e-5 * np.sqrt(N / 8.0))
     assert good, w
 
 
