@@ -249,9 +249,11 @@ def main():
     peak_alu = N_SM * SMSP_PER_SM * LANES * peaks["sm_max_mhz"] * 1e6 / 1e12      # T thread-instr/s
     per_launch_updates = float(M) * N * inner * K / max(launches, 1)
     achieved = I_ALG * per_launch_updates / (launch_ms * 1e-3) / 1e12
-    cpw = 128 // N
-    tile_bytes = 3328.0 * ((M + cpw - 1) // cpw)
-    hbm_achieved = 2.0 * tile_bytes / (launch_ms * 1e-3) / 1e9
+    # algorithmic state bytes per launch: read + write of the dense-slot
+    # state, 25 N bytes per chain (R 12N, A 12N, S N); the tiles the kernel really moves are larger
+    # (7552 B per 256 beads = 29.5 N per chain: anchors are float4 with the low part of x, plus Z)
+    alg_bytes = 2.0 * 25.0 * N * M
+    hbm_achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
     traffic = None
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tp):
@@ -268,11 +270,11 @@ def main():
         "e2e": e2e,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_alu, "unit": "T thread-instr/s",
                      "frac": achieved / peak_alu, "traffic": traffic,
-                     "kernel": "ssm_step_kernel<G=%d>" % (N // 4), "launch_ms": launch_ms,
+                     "kernel": "ssm_step_kernel<G=%d>" % (N // 8), "launch_ms": launch_ms,
                      "i_alg_per_bead_update": I_ALG,
                      "peak_how": "148 SM x 4 SMSP x 32 lanes x %.0f MHz (sm_max_mhz, %s)" % (peaks["sm_max_mhz"], peaks["source"]),
                      "hbm": {"achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                             "frac": hbm_achieved / peaks["hbm_gbs"], "bytes_per_launch": 2.0 * tile_bytes,
+                             "frac": hbm_achieved / peaks["hbm_gbs"], "bytes_per_launch": alg_bytes,
                              "peak_source": peaks["source"]}},
         "paper_context": {"gpu_bead_updates_per_s": 7.3e8, "cpu_bead_updates_per_s": 2.5e6,
                           "hardware": "Tesla C1060 / Core 2 Duo E8500 1 thread (PAPER.md Table 1)"},
