@@ -141,9 +141,13 @@ int ssm_reset_accumulators(ssm_ctx *ctx);
 /* Kernel launches issued so far by this ctx (all kernels of this library). */
 int64_t ssm_launch_count(const ssm_ctx *ctx);
 
-/* Set the number of time steps fused per kernel launch (1..128; default 64).  Results do
+/* Set the number of time steps fused per kernel launch (1..32; default 32).  Results do
  * not depend on it. */
 int ssm_set_fusion(ssm_ctx *ctx, int32_t steps_per_launch);
+
+/* Set the number of CTAs of the step kernel (1..default; 0 restores the default = as many
+ * as are resident at once, 2 per SM).  Results do not depend on it. */
+int ssm_set_grid(ssm_ctx *ctx, int32_t blocks);
 
 void ssm_destroy(ssm_ctx *ctx);
 

@@ -60,7 +60,7 @@ def lib():
         L.oracle_code23.argtypes = [C.c_uint32]; L.oracle_code23.restype = C.c_uint32
         L.oracle_u23.argtypes = [C.c_uint32]; L.oracle_u23.restype = C.c_double
         L.oracle_threshold23.argtypes = [C.c_double]; L.oracle_threshold23.restype = C.c_int64
-        L.oracle_box_muller.argtypes = [C.c_uint32, C.c_uint32, dp]
+        L.oracle_box_muller.argtypes = [C.c_uint32, dp]
         L.oracle_stream_normal.argtypes = [C.c_uint64, C.c_int, C.c_uint64, C.c_uint64, C.c_uint32]
         L.oracle_stream_normal.restype = C.c_double
         L.oracle_zmax.argtypes = [PP]; L.oracle_zmax.restype = C.c_int
@@ -110,9 +110,10 @@ def threshold23(p):
     return lib().oracle_threshold23(p)
 
 
-def box_muller(wa, wb):
+def box_muller(w):
+    """Two normals from one Philox word (16-bit codes in its low and high half)."""
     z = (C.c_double * 2)()
-    lib().oracle_box_muller(wa, wb, z)
+    lib().oracle_box_muller(w, z)
     return z[0], z[1]
 
 

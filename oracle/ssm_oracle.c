@@ -84,31 +84,34 @@ int64_t oracle_threshold23(double p)
     return (int64_t)t;
 }
 
-/* Box-Muller: r = sqrt(-2 ln u_a), theta = 2 pi (u_b - 1/2). */
-void oracle_box_muller(uint32_t wa, uint32_t wb, double z[2])
+/* Box-Muller on one Philox word (reading R24): the low and the high
+ * half of the word are two 16-bit codes ka, kb; u_a = (ka + 1/2) 2^-16, u_b = (kb + 1/2) 2^-16;
+ * r = sqrt(-2 ln u_a), theta = 2 pi (u_b - 1/2); (z0, z1) = (r cos theta, r sin theta).
+ * |z| <= sqrt(34 ln 2) = 4.86; E[z^2] = 1 - 5e-6 (pinned by enumeration in the tests). */
+void oracle_box_muller(uint32_t w, double z[2])
 {
-    double ua = oracle_u23(wa), ub = oracle_u23(wb);
+    double ua = ((double)(w & 0xFFFFu) + 0.5) * 0x1p-16;
+    double ub = ((double)(w >> 16) + 0.5) * 0x1p-16;
     double r = sqrt(-2.0 * log(ua));
     double th = 6.283185307179586476925286766559 * (ub - 0.5);
     z[0] = r * cos(th);
     z[1] = r * sin(th);
 }
 
-/* Normal number m of the stream (domain, step, chain): Philox call q = m>>2 gives
- * z_{4q},z_{4q+1} from words (0,1) and z_{4q+2},z_{4q+3} from words (2,3). */
+/* Normal number m of the stream (domain, step, chain): Philox call q = m>>3 gives the
+ * eight normals z_{8q+2e}, z_{8q+2e+1} from word e = 0..3. */
 static void normal_call(uint64_t seed, int domain, uint64_t step, uint64_t chain, uint32_t q,
-                        double z[4])
+                        double z[8])
 {
     uint32_t w[4];
     oracle_stream(seed, domain, step, chain, q, w);
-    oracle_box_muller(w[0], w[1], z);
-    oracle_box_muller(w[2], w[3], z + 2);
+    for (int e = 0; e < 4; ++e) oracle_box_muller(w[e], z + 2 * e);
 }
 double oracle_stream_normal(uint64_t seed, int domain, uint64_t step, uint64_t chain, uint32_t m)
 {
-    double z[4];
-    normal_call(seed, domain, step, chain, m >> 2, z);
-    return z[m & 3];
+    double z[8];
+    normal_call(seed, domain, step, chain, m >> 3, z);
+    return z[m & 7];
 }
 
 /* ------------------------------------------------------------------------- */
@@ -183,13 +186,12 @@ void oracle_init_chain(const oracle_params *p, uint64_t chain, double *R, double
     const int N = p->n_beads, zmax = oracle_zmax(p);
     /* 1. Gaussian bonds, variance b^2/3 per axis (eq 6); R_1 = 0 (reading R15) */
     R[0] = R[1] = R[2] = 0.0;
-    double z4[4];
+    double z8[8];
     for (int i = 0; i + 1 < N; ++i)
         for (int c = 0; c < 3; ++c) {
             uint32_t m = (uint32_t)(3 * i + c);
-            if ((m & 3) == 0 || (i == 0 && c == 0))
-                normal_call(p->seed, ORACLE_DOM_INIT_BOND, 0, chain, m >> 2, z4);
-            R[3 * (i + 1) + c] = R[3 * i + c] + sqrt(1.0 / 3.0) * z4[m & 3];
+            if ((m & 7) == 0) normal_call(p->seed, ORACLE_DOM_INIT_BOND, 0, chain, m >> 3, z8);
+            R[3 * (i + 1) + c] = R[3 * i + c] + sqrt(1.0 / 3.0) * z8[m & 7];
         }
     /* 2. Z ~ Poisson(N/N0) clamped at zmax (eq 12; reading R7) by inversion in the
      *    integer domain */
@@ -210,9 +212,9 @@ void oracle_init_chain(const oracle_params *p, uint64_t chain, double *R, double
         uint32_t w[4];
         oracle_stream(p->seed, ORACLE_DOM_INIT_SLOT, 0, chain, (uint32_t)j, w);
         S[j] = 1 + (int)(((uint64_t)w[0] * (uint64_t)N) >> 32);
-        normal_call(p->seed, ORACLE_DOM_INIT_ANCHOR, 0, chain, (uint32_t)j, z4);
+        normal_call(p->seed, ORACLE_DOM_INIT_ANCHOR, 0, chain, (uint32_t)j, z8);
         for (int c = 0; c < 3; ++c)
-            A[3 * j + c] = R[3 * (S[j] - 1) + c] + sqrt(p->n_s / 3.0) * z4[c];
+            A[3 * j + c] = R[3 * (S[j] - 1) + c] + sqrt(p->n_s / 3.0) * z8[c];
     }
     *Zout = Z;
 }
@@ -250,14 +252,14 @@ void oracle_step_chain(const oracle_params *p, uint64_t chain, uint64_t step, do
         for (int c = 0; c < 3; ++c) F[3 * s + c] -= (3.0 / p->n_s) * (R[3 * s + c] - A[3 * j + c]);
     }
     /* explicit Euler, eqs (44),(45) (reading R1); kappa_xy = shear_rate (eq 60) */
-    double z4[4];
+    double z8[8];
     for (int i = 0; i < N; ++i) {
         double ry = R[3 * i + 1];
         for (int c = 0; c < 3; ++c) {
             uint32_t m = (uint32_t)(3 * i + c);
-            if ((m & 3) == 0) normal_call(p->seed, ORACLE_DOM_NOISE, step, chain, m >> 2, z4);
+            if ((m & 7) == 0) normal_call(p->seed, ORACLE_DOM_NOISE, step, chain, m >> 3, z8);
             double flow = (c == 0) ? dt * shear_rate * ry : 0.0;
-            R[3 * i + c] = R[3 * i + c] + dt * F[3 * i + c] + flow + sqrt(2.0 * dt) * z4[m & 3];
+            R[3 * i + c] = R[3 * i + c] + dt * F[3 * i + c] + flow + sqrt(2.0 * dt) * z8[m & 7];
         }
     }
     for (int j = 0; j < Z; ++j) A[3 * j] = A[3 * j] + dt * shear_rate * A[3 * j + 1];
@@ -318,10 +320,10 @@ void oracle_step_chain(const oracle_params *p, uint64_t chain, uint64_t step, do
             if (code < T1) snew = 1;
             else if (code < T2) snew = N;
             if (snew) {
-                normal_call(p->seed, ORACLE_DOM_ANCHOR, step, chain, (uint32_t)k, z4);
+                normal_call(p->seed, ORACLE_DOM_ANCHOR, step, chain, (uint32_t)k, z8);
                 S[Zs] = snew;
                 for (int c = 0; c < 3; ++c)
-                    A[3 * Zs + c] = R[3 * (snew - 1) + c] + sqrt(p->n_s / 3.0) * z4[c];
+                    A[3 * Zs + c] = R[3 * (snew - 1) + c] + sqrt(p->n_s / 3.0) * z8[c];
                 ++Zs;
             }
         }

@@ -13,7 +13,7 @@ extern "C" {
 
 /* Philox stream domains */
 enum {
-    ORACLE_DOM_NOISE = 0,       /* step noise: normal m = 3*bead + axis                  */
+    ORACLE_DOM_NOISE = 0,       /* step noise: normal m = 3*bead + axis = normal m&7 of call m>>3 */
     ORACLE_DOM_SLOT = 1,        /* call j>>1: words 2(j&1), 2(j&1)+1 = u_hop, u_end of j  */
     ORACLE_DOM_ATTEMPT = 2,     /* call k>>2: word k&3 = uniform of construction attempt k*/
     ORACLE_DOM_ANCHOR = 3,      /* call k: normals 0..2 = anchor offset of attempt k      */
@@ -58,7 +58,7 @@ void     oracle_stream(uint64_t seed, int domain, uint64_t step, uint64_t chain,
 uint32_t oracle_code23(uint32_t w);
 double   oracle_u23(uint32_t w);
 int64_t  oracle_threshold23(double p);
-void     oracle_box_muller(uint32_t wa, uint32_t wb, double z[2]);
+void     oracle_box_muller(uint32_t w, double z[2]);
 double   oracle_stream_normal(uint64_t seed, int domain, uint64_t step, uint64_t chain, uint32_t m);
 int      oracle_zmax(const oracle_params *p);
 void     oracle_hop_probabilities(const oracle_params *p, const double *R, const double *A, int s,

@@ -16,7 +16,7 @@ SSM_OK, SSM_EINVAL, SSM_ENOMEM, SSM_ECUDA, SSM_ESTATE, SSM_ERANGE = 0, -1, -2, -
 
 EXPORTS = ["ssm_workspace_bytes", "ssm_init", "ssm_step", "ssm_stress_count", "ssm_stress", "ssm_stress_sums",
            "ssm_stress_sums_device", "ssm_chain_stress", "ssm_gt", "ssm_gt_sums", "ssm_get_state", "ssm_set_state",
-           "ssm_reset_accumulators", "ssm_launch_count", "ssm_set_fusion", "ssm_destroy", "ssm_last_error"]
+           "ssm_reset_accumulators", "ssm_launch_count", "ssm_set_fusion", "ssm_set_grid", "ssm_destroy", "ssm_last_error"]
 
 
 class Params(C.Structure):
@@ -60,6 +60,7 @@ def lib():
     L.ssm_reset_accumulators.argtypes = [vp]; L.ssm_reset_accumulators.restype = C.c_int
     L.ssm_launch_count.argtypes = [vp]; L.ssm_launch_count.restype = C.c_int64
     L.ssm_set_fusion.argtypes = [vp, C.c_int32]; L.ssm_set_fusion.restype = C.c_int
+    L.ssm_set_grid.argtypes = [vp, C.c_int32]; L.ssm_set_grid.restype = C.c_int
     L.ssm_destroy.argtypes = [vp]; L.ssm_destroy.restype = None
     L.ssm_last_error.argtypes = [vp]; L.ssm_last_error.restype = C.c_char_p
     _lib = L
@@ -195,6 +196,9 @@ class Ensemble:
 
     def set_fusion(self, steps_per_launch):
         self._ck(lib().ssm_set_fusion(self.h, steps_per_launch))
+
+    def set_grid(self, blocks):
+        self._ck(lib().ssm_set_grid(self.h, blocks))
 
     def synchronize(self):
         self.stream.synchronize()

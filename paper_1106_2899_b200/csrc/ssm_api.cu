@@ -40,7 +40,7 @@ struct ssm_ctx {
     cudaStream_t st;
     long long step;          // global step counter
     long long n_records;     // stress samples recorded since the last reset
-    int fuse, grid;
+    int fuse, grid, grid_default;
     long long launches;
     bool springs_on;
     StepParams sp;           // constant part filled at init
@@ -169,7 +169,7 @@ extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, s
     if (bps < 1) { delete c; return fail(nullptr, SSM_ECUDA, "step kernel does not fit on an SM"); }
     const long long want = (lay.n_tiles + kWarpsPerBlock - 1) / kWarpsPerBlock;
     const long long cap = (long long)n_sm * bps;
-    c->grid = (int)(want < cap ? want : cap);
+    c->grid = c->grid_default = (int)(want < cap ? want : cap);
 
     // constant launch parameters and integer decision thresholds (fp64 on the host)
     const double h = p->dt / p->zeta_s;
@@ -192,6 +192,7 @@ extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, s
     for (int K = 1; K <= 128; ++K) {
         const double pc = c->springs_on ? std::fmin(h / (p->n_0 * (double)K), 0.5) : 0.0;
         sp.t_c1[K] = threshold23(pc); sp.t_c2[K] = threshold23(2.0 * pc);
+        sp.w_c2[K] = sp.t_c2[K] ? (unsigned)((((unsigned long long)sp.t_c2[K]) << 9) - 1ull) : 0u;
     }
 
     InitParams ip;
@@ -408,6 +409,14 @@ extern "C" int ssm_set_fusion(ssm_ctx *c, int32_t t)
     if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
     if (t < 1 || t > kMaxFuse) return fail(c, SSM_EINVAL, "steps_per_launch out of range");
     c->fuse = t;
+    return SSM_OK;
+}
+
+extern "C" int ssm_set_grid(ssm_ctx *c, int32_t blocks)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (blocks < 0 || blocks > c->grid_default) return fail(c, SSM_EINVAL, "blocks out of range");
+    c->grid = blocks == 0 ? c->grid_default : blocks;
     return SSM_OK;
 }
 

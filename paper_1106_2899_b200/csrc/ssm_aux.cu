@@ -26,10 +26,10 @@ __global__ void __launch_bounds__(128) ssm_init_kernel(const __grid_constant__ I
 
     float R[128 * 3];
     R[0] = R[1] = R[2] = 0.0f;
-    float z4[4] = {0.f, 0.f, 0.f, 0.f};
-    for (int m = 0; m < 3 * (N - 1); ++m) {               // normal m = 3*bond + axis
-        if ((m & 3) == 0) normal_call(sk, P.rk, DOM_INIT_BOND, chain, (uint32_t)(m >> 2), P.bm_bond, z4);
-        R[m + 3] = R[m] + z4[m & 3];
+    float z8[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    for (int m = 0; m < 3 * (N - 1); ++m) {               // normal m = 3*bond + axis = normal m&7 of call m>>3
+        if ((m & 7) == 0) normal_call(sk, P.rk, DOM_INIT_BOND, chain, (uint32_t)(m >> 3), P.bm_bond, z8);
+        R[m + 3] = R[m] + z8[m & 7];
     }
     for (int i = 0; i < N; ++i)
         for (int c = 0; c < 3; ++c) *reinterpret_cast<float *>(st + off_R(k, N, i, c)) = R[3 * i + c];
@@ -48,8 +48,9 @@ __global__ void __launch_bounds__(128) ssm_init_kernel(const __grid_constant__ I
             uint32_t w[4];
             stream_call(sk, P.rk, DOM_INIT_SLOT, chain, (uint32_t)j, w);
             s = 1 + (int)__umulhi(w[0], (uint32_t)N);
-            normal_call(sk, P.rk, DOM_INIT_ANCHOR, chain, (uint32_t)j, P.bm_anchor, z4);
-            for (int c = 0; c < 3; ++c) a[c] = R[3 * (s - 1) + c] + z4[c];
+            float z3[3];
+            anchor_normals(sk, P.rk, DOM_INIT_ANCHOR, chain, (uint32_t)j, P.bm_anchor, z3);
+            for (int c = 0; c < 3; ++c) a[c] = R[3 * (s - 1) + c] + z3[c];
         }
         st[off_S(k, N, j)] = (unsigned char)s;
         for (int c = 0; c < 4; ++c) *reinterpret_cast<float *>(st + off_A(k, N, j, c)) = a[c];

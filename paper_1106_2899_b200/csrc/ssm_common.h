@@ -40,9 +40,11 @@ constexpr int kSmZ = 12544;      // int  [32]   Z per chain
 constexpr int kSmX = 12672;      // int  [33]   exclusive prefix of Z over the warp's chains (+ total), padded to 36
 constexpr int kSmEv = 12816;     // uint [64]   creation masks: created at bead 1 / at bead N, [2][chain][word]
 constexpr int kSmSamp = 13072;   // int  [32]   per-chain fixed-point sum of d_x d_y over slip-springs (sample steps)
-constexpr int kSmWarp = 13200;
+constexpr int kStageSteps = 16;  // recorded steps whose warp sums wait in kSmStage before they are added to the CTA sums
+constexpr int kSmStage = 13200;  // int  [16][12] warp sums of the last recorded steps (int32 fixed point)
+constexpr int kSmWarp = 13968;
 constexpr int kSmAcc = kWarpsPerBlock * kSmWarp;                          // int64 [kMaxFuse][12] per CTA
-constexpr int kSmStep = kSmAcc + kMaxFuse * 12 * 8;                       // 108,672 B: 2 CTAs per SM
+constexpr int kSmStep = kSmAcc + kMaxFuse * 12 * 8;                       // 114,816 B: 2 CTAs per SM (2 x (114,816 + 1024) <= 233,472)
 __host__ __device__ constexpr int rm_index(int bead_in_warp) { return bead_in_warp + (bead_in_warp >> 3); }
 __host__ __device__ constexpr int fx_index(int bead_in_warp) { return (bead_in_warp >> 3) * 28 + (bead_in_warp & 7) * 3; }
 
@@ -71,6 +73,8 @@ struct StepParams {
     float cs;         // 3/N_s                (eq 76)
     unsigned t_destroy;               // T(min{dt/zeta_s, 1})                 (eq 53)
     unsigned t_c1[129], t_c2[129];    // T(p_c(K)), T(2 p_c(K)), K = 1..128   (eqs 50, 51)
+    unsigned w_c2[129];               // largest Philox WORD w with (w >> 9) < T(2 p_c(K)): one compare on the minimum
+                                      // of a call's four words tells whether any of its attempts can succeed
 };
 
 struct InitParams {

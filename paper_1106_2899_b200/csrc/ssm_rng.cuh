@@ -12,7 +12,7 @@ namespace ssm {
 
 // stream domains
 enum : uint32_t {
-    DOM_NOISE = 0,        // per step: normal m = 3*bead + axis, call m>>2, normal m&3
+    DOM_NOISE = 0,        // per step: normal m = 3*bead + axis, call m>>3, normal m&7
     DOM_SLOT = 1,         // per step: call j>>1, words 2(j&1), 2(j&1)+1 = u_hop, u_end of slip-spring j
     DOM_ATTEMPT = 2,      // per step: call k>>2, word k&3 = uniform of construction attempt k
     DOM_ANCHOR = 3,       // per step: call k, normals 0..2 = anchor offset of attempt k
@@ -80,28 +80,42 @@ __device__ __forceinline__ float mufu_sqrt(float x)
     return y;
 }
 
-// Box-Muller: r = sigma sqrt(-2 ln u_a), theta = 2 pi (u_b - 1/2);
-// (z0, z1) = (r cos theta, r sin theta) are two N(0, sigma^2) numbers.
-// bm = -2 ln2 sigma^2, so that r^2 = bm log2(u_a).  The special-function unit evaluates
-// log2, sqrt, sin and cos (absolute error <= 2^-21.4 each in the ranges used here, DESIGN.md
-// section 8.2); theta = 2 pi x + pi 2^-23 with x = k 2^-23 - 1/2 formed exactly.
-__device__ __forceinline__ void box_muller(uint32_t wa, uint32_t wb, float bm, float& z0, float& z1)
+// Box-Muller on ONE Philox word (reading R24): the low and the high half
+// are 16-bit codes ka, kb; u_a = (ka + 1/2) 2^-16, theta = 2 pi ((kb + 1/2) 2^-16 - 1/2);
+// (z0, z1) = (r cos theta, r sin theta) with r = sigma sqrt(-2 ln u_a) are two N(0, sigma^2)
+// numbers, so a Philox call yields EIGHT normals.  bm = -2 ln2 sigma^2, so that
+// r^2 = bm log2(u_a).  The special-function unit evaluates log2, sqrt, sin and cos (absolute
+// error <= 2^-21.4 each in the ranges used here).  Both uniforms are
+// formed exactly: [1 + ka 2^-16] - [1 - 2^-17] and [1 + kb 2^-16] - 1.5 = kb 2^-16 - 1/2, then
+// theta = 2 pi x + pi 2^-16.
+__device__ __forceinline__ void box_muller(uint32_t w, float bm, float& z0, float& z1)
 {
-    const float ua = u23(wa);
-    const float x = __uint_as_float(0x3F800000u | (wb >> 9)) - 1.5f;          // k 2^-23 - 1/2, exact
-    const float th = fmaf(6.283185307179586f, x, 3.7450704e-07f);             // + pi 2^-23
+    const float ua = __uint_as_float(0x3F800000u | ((w & 0xFFFFu) << 7)) - 0.99999237f;    // (ka + 1/2) 2^-16
+    const float x = __uint_as_float(0x3F800000u | ((w >> 9) & 0x7FFF80u)) - 1.5f;          // kb 2^-16 - 1/2
+    const float th = fmaf(6.283185307179586f, x, 4.7936899e-05f);                          // + pi 2^-16
     const float r = mufu_sqrt(bm * __log2f(ua));
     z0 = r * __cosf(th); z1 = r * __sinf(th);
 }
 
-// the four normals of one call: (0,1) from words (0,1), (2,3) from words (2,3)
+// the eight normals of one call: (2e, 2e+1) from word e
 __device__ __forceinline__ void normal_call(const StreamKey& s, const unsigned (&rk)[20], uint32_t domain,
-                                            uint32_t chain, uint32_t call, float bm, float (&z)[4])
+                                            uint32_t chain, uint32_t call, float bm, float (&z)[8])
 {
     uint32_t w[4];
     stream_call(s, rk, domain, chain, call, w);
-    box_muller(w[0], w[1], bm, z[0], z[1]);
-    box_muller(w[2], w[3], bm, z[2], z[3]);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) box_muller(w[e], bm, z[2 * e], z[2 * e + 1]);
+}
+
+// normals 0..2 of a call (anchor offsets, eqs 15 and 52): words 0 and 1 only
+__device__ __forceinline__ void anchor_normals(const StreamKey& s, const unsigned (&rk)[20], uint32_t domain,
+                                               uint32_t chain, uint32_t call, float bm, float (&z)[3])
+{
+    uint32_t w[4];
+    stream_call(s, rk, domain, chain, call, w);
+    float unused;
+    box_muller(w[0], bm, z[0], z[1]);
+    box_muller(w[1], bm, z[2], unused);
 }
 
 }  // namespace ssm

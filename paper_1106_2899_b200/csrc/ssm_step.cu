@@ -53,6 +53,8 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     int *Xp = reinterpret_cast<int *>(wb + kSmX);
     unsigned *Ev = reinterpret_cast<unsigned *>(wb + kSmEv);
     int *Samp = reinterpret_cast<int *>(wb + kSmSamp);
+    int *Stage = reinterpret_cast<int *>(wb + kSmStage);
+    int4 *Stage4 = reinterpret_cast<int4 *>(wb + kSmStage);
     unsigned long long *acc = reinterpret_cast<unsigned long long *>(smem + kSmAcc);
 
     for (int i = threadIdx.x; i < kMaxFuse * 12; i += kBlockThreads) acc[i] = 0ull;
@@ -79,6 +81,16 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
         for (int st = CPW / 2; st >= 1; st >>= 1)
             if (f >= Xp[c + st]) c += st;
         j = f - Xp[c];
+    };
+
+    // add the staged warp sums of records [r0, r1) to the CTA's 64-bit sums
+    auto flush_stage = [&](int r0, int r1) {
+        __syncwarp();
+        for (int i = lane; i < (r1 - r0) * 12; i += 32) {
+            const int v = Stage[i];
+            if (v != 0) atomicAdd(acc + r0 * 12 + i, (unsigned long long)(long long)v);
+        }
+        __syncwarp();
     };
 
     const int nwarps = gridDim.x * kWarpsPerBlock;
@@ -131,6 +143,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
         __syncwarp();
 
         int rec = 0, smp = 0;           // records / correlator samples taken so far in this launch
+        int stage_base = 0;             // first record whose warp sums are still in the staging rows
         bool rec_prev = false, smp_prev = false;
         float sv[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, cnt = 0.f;   // sum d_a d_b and number of this lane's slip-springs
         for (int n = 0;; ++n) {
@@ -190,9 +203,11 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     // 12 shares by 256, and a 32-lane sum of shares * 2^18 fits 32 bits
                     const bool big = !(3.0f * (v[0] + v[1] + v[2]) < 240.0f && P.cs * (sv[0] + sv[1] + sv[2]) < 240.0f);
                     const float scale = (float)(1 << kStressShift);
-                    long long mine = 0;
+                    int4 *row = Stage4 + (rec - stage_base) * 3;
                     if (__any_sync(kFull, big)) {
-                        // rare (strongly stretched chains): sum the shares as two 32-bit halves
+                        // rare (strongly stretched chains): sum the shares as two 32-bit halves and add
+                        // them to the CTA sums directly; the staged row of this record is zero
+                        long long mine = 0;
 #pragma unroll
                         for (int i = 0; i < 12; ++i) {
                             const long long q = __float2ll_rn(t[i] * scale);
@@ -200,15 +215,22 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                             const int lo = __reduce_add_sync(kFull, (int)(q & 0xFFFF));
                             if (lane == i) mine = ((long long)hi << 16) + (long long)lo;
                         }
+                        if (lane < 12) atomicAdd(acc + rec * 12 + lane, (unsigned long long)mine);
+                        if (lane < 3) row[lane] = make_int4(0, 0, 0, 0);
                     } else {
+                        // one warp-wide integer add per component; lane 0 parks the 12 sums in the
+                        // warp's staging rows, which are added to the CTA sums every kStageSteps records
+                        int tot[12];
 #pragma unroll
-                        for (int i = 0; i < 12; ++i) {
-                            const int tot = __reduce_add_sync(kFull, __float2int_rn(t[i] * scale));
-                            if (lane == i) mine = (long long)tot;
+                        for (int i = 0; i < 12; ++i) tot[i] = __reduce_add_sync(kFull, __float2int_rn(t[i] * scale));
+                        if (lane == 0) {
+                            row[0] = make_int4(tot[0], tot[1], tot[2], tot[3]);
+                            row[1] = make_int4(tot[4], tot[5], tot[6], tot[7]);
+                            row[2] = make_int4(tot[8], tot[9], tot[10], tot[11]);
                         }
                     }
-                    if (lane < 12) atomicAdd(acc + rec * 12 + lane, (unsigned long long)mine);
                     ++rec;
+                    if (rec - stage_base == kStageSteps) { flush_stage(stage_base, rec); stage_base = rec; }
                 }
             }
             if (n == P.n_fuse) break;
@@ -221,20 +243,23 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
 
             // ================= bead phase: substep 1 (eq 44) =================
 #pragma unroll
-            for (int q = 0; q < 6; ++q) {
-                const int4 fx = Fx4[lane * 7 + q];
-                Fx4[lane * 7 + q] = make_int4(0, 0, 0, 0);
-                float z4[4];
-                normal_call(sk, P.rk, DOM_NOISE, chain, (uint32_t)(6 * l + q), P.bm_noise, z4);
-                const int fxa[4] = {fx.x, fx.y, fx.z, fx.w};
+            for (int q = 0; q < 3; ++q) {
+                float z8[8];
+                normal_call(sk, P.rk, DOM_NOISE, chain, (uint32_t)(3 * l + q), P.bm_noise, z8);
 #pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const int f = 4 * q + e, k = f / 3, c = f % 3;
-                    const float lap = b[f] - (k == 0 ? bl[c] : b[f - 3]);
-                    float inc = fmaf(P.dt3, lap, z4[e]);
-                    inc = fmaf((float)fxa[e], 1.0f / (float)(1 << kFxShift), inc);
-                    if (c == 0) inc = fmaf(P.gdt, r[f + 1], inc);
-                    r[f] += inc;
+                for (int h = 0; h < 2; ++h) {
+                    const int4 fx = Fx4[lane * 7 + 2 * q + h];
+                    Fx4[lane * 7 + 2 * q + h] = make_int4(0, 0, 0, 0);
+                    const int fxa[4] = {fx.x, fx.y, fx.z, fx.w};
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const int f = 8 * q + 4 * h + e, k = f / 3, c = f % 3;
+                        const float lap = b[f] - (k == 0 ? bl[c] : b[f - 3]);
+                        float inc = fmaf(P.dt3, lap, z8[4 * h + e]);
+                        inc = fmaf((float)fxa[e], 1.0f / (float)(1 << kFxShift), inc);
+                        if (c == 0) inc = fmaf(P.gdt, r[f + 1], inc);
+                        r[f] += inc;
+                    }
                 }
             }
 #pragma unroll
@@ -315,17 +340,22 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     int K = P.k_attempts > 0 ? (P.k_attempts < empty ? P.k_attempts : empty) : empty;
                     if (!valid) K = 0;
                     if (4 * l < K) {
-                        const unsigned t1 = P.t_c1[K], t2 = P.t_c2[K];
+                        // a success needs (w >> 9) < T(2 p_c) ~ 2e-3 2^23: one compare on the minimum
+                        // of the call's four words rules out all four attempts
+                        const unsigned wmax = P.w_c2[K];
                         for (int q = l; 4 * q < K; q += G) {
                             uint32_t w[4];
                             stream_call(sk, P.rk, DOM_ATTEMPT, chain, (uint32_t)q, w);
+                            if (min(min(w[0], w[1]), min(w[2], w[3])) <= wmax) {
+                                const unsigned t1 = P.t_c1[K], t2 = P.t_c2[K];
 #pragma unroll
-                            for (int e = 0; e < 4; ++e) {
-                                const int k = 4 * q + e;
-                                const unsigned code = code23(w[e]);
-                                if (k < K && code < t2) {
-                                    atomicOr(Ev + (code < t1 ? 0 : 1) * kEvStride + cw * WPC + (k >> 5), 1u << (k & 31));
-                                    event = true;
+                                for (int e = 0; e < 4; ++e) {
+                                    const int k = 4 * q + e;
+                                    const unsigned code = code23(w[e]);
+                                    if (k < K && code < t2) {
+                                        atomicOr(Ev + (code < t1 ? 0 : 1) * kEvStride + cw * WPC + (k >> 5), 1u << (k & 31));
+                                        event = true;
+                                    }
                                 }
                             }
                         }
@@ -364,10 +394,10 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                                 m &= m - 1u;
                                 const int k = 32 * wd + bit;
                                 const int snew = ((m1 >> bit) & 1u) ? 1 : N;
-                                float z4[4];
-                                normal_call(sk, P.rk, DOM_ANCHOR, chain, (uint32_t)k, P.bm_anchor, z4);   // eq 52
+                                float z3[3];
+                                anchor_normals(sk, P.rk, DOM_ANCHOR, chain, (uint32_t)k, P.bm_anchor, z3);   // eq 52
                                 const float4 rb = Rm[rm_index(base + snew - 1)];
-                                const float4 a = make_float4(rb.x + z4[0], rb.y + z4[1], rb.z + z4[2], 0.0f);
+                                const float4 a = make_float4(rb.x + z3[0], rb.y + z3[1], rb.z + z3[2], 0.0f);
                                 Sb[base + Zn] = (unsigned char)snew;
                                 A4[base + Zn] = a;
                                 ++Zn;
@@ -395,6 +425,8 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
             __syncwarp();
             rec_prev = record; smp_prev = sample;
         }
+
+        if (rec > stage_base) flush_stage(stage_base, rec);
 
         // ---- store the warp tile
         {

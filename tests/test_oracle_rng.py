@@ -87,14 +87,37 @@ def test_threshold23_equivalence_brute_force():
 
 
 def test_box_muller_closed_form_and_polar_identity():
-    # r^2 = -2 ln u_a and angle 2 pi (u_b - 1/2), "Box-Muller transform"
-    for wa, wb in [(0, 0), (0xFFFFFFFF, 0x80000000), (0x12345678, 0x9ABCDEF0), (1 << 31, 3 << 30)]:
-        z0, z1 = oracle.box_muller(wa, wb)
-        ua, ub = oracle.u23(wa), oracle.u23(wb)
+    # r^2 = -2 ln u_a and angle 2 pi (u_b - 1/2), "Box-Muller transform"; reading R24:
+    # u_a, u_b = midpoints of the 16-bit codes in the low / high half of one Philox word
+    for w in [0, 0xFFFFFFFF, 0x80000000, 0x12345678, 0x9ABCDEF0, 0x0000FFFF, 0xFFFF0000]:
+        z0, z1 = oracle.box_muller(w)
+        ua = ((w & 0xFFFF) + 0.5) / 65536.0
+        ub = ((w >> 16) + 0.5) / 65536.0
         assert math.isclose(z0 * z0 + z1 * z1, -2.0 * math.log(ua), rel_tol=1e-13)
         assert math.isclose(math.atan2(z1, z0), 2 * math.pi * (ub - 0.5), rel_tol=1e-12, abs_tol=1e-15)
-    z0, z1 = oracle.box_muller(0, 0)
-    assert abs(math.hypot(z0, z1)) < 5.8           # |normal| <= sqrt(2 ln 2^24) = 5.77
+    z0, z1 = oracle.box_muller(0)
+    assert abs(math.hypot(z0, z1)) < 4.86          # |normal| <= sqrt(2 ln 2^17) = 4.855
+
+
+def test_box_muller_16bit_grid_moments_by_enumeration():
+    """Reading R24 spends 16 bits per Box-Muller input.  The resulting normal is a discrete
+    law on 2^16 radii x 2^16 angles; its moments follow EXACTLY from enumerating the radii
+    (the angle average of cos^2 over the equally spaced half-offset grid is exactly 1/2, of
+    cos^4 exactly 3/8): E z^2 = E r^2 / 2, E z^4 = 3 E r^4 / 8.  They must agree with the
+    standard normal's to far better than the O(dt) = 1e-2 bias of the Euler scheme."""
+    k = np.arange(65536, dtype=np.float64)
+    r2 = -2.0 * np.log((k + 0.5) / 65536.0)
+    th = 2 * np.pi * ((k + 0.5) / 65536.0 - 0.5)
+    assert abs(np.mean(np.cos(th) ** 2) - 0.5) < 1e-15 and abs(np.mean(np.cos(th) ** 4) - 0.375) < 1e-15
+    assert abs(np.mean(np.cos(th))) < 1e-15 and abs(np.mean(np.cos(th) * np.sin(th))) < 1e-15
+    var = 0.5 * r2.mean(); m4 = 0.375 * (r2 ** 2).mean()
+    assert abs(var - 1.0) < 1e-5, var
+    assert abs(m4 - 3.0) < 5e-4, m4
+    # the oracle's own box_muller lands on that grid: radius from the low half, angle from the high half
+    for ka, kb in [(0, 0), (65535, 0), (123, 45678), (40000, 65535)]:
+        z0, z1 = oracle.box_muller(ka | (kb << 16))
+        assert math.isclose(z0 * z0 + z1 * z1, r2[ka], rel_tol=1e-13)
+        assert math.isclose(math.atan2(z1, z0), th[kb], rel_tol=1e-12, abs_tol=1e-15)
 
 
 def test_stream_normals_are_standard_normal():
@@ -104,11 +127,12 @@ def test_stream_normals_are_standard_normal():
     assert abs(z.var() - 1) < 4 * math.sqrt(2 / n)
     assert abs((z ** 4).mean() - 3) < 4 * math.sqrt(96 / n)
     assert stats.kstest(z, "norm").pvalue > 1e-3
-    # the four normals of one call are uncorrelated with each other
-    q = z.reshape(-1, 4)
+    # the eight normals of one call are uncorrelated with each other
+    q = z.reshape(-1, 8)
     c = np.corrcoef(q.T)
-    assert np.abs(c - np.eye(4)).max() < 5 / math.sqrt(n / 4)
-    # normal m comes from call m>>2: words (0,1) -> z0,z1 ; words (2,3) -> z2,z3
+    assert np.abs(c - np.eye(8)).max() < 5 / math.sqrt(n / 8)
+    # normal m comes from call m>>3: word e -> z_{2e}, z_{2e+1}
     w = oracle.stream(7, oracle.DOM_NOISE, 3, 11, 5)
-    a = oracle.box_muller(w[0], w[1]); b = oracle.box_muller(w[2], w[3])
-    assert [z[20], z[21], z[22], z[23]] == [a[0], a[1], b[0], b[1]]
+    want = [x for e in range(4) for x in oracle.box_muller(w[e])]
+    assert [z[40 + i] for i in range(8)] == want
+
