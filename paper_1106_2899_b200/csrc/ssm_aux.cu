@@ -22,13 +22,14 @@ __global__ void __launch_bounds__(128) ssm_init_kernel(const __grid_constant__ I
     const int N = P.n_beads, zmax = N;
     const uint32_t chain = (uint32_t)(P.chain_offset + (unsigned long long)k);
     const StreamKey sk = make_stream(0ull);
+    const BoxMuller bm_bond(P.bm_bond), bm_anchor(P.bm_anchor);
     unsigned char *st = P.state;
 
     float R[128 * 3];
     R[0] = R[1] = R[2] = 0.0f;
     float z8[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     for (int m = 0; m < 3 * (N - 1); ++m) {               // normal m = 3*bond + axis = normal m&7 of call m>>3
-        if ((m & 7) == 0) normal_call(sk, P.rk, DOM_INIT_BOND, chain, (uint32_t)(m >> 3), P.bm_bond, z8);
+        if ((m & 7) == 0) normal_call(sk, P.rk, DOM_INIT_BOND, chain, (uint32_t)(m >> 3), bm_bond, z8);
         R[m + 3] = R[m] + z8[m & 7];
     }
     for (int i = 0; i < N; ++i)
@@ -49,7 +50,7 @@ __global__ void __launch_bounds__(128) ssm_init_kernel(const __grid_constant__ I
             stream_call(sk, P.rk, DOM_INIT_SLOT, chain, (uint32_t)j, w);
             s = 1 + (int)__umulhi(w[0], (uint32_t)N);
             float z3[3];
-            anchor_normals(sk, P.rk, DOM_INIT_ANCHOR, chain, (uint32_t)j, P.bm_anchor, z3);
+            anchor_normals(sk, P.rk, DOM_INIT_ANCHOR, chain, (uint32_t)j, bm_anchor, z3);
             for (int c = 0; c < 3; ++c) a[c] = R[3 * (s - 1) + c] + z3[c];
         }
         st[off_S(k, N, j)] = (unsigned char)s;

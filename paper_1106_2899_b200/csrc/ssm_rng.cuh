@@ -80,42 +80,55 @@ __device__ __forceinline__ float mufu_sqrt(float x)
     return y;
 }
 
+__device__ __forceinline__ float mufu_lg2(float x)
+{
+    float y;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 // Box-Muller on ONE Philox word (reading R24): the low and the high half
 // are 16-bit codes ka, kb; u_a = (ka + 1/2) 2^-16, theta = 2 pi ((kb + 1/2) 2^-16 - 1/2);
 // (z0, z1) = (r cos theta, r sin theta) with r = sigma sqrt(-2 ln u_a) are two N(0, sigma^2)
 // numbers, so a Philox call yields EIGHT normals.  bm = -2 ln2 sigma^2, so that
 // r^2 = bm log2(u_a).  The special-function unit evaluates log2, sqrt, sin and cos (absolute
-// error <= 2^-21.4 each in the ranges used here).  Both uniforms are
-// formed exactly: [1 + ka 2^-16] - [1 - 2^-17] and [1 + kb 2^-16] - 1.5 = kb 2^-16 - 1/2, then
-// theta = 2 pi x + pi 2^-16.
-__device__ __forceinline__ void box_muller(uint32_t w, float bm, float& z0, float& z1)
-{
-    const float ua = __uint_as_float(0x3F800000u | ((w & 0xFFFFu) << 7)) - 0.99999237f;    // (ka + 1/2) 2^-16
-    const float x = __uint_as_float(0x3F800000u | ((w >> 9) & 0x7FFF80u)) - 1.5f;          // kb 2^-16 - 1/2
-    const float th = fmaf(6.283185307179586f, x, 4.7936899e-05f);                          // + pi 2^-16
-    const float r = mufu_sqrt(bm * __log2f(ua));
-    z0 = r * __cosf(th); z1 = r * __sinf(th);
-}
+// error <= 2^-21.4 each in the ranges used here; log2 is taken of
+// u_a in (0,1) itself so that it keeps its relative accuracy where u_a -> 1).  Both codes are
+// turned into floats exactly with one byte permute each: the bytes of the half word under
+// the exponent of 2^23 give the float 2^23 + k, and (2^23 + ka) 2^-16 - (128 - 2^-17) = u_a
+// is one exact fused multiply-add.
+struct BoxMuller {
+    float bm;            // -2 ln2 sigma^2
+    __device__ __forceinline__ explicit BoxMuller(float b) : bm(b) {}
+    __device__ __forceinline__ void operator()(uint32_t w, float& z0, float& z1) const
+    {
+        const float ua = fmaf(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610)), 1.52587890625e-05f, -127.99999237060547f);
+        const float kb = __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632)) - 8421376.0f;   // kb - 2^15
+        const float th = fmaf(kb, 9.5873799e-05f, 4.7936899e-05f);       // 2 pi 2^-16 (kb - 2^15) + pi 2^-16
+        const float r = mufu_sqrt(bm * mufu_lg2(ua));
+        z0 = r * __cosf(th); z1 = r * __sinf(th);
+    }
+};
 
 // the eight normals of one call: (2e, 2e+1) from word e
 __device__ __forceinline__ void normal_call(const StreamKey& s, const unsigned (&rk)[20], uint32_t domain,
-                                            uint32_t chain, uint32_t call, float bm, float (&z)[8])
+                                            uint32_t chain, uint32_t call, const BoxMuller& bm, float (&z)[8])
 {
     uint32_t w[4];
     stream_call(s, rk, domain, chain, call, w);
 #pragma unroll
-    for (int e = 0; e < 4; ++e) box_muller(w[e], bm, z[2 * e], z[2 * e + 1]);
+    for (int e = 0; e < 4; ++e) bm(w[e], z[2 * e], z[2 * e + 1]);
 }
 
 // normals 0..2 of a call (anchor offsets, eqs 15 and 52): words 0 and 1 only
 __device__ __forceinline__ void anchor_normals(const StreamKey& s, const unsigned (&rk)[20], uint32_t domain,
-                                               uint32_t chain, uint32_t call, float bm, float (&z)[3])
+                                               uint32_t chain, uint32_t call, const BoxMuller& bm, float (&z)[3])
 {
     uint32_t w[4];
     stream_call(s, rk, domain, chain, call, w);
     float unused;
-    box_muller(w[0], bm, z[0], z[1]);
-    box_muller(w[1], bm, z[2], unused);
+    bm(w[0], z[0], z[1]);
+    bm(w[1], z[2], unused);
 }
 
 }  // namespace ssm

@@ -57,6 +57,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     int4 *Stage4 = reinterpret_cast<int4 *>(wb + kSmStage);
     unsigned long long *acc = reinterpret_cast<unsigned long long *>(smem + kSmAcc);
 
+    const BoxMuller bm_noise(P.bm_noise), bm_anchor(P.bm_anchor);
     for (int i = threadIdx.x; i < kMaxFuse * 12; i += kBlockThreads) acc[i] = 0ull;
     for (int i = lane; i < 2 * kEvStride; i += 32) Ev[i] = 0u;
     Samp[lane] = 0;
@@ -192,17 +193,19 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                 if (rec_prev) {
                     // this lane's share: sum over its bonds of (3 b_a b_b - delta_ab) and over the
                     // slip-springs it handled of ((3/N_s) d_a d_b - delta_ab)
-                    const float s3 = valid ? 3.0f : 0.0f;
-                    const float nb = valid ? ((l == G - 1) ? 7.0f : 8.0f) : 0.0f;
+                    // (scaled by 2^kStressShift here, a power of two: the products are the same numbers)
+                    constexpr float scale = (float)(1 << kStressShift);
+                    const float s3 = valid ? 3.0f * scale : 0.0f, css = P.cs * scale;
+                    const float nb = valid ? ((l == G - 1) ? 7.0f * scale : 8.0f * scale) : 0.0f;
+                    const float cnts = cnt * scale;
                     float t[12];
                     t[0] = fmaf(s3, v[0], -nb); t[1] = fmaf(s3, v[1], -nb); t[2] = fmaf(s3, v[2], -nb);
                     t[3] = s3 * v[3]; t[4] = s3 * v[4]; t[5] = s3 * v[5];
-                    t[6] = fmaf(P.cs, sv[0], -cnt); t[7] = fmaf(P.cs, sv[1], -cnt); t[8] = fmaf(P.cs, sv[2], -cnt);
-                    t[9] = P.cs * sv[3]; t[10] = P.cs * sv[4]; t[11] = P.cs * sv[5];
+                    t[6] = fmaf(css, sv[0], -cnts); t[7] = fmaf(css, sv[1], -cnts); t[8] = fmaf(css, sv[2], -cnts);
+                    t[9] = css * sv[3]; t[10] = css * sv[4]; t[11] = css * sv[5];
                     // |off-diagonal| <= half the sum of two diagonals, so the two traces bound all
                     // 12 shares by 256, and a 32-lane sum of shares * 2^18 fits 32 bits
                     const bool big = !(3.0f * (v[0] + v[1] + v[2]) < 240.0f && P.cs * (sv[0] + sv[1] + sv[2]) < 240.0f);
-                    const float scale = (float)(1 << kStressShift);
                     int4 *row = Stage4 + (rec - stage_base) * 3;
                     if (__any_sync(kFull, big)) {
                         // rare (strongly stretched chains): sum the shares as two 32-bit halves and add
@@ -210,7 +213,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                         long long mine = 0;
 #pragma unroll
                         for (int i = 0; i < 12; ++i) {
-                            const long long q = __float2ll_rn(t[i] * scale);
+                            const long long q = __float2ll_rn(t[i]);
                             const int hi = __reduce_add_sync(kFull, (int)(q >> 16));
                             const int lo = __reduce_add_sync(kFull, (int)(q & 0xFFFF));
                             if (lane == i) mine = ((long long)hi << 16) + (long long)lo;
@@ -222,7 +225,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                         // warp's staging rows, which are added to the CTA sums every kStageSteps records
                         int tot[12];
 #pragma unroll
-                        for (int i = 0; i < 12; ++i) tot[i] = __reduce_add_sync(kFull, __float2int_rn(t[i] * scale));
+                        for (int i = 0; i < 12; ++i) tot[i] = __reduce_add_sync(kFull, __float2int_rn(t[i]));
                         if (lane == 0) {
                             row[0] = make_int4(tot[0], tot[1], tot[2], tot[3]);
                             row[1] = make_int4(tot[4], tot[5], tot[6], tot[7]);
@@ -245,7 +248,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
 #pragma unroll
             for (int q = 0; q < 3; ++q) {
                 float z8[8];
-                normal_call(sk, P.rk, DOM_NOISE, chain, (uint32_t)(3 * l + q), P.bm_noise, z8);
+                normal_call(sk, P.rk, DOM_NOISE, chain, (uint32_t)(3 * l + q), bm_noise, z8);
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
                     const int4 fx = Fx4[lane * 7 + 2 * q + h];
@@ -395,7 +398,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                                 const int k = 32 * wd + bit;
                                 const int snew = ((m1 >> bit) & 1u) ? 1 : N;
                                 float z3[3];
-                                anchor_normals(sk, P.rk, DOM_ANCHOR, chain, (uint32_t)k, P.bm_anchor, z3);   // eq 52
+                                anchor_normals(sk, P.rk, DOM_ANCHOR, chain, (uint32_t)k, bm_anchor, z3);   // eq 52
                                 const float4 rb = Rm[rm_index(base + snew - 1)];
                                 const float4 a = make_float4(rb.x + z3[0], rb.y + z3[1], rb.z + z3[2], 0.0f);
                                 Sb[base + Zn] = (unsigned char)snew;
