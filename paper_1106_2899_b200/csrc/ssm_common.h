@@ -35,13 +35,16 @@ constexpr int kSampleShift = 20;             // per-chain slip-spring virial (co
 constexpr int kSmRm = 0;         // float4[288] bead positions mirror (x, y, z, -), padded
 constexpr int kSmA = 4608;       // float4[256] anchors [chain][slot] (x, y, z, x low part)
 constexpr int kSmFx = 8704;      // int  [896]  fixed-point slip-spring displacement per bead coordinate, padded
-constexpr int kSmS = 12288;      // uint8[256]  bead index per slot (0xFF = destroyed in this step)
+constexpr int kSmS = 12288;      // uint8[256]  bead index per slot
 constexpr int kSmZ = 12544;      // int  [32]   Z per chain
 constexpr int kSmX = 12672;      // int  [33]   exclusive prefix of Z over the warp's chains (+ total), padded to 36
 constexpr int kSmEv = 12816;     // uint [64]   creation masks: created at bead 1 / at bead N, [2][chain][word]
 constexpr int kSmSamp = 13072;   // int  [32]   per-chain fixed-point sum of d_x d_y over slip-springs (sample steps)
-constexpr int kStageSteps = 16;  // recorded steps whose warp sums wait in kSmStage before they are added to the CTA sums
-constexpr int kSmStage = 13200;  // int  [16][12] warp sums of the last recorded steps (int32 fixed point)
+constexpr int kStageSteps = 8;   // recorded steps whose warp sums wait in kSmStage before they are added to the CTA sums
+constexpr int kSmStage = 13200;  // int  [8][12] warp sums of the last recorded steps (int32 fixed point)
+constexpr int kSmDm = 13584;     // uint [32]   destruction masks [chain][word]: bit j = slip-spring j was destroyed in this step
+constexpr int kSmMap = 13712;    // uint8[128]  dealing map: byte 4 lane + it = (chain << log2 N) | slot of the warp's
+                                 //             slip-spring number lane + 32 it (it = 0..3), rebuilt when some Z changes
 constexpr int kSmWarp = 13968;
 constexpr int kSmAcc = kWarpsPerBlock * kSmWarp;                          // int64 [kMaxFuse][12] per CTA
 constexpr int kSmStep = kSmAcc + kMaxFuse * 12 * 8;                       // 114,816 B: 2 CTAs per SM (2 x (114,816 + 1024) <= 233,472)

@@ -13,6 +13,8 @@
 // Mapping and layouts: ssm_common.h and DESIGN.md section 6.
 #include <cuda_runtime.h>
 
+#include <type_traits>
+
 #include "ssm_common.h"
 #include "ssm_rng.cuh"
 
@@ -35,7 +37,7 @@ __device__ __forceinline__ float mufu_ex2(float x)
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kEvStride = 32;     // words per event-mask type
 
-template <int G>
+template <int G, bool SHEAR>
 __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid_constant__ StepParams P)
 {
     constexpr int N = kBPL * G, CPW = 32 / G, LG = Log2<G>::v, LN = LG + 3, WPC = (N + 31) / 32;
@@ -52,6 +54,8 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     int *Zs = reinterpret_cast<int *>(wb + kSmZ);
     int *Xp = reinterpret_cast<int *>(wb + kSmX);
     unsigned *Ev = reinterpret_cast<unsigned *>(wb + kSmEv);
+    unsigned *Dm = reinterpret_cast<unsigned *>(wb + kSmDm);
+    unsigned char *Map = wb + kSmMap;
     int *Samp = reinterpret_cast<int *>(wb + kSmSamp);
     int *Stage = reinterpret_cast<int *>(wb + kSmStage);
     int4 *Stage4 = reinterpret_cast<int4 *>(wb + kSmStage);
@@ -61,6 +65,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     for (int i = threadIdx.x; i < kMaxFuse * 12; i += kBlockThreads) acc[i] = 0ull;
     for (int i = lane; i < 2 * kEvStride; i += 32) Ev[i] = 0u;
     Samp[lane] = 0;
+    Dm[lane] = 0u;
     __syncthreads();
 
     // exclusive prefix of Z over the warp's chains: slip-spring f of the warp (0 <= f < Tz)
@@ -82,6 +87,27 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
         for (int st = CPW / 2; st >= 1; st >>= 1)
             if (f >= Xp[c + st]) c += st;
         j = f - Xp[c];
+    };
+
+    // dealing cache: byte it of cj = (c << LN) | j of this lane's slip-spring number lane + 32 it
+    // (it = 0..3).  It only changes when some Z of the warp changes, so it is rebuilt after
+    // rescan(): the lanes of a chain write the entries of their chain's slip-springs into Map.
+    unsigned cj = 0u;
+    auto remap = [&]() {
+        const int z = Zs[cw], x0 = Xp[cw];
+        for (int j = l; j < z; j += G) {
+            const int f = x0 + j;
+            if (f < 128) Map[((f & 31) << 2) | (f >> 5)] = (unsigned char)((cw << LN) | j);
+        }
+        __syncwarp();
+        cj = reinterpret_cast<const unsigned *>(Map)[lane];
+    };
+    // (c << LN) | j of slip-spring number f = lane + 32 it of the warp (f < Tz)
+    auto slot_index = [&](int it, int f) -> int {
+        if (it < 4) return (int)((cj >> (8 * it)) & 0xFFu);
+        int c, j;
+        locate(f, c, j);
+        return (c << LN) | j;
     };
 
     // add the staged warp sums of records [r0, r1) to the CTA's 64-bit sums
@@ -125,14 +151,13 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
         rescan();
         __syncwarp();
         int Tz = Xp[CPW];
+        remap();
 
         // forces of the loaded state: scatter -dt (3/N_s) (R_S - A) of every slip-spring into
         // the fixed-point accumulators of bead S (eq 1; used by the first bead phase)
         if (P.springs_on) {
-            for (int f = lane; f < Tz; f += 32) {
-                int c, j;
-                locate(f, c, j);
-                const int base = c << LN, sidx = base + j;
+            for (int it = 0, f = lane; f < Tz; f += 32, ++it) {
+                const int sidx = slot_index(it, f), base = sidx & ~(N - 1);
                 const int s = Sb[sidx];
                 const float4 a = A4[sidx], rb = Rm[rm_index(base + s - 1)];
                 int *fp = Fx + fx_index(base + s - 1);
@@ -260,7 +285,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                         const float lap = b[f] - (k == 0 ? bl[c] : b[f - 3]);
                         float inc = fmaf(P.dt3, lap, z8[4 * h + e]);
                         inc = fmaf((float)fxa[e], 1.0f / (float)(1 << kFxShift), inc);
-                        if (c == 0) inc = fmaf(P.gdt, r[f + 1], inc);
+                        if (SHEAR && c == 0) inc = fmaf(P.gdt, r[f + 1], inc);
                         r[f] += inc;
                     }
                 }
@@ -275,66 +300,93 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
             cnt = 0.0f;
             if (P.springs_on) {
                 bool event = false;
-                for (int f = lane; f < Tz; f += 32) {
-                    int c, j;
-                    locate(f, c, j);
-                    const int base = c << LN, sidx = base + j;
-                    uint32_t w[4];
-                    stream_call(sk, P.rk, DOM_SLOT, chain0 + (uint32_t)c, (uint32_t)(j >> 1), w);
-                    const uint32_t w_hop = (j & 1) ? w[2] : w[0], w_end = (j & 1) ? w[3] : w[1];
-                    const int s = Sb[sidx];                                   // 1..N
-                    float4 a = A4[sidx];
-                    if (P.gdt != 0.0f) {
-                        // eq 45 with kappa_xy only: A_x += dt gamma_dot A_y, as a compensated
-                        // (two-sum) update of (A_x, low part): the increment is the same every
-                        // step, so a plain fp32 sum would drift linearly instead of randomly
-                        const float t = fmaf(P.gdt, a.y, a.w);
-                        const float sum = a.x + t;
-                        const float bb = sum - a.x;
-                        a.w = (a.x - (sum - bb)) + (t - bb);
-                        a.x = sum;
-                        A4[sidx] = a;
+                // U slip-springs per lane in one straight-line pass (numbers lane + 32 (it0 + u)), so
+                // that the U Philox chains and the U dependent load -> exp -> compare -> scatter
+                // chains overlap
+                auto slot_round = [&](auto U_, int it0) {
+                    constexpr int U = decltype(U_)::value;
+                    int sx[U], s[U];
+                    bool act[U];
+                    uint32_t w_hop[U], w_end[U];
+                    float4 a[U];
+#pragma unroll
+                    for (int u = 0; u < U; ++u) {
+                        const int f = lane + 32 * (it0 + u);
+                        act[u] = f < Tz;
+                        sx[u] = slot_index(it0 + u, act[u] ? f : 0);
+                        const int c = sx[u] >> LN, j = sx[u] & (N - 1);
+                        uint32_t w[4];
+                        stream_call(sk, P.rk, DOM_SLOT, chain0 + (uint32_t)c, (uint32_t)(j >> 1), w);
+                        w_hop[u] = (j & 1) ? w[2] : w[0];
+                        w_end[u] = (j & 1) ? w[3] : w[1];
+                        s[u] = max((int)Sb[sx[u]], 1);       // 1..N (an idle lane may look at an empty slot: any bead will do)
+                        a[u] = A4[sx[u]];
                     }
-                    // Glauber hop (eqs 23, 24 with the cap of eqs 48, 49):
-                    // p+- = min{ h [1 - tanh x+-], 1/2 } = min{ 2h / (1 + e^{2 x+-}), 1/2 },
-                    // x+- = (3/4N_s)(|R_{s+-1}-A|^2 - |R_s-A|^2)
-                    //     = (3/4N_s)(R_{s+-1}-R_s).(R_{s+-1}+R_s-2A)   (no cancellation)
-                    const float4 r0 = Rm[rm_index(base + s - 1)];
-                    const float4 rp = Rm[rm_index(base + (s < N ? s : N - 1))];
-                    const float4 rm = Rm[rm_index(base + (s > 1 ? s - 2 : 0))];
-                    const float ax2 = 2.0f * a.x, ay2 = 2.0f * a.y, az2 = 2.0f * a.z;
-                    float dp = (rp.x - r0.x) * ((rp.x + r0.x) - ax2);
-                    dp = fmaf(rp.y - r0.y, (rp.y + r0.y) - ay2, dp);
-                    dp = fmaf(rp.z - r0.z, (rp.z + r0.z) - az2, dp);
-                    float dm = (rm.x - r0.x) * ((rm.x + r0.x) - ax2);
-                    dm = fmaf(rm.y - r0.y, (rm.y + r0.y) - ay2, dm);
-                    dm = fmaf(rm.z - r0.z, (rm.z + r0.z) - az2, dm);
-                    float pp = fminf(__fdividef(P.h2, 1.0f + mufu_ex2(P.q2l * dp)), 0.5f);
-                    float pm = fminf(__fdividef(P.h2, 1.0f + mufu_ex2(P.q2l * dm)), 0.5f);
-                    if (s == N) pp = 0.0f;
-                    if (s == 1) pm = 0.0f;
-                    const float u = u23(w_hop);
-                    int sn = s;
-                    float4 rn = r0;
-                    if (u < pp) { sn = s + 1; rn = rp; }
-                    else if (u < pp + pm) { sn = s - 1; rn = rm; }
-                    // destruction at the ends (eq 53), integer-domain comparison
-                    const bool destroyed = (sn == 1 || sn == N) && code23(w_end) < P.t_destroy;
-                    event |= destroyed;
-                    if (destroyed || sn != s) Sb[sidx] = (unsigned char)(destroyed ? 0xFF : sn);   // 0xFF: removed in the rare path
-                    // a destroyed slip-spring exerts no force and has no virial: zero displacement
-                    const float dx = destroyed ? 0.0f : rn.x - a.x, dy = destroyed ? 0.0f : rn.y - a.y,
-                                dz = destroyed ? 0.0f : rn.z - a.z;
-                    int *fp = Fx + fx_index(base + sn - 1);
-                    atomicAdd(fp, __float2int_rn(-P.fx_scale * dx));
-                    atomicAdd(fp + 1, __float2int_rn(-P.fx_scale * dy));
-                    atomicAdd(fp + 2, __float2int_rn(-P.fx_scale * dz));
-                    if (record) {
+#pragma unroll
+                    for (int u = 0; u < U; ++u) {
+                        const int base = sx[u] & ~(N - 1);
+                        if (SHEAR) {
+                            // eq 45 with kappa_xy only: A_x += dt gamma_dot A_y, as a compensated
+                            // (two-sum) update of (A_x, low part): the increment is the same every
+                            // step, so a plain fp32 sum would drift linearly instead of randomly
+                            const float t = fmaf(P.gdt, a[u].y, a[u].w);
+                            const float sum = a[u].x + t;
+                            const float bb = sum - a[u].x;
+                            a[u].w = (a[u].x - (sum - bb)) + (t - bb);
+                            a[u].x = sum;
+                            if (act[u]) A4[sx[u]] = a[u];
+                        }
+                        // Glauber hop (eqs 23, 24 with the cap of eqs 48, 49):
+                        // p+- = min{ h [1 - tanh x+-], 1/2 } = min{ 2h / (1 + e^{2 x+-}), 1/2 },
+                        // x+- = (3/4N_s)(|R_{s+-1}-A|^2 - |R_s-A|^2)
+                        const int b0 = base + s[u] - 1;
+                        const float4 r0 = Rm[rm_index(b0)];
+                        const float4 rp = Rm[rm_index(b0 + (s[u] < N ? 1 : 0))];
+                        const float4 rm = Rm[rm_index(b0 - (s[u] > 1 ? 1 : 0))];
+                        const float d0x = r0.x - a[u].x, d0y = r0.y - a[u].y, d0z = r0.z - a[u].z;
+                        const float dpx = rp.x - a[u].x, dpy = rp.y - a[u].y, dpz = rp.z - a[u].z;
+                        const float dmx = rm.x - a[u].x, dmy = rm.y - a[u].y, dmz = rm.z - a[u].z;
+                        const float e0 = fmaf(d0z, d0z, fmaf(d0y, d0y, d0x * d0x));
+                        const float ep = fmaf(dpz, dpz, fmaf(dpy, dpy, dpx * dpx));
+                        const float em = fmaf(dmz, dmz, fmaf(dmy, dmy, dmx * dmx));
+                        float pp = fminf(__fdividef(P.h2, 1.0f + mufu_ex2(P.q2l * (ep - e0))), 0.5f);
+                        float pm = fminf(__fdividef(P.h2, 1.0f + mufu_ex2(P.q2l * (em - e0))), 0.5f);
+                        if (s[u] == N) pp = 0.0f;
+                        if (s[u] == 1) pm = 0.0f;
+                        const float uu = u23(w_hop[u]);
+                        const bool up = uu < pp, dn = !up && uu < pp + pm;
+                        const int sn = s[u] + (up ? 1 : 0) - (dn ? 1 : 0);
+                        // destruction at the ends (eq 53), integer-domain comparison
+                        const bool destroyed = (sn == 1 || sn == N) && code23(w_end[u]) < P.t_destroy;
+                        const bool live = act[u] && !destroyed;
+                        if (act[u] && sn != s[u]) Sb[sx[u]] = (unsigned char)sn;
+                        if (act[u] && destroyed) {
+                            const int j = sx[u] & (N - 1);
+                            atomicOr(Dm + (sx[u] >> LN) * WPC + (j >> 5), 1u << (j & 31));
+                            event = true;
+                        }
+                        // a destroyed slip-spring exerts no force and has no virial: zero displacement
+                        const float dx = live ? (up ? dpx : (dn ? dmx : d0x)) : 0.0f;
+                        const float dy = live ? (up ? dpy : (dn ? dmy : d0y)) : 0.0f;
+                        const float dz = live ? (up ? dpz : (dn ? dmz : d0z)) : 0.0f;
+                        if (live) {
+                            int *fp = Fx + fx_index(b0 + sn - s[u]);
+                            atomicAdd(fp, __float2int_rn(-P.fx_scale * dx));
+                            atomicAdd(fp + 1, __float2int_rn(-P.fx_scale * dy));
+                            atomicAdd(fp + 2, __float2int_rn(-P.fx_scale * dz));
+                        }
                         sv[0] = fmaf(dx, dx, sv[0]); sv[1] = fmaf(dy, dy, sv[1]); sv[2] = fmaf(dz, dz, sv[2]);
                         sv[3] = fmaf(dx, dy, sv[3]); sv[4] = fmaf(dy, dz, sv[4]); sv[5] = fmaf(dz, dx, sv[5]);
-                        cnt += destroyed ? 0.0f : 1.0f;
+                        cnt += live ? 1.0f : 0.0f;
+                        if (sample && live) atomicAdd(Samp + (sx[u] >> LN), __float2int_rn(dx * dy * (float)(1 << kSampleShift)));
                     }
-                    if (sample) atomicAdd(Samp + c, __float2int_rn(dx * dy * (float)(1 << kSampleShift)));
+                };
+                {
+                    const int nit = (Tz + 31) >> 5;
+                    int it0 = 0;
+                    // (two slip-springs per lane per pass was measured slower: the larger loop body
+                    // costs more instruction-fetch stalls than the overlap wins)
+                    for (; it0 < nit; ++it0) slot_round(std::integral_constant<int, 1>(), it0);
                 }
                 // construction attempts (eqs 50, 51), drawn by the chain's own lanes: attempt k
                 // uses word k&3 of call k>>2; K = N - Z or a fixed K
@@ -374,17 +426,18 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                         const int base = cw << LN;
                         int Zn = Z0;
                         bool changed = false;
-                        for (int wd = (Z0 - 1) >> 2; wd >= 0; --wd) {
-                            unsigned m = __vcmpeq4(reinterpret_cast<const unsigned *>(Sb + base)[wd], 0xFFFFFFFFu);
+#pragma unroll
+                        for (int wd = WPC - 1; wd >= 0; --wd) {
+                            unsigned m = Dm[cw * WPC + wd];
+                            if (m) { Dm[cw * WPC + wd] = 0u; changed = true; }
                             while (m) {
-                                const int bit = 31 - __clz(m);            // highest marked byte first
-                                m &= ~(0xFFu << (bit & 24));
-                                const int j = 4 * wd + (bit >> 3);
+                                const int bit = 31 - __clz(m);            // highest slot first
+                                m &= ~(1u << bit);
+                                const int j = 32 * wd + bit;
                                 --Zn;
                                 if (j != Zn) { Sb[base + j] = Sb[base + Zn]; A4[base + j] = A4[base + Zn]; }
                                 Sb[base + Zn] = 0;
                                 A4[base + Zn] = make_float4(0.f, 0.f, 0.f, 0.f);
-                                changed = true;
                             }
                         }
 #pragma unroll
@@ -423,6 +476,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     rescan();
                     __syncwarp();
                     Tz = Xp[CPW];
+                    remap();
                 }
             }
             __syncwarp();
@@ -458,25 +512,32 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
 // ---------------------------------------------------------------------------------------
 // host-side launcher
 // ---------------------------------------------------------------------------------------
-template <int G>
-static cudaError_t launch_g(const StepParams &p, int grid, cudaStream_t st)
+template <int G, bool SHEAR>
+static cudaError_t launch_gs(const StepParams &p, int grid, cudaStream_t st)
 {
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(ssm_step_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmStep);
+        cudaError_t e = cudaFuncSetAttribute(ssm_step_kernel<G, SHEAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmStep);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    ssm_step_kernel<G><<<grid, kBlockThreads, kSmStep, st>>>(p);
+    ssm_step_kernel<G, SHEAR><<<grid, kBlockThreads, kSmStep, st>>>(p);
     return cudaGetLastError();
+}
+
+// the affine term of eqs 44, 45 is compiled in only when a velocity gradient is applied
+template <int G>
+static cudaError_t launch_g(const StepParams &p, int grid, cudaStream_t st)
+{
+    return p.gdt != 0.0f ? launch_gs<G, true>(p, grid, st) : launch_gs<G, false>(p, grid, st);
 }
 
 template <int G>
 static cudaError_t occupancy_g(int *blocks_per_sm)
 {
-    cudaError_t e = cudaFuncSetAttribute(ssm_step_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmStep);
+    cudaError_t e = cudaFuncSetAttribute(ssm_step_kernel<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmStep);
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, ssm_step_kernel<G>, kBlockThreads, kSmStep);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, ssm_step_kernel<G, true>, kBlockThreads, kSmStep);
 }
 
 cudaError_t step_occupancy(int n_beads, int *blocks_per_sm)
