@@ -312,10 +312,16 @@ void oracle_step_chain(const oracle_params *p, uint64_t chain, uint64_t step, do
     if (K > 0) {
         const double pc = fmin(h / (p->n_0 * (double)K), 0.5);
         const int64_t T1 = oracle_threshold23(pc), T2 = oracle_threshold23(2.0 * pc);
+        uint32_t w[4] = {0, 0, 0, 0};
         for (int k = 0; k < K; ++k) {
-            uint32_t w[4];
-            oracle_stream(p->seed, ORACLE_DOM_ATTEMPT, step, chain, (uint32_t)(k >> 2), w);
-            int64_t code = (int64_t)oracle_code23(w[k & 3]);
+            /* uniform of attempt k (reading R22): u = (code + 1/2) 2^-23 with the 23-bit
+             * code = (h << 7) | e; h = 16-bit half (k&1) of word (k&7)>>1 of ATTEMPT call k>>3,
+             * e = top 7 bits of word 2 of ANCHOR call k (whose words 0, 1 give the anchor offset) */
+            uint32_t wa[4];
+            if ((k & 7) == 0) oracle_stream(p->seed, ORACLE_DOM_ATTEMPT, step, chain, (uint32_t)(k >> 3), w);
+            oracle_stream(p->seed, ORACLE_DOM_ANCHOR, step, chain, (uint32_t)k, wa);
+            uint32_t h = (w[(k & 7) >> 1] >> (16 * (k & 1))) & 0xFFFFu;
+            int64_t code = (int64_t)((h << 7) | (wa[2] >> 25));
             int snew = 0;
             if (code < T1) snew = 1;
             else if (code < T2) snew = N;

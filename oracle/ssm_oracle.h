@@ -15,8 +15,9 @@ extern "C" {
 enum {
     ORACLE_DOM_NOISE = 0,       /* step noise: normal m = 3*bead + axis = normal m&7 of call m>>3 */
     ORACLE_DOM_SLOT = 1,        /* call j>>1: words 2(j&1), 2(j&1)+1 = u_hop, u_end of j  */
-    ORACLE_DOM_ATTEMPT = 2,     /* call k>>2: word k&3 = uniform of construction attempt k*/
-    ORACLE_DOM_ANCHOR = 3,      /* call k: normals 0..2 = anchor offset of attempt k      */
+    ORACLE_DOM_ATTEMPT = 2,     /* call k>>3: half k&1 of word (k&7)>>1 = high 16 bits of the 23-bit code of attempt k */
+    ORACLE_DOM_ANCHOR = 3,      /* call k: normals 0..2 (words 0, 1) = anchor offset of attempt k; top 7 bits of word 2 =
+                                   low 7 bits of its 23-bit code */
     ORACLE_DOM_INIT_BOND = 4,   /* step 0: normal m = 3*bond + axis                       */
     ORACLE_DOM_INIT_Z = 5,      /* step 0, call 0, word 0 -> Z                            */
     ORACLE_DOM_INIT_SLOT = 6,   /* step 0, call j, word 0 -> S_j                          */

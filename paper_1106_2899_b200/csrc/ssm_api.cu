@@ -192,7 +192,7 @@ extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, s
     for (int K = 1; K <= 128; ++K) {
         const double pc = c->springs_on ? std::fmin(h / (p->n_0 * (double)K), 0.5) : 0.0;
         sp.t_c1[K] = threshold23(pc); sp.t_c2[K] = threshold23(2.0 * pc);
-        sp.w_c2[K] = sp.t_c2[K] ? (unsigned)((((unsigned long long)sp.t_c2[K]) << 9) - 1ull) : 0u;
+        sp.h_c2[K] = sp.t_c2[K] ? (int)((sp.t_c2[K] - 1u) >> 7) : -1;
     }
 
     InitParams ip;

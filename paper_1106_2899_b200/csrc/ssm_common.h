@@ -38,7 +38,7 @@ constexpr int kSmFx = 8704;      // int  [896]  fixed-point slip-spring displace
 constexpr int kSmS = 12288;      // uint8[256]  bead index per slot
 constexpr int kSmZ = 12544;      // int  [32]   Z per chain
 constexpr int kSmX = 12672;      // int  [33]   exclusive prefix of Z over the warp's chains (+ total), padded to 36
-constexpr int kSmEv = 12816;     // uint [64]   creation masks: created at bead 1 / at bead N, [2][chain][word]
+constexpr int kSmEv = 12816;     // uint [32]   construction candidates [chain][word]: bit k = attempt k passed the 16-bit test (+128 B spare)
 constexpr int kSmSamp = 13072;   // int  [32]   per-chain fixed-point sum of d_x d_y over slip-springs (sample steps)
 constexpr int kStageSteps = 8;   // recorded steps whose warp sums wait in kSmStage before they are added to the CTA sums
 constexpr int kSmStage = 13200;  // int  [8][12] warp sums of the last recorded steps (int32 fixed point)
@@ -76,8 +76,8 @@ struct StepParams {
     float cs;         // 3/N_s                (eq 76)
     unsigned t_destroy;               // T(min{dt/zeta_s, 1})                 (eq 53)
     unsigned t_c1[129], t_c2[129];    // T(p_c(K)), T(2 p_c(K)), K = 1..128   (eqs 50, 51)
-    unsigned w_c2[129];               // largest Philox WORD w with (w >> 9) < T(2 p_c(K)): one compare on the minimum
-                                      // of a call's four words tells whether any of its attempts can succeed
+    int h_c2[129];                    // the 23-bit code of attempt k is (h << 7) | e with a 16-bit h (reading R22):
+                                      // h <= h_c2[K] = (T(2 p_c(K)) - 1) >> 7 is necessary for success (-1: never)
 };
 
 struct InitParams {

@@ -14,8 +14,9 @@ namespace ssm {
 enum : uint32_t {
     DOM_NOISE = 0,        // per step: normal m = 3*bead + axis, call m>>3, normal m&7
     DOM_SLOT = 1,         // per step: call j>>1, words 2(j&1), 2(j&1)+1 = u_hop, u_end of slip-spring j
-    DOM_ATTEMPT = 2,      // per step: call k>>2, word k&3 = uniform of construction attempt k
-    DOM_ANCHOR = 3,       // per step: call k, normals 0..2 = anchor offset of attempt k
+    DOM_ATTEMPT = 2,      // per step: call k>>3, half k&1 of word (k&7)>>1 = high 16 bits of the 23-bit code of attempt k
+    DOM_ANCHOR = 3,       // per step: call k, normals 0..2 (words 0, 1) = anchor offset of attempt k,
+                          //           top 7 bits of word 2 = low 7 bits of its 23-bit code
     DOM_INIT_BOND = 4,    // step 0: normal m = 3*bond + axis
     DOM_INIT_Z = 5,       // step 0, call 0, word 0 -> Z
     DOM_INIT_SLOT = 6,    // step 0, call j, word 0 -> S_j

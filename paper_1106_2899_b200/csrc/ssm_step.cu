@@ -35,7 +35,6 @@ __device__ __forceinline__ float mufu_ex2(float x)
 }
 
 constexpr unsigned kFull = 0xffffffffu;
-constexpr int kEvStride = 32;     // words per event-mask type
 
 template <int G, bool SHEAR>
 __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid_constant__ StepParams P)
@@ -63,7 +62,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
 
     const BoxMuller bm_noise(P.bm_noise), bm_anchor(P.bm_anchor);
     for (int i = threadIdx.x; i < kMaxFuse * 12; i += kBlockThreads) acc[i] = 0ull;
-    for (int i = lane; i < 2 * kEvStride; i += 32) Ev[i] = 0u;
+    Ev[lane] = 0u;
     Samp[lane] = 0;
     Dm[lane] = 0u;
     __syncthreads();
@@ -388,29 +387,28 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     // costs more instruction-fetch stalls than the overlap wins)
                     for (; it0 < nit; ++it0) slot_round(std::integral_constant<int, 1>(), it0);
                 }
-                // construction attempts (eqs 50, 51), drawn by the chain's own lanes: attempt k
-                // uses word k&3 of call k>>2; K = N - Z or a fixed K
+                // construction attempts (eqs 50, 51), drawn by the chain's own lanes; K = N - Z
+                // or a fixed K.  The 23-bit code of attempt k is (h << 7) | e (DESIGN.md
+                // reading R22): h is a 16-bit half of ATTEMPT call k>>3, so ONE call per lane covers the
+                // chain's K <= 8G attempts; e comes from the ANCHOR call, which only a candidate
+                // (h <= (T(2 p_c) - 1) >> 7, about 2e-3 per attempt) ever evaluates.
                 {
                     const int empty = N - Z0;
                     int K = P.k_attempts > 0 ? (P.k_attempts < empty ? P.k_attempts : empty) : empty;
                     if (!valid) K = 0;
-                    if (4 * l < K) {
-                        // a success needs (w >> 9) < T(2 p_c) ~ 2e-3 2^23: one compare on the minimum
-                        // of the call's four words rules out all four attempts
-                        const unsigned wmax = P.w_c2[K];
-                        for (int q = l; 4 * q < K; q += G) {
-                            uint32_t w[4];
-                            stream_call(sk, P.rk, DOM_ATTEMPT, chain, (uint32_t)q, w);
-                            if (min(min(w[0], w[1]), min(w[2], w[3])) <= wmax) {
-                                const unsigned t1 = P.t_c1[K], t2 = P.t_c2[K];
+                    if (8 * l < K) {
+                        uint32_t w[4];
+                        stream_call(sk, P.rk, DOM_ATTEMPT, chain, (uint32_t)l, w);
+                        const int hmax = P.h_c2[K];
+                        const unsigned m2 = __vminu2(__vminu2(w[0], w[1]), __vminu2(w[2], w[3]));
+                        if ((int)min(m2 & 0xFFFFu, m2 >> 16) <= hmax) {
 #pragma unroll
-                                for (int e = 0; e < 4; ++e) {
-                                    const int k = 4 * q + e;
-                                    const unsigned code = code23(w[e]);
-                                    if (k < K && code < t2) {
-                                        atomicOr(Ev + (code < t1 ? 0 : 1) * kEvStride + cw * WPC + (k >> 5), 1u << (k & 31));
-                                        event = true;
-                                    }
+                            for (int e = 0; e < 8; ++e) {
+                                const int k = 8 * l + e;
+                                const int h = (int)((w[e >> 1] >> (16 * (e & 1))) & 0xFFFFu);
+                                if (k < K && h <= hmax) {
+                                    atomicOr(Ev + cw * WPC + (k >> 5), 1u << (k & 31));
+                                    event = true;
                                 }
                             }
                         }
@@ -440,33 +438,40 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                                 A4[base + Zn] = make_float4(0.f, 0.f, 0.f, 0.f);
                             }
                         }
+                        const int K0 = P.k_attempts > 0 ? min(P.k_attempts, N - Z0) : N - Z0;
 #pragma unroll
                         for (int wd = 0; wd < WPC; ++wd) {
-                            const unsigned m1 = Ev[cw * WPC + wd];
-                            unsigned m = m1 | Ev[kEvStride + cw * WPC + wd];
-                            if (m) { Ev[cw * WPC + wd] = 0u; Ev[kEvStride + cw * WPC + wd] = 0u; changed = true; }
+                            unsigned m = Ev[cw * WPC + wd];
+                            if (m) Ev[cw * WPC + wd] = 0u;
                             while (m) {
                                 const int bit = __ffs(m) - 1;
                                 m &= m - 1u;
                                 const int k = 32 * wd + bit;
-                                const int snew = ((m1 >> bit) & 1u) ? 1 : N;
-                                float z3[3];
-                                anchor_normals(sk, P.rk, DOM_ANCHOR, chain, (uint32_t)k, bm_anchor, z3);   // eq 52
+                                // the candidate's full code: 16 bits of its ATTEMPT half, 7 bits of ANCHOR word 2
+                                uint32_t w[4], wa[4];
+                                stream_call(sk, P.rk, DOM_ATTEMPT, chain, (uint32_t)(k >> 3), w);
+                                stream_call(sk, P.rk, DOM_ANCHOR, chain, (uint32_t)k, wa);
+                                const unsigned h = (w[(k & 7) >> 1] >> (16 * (k & 1))) & 0xFFFFu;
+                                const unsigned code = (h << 7) | (wa[2] >> 25);
+                                if (code >= P.t_c2[K0]) continue;
+                                const int snew = code < P.t_c1[K0] ? 1 : N;
+                                float z3[3], unused;
+                                bm_anchor(wa[0], z3[0], z3[1]);                                       // eq 52
+                                bm_anchor(wa[1], z3[2], unused);
                                 const float4 rb = Rm[rm_index(base + snew - 1)];
                                 const float4 a = make_float4(rb.x + z3[0], rb.y + z3[1], rb.z + z3[2], 0.0f);
                                 Sb[base + Zn] = (unsigned char)snew;
                                 A4[base + Zn] = a;
                                 ++Zn;
+                                changed = true;
                                 const float dx = rb.x - a.x, dy = rb.y - a.y, dz = rb.z - a.z;
                                 int *fp = Fx + fx_index(base + snew - 1);
                                 atomicAdd(fp, __float2int_rn(-P.fx_scale * dx));
                                 atomicAdd(fp + 1, __float2int_rn(-P.fx_scale * dy));
                                 atomicAdd(fp + 2, __float2int_rn(-P.fx_scale * dz));
-                                if (record) {
-                                    sv[0] = fmaf(dx, dx, sv[0]); sv[1] = fmaf(dy, dy, sv[1]); sv[2] = fmaf(dz, dz, sv[2]);
-                                    sv[3] = fmaf(dx, dy, sv[3]); sv[4] = fmaf(dy, dz, sv[4]); sv[5] = fmaf(dz, dx, sv[5]);
-                                    cnt += 1.0f;
-                                }
+                                sv[0] = fmaf(dx, dx, sv[0]); sv[1] = fmaf(dy, dy, sv[1]); sv[2] = fmaf(dz, dz, sv[2]);
+                                sv[3] = fmaf(dx, dy, sv[3]); sv[4] = fmaf(dy, dz, sv[4]); sv[5] = fmaf(dz, dx, sv[5]);
+                                cnt += 1.0f;
                                 if (sample) atomicAdd(Samp + cw, __float2int_rn(dx * dy * (float)(1 << kSampleShift)));
                             }
                         }
