@@ -67,19 +67,9 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     Dm[lane] = 0u;
     __syncthreads();
 
-    // exclusive prefix of Z over the warp's chains: slip-spring f of the warp (0 <= f < Tz)
-    // belongs to the chain c with Xp[c] <= f < Xp[c+1] and is its slot f - Xp[c]
-    auto rescan = [&]() {
-        const int z = lane < CPW ? Zs[lane] : 0;
-        int incl = z;
-#pragma unroll
-        for (int o = 1; o < CPW; o <<= 1) {
-            const int t = __shfl_up_sync(kFull, incl, o);
-            if (lane >= o) incl += t;
-        }
-        if (lane < CPW) Xp[lane + 1] = incl;
-        if (lane == 0) Xp[0] = 0;
-    };
+    // dealing: slip-spring f of the warp (0 <= f < Tz) belongs to the chain c with
+    // Xp[c] <= f < Xp[c+1] (Xp = exclusive prefix of Z over the warp's chains) and is its slot
+    // f - Xp[c]
     auto locate = [&](int f, int &c, int &j) {
         c = 0;
 #pragma unroll
@@ -89,17 +79,30 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     };
 
     // dealing cache: byte it of cj = (c << LN) | j of this lane's slip-spring number lane + 32 it
-    // (it = 0..3).  It only changes when some Z of the warp changes, so it is rebuilt after
-    // rescan(): the lanes of a chain write the entries of their chain's slip-springs into Map.
+    // (it = 0..3).  It only changes when some Z of the warp changes.  deal(z) takes the Z of the
+    // lane's own chain, forms the prefix over the chains with shuffles (every lane of a chain
+    // holds the same z, so a scan over lanes with strides G, 2G, .. is a scan over chains), lets
+    // the lanes of a chain write the entries of their chain's slip-springs into Map, and returns
+    // the warp's total Tz.  Xp is kept for locate(), which serves slip-springs number >= 128 only.
     unsigned cj = 0u;
-    auto remap = [&]() {
-        const int z = Zs[cw], x0 = Xp[cw];
+    auto deal = [&](int z) -> int {
+        int incl = z;
+#pragma unroll
+        for (int o = G; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(kFull, incl, o);
+            if (lane >= o) incl += t;
+        }
+        const int total = __shfl_sync(kFull, incl, 31);
+        const int x0 = incl - z;
+        if (l == 0) Xp[cw + 1] = incl;
+        if (lane == 0) Xp[0] = 0;
         for (int j = l; j < z; j += G) {
             const int f = x0 + j;
             if (f < 128) Map[((f & 31) << 2) | (f >> 5)] = (unsigned char)((cw << LN) | j);
         }
         __syncwarp();
         cj = reinterpret_cast<const unsigned *>(Map)[lane];
+        return total;
     };
     // (c << LN) | j of slip-spring number f = lane + 32 it of the warp (f < Tz)
     auto slot_index = [&](int it, int f) -> int {
@@ -147,10 +150,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
             for (int k = 0; k < 8; ++k) Rm[lane * 9 + k] = make_float4(r[3 * k], r[3 * k + 1], r[3 * k + 2], 0.0f);
         }
         __syncwarp();
-        rescan();
-        __syncwarp();
-        int Tz = Xp[CPW];
-        remap();
+        int Tz = deal(Zs[cw]);
 
         // forces of the loaded state: scatter -dt (3/N_s) (R_S - A) of every slip-spring into
         // the fixed-point accumulators of bead S (eq 1; used by the first bead phase)
@@ -416,13 +416,13 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                 }
                 if (__any_sync(kFull, event)) {
                     __syncwarp();
+                    int Zn = Z0;
                     if (l == 0) {
                         // rare path, one lane per chain: re-index the chain's slip-springs so that
                         // they occupy slots 0..Z-1.  Destroyed ones are visited from the
                         // last to the first and replaced by the last one; new ones are appended in
                         // attempt order (reading R21).
                         const int base = cw << LN;
-                        int Zn = Z0;
                         bool changed = false;
 #pragma unroll
                         for (int wd = WPC - 1; wd >= 0; --wd) {
@@ -478,10 +478,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                         if (changed) Zs[cw] = Zn;
                     }
                     __syncwarp();
-                    rescan();
-                    __syncwarp();
-                    Tz = Xp[CPW];
-                    remap();
+                    Tz = deal(__shfl_sync(kFull, Zn, cw << LG));
                 }
             }
             __syncwarp();
