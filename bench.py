@@ -30,7 +30,7 @@ if ROOT not in sys.path:
 # Frozen algorithmic thread-instruction count per bead-update of the N = 32, <Z> = 8 step
 # (DESIGN.md section 9.2).  The roofline numerator is I_ALG x bead-updates/s, NOT the number
 # of instructions the kernel happens to execute, so padding cannot raise the fraction.
-I_ALG = 100.0
+I_ALG = 95.0
 N_SM, SMSP_PER_SM, LANES = 148, 4, 32
 
 
@@ -55,6 +55,23 @@ def measured_peaks():
         d = json.load(open(p))
         return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)), "source": "measured"}
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
+
+
+def ncu_traffic(n_beads, n_chains):
+    """DRAM bytes per launch of the step kernel (dram__bytes_read.sum + dram__bytes_write.sum)
+    from the committed `ncu --set full` capture of this workload; None for other workloads."""
+    if (n_beads, n_chains) != (32, 1 << 20):
+        return None
+    path = os.path.join(ROOT, "profiles", "r1_v4_step_kernel_metrics.csv")
+    try:
+        import csv
+        tot = 0.0
+        for name, unit, value in csv.reader(open(path)):
+            if name in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                tot += float(value) * {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}[unit]
+        return tot or None
+    except (OSError, ValueError, KeyError):
+        return None
 
 
 class ClockSampler:
@@ -254,13 +271,7 @@ def main():
     # (7552 B per 256 beads = 29.5 N per chain: anchors are float4 with the low part of x, plus Z)
     alg_bytes = 2.0 * 25.0 * N * M
     hbm_achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tp):
-        try:
-            traffic = json.load(open(tp)).get("dram_bytes_per_launch")
-        except Exception:
-            traffic = None
+    traffic = ncu_traffic(N, M)
     line = {
         "metric": "bead-updates/s", "value": value, "unit": "bead-updates/s", "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
