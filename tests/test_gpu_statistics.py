@@ -138,6 +138,48 @@ def test_full_size_c4_in_the_bench_launch_configuration(ssm):
     assert np.all(np.abs(s[:, 3:6]) < 0.03) and np.all(np.abs(s[:, 9:]) < 0.03)  # no flow: shear components vanish
 
 
+@pytest.mark.parametrize("N,M,dt,rate,seed", [(16, 65536, 0.01, 0.0, 2), (32, 262144, 0.01, 0.1, 3), (128, 131072, 0.005, 1e-3, 5)])
+def test_full_size_c2_c3_c5_sampled_chains(ssm, N, M, dt, rate, seed):
+    """BASELINE.json configs[1], [2], [4] at their full ensemble sizes (65,536 x 16; 262,144 x 32 under
+    start-up shear; 131,072 x 128 at dt = 0.005 under shear: the shared-memory-resident long chains),
+    default launch geometry: sampled chains re-run one by one by the oracle from the GPU's own
+    initial state, and the any-size slot invariants on all chains."""
+    steps = 48
+    g = ssm.Ensemble(N, M, dt=dt, seed=seed, stress_every=10, stress_capacity=8, sample_every=10,
+                     corr_levels=4, corr_bins=16, corr_groups=32)
+    R0, A0, S0, _ = g.get_state()
+    g.step(steps, shear_rate=rate)
+    R1, A1, S1, step = g.get_state()
+    assert step == steps
+    rng = np.random.default_rng(seed)
+    picks = np.unique(np.concatenate([[0, 1, M - 2, M - 1], rng.integers(0, M, 28)]))
+    compared = 0
+    for k in picks:
+        e = oracle.Ensemble(N, 1, dt=dt, seed=seed, chain_offset=int(k), init=False)
+        Rk, Ak, Sk, Zk = from_external(R0[:, :, k:k + 1], A0[:, :, k:k + 1], S0[:, k:k + 1])
+        e.R[:], e.A[:], e.S[:], e.Z[:] = Rk, Ak, Sk, Zk
+        e.run(steps, shear_rate=rate, guard=GUARD)
+        if e.first_fragile[0] >= 0:
+            continue
+        Rg, Ag, Sg, Zg = from_external(R1[:, :, k:k + 1], A1[:, :, k:k + 1], S1[:, k:k + 1])
+        assert np.array_equal(Sg, e.S) and np.array_equal(Zg, e.Z), "chain %d: slip-spring indices differ" % k
+        ok, w = close(Rg, e.R)
+        assert ok, "chain %d: positions off by %.3g" % (k, w)
+        occ = e.S > 0
+        ok, w = close(Ag[occ], e.A[occ])
+        assert ok, "chain %d: anchors off by %.3g" % (k, w)
+        compared += 1
+    assert compared >= len(picks) - (4 if N < 128 else 12)
+    occ = S1 > 0
+    Z = occ.sum(0)
+    assert np.array_equal(occ, np.arange(N)[:, None] < Z[None, :])
+    assert S1.max() <= N and Z.max() <= N
+    assert abs(Z.mean() - N / 4.0) < 0.02 * N
+    assert g.stress().shape == (4, 12)
+    t, G, se = g.gt()
+    assert len(t) > 0 and np.all(np.isfinite(G)) and abs(G[0] * N / (N - 1) - 1.0) < 0.1
+
+
 def test_edge_cases(ssm):
     # one chain, and chain counts that leave a ragged warp tile, against the oracle
     for N, M in ((8, 1), (16, 3), (128, 1)):
