@@ -38,7 +38,7 @@ constexpr int kSmFx = 8704;      // int  [896]  fixed-point slip-spring displace
 constexpr int kSmS = 12288;      // uint8[256]  bead index per slot
 constexpr int kSmZ = 12544;      // int  [32]   Z per chain
 constexpr int kSmX = 12672;      // int  [33]   exclusive prefix of Z over the warp's chains (+ total), padded to 36
-constexpr int kSmEv = 12816;     // uint [32]   construction candidates [chain][word]: bit k = attempt k passed the 16-bit test (+128 B spare)
+constexpr int kSmEv = 12816;     // uint [64]   construction candidates [chain][word]: bit k = attempt k passed the 16-bit test; [32 + chain] = (k << 16) | half of the chain's latest candidate
 constexpr int kSmSamp = 13072;   // int  [32]   per-chain fixed-point sum of d_x d_y over slip-springs (sample steps)
 constexpr int kStageSteps = 8;   // recorded steps whose warp sums wait in kSmStage before they are added to the CTA sums
 constexpr int kSmStage = 13200;  // int  [8][12] warp sums of the last recorded steps (int32 fixed point)

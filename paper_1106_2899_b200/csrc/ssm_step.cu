@@ -408,6 +408,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                                 const int h = (int)((w[e >> 1] >> (16 * (e & 1))) & 0xFFFFu);
                                 if (k < K && h <= hmax) {
                                     atomicOr(Ev + cw * WPC + (k >> 5), 1u << (k & 31));
+                                    Ev[32 + cw] = ((unsigned)k << 16) | (unsigned)h;   // the chain's latest candidate and its half
                                     event = true;
                                 }
                             }
@@ -448,10 +449,15 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                                 m &= m - 1u;
                                 const int k = 32 * wd + bit;
                                 // the candidate's full code: 16 bits of its ATTEMPT half, 7 bits of ANCHOR word 2
-                                uint32_t w[4], wa[4];
-                                stream_call(sk, P.rk, DOM_ATTEMPT, chain, (uint32_t)(k >> 3), w);
+                                uint32_t wa[4];
                                 stream_call(sk, P.rk, DOM_ANCHOR, chain, (uint32_t)k, wa);
-                                const unsigned h = (w[(k & 7) >> 1] >> (16 * (k & 1))) & 0xFFFFu;
+                                const unsigned cd = Ev[32 + cw];
+                                unsigned h = cd & 0xFFFFu;
+                                if ((cd >> 16) != (unsigned)k) {       // several candidates in one chain: draw the half again
+                                    uint32_t w[4];
+                                    stream_call(sk, P.rk, DOM_ATTEMPT, chain, (uint32_t)(k >> 3), w);
+                                    h = (w[(k & 7) >> 1] >> (16 * (k & 1))) & 0xFFFFu;
+                                }
                                 const unsigned code = (h << 7) | (wa[2] >> 25);
                                 if (code >= P.t_c2[K0]) continue;
                                 const int snew = code < P.t_c1[K0] ? 1 : N;
