@@ -46,6 +46,8 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=20.0)
+    ap.add_argument("--table1", action="store_true",
+                    help="context only: the paper's Table 1 shapes (65,536 beads, 1e4 steps) timed on this GPU")
     return ap.parse_args()
 
 
@@ -167,10 +169,34 @@ def workload_config(a, chains_per_gpu, inner, world):
                    if a.impl == "ours" else "CPU arm: bounded sample of the workload on the host cores")}
 
 
+def run_table1():
+    """PAPER.md Table 1 (lines 706-719): N x M = 16x4096 .. 128x512 (65,536 beads), dt = 0.01, 1e4 steps
+    from the equilibrium start, shear rate 0 and 0.05, K = N - Z.  Context beside the paper's
+    own times (Tesla C1060); 65,536 beads are 256 warp tiles and cannot fill a B200."""
+    import torch
+    import paper_1106_2899_b200 as ssm
+    paper = {(16, 0.0): 8.97e-1, (16, 0.05): 8.95e-1, (32, 0.0): 9.02e-1, (32, 0.05): 8.95e-1,
+             (64, 0.0): 8.70e-1, (64, 0.05): 8.63e-1, (128, 0.0): 8.45e-1, (128, 0.05): 8.40e-1}
+    rows = []
+    for N in (16, 32, 64, 128):
+        for rate in (0.0, 0.05):
+            g = ssm.Ensemble(N, 65536 // N, seed=1)
+            g.step(64, rate)                                  # warm-up (and the kernel variant's first launch)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); g.step(10000, rate); e1.record(); torch.cuda.synchronize()
+            t = e0.elapsed_time(e1) * 1e-3
+            rows.append({"n_beads": N, "n_chains": 65536 // N, "shear_rate": rate, "steps": 10000, "seconds": t,
+                         "bead_updates_per_s": 65536 * 1e4 / t, "paper_gpu_seconds": paper[(N, rate)]})
+    print(json.dumps({"workload": "PAPER.md Table 1 (context)", "rows": rows}))
+
+
 def main():
     a = parse()
     if a.impl == "reference":
         return run_reference(a)
+    if a.table1:
+        return run_table1()
 
     import torch
     import torch.distributed as dist
