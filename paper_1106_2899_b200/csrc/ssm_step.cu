@@ -13,8 +13,6 @@
 // Mapping and layouts: ssm_common.h and DESIGN.md section 6.
 #include <cuda_runtime.h>
 
-#include <type_traits>
-
 #include "ssm_common.h"
 #include "ssm_rng.cuh"
 
@@ -299,93 +297,72 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
             cnt = 0.0f;
             if (P.springs_on) {
                 bool event = false;
-                // U slip-springs per lane in one straight-line pass (numbers lane + 32 (it0 + u)), so
-                // that the U Philox chains and the U dependent load -> exp -> compare -> scatter
-                // chains overlap
-                auto slot_round = [&](auto U_, int it0) {
-                    constexpr int U = decltype(U_)::value;
-                    int sx[U], s[U];
-                    bool act[U];
-                    uint32_t w_hop[U], w_end[U];
-                    float4 a[U];
-#pragma unroll
-                    for (int u = 0; u < U; ++u) {
-                        const int f = lane + 32 * (it0 + u);
-                        act[u] = f < Tz;
-                        sx[u] = slot_index(it0 + u, act[u] ? f : 0);
-                        const int c = sx[u] >> LN, j = sx[u] & (N - 1);
-                        uint32_t w[4];
-                        stream_call(sk, P.rk, DOM_SLOT, chain0 + (uint32_t)c, (uint32_t)(j >> 1), w);
-                        w_hop[u] = (j & 1) ? w[2] : w[0];
-                        w_end[u] = (j & 1) ? w[3] : w[1];
-                        s[u] = max((int)Sb[sx[u]], 1);       // 1..N (an idle lane may look at an empty slot: any bead will do)
-                        a[u] = A4[sx[u]];
+                // one slip-spring per lane per pass: number f = lane + 32 it of the warp.  (Two or three
+                // per lane in one straight-line pass were measured slower: 8.2 and 9.1 ms against 7.7 ms
+                // per launch; the extra predicated-off pass costs more than the overlap of the chains wins.)
+                const int nit = (Tz + 31) >> 5;
+                for (int it = 0; it < nit; ++it) {
+                    const int f = lane + 32 * it;
+                    const bool act = f < Tz;
+                    const int sx = slot_index(it, act ? f : 0), c = sx >> LN, j = sx & (N - 1), base = sx & ~(N - 1);
+                    uint32_t w[4];
+                    stream_call(sk, P.rk, DOM_SLOT, chain0 + (uint32_t)c, (uint32_t)(j >> 1), w);
+                    const uint32_t w_hop = (j & 1) ? w[2] : w[0], w_end = (j & 1) ? w[3] : w[1];
+                    const int s = max((int)Sb[sx], 1);       // 1..N (an idle lane may look at an empty slot: any bead will do)
+                    float4 a = A4[sx];
+                    if (SHEAR) {
+                        // eq 45 with kappa_xy only: A_x += dt gamma_dot A_y, as a compensated
+                        // (two-sum) update of (A_x, low part): the increment is the same every
+                        // step, so a plain fp32 sum would drift linearly instead of randomly
+                        const float t = fmaf(P.gdt, a.y, a.w);
+                        const float sum = a.x + t;
+                        const float bb = sum - a.x;
+                        a.w = (a.x - (sum - bb)) + (t - bb);
+                        a.x = sum;
+                        if (act) A4[sx] = a;
                     }
-#pragma unroll
-                    for (int u = 0; u < U; ++u) {
-                        const int base = sx[u] & ~(N - 1);
-                        if (SHEAR) {
-                            // eq 45 with kappa_xy only: A_x += dt gamma_dot A_y, as a compensated
-                            // (two-sum) update of (A_x, low part): the increment is the same every
-                            // step, so a plain fp32 sum would drift linearly instead of randomly
-                            const float t = fmaf(P.gdt, a[u].y, a[u].w);
-                            const float sum = a[u].x + t;
-                            const float bb = sum - a[u].x;
-                            a[u].w = (a[u].x - (sum - bb)) + (t - bb);
-                            a[u].x = sum;
-                            if (act[u]) A4[sx[u]] = a[u];
-                        }
-                        // Glauber hop (eqs 23, 24 with the cap of eqs 48, 49):
-                        // p+- = min{ h [1 - tanh x+-], 1/2 } = min{ 2h / (1 + e^{2 x+-}), 1/2 },
-                        // x+- = (3/4N_s)(|R_{s+-1}-A|^2 - |R_s-A|^2)
-                        const int b0 = base + s[u] - 1;
-                        const float4 r0 = Rm[rm_index(b0)];
-                        const float4 rp = Rm[rm_index(b0 + (s[u] < N ? 1 : 0))];
-                        const float4 rm = Rm[rm_index(b0 - (s[u] > 1 ? 1 : 0))];
-                        const float d0x = r0.x - a[u].x, d0y = r0.y - a[u].y, d0z = r0.z - a[u].z;
-                        const float dpx = rp.x - a[u].x, dpy = rp.y - a[u].y, dpz = rp.z - a[u].z;
-                        const float dmx = rm.x - a[u].x, dmy = rm.y - a[u].y, dmz = rm.z - a[u].z;
-                        const float e0 = fmaf(d0z, d0z, fmaf(d0y, d0y, d0x * d0x));
-                        const float ep = fmaf(dpz, dpz, fmaf(dpy, dpy, dpx * dpx));
-                        const float em = fmaf(dmz, dmz, fmaf(dmy, dmy, dmx * dmx));
-                        float pp = fminf(__fdividef(P.h2, 1.0f + mufu_ex2(P.q2l * (ep - e0))), 0.5f);
-                        float pm = fminf(__fdividef(P.h2, 1.0f + mufu_ex2(P.q2l * (em - e0))), 0.5f);
-                        if (s[u] == N) pp = 0.0f;
-                        if (s[u] == 1) pm = 0.0f;
-                        const float uu = u23(w_hop[u]);
-                        const bool up = uu < pp, dn = !up && uu < pp + pm;
-                        const int sn = s[u] + (up ? 1 : 0) - (dn ? 1 : 0);
-                        // destruction at the ends (eq 53), integer-domain comparison
-                        const bool destroyed = (sn == 1 || sn == N) && code23(w_end[u]) < P.t_destroy;
-                        const bool live = act[u] && !destroyed;
-                        if (act[u] && sn != s[u]) Sb[sx[u]] = (unsigned char)sn;
-                        if (act[u] && destroyed) {
-                            const int j = sx[u] & (N - 1);
-                            atomicOr(Dm + (sx[u] >> LN) * WPC + (j >> 5), 1u << (j & 31));
-                            event = true;
-                        }
-                        // a destroyed slip-spring exerts no force and has no virial: zero displacement
-                        const float dx = live ? (up ? dpx : (dn ? dmx : d0x)) : 0.0f;
-                        const float dy = live ? (up ? dpy : (dn ? dmy : d0y)) : 0.0f;
-                        const float dz = live ? (up ? dpz : (dn ? dmz : d0z)) : 0.0f;
-                        if (live) {
-                            int *fp = Fx + fx_index(b0 + sn - s[u]);
-                            atomicAdd(fp, __float2int_rn(-P.fx_scale * dx));
-                            atomicAdd(fp + 1, __float2int_rn(-P.fx_scale * dy));
-                            atomicAdd(fp + 2, __float2int_rn(-P.fx_scale * dz));
-                        }
-                        sv[0] = fmaf(dx, dx, sv[0]); sv[1] = fmaf(dy, dy, sv[1]); sv[2] = fmaf(dz, dz, sv[2]);
-                        sv[3] = fmaf(dx, dy, sv[3]); sv[4] = fmaf(dy, dz, sv[4]); sv[5] = fmaf(dz, dx, sv[5]);
-                        cnt += live ? 1.0f : 0.0f;
-                        if (sample && live) atomicAdd(Samp + (sx[u] >> LN), __float2int_rn(dx * dy * (float)(1 << kSampleShift)));
+                    // Glauber hop (eqs 23, 24 with the cap of eqs 48, 49):
+                    // p+- = min{ h [1 - tanh x+-], 1/2 } = min{ 2h / (1 + e^{2 x+-}), 1/2 },
+                    // x+- = (3/4N_s)(|R_{s+-1}-A|^2 - |R_s-A|^2)
+                    const int b0 = base + s - 1;
+                    const float4 r0 = Rm[rm_index(b0)];
+                    const float4 rp = Rm[rm_index(b0 + (s < N ? 1 : 0))];
+                    const float4 rm = Rm[rm_index(b0 - (s > 1 ? 1 : 0))];
+                    const float d0x = r0.x - a.x, d0y = r0.y - a.y, d0z = r0.z - a.z;
+                    const float dpx = rp.x - a.x, dpy = rp.y - a.y, dpz = rp.z - a.z;
+                    const float dmx = rm.x - a.x, dmy = rm.y - a.y, dmz = rm.z - a.z;
+                    const float e0 = fmaf(d0z, d0z, fmaf(d0y, d0y, d0x * d0x));
+                    const float ep = fmaf(dpz, dpz, fmaf(dpy, dpy, dpx * dpx));
+                    const float em = fmaf(dmz, dmz, fmaf(dmy, dmy, dmx * dmx));
+                    float pp = fminf(__fdividef(P.h2, 1.0f + mufu_ex2(P.q2l * (ep - e0))), 0.5f);
+                    float pm = fminf(__fdividef(P.h2, 1.0f + mufu_ex2(P.q2l * (em - e0))), 0.5f);
+                    if (s == N) pp = 0.0f;
+                    if (s == 1) pm = 0.0f;
+                    const float uu = u23(w_hop);
+                    const bool up = uu < pp, dn = !up && uu < pp + pm;
+                    const int sn = s + (up ? 1 : 0) - (dn ? 1 : 0);
+                    // destruction at the ends (eq 53), integer-domain comparison
+                    const bool destroyed = (sn == 1 || sn == N) && code23(w_end) < P.t_destroy;
+                    const bool live = act && !destroyed;
+                    if (act && sn != s) Sb[sx] = (unsigned char)sn;
+                    if (act && destroyed) {
+                        atomicOr(Dm + c * WPC + (j >> 5), 1u << (j & 31));
+                        event = true;
                     }
-                };
-                {
-                    const int nit = (Tz + 31) >> 5;
-                    int it0 = 0;
-                    // (two slip-springs per lane per pass was measured slower: the larger loop body
-                    // costs more instruction-fetch stalls than the overlap wins)
-                    for (; it0 < nit; ++it0) slot_round(std::integral_constant<int, 1>(), it0);
+                    // a destroyed slip-spring exerts no force and has no virial: zero displacement
+                    const float dx = live ? (up ? dpx : (dn ? dmx : d0x)) : 0.0f;
+                    const float dy = live ? (up ? dpy : (dn ? dmy : d0y)) : 0.0f;
+                    const float dz = live ? (up ? dpz : (dn ? dmz : d0z)) : 0.0f;
+                    if (live) {
+                        int *fp = Fx + fx_index(b0 + sn - s);
+                        atomicAdd(fp, __float2int_rn(-P.fx_scale * dx));
+                        atomicAdd(fp + 1, __float2int_rn(-P.fx_scale * dy));
+                        atomicAdd(fp + 2, __float2int_rn(-P.fx_scale * dz));
+                    }
+                    sv[0] = fmaf(dx, dx, sv[0]); sv[1] = fmaf(dy, dy, sv[1]); sv[2] = fmaf(dz, dz, sv[2]);
+                    sv[3] = fmaf(dx, dy, sv[3]); sv[4] = fmaf(dy, dz, sv[4]); sv[5] = fmaf(dz, dx, sv[5]);
+                    cnt += live ? 1.0f : 0.0f;
+                    if (sample && live) atomicAdd(Samp + c, __float2int_rn(dx * dy * (float)(1 << kSampleShift)));
                 }
                 // construction attempts (eqs 50, 51), drawn by the chain's own lanes; K = N - Z
                 // or a fixed K.  The 23-bit code of attempt k is (h << 7) | e (DESIGN.md
