@@ -248,3 +248,36 @@ def test_translation_invariance_of_the_dynamics():
     a.run(40); b.run(40)
     assert np.array_equal(a.S, b.S)
     assert np.allclose(np.diff(a.R, axis=1), np.diff(b.R, axis=1), atol=1e-11)
+
+
+def test_construction_attempt_uniform_is_assembled_as_reading_r22_states():
+    """DESIGN.md reading R22: attempt k has the 23-bit code (h << 7) | e with h = half k&1 of
+    word (k&7)>>1 of ATTEMPT call k>>3 and e = top 7 bits of word 2 of ANCHOR call k; success at
+    bead 1 if code < T(p_c), at bead N if code < T(2 p_c) (eqs 50, 51), the anchor from normals
+    0..2 of the same ANCHOR call (eq 52).  An empty chain is stepped once at many step numbers
+    and the slip-springs that appear are compared with that statement written against the raw
+    stream (the big-integer Philox pins the stream itself)."""
+    N, seed = 16, 11
+    h = 0.01 / 0.1
+    pc = h / (4.0 * N)                                   # K = N - Z = N attempts (P:L370)
+    T1, T2 = oracle.threshold23(pc), oracle.threshold23(2.0 * pc)
+    made = 0
+    for step in range(1500):
+        e = oracle.Ensemble(N, 1, seed=seed, chain_offset=7)
+        e.S[:] = 0; e.A[:] = 0.0; e.Z[:] = 0
+        e.step = step
+        e.run(1)
+        want = []
+        for k in range(N):
+            w = oracle.stream(seed, oracle.DOM_ATTEMPT, step, 7, k >> 3)
+            wa = oracle.stream(seed, oracle.DOM_ANCHOR, step, 7, k)
+            code = (((w[(k & 7) >> 1] >> (16 * (k & 1))) & 0xFFFF) << 7) | (wa[2] >> 25)
+            if code < T2:
+                z0, z1 = oracle.box_muller(wa[0]); z2, _ = oracle.box_muller(wa[1])
+                want.append((1 if code < T1 else N, (z0, z1, z2)))
+        assert e.Z[0] == len(want)
+        for j, (s, z) in enumerate(want):
+            assert e.S[0, j] == s
+            assert np.allclose(e.A[0, j], e.R[0, s - 1] + np.sqrt(0.5 / 3.0) * np.array(z), rtol=0, atol=1e-12)
+        made += len(want)
+    assert 40 < made < 120                               # 2 h / N0 = 0.05 per step expected
