@@ -179,3 +179,20 @@ def test_correlator_matches_oracle_on_identical_trajectories(ssm):
     assert np.allclose(t0, t1)
     assert np.allclose(G1, G0, rtol=0, atol=2e-4 * np.abs(G0).max())
     assert np.allclose(se1, se0, rtol=0.02, atol=1e-6)
+
+
+def test_device_view_of_the_stress_sums_is_what_the_exchange_reduces(ssm):
+    """the only multi-GPU exchange is an in-place int64 all-reduce of the
+    fixed-point sums inside the workspace; the device view must alias exactly what ssm_stress_sums
+    and ssm_stress report (one rank: the reduction is the identity)."""
+    import torch
+    from paper_1106_2899_b200 import shard
+    g = ssm.Ensemble(16, 300, seed=31, stress_every=1, stress_capacity=40)
+    g.step(40)
+    dev = g.stress_sums_device(5, 20)
+    assert dev.is_cuda and dev.dtype == torch.int64 and tuple(dev.shape) == (20, 12)
+    shard.allreduce_sums(dev)
+    torch.cuda.synchronize()
+    host = g.stress_sums()[5:25]
+    assert np.array_equal(dev.cpu().numpy(), host)
+    assert np.allclose(shard.stress_means(host, 300), g.stress(5, 20), rtol=0, atol=1e-12)
