@@ -123,6 +123,22 @@ int ssm_chain_stress(ssm_ctx *ctx, float *out, int pointers_are_device);
  * error over chain groups.  All (host). */
 int ssm_gt(ssm_ctx *ctx, int32_t *n_lags, double *h_lag_time, double *h_G, double *h_se);
 
+/* Host post-processing of a tabulated G(t) (section 4.1); no device work, no ctx.
+ * h_t[n_lags] strictly increasing lag times >= 0 (as ssm_gt returns them), h_G[n_lags].  All (host).
+ *  ssm_moduli : storage and loss moduli, eqs (55), (56), by the trapezoidal rule the paper names
+ *               (P:L392), the integral truncated at the last lag: h_storage[q] = G'(h_omega[q]),
+ *               h_loss[q] = G''(h_omega[q]); the dynamic viscosity of eq (64) is
+ *               sqrt(G'^2 + G''^2).
+ *  ssm_eta0   : zero-shear viscosity, eq (59), trapezoidal rule.
+ *  ssm_tau_d  : longest relaxation time, eq (58): -1 / slope of the least-squares line through
+ *               ln G(t) over t_lo <= t <= t_hi (points with G <= 0 skipped); SSM_ERANGE if the
+ *               window holds fewer than two usable points or the slope is not negative.
+ * SSM_EINVAL on NULL pointers, n_lags < 2, lag times not increasing, negative frequencies. */
+int ssm_moduli(int32_t n_lags, const double *h_t, const double *h_G, int32_t n_omega, const double *h_omega,
+               double *h_storage, double *h_loss);
+int ssm_eta0(int32_t n_lags, const double *h_t, const double *h_G, double *h_eta0);
+int ssm_tau_d(int32_t n_lags, const double *h_t, const double *h_G, double t_lo, double t_hi, double *h_tau_d);
+
 /* Raw correlator sums for multi-GPU reduction: h_sum (host) [groups][levels][bins] double,
  * h_count (host) [groups][levels][bins] int64. */
 int ssm_gt_sums(ssm_ctx *ctx, double *h_sum, int64_t *h_count);

@@ -16,7 +16,8 @@ SSM_OK, SSM_EINVAL, SSM_ENOMEM, SSM_ECUDA, SSM_ESTATE, SSM_ERANGE = 0, -1, -2, -
 
 EXPORTS = ["ssm_workspace_bytes", "ssm_init", "ssm_step", "ssm_stress_count", "ssm_stress", "ssm_stress_sums",
            "ssm_stress_sums_device", "ssm_chain_stress", "ssm_gt", "ssm_gt_sums", "ssm_get_state", "ssm_set_state",
-           "ssm_reset_accumulators", "ssm_launch_count", "ssm_set_fusion", "ssm_set_grid", "ssm_destroy", "ssm_last_error"]
+           "ssm_reset_accumulators", "ssm_launch_count", "ssm_set_fusion", "ssm_set_grid", "ssm_destroy", "ssm_last_error",
+           "ssm_moduli", "ssm_eta0", "ssm_tau_d"]
 
 
 class Params(C.Structure):
@@ -63,6 +64,9 @@ def lib():
     L.ssm_set_grid.argtypes = [vp, C.c_int32]; L.ssm_set_grid.restype = C.c_int
     L.ssm_destroy.argtypes = [vp]; L.ssm_destroy.restype = None
     L.ssm_last_error.argtypes = [vp]; L.ssm_last_error.restype = C.c_char_p
+    L.ssm_moduli.argtypes = [C.c_int32, dp, dp, C.c_int32, dp, dp, dp]; L.ssm_moduli.restype = C.c_int
+    L.ssm_eta0.argtypes = [C.c_int32, dp, dp, dp]; L.ssm_eta0.restype = C.c_int
+    L.ssm_tau_d.argtypes = [C.c_int32, dp, dp, C.c_double, C.c_double, dp]; L.ssm_tau_d.restype = C.c_int
     _lib = L
     return L
 
@@ -73,6 +77,40 @@ def library_path():
 
 def workspace_bytes(params):
     return lib().ssm_workspace_bytes(C.byref(params))
+
+
+def _d(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _ck0(rc, what):
+    if rc != SSM_OK:
+        raise SsmError(rc, what)
+
+
+def moduli(t, G, omega):
+    """ssm_moduli: (G'(omega), G''(omega)) of a tabulated G(t), eqs 55-56."""
+    t, tp = _d(t); G, Gp = _d(G); w, wp = _d(omega)
+    g1 = np.zeros(len(w)); g2 = np.zeros(len(w))
+    _ck0(lib().ssm_moduli(len(t), tp, Gp, len(w), wp, _d(g1)[1], _d(g2)[1]), "ssm_moduli: bad arguments")
+    return g1, g2
+
+
+def eta0(t, G):
+    """ssm_eta0: zero-shear viscosity, eq 59."""
+    t, tp = _d(t); G, Gp = _d(G)
+    out = C.c_double()
+    _ck0(lib().ssm_eta0(len(t), tp, Gp, C.byref(out)), "ssm_eta0: bad arguments")
+    return out.value
+
+
+def tau_d(t, G, t_lo, t_hi):
+    """ssm_tau_d: longest relaxation time from the tail slope of ln G(t), eq 58."""
+    t, tp = _d(t); G, Gp = _d(G)
+    out = C.c_double()
+    _ck0(lib().ssm_tau_d(len(t), tp, Gp, float(t_lo), float(t_hi), C.byref(out)), "ssm_tau_d: bad arguments or no decaying tail in the window")
+    return out.value
 
 
 class Ensemble:

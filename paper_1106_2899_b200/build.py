@@ -12,7 +12,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libssm.so")
-SOURCES = ["ssm_step.cu", "ssm_aux.cu", "ssm_api.cu"]
+SOURCES = ["ssm_step.cu", "ssm_aux.cu", "ssm_api.cu", "ssm_rheo.cu"]
 HEADERS = ["ssm_common.h", "ssm_rng.cuh", os.path.join("..", "..", "include", "ssm.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--fmad=true", "-Xcompiler", "-fPIC", "-shared", "-cudart", "shared"]

@@ -224,3 +224,29 @@ def test_capacity_and_probability_caps(ssm):
         assert n >= 0.6 * M
         assert e.Z.max() <= N
     assert kw == dict(zeta_s=0.02)
+
+
+def test_rouse_limit_gt_to_viscosity_and_relaxation_time(ssm):
+    """ssm_gt -> ssm_eta0 / ssm_tau_d / ssm_moduli (eqs 55-59) on the GPU's own correlator output in
+    the Rouse limit, where G is a closed form of the Euler map: G(n dt) N =
+    sum_p (1 - k_p dt)^(2n) / (1 - k_p dt/2)^2, k_p = 12 sin^2(p pi/2N).  The expected numbers are
+    the ORACLE's post-processing of that exact table on the same lags (the fast modes are shorter
+    than the sampling interval 0.1, so the trapezoidal rule of P:L392 is not the continuum integral)."""
+    from oracle import rheology as ref
+    N, M, steps, dt = 8, 8192, 12000, 0.01
+    g = ssm.Ensemble(N, M, n_0=0.0, seed=77, sample_every=10, corr_levels=7, corr_bins=16, corr_groups=32)
+    g.step(steps)
+    t, G, se = g.gt()
+    kp = 12.0 * np.sin(np.arange(1, N) * np.pi / (2 * N)) ** 2
+    tau1 = 1.0 / (2.0 * kp[0])
+    keep = t <= 8.0 * tau1                                    # beyond that the table is noise
+    t, G = t[keep], G[keep]
+    Gx = ((1.0 - kp[None, :] * dt) ** (2.0 * t[:, None] / dt) / (1.0 - kp[None, :] * dt / 2.0) ** 2).sum(1) / N
+    eta, eta_x = ssm.eta0(t, G), ref.eta0(t, Gx)
+    assert abs(eta - eta_x) < 0.04 * eta_x, (eta, eta_x)
+    td, td_x = ssm.tau_d(t, G, 1.0 * tau1, 3.0 * tau1), ref.tau_d(t, Gx, 1.0 * tau1, 3.0 * tau1)
+    assert abs(td - td_x) < 0.08 * td_x, (td, td_x)
+    w = np.array([0.2 / tau1, 1.0 / tau1])
+    g1, g2 = ssm.moduli(t, G, w)
+    x1, x2 = ref.moduli(t, Gx, w)
+    assert np.allclose(g1, x1, rtol=0.1) and np.allclose(g2, x2, rtol=0.1), (g1, x1, g2, x2)
