@@ -31,6 +31,9 @@ if ROOT not in sys.path:
 # (DESIGN.md section 9.2).  The roofline numerator is I_ALG x bead-updates/s, NOT the number
 # of instructions the kernel happens to execute, so padding cannot raise the fraction.
 I_ALG = 95.0
+# of which 32 x 32 -> 64-bit multiplies (IMAD.WIDE) of Philox: 0.594 calls x 20.  They are not full-rate
+# instructions on B200; ssm_issue_rates() measures their cost live for the rate-weighted fraction.
+I_ALG_WIDE = 0.59375 * 20.0
 N_SM, SMSP_PER_SM, LANES = 148, 4, 32
 
 
@@ -299,6 +302,9 @@ def main():
     alg_bytes = 2.0 * 25.0 * N * M
     hbm_achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
     traffic = ncu_traffic(N, M)
+    rates = g.issue_rates()
+    i_alg_cycles = (I_ALG - I_ALG_WIDE) + I_ALG_WIDE * max(1.0, rates["imad_wide"])
+    weighted = i_alg_cycles * per_launch_updates / (launch_ms * 1e-3) / 1e12
     line = {
         "metric": "bead-updates/s", "value": value, "unit": "bead-updates/s", "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -310,6 +316,11 @@ def main():
                      "frac": achieved / peak_alu, "traffic": traffic,
                      "kernel": "ssm_step_kernel<G=%d>" % (N // 8), "launch_ms": launch_ms,
                      "i_alg_per_bead_update": I_ALG,
+                     "rate_weighted": {"frac": weighted / peak_alu, "i_alg_issue_cycles_per_bead_update": i_alg_cycles,
+                                       "measured_cycles_per_warp_instruction": rates,
+                                       "how": "as frac, but the %.1f IMAD.WIDE of the algorithmic count are charged the "
+                                              "issue cycles ssm_issue_rates() measures for them on this GPU instead of 1"
+                                              % I_ALG_WIDE},
                      "peak_how": "148 SM x 4 SMSP x 32 lanes x %.0f MHz (sm_max_mhz, %s)" % (peaks["sm_max_mhz"], peaks["source"]),
                      "hbm": {"achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                              "frac": hbm_achieved / peaks["hbm_gbs"], "bytes_per_launch": alg_bytes,

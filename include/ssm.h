@@ -123,6 +123,13 @@ int ssm_chain_stress(ssm_ctx *ctx, float *out, int pointers_are_device);
  * error over chain groups.  All (host). */
 int ssm_gt(ssm_ctx *ctx, int32_t *n_lags, double *h_lag_time, double *h_G, double *h_se);
 
+/* Diagnostic for the roofline: measured cycles per warp instruction per
+ * scheduler, at the step kernel's residency (4 warps per scheduler), of h_cycles[0] FFMA,
+ * [1] LOP3/IADD3/SHF, [2] IMAD, [3] IMAD.WIDE (the 32 x 32 -> 64-bit multiply of Philox).
+ * Runs four short kernels on the ctx's stream, uses the workspace's staging area (nothing of
+ * the ensemble is touched) and synchronises.  h_cycles (host)[4]. */
+int ssm_issue_rates(ssm_ctx *ctx, double *h_cycles);
+
 /* Host post-processing of a tabulated G(t) (section 4.1); no device work, no ctx.
  * h_t[n_lags] strictly increasing lag times >= 0 (as ssm_gt returns them), h_G[n_lags].  All (host).
  *  ssm_moduli : storage and loss moduli, eqs (55), (56), by the trapezoidal rule the paper names

@@ -17,7 +17,7 @@ SSM_OK, SSM_EINVAL, SSM_ENOMEM, SSM_ECUDA, SSM_ESTATE, SSM_ERANGE = 0, -1, -2, -
 EXPORTS = ["ssm_workspace_bytes", "ssm_init", "ssm_step", "ssm_stress_count", "ssm_stress", "ssm_stress_sums",
            "ssm_stress_sums_device", "ssm_chain_stress", "ssm_gt", "ssm_gt_sums", "ssm_get_state", "ssm_set_state",
            "ssm_reset_accumulators", "ssm_launch_count", "ssm_set_fusion", "ssm_set_grid", "ssm_destroy", "ssm_last_error",
-           "ssm_moduli", "ssm_eta0", "ssm_tau_d"]
+           "ssm_moduli", "ssm_eta0", "ssm_tau_d", "ssm_issue_rates"]
 
 
 class Params(C.Structure):
@@ -64,6 +64,7 @@ def lib():
     L.ssm_set_grid.argtypes = [vp, C.c_int32]; L.ssm_set_grid.restype = C.c_int
     L.ssm_destroy.argtypes = [vp]; L.ssm_destroy.restype = None
     L.ssm_last_error.argtypes = [vp]; L.ssm_last_error.restype = C.c_char_p
+    L.ssm_issue_rates.argtypes = [vp, dp]; L.ssm_issue_rates.restype = C.c_int
     L.ssm_moduli.argtypes = [C.c_int32, dp, dp, C.c_int32, dp, dp, dp]; L.ssm_moduli.restype = C.c_int
     L.ssm_eta0.argtypes = [C.c_int32, dp, dp, dp]; L.ssm_eta0.restype = C.c_int
     L.ssm_tau_d.argtypes = [C.c_int32, dp, dp, C.c_double, C.c_double, dp]; L.ssm_tau_d.restype = C.c_int
@@ -234,6 +235,13 @@ class Ensemble:
 
     def set_fusion(self, steps_per_launch):
         self._ck(lib().ssm_set_fusion(self.h, steps_per_launch))
+
+    def issue_rates(self):
+        """ssm_issue_rates: cycles per warp instruction per scheduler of FFMA, LOP3-class, IMAD, IMAD.WIDE."""
+        out = np.zeros(4)
+        with self._torch.cuda.device(self.device):
+            self._ck(lib().ssm_issue_rates(self.h, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return {"ffma": out[0], "alu": out[1], "imad": out[2], "imad_wide": out[3]}
 
     def set_grid(self, blocks):
         self._ck(lib().ssm_set_grid(self.h, blocks))

@@ -18,6 +18,7 @@ namespace ssm {
 cudaError_t step_occupancy(int n_beads, int *blocks_per_sm);
 cudaError_t launch_step(int n_beads, const StepParams &p, int grid, cudaStream_t st);
 cudaError_t launch_init(const InitParams &p, cudaStream_t st);
+cudaError_t measure_rates(unsigned *d_scratch, int blocks, cudaStream_t st, double cycles[4]);
 cudaError_t launch_xfer(bool do_export, unsigned char *state, float *R, float *A, unsigned char *S, int N,
                         long long k0, long long nk, long long pitch, cudaStream_t st);
 cudaError_t launch_chain_stress(const unsigned char *state, float *out, int N, long long M, float cs, cudaStream_t st);
@@ -101,7 +102,10 @@ static Layout make_layout(const ssm_params *p)
     L.csum = o; if (corr) o = align_up(o + (size_t)p->corr_groups * p->corr_levels * p->corr_bins * 8, 256);
     // staging for host-pointer get/set state and chain stress: chunks of <= 65536 chains
     L.stage_chains = p->n_chains < 65536 ? p->n_chains : 65536;
-    L.stage = o; o = align_up(o + (size_t)L.stage_chains * (size_t)(29 * p->n_beads > 48 ? 29 * p->n_beads : 48), 256);
+    // (at least 1 MB, so that the issue-rate probe's scratch of 2 kB per SM fits any ensemble)
+    size_t stage_bytes = (size_t)L.stage_chains * (size_t)(29 * p->n_beads > 48 ? 29 * p->n_beads : 48);
+    if (stage_bytes < ((size_t)1 << 20)) stage_bytes = (size_t)1 << 20;
+    L.stage = o; o = align_up(o + stage_bytes, 256);
     L.total = o;
     return L;
 }
@@ -409,6 +413,22 @@ extern "C" int ssm_set_fusion(ssm_ctx *c, int32_t t)
     if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
     if (t < 1 || t > kMaxFuse) return fail(c, SSM_EINVAL, "steps_per_launch out of range");
     c->fuse = t;
+    return SSM_OK;
+}
+
+extern "C" int ssm_issue_rates(ssm_ctx *c, double *h_cycles)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (!h_cycles) return fail(c, SSM_EINVAL, "h_cycles is NULL");
+    int dev = 0, sms = 0;
+    CK(c, cudaGetDevice(&dev));
+    CK(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const size_t need = (size_t)(1 + sms * 512) * sizeof(unsigned);
+    if (need > c->lay.total - c->lay.stage) return fail(c, SSM_ENOMEM, "staging area too small for the issue-rate probe");
+    double raw[4];
+    CK(c, measure_rates(reinterpret_cast<unsigned *>(c->ws + c->lay.stage), sms, c->st, raw));
+    h_cycles[0] = raw[0]; h_cycles[1] = raw[1]; h_cycles[2] = raw[2];
+    h_cycles[3] = 2.0 * raw[3] - raw[1];          // the probe's pair is IMAD.WIDE + LOP3
     return SSM_OK;
 }
 

@@ -207,3 +207,60 @@ cudaError_t launch_corr(const CorrParams &c, cudaStream_t st)
 }
 
 }  // namespace ssm
+
+namespace ssm {
+// ---------------------------------------------------------------------------------------
+// Issue-rate probe: cycles per warp instruction per scheduler for the
+// instruction classes of the step kernel, measured with 4 warps per scheduler (the step
+// kernel's residency) and 4 independent chains per lane.  OP 0: FFMA, 1: LOP3/IADD3/SHF,
+// 2: IMAD, 3: IMAD.WIDE (+ one LOP3, subtracted on the host with the rate of OP 1).
+// ---------------------------------------------------------------------------------------
+template <int OP>
+__global__ void __launch_bounds__(512) ssm_rate_kernel(unsigned *out, int iters, unsigned seed)
+{
+    constexpr int ILP = 4;
+    unsigned a[ILP], b[ILP]; float f[ILP], g[ILP];
+#pragma unroll
+    for (int i = 0; i < ILP; ++i) { a[i] = seed + threadIdx.x * 7u + i; b[i] = seed * 3u + i; f[i] = a[i] * 1e-3f; g[i] = 1.0001f + i; }
+    const long long t0 = clock64();
+    for (int n = 0; n < iters; ++n) {
+#pragma unroll
+        for (int i = 0; i < ILP; ++i) {
+            if (OP == 0) f[i] = fmaf(f[i], g[i], 0.5f);
+            if (OP == 1) { a[i] = (a[i] ^ b[i]) + 0x9E3779B9u; a[i] ^= a[i] >> 7; }
+            if (OP == 2) a[i] = a[i] * 0xD2511F53u + b[i];
+            if (OP == 3) { const unsigned long long p = (unsigned long long)a[i] * 0xD2511F53u; a[i] = (unsigned)(p >> 32) ^ (unsigned)p; }
+        }
+    }
+    const long long t1 = clock64();
+    unsigned r = 0;
+#pragma unroll
+    for (int i = 0; i < ILP; ++i) r += a[i] + b[i] + __float_as_uint(f[i]);
+    out[1 + blockIdx.x * blockDim.x + threadIdx.x] = r;
+    if (threadIdx.x == 0 && blockIdx.x == 0) out[0] = (unsigned)(t1 - t0);
+}
+
+// out: device scratch of at least (1 + blocks * 512) words; cycles[4] as described above (raw,
+// per warp instruction of the loop body: 1, 4, 1 and 2 instructions per chain and iteration)
+cudaError_t measure_rates(unsigned *d_scratch, int blocks, cudaStream_t st, double cycles[4])
+{
+    const int iters = 4000, ilp = 4, warps_per_smsp = 4;
+    const int per_iter[4] = {1, 4, 1, 2};
+    for (int op = 0; op < 4; ++op) {
+        for (int rep = 0; rep < 2; ++rep) {                      // first launch warms the instruction cache
+            switch (op) {
+                case 0: ssm_rate_kernel<0><<<blocks, 512, 0, st>>>(d_scratch, iters, 1u); break;
+                case 1: ssm_rate_kernel<1><<<blocks, 512, 0, st>>>(d_scratch, iters, 1u); break;
+                case 2: ssm_rate_kernel<2><<<blocks, 512, 0, st>>>(d_scratch, iters, 1u); break;
+                default: ssm_rate_kernel<3><<<blocks, 512, 0, st>>>(d_scratch, iters, 1u); break;
+            }
+        }
+        unsigned cyc = 0;
+        cudaError_t e = cudaMemcpyAsync(&cyc, d_scratch, sizeof cyc, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return e;
+        cycles[op] = (double)cyc / ((double)iters * ilp * per_iter[op] * warps_per_smsp);
+    }
+    return cudaGetLastError();
+}
+}  // namespace ssm

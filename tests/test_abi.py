@@ -75,10 +75,11 @@ def test_no_cpu_fallback():
         m.Ensemble(32, 16)
     # the C ABI itself refuses too
     h = C.c_void_p()
-    buf = C.create_string_buffer(1 << 20)
-    base = (C.addressof(buf) + 255) // 256 * 256
     p = _params(n_chains=16)
-    rc = m.lib().ssm_init(C.byref(h), C.byref(p), C.c_void_p(base), 1 << 19, None)
+    need = m.lib().ssm_workspace_bytes(C.byref(p))
+    buf = C.create_string_buffer(need + 256)
+    base = (C.addressof(buf) + 255) // 256 * 256
+    rc = m.lib().ssm_init(C.byref(h), C.byref(p), C.c_void_p(base), need, None)
     assert rc == m.SSM_ECUDA
     assert b"no CUDA device" in m.lib().ssm_last_error(None)
 

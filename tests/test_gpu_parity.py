@@ -196,3 +196,16 @@ def test_device_view_of_the_stress_sums_is_what_the_exchange_reduces(ssm):
     host = g.stress_sums()[5:25]
     assert np.array_equal(dev.cpu().numpy(), host)
     assert np.allclose(shard.stress_means(host, 300), g.stress(5, 20), rtol=0, atol=1e-12)
+
+
+def test_issue_rate_probe(ssm):
+    """ssm_issue_rates: plain ALU and FP32 instructions issue about once per
+    cycle per scheduler, IMAD at half rate, and the 32 x 32 -> 64-bit multiply of Philox slower still."""
+    g = ssm.Ensemble(8, 64, seed=1)
+    r = g.issue_rates()
+    assert 0.9 < r["ffma"] < 1.6 and 0.9 < r["alu"] < 1.6
+    assert 1.7 < r["imad"] < 2.6
+    assert 3.0 < r["imad_wide"] < 6.0
+    R, A, S, step = g.get_state()          # the probe used the staging area only
+    g2 = ssm.Ensemble(8, 64, seed=1)
+    assert np.array_equal(R, g2.get_state()[0]) and np.array_equal(S, g2.get_state()[2])
