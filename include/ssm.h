@@ -72,7 +72,7 @@ typedef struct {
     int32_t  sample_every;    /* feed the G(t) correlator after every k-th step; 0 = off          */
     int32_t  corr_levels;     /* multi-tau levels (16); averaging factor m = 2 fixed              */
     int32_t  corr_bins;       /* bins per level (16), even, <= 32                                 */
-    int32_t  corr_groups;     /* chain groups for the standard error (32); group = chain % groups */
+    int32_t  corr_groups;     /* chain groups for the standard error (32); group = (chain / 32) % groups */
     int32_t  k_attempts;      /* K of eqs (50), (51), "an integer parameter which can depend on Z"    */
                               /* (P:L328): 0 = K = N - Z (the paper's GPU choice);           */
                               /* k > 0 = K = min(k, N - Z) (k = 1 is the paper's CPU choice)         */

@@ -474,7 +474,7 @@ static void *worker(void *arg)
                     for (int t = 0; t < 6; ++t) { o[t] += sig[t]; o[6 + t] += sigv[t]; }
                 }
                 if (smp)
-                    oracle_corr_push(w->corr, k, (int)(chain % (uint64_t)w->corr->groups),
+                    oracle_corr_push(w->corr, k, (int)((chain / 32) % (uint64_t)w->corr->groups),   /* DESIGN.md section 7 */
                                      sig[3], sig[3] + sigv[3]);
             }
         }

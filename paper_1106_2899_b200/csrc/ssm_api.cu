@@ -450,15 +450,18 @@ extern "C" int ssm_gt_sums(ssm_ctx *c, double *h_sum, int64_t *h_count)
     std::vector<long long> raw(n);
     CK(c, cudaMemcpyAsync(raw.data(), c->ws + c->lay.csum, n * 8, cudaMemcpyDeviceToHost, c->st));
     CK(c, cudaStreamSynchronize(c->st));
-    for (int g = 0; g < p.corr_groups; ++g) {
-        // chains of this group among the local ones: global index = chain_offset + k, group = index % groups
-        const unsigned long long first = (p.chain_offset % (unsigned)p.corr_groups);
-        long long ng = 0;
-        {   // count k in [0, M) with (first + k) % groups == g
-            const long long G = p.corr_groups, M = p.n_chains;
-            const long long r = ((long long)g - (long long)first % G + G) % G;
-            ng = r < M ? (M - 1 - r) / G + 1 : 0;
+    // chains per group among the local ones: global index = chain_offset + k, group = (index / 32) % groups
+    // (a warp of the correlator kernel, 32 consecutive chains, feeds one group)
+    std::vector<long long> per_group((size_t)p.corr_groups, 0);
+    {
+        const unsigned long long lo = p.chain_offset, hi = p.chain_offset + (unsigned long long)p.n_chains;   // [lo, hi)
+        for (unsigned long long b = lo >> 5; (b << 5) < hi; ++b) {
+            const unsigned long long b0 = b << 5, b1 = b0 + 32;
+            per_group[(size_t)(b % (unsigned)p.corr_groups)] += (long long)((b1 < hi ? b1 : hi) - (b0 > lo ? b0 : lo));
         }
+    }
+    for (int g = 0; g < p.corr_groups; ++g) {
+        const long long ng = per_group[(size_t)g];
         for (int lev = 0; lev < p.corr_levels; ++lev)
             for (int q = 0; q < p.corr_bins; ++q) {
                 const size_t i = ((size_t)g * p.corr_levels + lev) * p.corr_bins + q;

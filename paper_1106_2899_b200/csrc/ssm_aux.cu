@@ -166,32 +166,47 @@ cudaError_t launch_chain_stress(const unsigned char *state, float *out, int N, l
 // ---------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) ssm_corr_kernel(const __grid_constant__ CorrParams C)
 {
-    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= C.M) return;
-    const int L = C.L, Pb = C.Pb;
-    const int group = (int)((C.chain_offset + (unsigned long long)k) % (unsigned)C.groups);
+    const long long k0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool valid = k0 < C.M;
+    const long long k = valid ? k0 : C.M - 1;           // idle lanes of the last warp shadow a real chain and add 0
+    const int L = C.L, Pb = C.Pb, lane = threadIdx.x & 31;
+    // group = (global chain index / 32) % groups: the same for the whole warp when the local chain 0
+    // sits on a multiple of 32 (always, unless a shard starts elsewhere)
+    const int group = (int)(((C.chain_offset + (unsigned long long)k) >> 5) % (unsigned)C.groups);
+    const bool one_group = __all_sync(0xffffffffu, group == __shfl_sync(0xffffffffu, group, 0));
     long long *gsum = C.sum + (long long)group * L * Pb;
     unsigned char pos[kCorrMaxLevels], fil[kCorrMaxLevels], par[kCorrMaxLevels];
     for (int lev = 0; lev < L; ++lev) { pos[lev] = C.pos[lev]; fil[lev] = C.filled[lev]; par[lev] = C.parity[lev]; }
     for (int s = 0; s < C.n_samples; ++s) {
         const float2 fg = C.samples[(long long)s * C.M + k];
         float f = fg.x, g = fg.y;
-        for (int lev = 0; lev < L; ++lev) {
+        for (int lev = 0; lev < L; ++lev) {              // (every bound in here is the same for all chains)
             const long long lm = (long long)lev * C.M + k;
             float *ring = C.ring + (long long)lev * Pb * C.M + k;
             const int p0 = pos[lev];
-            ring[(long long)p0 * C.M] = g;
+            if (valid) ring[(long long)p0 * C.M] = g;
             if (fil[lev] < Pb) ++fil[lev];
             const int kmin = lev == 0 ? 0 : Pb / 2;
             for (int q = kmin; q < fil[lev]; ++q) {
                 int idx = p0 - q; if (idx < 0) idx += Pb;
-                const float prod = f * ring[(long long)idx * C.M];
-                atomicAdd(reinterpret_cast<unsigned long long *>(gsum + lev * Pb + q),
-                          (unsigned long long)__double2ll_rn((double)prod * 65536.0));
+                const float prod = valid ? f * ring[(long long)idx * C.M] : 0.0f;
+                const long long v = __float2ll_rn(prod * 65536.0f);      // fixed point 2^-16
+                if (one_group) {
+                    // exact warp sum of the 64-bit values as two 32-bit integer reductions:
+                    // v = hi 2^20 + lo, 0 <= lo < 2^20 (|v| < 2^46 keeps the sum of 32 hi's in 32 bits)
+                    const int hi = __reduce_add_sync(0xffffffffu, (int)(v >> 20));
+                    const int lo = __reduce_add_sync(0xffffffffu, (int)(v & 0xFFFFF));
+                    if (lane == 0)
+                        atomicAdd(reinterpret_cast<unsigned long long *>(gsum + lev * Pb + q),
+                                  (unsigned long long)(((long long)hi << 20) + (long long)lo));
+                } else if (valid) {
+                    atomicAdd(reinterpret_cast<unsigned long long *>(gsum + lev * Pb + q), (unsigned long long)v);
+                }
             }
             pos[lev] = (unsigned char)((p0 + 1) % Pb);
             if (par[lev] == 0) {
-                C.acc_f[lm] = f; C.acc_g[lm] = g; par[lev] = 1;
+                if (valid) { C.acc_f[lm] = f; C.acc_g[lm] = g; }
+                par[lev] = 1;
                 break;
             }
             f = 0.5f * (C.acc_f[lm] + f); g = 0.5f * (C.acc_g[lm] + g);
