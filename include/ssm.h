@@ -123,6 +123,15 @@ int ssm_chain_stress(ssm_ctx *ctx, float *out, int pointers_are_device);
  * error over chain groups.  All (host). */
 int ssm_gt(ssm_ctx *ctx, int32_t *n_lags, double *h_lag_time, double *h_G, double *h_se);
 
+/* Relative contribution of the virtual stress to the relaxation modulus, eq (66):
+ *   dGv(t) = [<sv(t) s(0)> + <sv(t) sv(0)>] / [<s(t) s(0)> + <s(t) sv(0)>],  s = sigma_xy, sv = sigma^(v)_xy,
+ * from the same multi-tau correlator (it also keeps the sums of g_new g_old, g = s + sv, so that the
+ * numerator is <g(t) g(0)> - <s(t) g(0)>).  Arguments as ssm_gt; h_se = standard error of the ratio
+ * over chain groups (may be NULL).  ssm_gt_sums_virtual returns the raw g g sums,
+ * h_sum_gg (host) [groups][levels][bins], for a multi-GPU reduction beside ssm_gt_sums. */
+int ssm_gt_virtual(ssm_ctx *ctx, int32_t *n_lags, double *h_lag_time, double *h_dgv, double *h_se);
+int ssm_gt_sums_virtual(ssm_ctx *ctx, double *h_sum_gg);
+
 /* Diagnostic for the roofline: measured cycles per warp instruction per
  * scheduler, at the step kernel's residency (4 warps per scheduler), of h_cycles[0] FFMA,
  * [1] LOP3/IADD3/SHF, [2] IMAD, [3] IMAD.WIDE (the 32 x 32 -> 64-bit multiply of Philox).

@@ -75,6 +75,8 @@ def lib():
         L.oracle_corr_push.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_double, C.c_double]
         L.oracle_corr_result.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_int, dp, dp, dp]
         L.oracle_corr_result.restype = C.c_int
+        L.oracle_corr_result_virtual.argtypes = [C.c_void_p, C.c_double, C.c_int, dp, dp, dp]
+        L.oracle_corr_result_virtual.restype = C.c_int
         L.oracle_run.argtypes = [PP, C.POINTER(State), C.c_int64, C.c_double, C.c_int, dp, C.c_int,
                                  C.c_void_p, C.c_double, C.c_int]
         L.oracle_run.restype = C.c_int64
@@ -137,6 +139,14 @@ class Correlator:
         n = lib().oracle_corr_result(self.h, n_beads, base_dt, cap, _dp(t), _dp(G), _dp(se))
         assert n >= 0
         return t[:n].copy(), G[:n].copy(), se[:n].copy()
+
+    def result_virtual(self, base_dt):
+        """eq 66: relative contribution of the virtual stress to G(t), with its standard error."""
+        cap = self.levels * self.bins
+        t = np.zeros(cap); d = np.zeros(cap); se = np.zeros(cap)
+        n = lib().oracle_corr_result_virtual(self.h, base_dt, cap, _dp(t), _dp(d), _dp(se))
+        assert n >= 0
+        return t[:n].copy(), d[:n].copy(), se[:n].copy()
 
     def __del__(self):
         if getattr(self, "h", None):

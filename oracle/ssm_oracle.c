@@ -354,10 +354,12 @@ static void corr_insert(oracle_corr *c, int64_t chain_local, int group, int lev,
     if (*fil < P) ++*fil;
     const int kmin = lev == 0 ? 0 : P / m;
     double *C = c->sum + ((size_t)group * L + lev) * P;
+    double *C2 = c->sum_gg + ((size_t)group * L + lev) * P;
     int64_t *cnt = c->count + ((size_t)group * L + lev) * P;
     for (int k = kmin; k < P && k < *fil; ++k) {
         int idx = *pos - k; if (idx < 0) idx += P;
         C[k] += f * ring[idx];
+        C2[k] += g * ring[idx];           /* for the virtual-stress contribution, eq (66) */
         cnt[k] += 1;
     }
     *pos = (*pos + 1) % P;
@@ -384,6 +386,7 @@ oracle_corr *oracle_corr_create(int64_t n_chains, int levels, int bins, int grou
     c->acc_g = (double *)calloc(nl, sizeof(double));
     c->acc_n = (int *)calloc(nl, sizeof(int));
     c->sum = (double *)calloc((size_t)groups * levels * bins, sizeof(double));
+    c->sum_gg = (double *)calloc((size_t)groups * levels * bins, sizeof(double));
     c->count = (int64_t *)calloc((size_t)groups * levels * bins, sizeof(int64_t));
     return c;
 }
@@ -391,7 +394,7 @@ void oracle_corr_destroy(oracle_corr *c)
 {
     if (!c) return;
     free(c->ring); free(c->pos); free(c->filled); free(c->acc_f); free(c->acc_g); free(c->acc_n);
-    free(c->sum); free(c->count); free(c);
+    free(c->sum); free(c->sum_gg); free(c->count); free(c);
 }
 void oracle_corr_push(oracle_corr *c, int64_t chain_local, int group, double f, double g)
 {
@@ -429,6 +432,46 @@ int oracle_corr_result(const oracle_corr *c, int n_beads, double base_dt, int ca
                             double v = c->sum[((size_t)g * L + lev) * P + k] / ((double)cg * n_beads) - mean;
                             var += v * v;
                         }
+                    }
+                    se[n] = sqrt(var / (used - 1) / used);
+                } else se[n] = NAN;
+            }
+            ++n;
+        }
+    return n;
+}
+
+/* Relative contribution of the virtual stress to the relaxation modulus, eq (66) P:L438:
+ *   dGv(t) = [<sv(t) s(0)> + <sv(t) sv(0)>] / [<s(t) s(0)> + <s(t) sv(0)>],  s = sigma_xy, sv = sigma^(v)_xy.
+ * With g = s + sv the denominator is <s(t) g(0)> (the sums of eq 43) and the numerator is
+ * <sv(t) g(0)> = <g(t) g(0)> - <s(t) g(0)>.  se = std over groups of the per-group ratio / sqrt(groups). */
+int oracle_corr_result_virtual(const oracle_corr *c, double base_dt, int cap,
+                               double *lag_time, double *dGv, double *se)
+{
+    const int L = c->levels, P = c->bins, Gn = c->groups;
+    int n = 0;
+    for (int lev = 0; lev < L; ++lev)
+        for (int k = (lev == 0 ? 0 : P / 2); k < P; ++k) {
+            double sfg = 0.0, sgg = 0.0; int64_t cn = 0;
+            for (int g = 0; g < Gn; ++g) {
+                size_t i = ((size_t)g * L + lev) * P + k;
+                sfg += c->sum[i]; sgg += c->sum_gg[i]; cn += c->count[i];
+            }
+            if (cn == 0) continue;
+            if (n >= cap) return -1;
+            lag_time[n] = (double)k * ldexp(1.0, lev) * base_dt;
+            dGv[n] = (sgg - sfg) / sfg;
+            if (se) {
+                double mean = 0.0, var = 0.0; int used = 0;
+                for (int g = 0; g < Gn; ++g) {
+                    size_t i = ((size_t)g * L + lev) * P + k;
+                    if (c->count[i] > 0) { mean += (c->sum_gg[i] - c->sum[i]) / c->sum[i]; ++used; }
+                }
+                if (used > 1) {
+                    mean /= used;
+                    for (int g = 0; g < Gn; ++g) {
+                        size_t i = ((size_t)g * L + lev) * P + k;
+                        if (c->count[i] > 0) { double v = (c->sum_gg[i] - c->sum[i]) / c->sum[i] - mean; var += v * v; }
                     }
                     se[n] = sqrt(var / (used - 1) / used);
                 } else se[n] = NAN;

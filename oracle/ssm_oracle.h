@@ -51,7 +51,8 @@ typedef struct {
 typedef struct {
     int64_t n_chains; int levels, bins, groups;
     double *ring; int *pos, *filled; double *acc_f, *acc_g; int *acc_n;
-    double *sum; int64_t *count;   /* [groups][levels][bins] */
+    double *sum; int64_t *count;   /* [groups][levels][bins]: sum of f_new g_old (eq 43) */
+    double *sum_gg;                /* [groups][levels][bins]: sum of g_new g_old (eq 66) */
 } oracle_corr;
 
 void     oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
@@ -75,6 +76,8 @@ void     oracle_corr_destroy(oracle_corr *c);
 void     oracle_corr_push(oracle_corr *c, int64_t chain_local, int group, double f, double g);
 int      oracle_corr_result(const oracle_corr *c, int n_beads, double base_dt, int cap,
                             double *lag_time, double *G, double *se);
+int      oracle_corr_result_virtual(const oracle_corr *c, double base_dt, int cap,
+                                    double *lag_time, double *dGv, double *se);
 int64_t  oracle_run(const oracle_params *p, oracle_state *st, int64_t n_steps, double shear_rate,
                     int stress_every, double *stress_out, int sample_every, oracle_corr *corr,
                     double guard, int n_threads);

@@ -17,7 +17,8 @@ SSM_OK, SSM_EINVAL, SSM_ENOMEM, SSM_ECUDA, SSM_ESTATE, SSM_ERANGE = 0, -1, -2, -
 EXPORTS = ["ssm_workspace_bytes", "ssm_init", "ssm_step", "ssm_stress_count", "ssm_stress", "ssm_stress_sums",
            "ssm_stress_sums_device", "ssm_chain_stress", "ssm_gt", "ssm_gt_sums", "ssm_get_state", "ssm_set_state",
            "ssm_reset_accumulators", "ssm_launch_count", "ssm_set_fusion", "ssm_set_grid", "ssm_destroy", "ssm_last_error",
-           "ssm_moduli", "ssm_eta0", "ssm_tau_d", "ssm_issue_rates"]
+           "ssm_moduli", "ssm_eta0", "ssm_tau_d", "ssm_issue_rates",
+           "ssm_gt_virtual", "ssm_gt_sums_virtual"]
 
 
 class Params(C.Structure):
@@ -65,6 +66,8 @@ def lib():
     L.ssm_destroy.argtypes = [vp]; L.ssm_destroy.restype = None
     L.ssm_last_error.argtypes = [vp]; L.ssm_last_error.restype = C.c_char_p
     L.ssm_issue_rates.argtypes = [vp, dp]; L.ssm_issue_rates.restype = C.c_int
+    L.ssm_gt_virtual.argtypes = [vp, C.POINTER(C.c_int32), dp, dp, dp]; L.ssm_gt_virtual.restype = C.c_int
+    L.ssm_gt_sums_virtual.argtypes = [vp, dp]; L.ssm_gt_sums_virtual.restype = C.c_int
     L.ssm_moduli.argtypes = [C.c_int32, dp, dp, C.c_int32, dp, dp, dp]; L.ssm_moduli.restype = C.c_int
     L.ssm_eta0.argtypes = [C.c_int32, dp, dp, dp]; L.ssm_eta0.restype = C.c_int
     L.ssm_tau_d.argtypes = [C.c_int32, dp, dp, C.c_double, C.c_double, dp]; L.ssm_tau_d.restype = C.c_int
@@ -181,6 +184,15 @@ class Ensemble:
             return a
         self._ck(lib().ssm_chain_stress(self.h, C.c_void_p(out.data_ptr()), 1))
         return out
+
+    def gt_virtual(self):
+        """ssm_gt_virtual: (lag times, dGv(t) of eq 66, standard error)."""
+        cap = self.p.corr_levels * self.p.corr_bins
+        n = C.c_int32(cap)
+        t = np.zeros(cap); d = np.zeros(cap); se = np.zeros(cap)
+        dd = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+        self._ck(lib().ssm_gt_virtual(self.h, C.byref(n), dd(t), dd(d), dd(se)))
+        return t[:n.value].copy(), d[:n.value].copy(), se[:n.value].copy()
 
     def gt(self):
         cap = self.p.corr_levels * self.p.corr_bins

@@ -99,7 +99,8 @@ static Layout make_layout(const ssm_params *p)
     L.ring = o; if (corr) o = align_up(o + (size_t)p->corr_levels * p->corr_bins * M * 4, 256);
     L.accf = o; if (corr) o = align_up(o + (size_t)p->corr_levels * M * 4, 256);
     L.accg = o; if (corr) o = align_up(o + (size_t)p->corr_levels * M * 4, 256);
-    L.csum = o; if (corr) o = align_up(o + (size_t)p->corr_groups * p->corr_levels * p->corr_bins * 8, 256);
+    // two sum arrays: f_new g_old (eq 43) and g_new g_old (eq 66)
+    L.csum = o; if (corr) o = align_up(o + 2 * (size_t)p->corr_groups * p->corr_levels * p->corr_bins * 8, 256);
     // staging for host-pointer get/set state and chain stress: chunks of <= 65536 chains
     L.stage_chains = p->n_chains < 65536 ? p->n_chains : 65536;
     // (at least 1 MB, so that the issue-rate probe's scratch of 2 kB per SM fits any ensemble)
@@ -277,6 +278,7 @@ extern "C" int ssm_step(ssm_ctx *c, int64_t n_steps, double shear_rate)
             cp.acc_f = reinterpret_cast<float *>(c->ws + c->lay.accf);
             cp.acc_g = reinterpret_cast<float *>(c->ws + c->lay.accg);
             cp.sum = reinterpret_cast<long long *>(c->ws + c->lay.csum);
+            cp.sum_gg = cp.sum + (size_t)p.corr_groups * p.corr_levels * p.corr_bins;
             cp.M = p.n_chains; cp.chain_offset = p.chain_offset;
             cp.n_samples = (int)nsmp; cp.L = p.corr_levels; cp.Pb = p.corr_bins; cp.groups = p.corr_groups;
             std::memcpy(cp.pos, c->cpos, sizeof cp.pos); std::memcpy(cp.filled, c->cfil, sizeof cp.filled);
@@ -469,6 +471,67 @@ extern "C" int ssm_gt_sums(ssm_ctx *c, double *h_sum, int64_t *h_count)
                 h_count[i] = c->ccount[(size_t)lev * 32 + q] * ng;
             }
     }
+    return SSM_OK;
+}
+
+extern "C" int ssm_gt_sums_virtual(ssm_ctx *c, double *h_sum_gg)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    const ssm_params &p = c->p;
+    if (p.sample_every <= 0) return fail(c, SSM_ESTATE, "correlator is off (sample_every = 0)");
+    if (!h_sum_gg) return fail(c, SSM_EINVAL, "NULL output");
+    const size_t n = (size_t)p.corr_groups * p.corr_levels * p.corr_bins;
+    std::vector<long long> raw(n);
+    CK(c, cudaMemcpyAsync(raw.data(), c->ws + c->lay.csum + n * 8, n * 8, cudaMemcpyDeviceToHost, c->st));
+    CK(c, cudaStreamSynchronize(c->st));
+    for (size_t i = 0; i < n; ++i) h_sum_gg[i] = (double)raw[i] / 65536.0;
+    return SSM_OK;
+}
+
+// eq (66): dGv(t) = <sv(t) g(0)> / <s(t) g(0)> = (sum_gg - sum_fg) / sum_fg, g = s + sv
+extern "C" int ssm_gt_virtual(ssm_ctx *c, int32_t *n_lags, double *h_t, double *h_dgv, double *h_se)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (!n_lags || !h_t || !h_dgv) return fail(c, SSM_EINVAL, "NULL output");
+    const ssm_params &p = c->p;
+    if (p.sample_every <= 0) return fail(c, SSM_ESTATE, "correlator is off (sample_every = 0)");
+    const int L = p.corr_levels, Pb = p.corr_bins, Gn = p.corr_groups;
+    const size_t n_all = (size_t)Gn * L * Pb;
+    std::vector<double> fg(n_all), gg(n_all); std::vector<int64_t> cnt(n_all);
+    int rc = ssm_gt_sums(c, fg.data(), cnt.data());
+    if (rc == SSM_OK) rc = ssm_gt_sums_virtual(c, gg.data());
+    if (rc != SSM_OK) return rc;
+    const double base = p.dt * p.sample_every;
+    int n = 0;
+    for (int lev = 0; lev < L; ++lev)
+        for (int q = (lev == 0 ? 0 : Pb / 2); q < Pb; ++q) {
+            double sfg = 0.0, sgg = 0.0; int64_t cn = 0;
+            for (int g = 0; g < Gn; ++g) {
+                const size_t i = ((size_t)g * L + lev) * Pb + q;
+                sfg += fg[i]; sgg += gg[i]; cn += cnt[i];
+            }
+            if (cn == 0) continue;
+            if (n >= *n_lags) return fail(c, SSM_ERANGE, "n_lags capacity too small");
+            h_t[n] = (double)q * std::ldexp(1.0, lev) * base;
+            h_dgv[n] = (sgg - sfg) / sfg;
+            if (h_se) {
+                double mean = 0.0, var = 0.0; int used = 0;
+                for (int g = 0; g < Gn; ++g) {
+                    const size_t i = ((size_t)g * L + lev) * Pb + q;
+                    if (cnt[i] > 0) { mean += (gg[i] - fg[i]) / fg[i]; ++used; }
+                }
+                if (used > 1) {
+                    mean /= used;
+                    for (int g = 0; g < Gn; ++g) {
+                        const size_t i = ((size_t)g * L + lev) * Pb + q;
+                        if (cnt[i] > 0) { const double v = (gg[i] - fg[i]) / fg[i] - mean; var += v * v; }
+                    }
+                    h_se[n] = std::sqrt(var / (used - 1) / used);
+                } else h_se[n] = NAN;
+            }
+            ++n;
+        }
+    *n_lags = n;
     return SSM_OK;
 }
 

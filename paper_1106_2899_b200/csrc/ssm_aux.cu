@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(256) ssm_corr_kernel(const __grid_constant__ C
     // sits on a multiple of 32 (always, unless a shard starts elsewhere)
     const int group = (int)(((C.chain_offset + (unsigned long long)k) >> 5) % (unsigned)C.groups);
     const bool one_group = __all_sync(0xffffffffu, group == __shfl_sync(0xffffffffu, group, 0));
-    long long *gsum = C.sum + (long long)group * L * Pb;
+    long long *gsum = C.sum + (long long)group * L * Pb, *gsum2 = C.sum_gg + (long long)group * L * Pb;
     unsigned char pos[kCorrMaxLevels], fil[kCorrMaxLevels], par[kCorrMaxLevels];
     for (int lev = 0; lev < L; ++lev) { pos[lev] = C.pos[lev]; fil[lev] = C.filled[lev]; par[lev] = C.parity[lev]; }
     for (int s = 0; s < C.n_samples; ++s) {
@@ -189,18 +189,25 @@ __global__ void __launch_bounds__(256) ssm_corr_kernel(const __grid_constant__ C
             const int kmin = lev == 0 ? 0 : Pb / 2;
             for (int q = kmin; q < fil[lev]; ++q) {
                 int idx = p0 - q; if (idx < 0) idx += Pb;
-                const float prod = valid ? f * ring[(long long)idx * C.M] : 0.0f;
-                const long long v = __float2ll_rn(prod * 65536.0f);      // fixed point 2^-16
+                const float old = valid ? ring[(long long)idx * C.M] : 0.0f;
+                // fixed point 2^-16: f_new g_old for G(t) (eq 43), g_new g_old for the virtual-stress share (eq 66)
+                const long long v = __float2ll_rn(f * old * 65536.0f), v2 = __float2ll_rn(g * old * 65536.0f);
                 if (one_group) {
-                    // exact warp sum of the 64-bit values as two 32-bit integer reductions:
+                    // exact warp sums of the 64-bit values as two 32-bit integer reductions each:
                     // v = hi 2^20 + lo, 0 <= lo < 2^20 (|v| < 2^46 keeps the sum of 32 hi's in 32 bits)
                     const int hi = __reduce_add_sync(0xffffffffu, (int)(v >> 20));
                     const int lo = __reduce_add_sync(0xffffffffu, (int)(v & 0xFFFFF));
-                    if (lane == 0)
+                    const int hi2 = __reduce_add_sync(0xffffffffu, (int)(v2 >> 20));
+                    const int lo2 = __reduce_add_sync(0xffffffffu, (int)(v2 & 0xFFFFF));
+                    if (lane == 0) {
                         atomicAdd(reinterpret_cast<unsigned long long *>(gsum + lev * Pb + q),
                                   (unsigned long long)(((long long)hi << 20) + (long long)lo));
+                        atomicAdd(reinterpret_cast<unsigned long long *>(gsum2 + lev * Pb + q),
+                                  (unsigned long long)(((long long)hi2 << 20) + (long long)lo2));
+                    }
                 } else if (valid) {
                     atomicAdd(reinterpret_cast<unsigned long long *>(gsum + lev * Pb + q), (unsigned long long)v);
+                    atomicAdd(reinterpret_cast<unsigned long long *>(gsum2 + lev * Pb + q), (unsigned long long)v2);
                 }
             }
             pos[lev] = (unsigned char)((p0 + 1) % Pb);

@@ -97,7 +97,8 @@ struct CorrParams {
     const float2 *samples;     // [n_samples][M] (f, g) = (sigma_xy, sigma_xy + sigma^(v)_xy)
     float *ring;               // [L][P][M] block-averaged g history
     float *acc_f, *acc_g;      // [L][M] first element of the pending pair
-    long long *sum;            // [groups][L][P] int64 fixed point (2^-16)
+    long long *sum;            // [groups][L][P] int64 fixed point (2^-16): f_new g_old (eq 43)
+    long long *sum_gg;         // [groups][L][P] int64 fixed point (2^-16): g_new g_old (eq 66)
     long long M;
     unsigned long long chain_offset;
     int n_samples, L, Pb, groups;

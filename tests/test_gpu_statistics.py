@@ -250,3 +250,25 @@ def test_rouse_limit_gt_to_viscosity_and_relaxation_time(ssm):
     g1, g2 = ssm.moduli(t, G, w)
     x1, x2 = ref.moduli(t, Gx, w)
     assert np.allclose(g1, x1, rtol=0.1) and np.allclose(g2, x2, rtol=0.1), (g1, x1, g2, x2)
+
+
+def test_virtual_stress_contribution_gpu_vs_oracle(ssm):
+    """eq 66 from the GPU correlator (ssm_gt_virtual) against the oracle's independent estimate,
+    within 3 combined standard errors, and against the closed form at t = 0."""
+    N, steps, levels, groups = 32, 5000, 6, 32
+    e = oracle.Ensemble(N, 512, seed=301)
+    c = oracle.Correlator(512, levels=levels, bins=16, groups=groups)
+    e.run(steps, sample_every=10, corr=c, n_threads=8)
+    t0, d0, se0 = c.result_virtual(0.1)
+    g = ssm.Ensemble(N, 8192, seed=302, sample_every=10, corr_levels=levels, corr_bins=16, corr_groups=groups)
+    g.step(steps)
+    t1, d1, se1 = g.gt_virtual()
+    assert np.allclose(t0, t1)
+    z = (d1 - d0) / np.sqrt(se0 ** 2 + se1 ** 2)
+    assert np.mean(np.abs(z) < 3.0) >= 0.95 and np.abs(z).max() < 4.5, z
+    static = (N / 4.0) / (N - 1.0)
+    assert abs(d1[0] - static) < 0.05 * static
+    # Rouse limit: no virtual stress at all
+    r = ssm.Ensemble(8, 1024, n_0=0.0, seed=5, sample_every=10, corr_levels=3, corr_bins=16, corr_groups=32)
+    r.step(600)
+    assert np.allclose(r.gt_virtual()[1], 0.0, atol=1e-12)
