@@ -164,12 +164,16 @@ def test_split_runs_fusion_depth_and_ensemble_size_do_not_change_results(ssm):
     assert np.array_equal(R, R0[:, :, 128:192]) and np.array_equal(S, S0[:, 128:192])
 
 
-def test_correlator_matches_oracle_on_identical_trajectories(ssm):
+@pytest.mark.parametrize("M,offset", [(512, 0), (500, 7)])
+def test_correlator_matches_oracle_on_identical_trajectories(ssm, M, offset):
     """Rouse limit (no forks): GPU multi-tau sums against the oracle's correlator fed by
-    the oracle's own stresses of the same trajectories."""
-    N, M, steps = 8, 512, 2000
-    e = oracle.Ensemble(N, M, n_0=0.0, seed=13)
-    g = ssm.Ensemble(N, M, n_0=0.0, seed=13, sample_every=10, corr_levels=6, corr_bins=16, corr_groups=32)
+    the oracle's own stresses of the same trajectories.  (500, 7): a ragged last warp and a
+    shard that does not start on a multiple of 32, so that a warp's chains fall into two
+    groups (the per-lane path of the correlator kernel)."""
+    N, steps = 8, 2000
+    e = oracle.Ensemble(N, M, n_0=0.0, seed=13, chain_offset=offset)
+    g = ssm.Ensemble(N, M, n_0=0.0, seed=13, chain_offset=offset, sample_every=10, corr_levels=6, corr_bins=16,
+                     corr_groups=32)
     upload(e, g)
     corr = oracle.Correlator(M, levels=6, bins=16, groups=32)
     e.run(steps, sample_every=10, corr=corr)
