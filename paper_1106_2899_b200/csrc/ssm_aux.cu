@@ -21,7 +21,7 @@ __global__ void __launch_bounds__(128) ssm_init_kernel(const __grid_constant__ I
     if (k >= P.n_chains_padded) return;
     const int N = P.n_beads, zmax = N;
     const uint32_t chain = (uint32_t)(P.chain_offset + (unsigned long long)k);
-    const StreamKey sk = make_stream(0ull);
+    const StreamKey sk = make_stream(0ull, P.rk);
     const BoxMuller bm_bond(P.bm_bond), bm_anchor(P.bm_anchor);
     unsigned char *st = P.state;
 

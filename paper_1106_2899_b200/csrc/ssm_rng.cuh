@@ -51,19 +51,54 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 }
 
 // counter = (step low 32, domain<<28 | step bits 32..59, global chain index, item)
+//
+// The first counter word (the step) is the same for every call of a time step, so what the
+// first round makes of it is formed ONCE per step: M0 * step gives hi ^ k1 (xored with the
+// item in round 1) and lo ^ (k1 + W1) (xored with a product in round 2).  A call then spends
+// one wide multiply in round 1 instead of two, and the two xors that would take two uniform
+// operands take one.  The result is Philox4x32-10 of the counter above, bit for bit.
 struct StreamKey {
-    uint32_t c0, c1hi;      // step low 32 bits, step bits 32..59
+    uint32_t c1hi;          // step bits 32..59
+    uint32_t a1;            // hi(M0 * step low 32) ^ rk[1]
+    uint32_t b3;            // lo(M0 * step low 32) ^ rk[3]
 };
-__device__ __forceinline__ StreamKey make_stream(unsigned long long step)
+__device__ __forceinline__ StreamKey make_stream(unsigned long long step, const unsigned (&rk)[20])
 {
-    StreamKey s; s.c0 = (uint32_t)step;
+    const uint64_t p0 = (uint64_t)0xD2511F53u * (uint32_t)step;
+    StreamKey s;
     s.c1hi = (uint32_t)(step >> 32) & 0x0FFFFFFFu;
+    s.a1 = (uint32_t)(p0 >> 32) ^ rk[1];
+    s.b3 = (uint32_t)p0 ^ rk[3];
     return s;
 }
 __device__ __forceinline__ void stream_call(const StreamKey& s, const unsigned (&rk)[20], uint32_t domain,
                                             uint32_t chain, uint32_t item, uint32_t (&w)[4])
 {
-    philox4x32_10(s.c0, (domain << 28) | s.c1hi, chain, item, rk, w);
+    constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+    // round 1 on (step, domain | step hi, chain, item)
+    const uint64_t q1 = (uint64_t)M1 * chain;
+    uint32_t c0 = (uint32_t)(q1 >> 32) ^ (((domain << 28) | s.c1hi) ^ rk[0]);
+    uint32_t c1 = (uint32_t)q1;
+    uint32_t c2 = s.a1 ^ item;
+    // round 2: its c3 is lo(M0 * step), already folded with rk[3] into b3
+    {
+        const uint64_t p0 = (uint64_t)M0 * c0;
+        const uint64_t p1 = (uint64_t)M1 * c2;
+        c0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk[2];
+        c2 = (uint32_t)(p0 >> 32) ^ s.b3;
+        c1 = (uint32_t)p1;
+        const uint32_t c3 = (uint32_t)p0;
+        uint32_t d3 = c3;
+#pragma unroll
+        for (int r = 2; r < 10; ++r) {
+            const uint64_t t0 = (uint64_t)M0 * c0;
+            const uint64_t t1 = (uint64_t)M1 * c2;
+            c0 = (uint32_t)(t1 >> 32) ^ c1 ^ rk[2 * r];
+            c2 = (uint32_t)(t0 >> 32) ^ d3 ^ rk[2 * r + 1];
+            c1 = (uint32_t)t1; d3 = (uint32_t)t0;
+        }
+        w[0] = c0; w[1] = c1; w[2] = c2; w[3] = d3;
+    }
 }
 
 // 23-bit code k = w >> 9 and the uniform u = (k + 1/2) 2^-23 in (0,1); exact in fp32:

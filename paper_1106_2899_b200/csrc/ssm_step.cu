@@ -261,7 +261,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
             if (n == P.n_fuse) break;
 
             const unsigned long long step = P.step0 + (unsigned long long)n;
-            const StreamKey sk = make_stream(step);
+            const StreamKey sk = make_stream(step, P.rk);
             const bool record = (P.rec_mask >> n) & 1u;
             const bool sample = (P.smp_mask >> n) & 1u;
             const int Z0 = Zs[cw];
