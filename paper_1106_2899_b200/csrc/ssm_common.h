@@ -28,11 +28,12 @@ constexpr int kFxShift = 26;                 // slip-spring displacement fixed p
 constexpr int kStressShift = 18;             // ensemble stress fixed point: 2^-18 kT per lane share
 constexpr int kSampleShift = 20;             // per-chain slip-spring virial (correlator samples): 2^-20
 
-// per-warp shared memory of the step kernel.  Two arrays are padded so that the bead lanes'
-// 16-byte accesses (one per lane, consecutive lanes) fall into distinct banks:
-//   bead b of the warp (0..255) sits at float4 index  b + (b >> 3)      (9 float4 per lane)
-//   its coordinate c at int index  (b >> 3) * 28 + (b & 7) * 3 + c      (28 ints per lane)
-constexpr int kSmRm = 0;         // float4[288] bead positions mirror (x, y, z, -), padded
+// per-warp shared memory of the step kernel.  The bead positions and the slip-spring force
+// accumulators share one index: coordinate c of bead b of the warp (0..255) sits at word
+//   (b >> 3) * 28 + (b & 7) * 3 + c      (28 words per lane: 24 used + 4 of padding)
+// so that the bead lanes move their 24 words as 6 aligned 16-byte accesses (consecutive lanes
+// 112 bytes apart: conflict-free) and the position mirror is the lane's register image as it is.
+constexpr int kSmRm = 0;         // float[896]  bead positions mirror (+1 kB spare up to kSmA)
 constexpr int kSmA = 4608;       // float4[256] anchors [chain][slot] (x, y, z, x low part)
 constexpr int kSmFx = 8704;      // int  [896]  fixed-point slip-spring displacement per bead coordinate, padded
 constexpr int kSmS = 12288;      // uint8[256]  bead index per slot
@@ -48,7 +49,6 @@ constexpr int kSmMap = 13712;    // uint8[128]  dealing map: byte 4 lane + it = 
 constexpr int kSmWarp = 13968;
 constexpr int kSmAcc = kWarpsPerBlock * kSmWarp;                          // int64 [kMaxFuse][12] per CTA
 constexpr int kSmStep = kSmAcc + kMaxFuse * 12 * 8;                       // 114,816 B: 2 CTAs per SM (2 x (114,816 + 1024) <= 233,472)
-__host__ __device__ constexpr int rm_index(int bead_in_warp) { return bead_in_warp + (bead_in_warp >> 3); }
 __host__ __device__ constexpr int fx_index(int bead_in_warp) { return (bead_in_warp >> 3) * 28 + (bead_in_warp & 7) * 3; }
 
 struct StepParams {

@@ -43,7 +43,11 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int l = lane & (G - 1), cw = lane >> LG;
     unsigned char *wb = smem + warp * kSmWarp;
-    float4 *Rm = reinterpret_cast<float4 *>(wb + kSmRm);
+    // mirror of the bead positions: the lane's 24 register floats as they are (6 x 16 bytes,
+    // 28 floats per lane: the same index as Fx), read by the slot phase as three scalars per bead
+    float *Rf = reinterpret_cast<float *>(wb + kSmRm);
+    float4 *Rf4 = reinterpret_cast<float4 *>(wb + kSmRm);
+    auto bead = [&](int fi) -> float4 { return make_float4(Rf[fi], Rf[fi + 1], Rf[fi + 2], 0.0f); };
     float4 *A4 = reinterpret_cast<float4 *>(wb + kSmA);
     int *Fx = reinterpret_cast<int *>(wb + kSmFx);
     int4 *Fx4 = reinterpret_cast<int4 *>(wb + kSmFx);
@@ -145,7 +149,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
             reinterpret_cast<uint2 *>(Sb)[lane] = reinterpret_cast<const uint2 *>(tp + kTileS)[lane];
             Zs[lane] = reinterpret_cast<const int *>(tp + kTileZ)[lane];
 #pragma unroll
-            for (int k = 0; k < 8; ++k) Rm[lane * 9 + k] = make_float4(r[3 * k], r[3 * k + 1], r[3 * k + 2], 0.0f);
+            for (int v = 0; v < 6; ++v) Rf4[lane * 7 + v] = make_float4(r[4 * v], r[4 * v + 1], r[4 * v + 2], r[4 * v + 3]);
         }
         __syncwarp();
         int Tz = deal(Zs[cw]);
@@ -156,7 +160,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
             for (int it = 0, f = lane; f < Tz; f += 32, ++it) {
                 const int sidx = slot_index(it, f), base = sidx & ~(N - 1);
                 const int s = Sb[sidx];
-                const float4 a = A4[sidx], rb = Rm[rm_index(base + s - 1)];
+                const float4 a = A4[sidx], rb = bead(fx_index(base + s - 1));
                 int *fp = Fx + fx_index(base + s - 1);
                 atomicAdd(fp, __float2int_rn(-P.fx_scale * (rb.x - a.x)));
                 atomicAdd(fp + 1, __float2int_rn(-P.fx_scale * (rb.y - a.y)));
@@ -288,7 +292,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                 }
             }
 #pragma unroll
-            for (int k = 0; k < 8; ++k) Rm[lane * 9 + k] = make_float4(r[3 * k], r[3 * k + 1], r[3 * k + 2], 0.0f);
+            for (int v = 0; v < 6; ++v) Rf4[lane * 7 + v] = make_float4(r[4 * v], r[4 * v + 1], r[4 * v + 2], r[4 * v + 3]);
             __syncwarp();
 
             // ================= slot phase: substeps 2 and 3 =================
@@ -325,9 +329,11 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     // p+- = min{ h [1 - tanh x+-], 1/2 } = min{ 2h / (1 + e^{2 x+-}), 1/2 },
                     // x+- = (3/4N_s)(|R_{s+-1}-A|^2 - |R_s-A|^2)
                     const int b0 = base + s - 1;
-                    const float4 r0 = Rm[rm_index(b0)];
-                    const float4 rp = Rm[rm_index(b0 + (s < N ? 1 : 0))];
-                    const float4 rm = Rm[rm_index(b0 - (s > 1 ? 1 : 0))];
+                    // neighbours along the chain are 3 floats away, 7 across a lane boundary (4 floats of padding)
+                    const int fi = fx_index(b0), kb = b0 & 7;
+                    const float4 r0 = bead(fi);
+                    const float4 rp = bead(fi + (s < N ? (kb == 7 ? 7 : 3) : 0));
+                    const float4 rm = bead(fi - (s > 1 ? (kb == 0 ? 7 : 3) : 0));
                     const float d0x = r0.x - a.x, d0y = r0.y - a.y, d0z = r0.z - a.z;
                     const float dpx = rp.x - a.x, dpy = rp.y - a.y, dpz = rp.z - a.z;
                     const float dmx = rm.x - a.x, dmy = rm.y - a.y, dmz = rm.z - a.z;
@@ -354,7 +360,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     const float dy = live ? (up ? dpy : (dn ? dmy : d0y)) : 0.0f;
                     const float dz = live ? (up ? dpz : (dn ? dmz : d0z)) : 0.0f;
                     if (live) {
-                        int *fp = Fx + fx_index(b0 + sn - s);
+                        int *fp = Fx + fi + (up ? (kb == 7 ? 7 : 3) : 0) - (dn ? (kb == 0 ? 7 : 3) : 0);
                         atomicAdd(fp, __float2int_rn(-P.fx_scale * dx));
                         atomicAdd(fp + 1, __float2int_rn(-P.fx_scale * dy));
                         atomicAdd(fp + 2, __float2int_rn(-P.fx_scale * dz));
@@ -441,7 +447,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                                 float z3[3], unused;
                                 bm_anchor(wa[0], z3[0], z3[1]);                                       // eq 52
                                 bm_anchor(wa[1], z3[2], unused);
-                                const float4 rb = Rm[rm_index(base + snew - 1)];
+                                const float4 rb = bead(fx_index(base + snew - 1));
                                 const float4 a = make_float4(rb.x + z3[0], rb.y + z3[1], rb.z + z3[2], 0.0f);
                                 Sb[base + Zn] = (unsigned char)snew;
                                 A4[base + Zn] = a;
