@@ -355,20 +355,19 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                         atomicOr(Dm + c * WPC + (j >> 5), 1u << (j & 31));
                         event = true;
                     }
-                    // a destroyed slip-spring exerts no force and has no virial: zero displacement
-                    const float dx = live ? (up ? dpx : (dn ? dmx : d0x)) : 0.0f;
-                    const float dy = live ? (up ? dpy : (dn ? dmy : d0y)) : 0.0f;
-                    const float dz = live ? (up ? dpz : (dn ? dmz : d0z)) : 0.0f;
+                    // a destroyed slip-spring exerts no force and has no virial
                     if (live) {
+                        const float dx = up ? dpx : (dn ? dmx : d0x), dy = up ? dpy : (dn ? dmy : d0y),
+                                    dz = up ? dpz : (dn ? dmz : d0z);
                         int *fp = Fx + fi + (up ? (kb == 7 ? 7 : 3) : 0) - (dn ? (kb == 0 ? 7 : 3) : 0);
                         atomicAdd(fp, __float2int_rn(-P.fx_scale * dx));
                         atomicAdd(fp + 1, __float2int_rn(-P.fx_scale * dy));
                         atomicAdd(fp + 2, __float2int_rn(-P.fx_scale * dz));
+                        sv[0] = fmaf(dx, dx, sv[0]); sv[1] = fmaf(dy, dy, sv[1]); sv[2] = fmaf(dz, dz, sv[2]);
+                        sv[3] = fmaf(dx, dy, sv[3]); sv[4] = fmaf(dy, dz, sv[4]); sv[5] = fmaf(dz, dx, sv[5]);
+                        cnt += 1.0f;
+                        if (sample) atomicAdd(Samp + c, __float2int_rn(dx * dy * (float)(1 << kSampleShift)));
                     }
-                    sv[0] = fmaf(dx, dx, sv[0]); sv[1] = fmaf(dy, dy, sv[1]); sv[2] = fmaf(dz, dz, sv[2]);
-                    sv[3] = fmaf(dx, dy, sv[3]); sv[4] = fmaf(dy, dz, sv[4]); sv[5] = fmaf(dz, dx, sv[5]);
-                    cnt += live ? 1.0f : 0.0f;
-                    if (sample && live) atomicAdd(Samp + c, __float2int_rn(dx * dy * (float)(1 << kSampleShift)));
                 }
                 // construction attempts (eqs 50, 51), drawn by the chain's own lanes; K = N - Z
                 // or a fixed K.  The 23-bit code of attempt k is (h << 7) | e (DESIGN.md
