@@ -48,7 +48,8 @@ constexpr int kSmMap = 13712;    // uint8[128]  dealing map: byte 4 lane + it = 
                                  //             slip-spring number lane + 32 it (it = 0..3), rebuilt when some Z changes
 constexpr int kSmWarp = 13968;
 constexpr int kSmAcc = kWarpsPerBlock * kSmWarp;                          // int64 [kMaxFuse][12] per CTA
-constexpr int kSmStep = kSmAcc + kMaxFuse * 12 * 8;                       // 114,816 B: 2 CTAs per SM (2 x (114,816 + 1024) <= 233,472)
+constexpr int kSmKeys = kSmAcc + kMaxFuse * 12 * 8;                       // uint [20] Philox round keys (+ padding to 128 B)
+constexpr int kSmStep = kSmKeys + 128;                                    // 114,944 B: 2 CTAs per SM (2 x (114,944 + 1024) <= 233,472)
 __host__ __device__ constexpr int fx_index(int bead_in_warp) { return (bead_in_warp >> 3) * 28 + (bead_in_warp & 7) * 3; }
 
 struct StepParams {

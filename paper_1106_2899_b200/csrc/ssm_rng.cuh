@@ -71,34 +71,45 @@ __device__ __forceinline__ StreamKey make_stream(unsigned long long step, const 
     s.b3 = (uint32_t)p0 ^ rk[3];
     return s;
 }
+// The round keys of rounds 2..10 come from a copy in SHARED memory when the caller has one
+// (rk_sm, 16-byte aligned, 20 words): five 16-byte broadcast loads put them straight into
+// registers.  Read from the kernel parameters they arrive in uniform registers, and ptxas then
+// spends a register move per key and call on them (measured: 18 moves per call in the slot pass).
+template <bool SM = false>
 __device__ __forceinline__ void stream_call(const StreamKey& s, const unsigned (&rk)[20], uint32_t domain,
-                                            uint32_t chain, uint32_t item, uint32_t (&w)[4])
+                                            uint32_t chain, uint32_t item, uint32_t (&w)[4],
+                                            const uint4 *rk_sm = nullptr)
 {
     constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+    unsigned k[20];
+    if (SM) {
+#pragma unroll
+        for (int i = 0; i < 5; ++i) { const uint4 t = rk_sm[i]; k[4 * i] = t.x; k[4 * i + 1] = t.y; k[4 * i + 2] = t.z; k[4 * i + 3] = t.w; }
+    } else {
+#pragma unroll
+        for (int i = 0; i < 20; ++i) k[i] = rk[i];
+    }
     // round 1 on (step, domain | step hi, chain, item)
     const uint64_t q1 = (uint64_t)M1 * chain;
     uint32_t c0 = (uint32_t)(q1 >> 32) ^ (((domain << 28) | s.c1hi) ^ rk[0]);
     uint32_t c1 = (uint32_t)q1;
     uint32_t c2 = s.a1 ^ item;
     // round 2: its c3 is lo(M0 * step), already folded with rk[3] into b3
-    {
-        const uint64_t p0 = (uint64_t)M0 * c0;
-        const uint64_t p1 = (uint64_t)M1 * c2;
-        c0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk[2];
-        c2 = (uint32_t)(p0 >> 32) ^ s.b3;
-        c1 = (uint32_t)p1;
-        const uint32_t c3 = (uint32_t)p0;
-        uint32_t d3 = c3;
+    const uint64_t p0 = (uint64_t)M0 * c0;
+    const uint64_t p1 = (uint64_t)M1 * c2;
+    c0 = (uint32_t)(p1 >> 32) ^ c1 ^ k[2];
+    c2 = (uint32_t)(p0 >> 32) ^ s.b3;
+    c1 = (uint32_t)p1;
+    uint32_t c3 = (uint32_t)p0;
 #pragma unroll
-        for (int r = 2; r < 10; ++r) {
-            const uint64_t t0 = (uint64_t)M0 * c0;
-            const uint64_t t1 = (uint64_t)M1 * c2;
-            c0 = (uint32_t)(t1 >> 32) ^ c1 ^ rk[2 * r];
-            c2 = (uint32_t)(t0 >> 32) ^ d3 ^ rk[2 * r + 1];
-            c1 = (uint32_t)t1; d3 = (uint32_t)t0;
-        }
-        w[0] = c0; w[1] = c1; w[2] = c2; w[3] = d3;
+    for (int r = 2; r < 10; ++r) {
+        const uint64_t t0 = (uint64_t)M0 * c0;
+        const uint64_t t1 = (uint64_t)M1 * c2;
+        c0 = (uint32_t)(t1 >> 32) ^ c1 ^ k[2 * r];
+        c2 = (uint32_t)(t0 >> 32) ^ c3 ^ k[2 * r + 1];
+        c1 = (uint32_t)t1; c3 = (uint32_t)t0;
     }
+    w[0] = c0; w[1] = c1; w[2] = c2; w[3] = c3;
 }
 
 // 23-bit code k = w >> 9 and the uniform u = (k + 1/2) 2^-23 in (0,1); exact in fp32:
@@ -147,11 +158,13 @@ struct BoxMuller {
 };
 
 // the eight normals of one call: (2e, 2e+1) from word e
+template <bool SM = false>
 __device__ __forceinline__ void normal_call(const StreamKey& s, const unsigned (&rk)[20], uint32_t domain,
-                                            uint32_t chain, uint32_t call, const BoxMuller& bm, float (&z)[8])
+                                            uint32_t chain, uint32_t call, const BoxMuller& bm, float (&z)[8],
+                                            const uint4 *rk_sm = nullptr)
 {
     uint32_t w[4];
-    stream_call(s, rk, domain, chain, call, w);
+    stream_call<SM>(s, rk, domain, chain, call, w, rk_sm);
 #pragma unroll
     for (int e = 0; e < 4; ++e) bm(w[e], z[2 * e], z[2 * e + 1]);
 }

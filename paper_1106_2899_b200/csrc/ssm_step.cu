@@ -63,6 +63,8 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     unsigned long long *acc = reinterpret_cast<unsigned long long *>(smem + kSmAcc);
 
     const BoxMuller bm_noise(P.bm_noise), bm_anchor(P.bm_anchor);
+    const uint4 *Keys = reinterpret_cast<const uint4 *>(smem + kSmKeys);
+    if (threadIdx.x < 20) reinterpret_cast<unsigned *>(smem + kSmKeys)[threadIdx.x] = P.rk[threadIdx.x];
     for (int i = threadIdx.x; i < kMaxFuse * 12; i += kBlockThreads) acc[i] = 0ull;
     Ev[lane] = 0u;
     Samp[lane] = 0;
@@ -274,7 +276,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
 #pragma unroll
             for (int q = 0; q < 3; ++q) {
                 float z8[8];
-                normal_call(sk, P.rk, DOM_NOISE, chain, (uint32_t)(3 * l + q), bm_noise, z8);
+                normal_call<true>(sk, P.rk, DOM_NOISE, chain, (uint32_t)(3 * l + q), bm_noise, z8, Keys);
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
                     const int4 fx = Fx4[lane * 7 + 2 * q + h];
@@ -310,7 +312,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     const bool act = f < Tz;
                     const int sx = slot_index(it, act ? f : 0), c = sx >> LN, j = sx & (N - 1), base = sx & ~(N - 1);
                     uint32_t w[4];
-                    stream_call(sk, P.rk, DOM_SLOT, chain0 + (uint32_t)c, (uint32_t)(j >> 1), w);
+                    stream_call<true>(sk, P.rk, DOM_SLOT, chain0 + (uint32_t)c, (uint32_t)(j >> 1), w, Keys);
                     const uint32_t w_hop = (j & 1) ? w[2] : w[0], w_end = (j & 1) ? w[3] : w[1];
                     const int s = max((int)Sb[sx], 1);       // 1..N (an idle lane may look at an empty slot: any bead will do)
                     float4 a = A4[sx];
@@ -380,7 +382,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     if (!valid) K = 0;
                     if (8 * l < K) {
                         uint32_t w[4];
-                        stream_call(sk, P.rk, DOM_ATTEMPT, chain, (uint32_t)l, w);
+                        stream_call<true>(sk, P.rk, DOM_ATTEMPT, chain, (uint32_t)l, w, Keys);
                         const int hmax = P.h_c2[K];
                         const unsigned m2 = __vminu2(__vminu2(w[0], w[1]), __vminu2(w[2], w[3]));
                         if ((int)min(m2 & 0xFFFFu, m2 >> 16) <= hmax) {
