@@ -538,11 +538,23 @@ int64_t oracle_run(const oracle_params *p, oracle_state *st, int64_t n_steps, do
     if ((int64_t)n_threads > M) n_threads = (int)M;
     work_t *w = (work_t *)calloc((size_t)n_threads, sizeof(work_t));
     pthread_t *th = (pthread_t *)calloc((size_t)n_threads, sizeof(pthread_t));
+    /* Correlator sums are shared by the chains of a group: each thread adds into PRIVATE copies of
+     * the sum / count arrays (rings and pending pairs are per chain, hence disjoint), merged below
+     * in thread order, so that a multi-threaded run has no race and is reproducible. */
+    const size_t nsum = corr ? (size_t)corr->groups * corr->levels * corr->bins : 0;
+    oracle_corr *priv = corr && n_threads > 1 ? (oracle_corr *)calloc((size_t)n_threads, sizeof(oracle_corr)) : NULL;
     for (int t = 0; t < n_threads; ++t) {
         w[t].p = p; w[t].st = st; w[t].k0 = M * t / n_threads; w[t].k1 = M * (t + 1) / n_threads;
         w[t].n_steps = n_steps; w[t].shear_rate = shear_rate; w[t].stress_every = stress_every;
         w[t].stress_sum = n_samples ? (double *)calloc((size_t)n_samples * 12, sizeof(double)) : NULL;
         w[t].sample_every = sample_every; w[t].corr = corr; w[t].guard = guard;
+        if (priv) {
+            priv[t] = *corr;
+            priv[t].sum = (double *)calloc(nsum, sizeof(double));
+            priv[t].sum_gg = (double *)calloc(nsum, sizeof(double));
+            priv[t].count = (int64_t *)calloc(nsum, sizeof(int64_t));
+            w[t].corr = &priv[t];
+        }
     }
     if (n_threads == 1) worker(&w[0]);
     else {
@@ -553,6 +565,15 @@ int64_t oracle_run(const oracle_params *p, oracle_state *st, int64_t n_steps, do
         double s = 0.0;
         for (int t = 0; t < n_threads; ++t) s += w[t].stress_sum[i];
         stress_out[i] = s / (double)M;
+    }
+    if (priv) {
+        for (int t = 0; t < n_threads; ++t) {
+            for (size_t i = 0; i < nsum; ++i) {
+                corr->sum[i] += priv[t].sum[i]; corr->sum_gg[i] += priv[t].sum_gg[i]; corr->count[i] += priv[t].count[i];
+            }
+            free(priv[t].sum); free(priv[t].sum_gg); free(priv[t].count);
+        }
+        free(priv);
     }
     for (int t = 0; t < n_threads; ++t) free(w[t].stress_sum);
     free(w); free(th);

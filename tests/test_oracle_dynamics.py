@@ -225,3 +225,20 @@ def test_virtual_stress_contribution_matches_the_printed_25_percent_and_its_stat
     t2, G, _ = c.result(N, 0.1)
     # G(0) N = <s g> = (N - 1)(1 + O(dt)): the Euler map inflates it by about 6 % at dt = 0.01
     assert np.allclose(t, t2) and 1.0 < G[0] * N / (N - 1) < 1.13
+
+
+def test_correlator_sums_do_not_depend_on_the_number_of_oracle_threads():
+    """The oracle's driver splits chains over threads; chains of one group may land on different
+    threads, so every thread adds into private sums that are merged afterwards.  1 thread and 8
+    threads must agree to rounding, and two 8-thread runs exactly."""
+    def run(nt):
+        e = oracle.Ensemble(8, 200, seed=5)
+        c = oracle.Correlator(200, levels=4, bins=16, groups=8)
+        s = e.run(400, stress_every=10, sample_every=10, corr=c, n_threads=nt)
+        return c.result(8, 0.1), c.result_virtual(0.1), s
+    a, b, b2 = run(1), run(8), run(8)
+    for x, y in ((a, b), (b, b2)):
+        assert np.allclose(x[0][1], y[0][1], rtol=0, atol=1e-12) and np.allclose(x[0][2], y[0][2], rtol=0, atol=1e-12)
+        assert np.allclose(x[1][1], y[1][1], rtol=0, atol=1e-10)
+        assert np.allclose(x[2], y[2], rtol=0, atol=1e-12)
+    assert np.array_equal(b[0][1], b2[0][1])
