@@ -76,6 +76,10 @@ typedef struct {
     int32_t  k_attempts;      /* K of eqs (50), (51), "an integer parameter which can depend on Z"    */
                               /* (P:L328): 0 = K = N - Z (the paper's GPU choice);           */
                               /* k > 0 = K = min(k, N - Z) (k = 1 is the paper's CPU choice)         */
+    int32_t  corr_components; /* 0 or 1: the correlator follows sigma_xy (eq 43 as printed); 3: xy, yz and  */
+                              /* zx each keep their own history and feed the same sums -- the equilibrium   */
+                              /* ensemble is isotropic, so this is the same G(t) from three times the data  */
+                              /* (meaningful without flow only)                                             */
 } ssm_params;
 
 /* Bytes of device workspace ssm_init() needs for these parameters (0 on bad parameters). */

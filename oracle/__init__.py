@@ -71,6 +71,8 @@ def lib():
         L.oracle_step_chain.argtypes = [PP, C.c_uint64, C.c_uint64, C.c_double, dp, dp, i32p, i32p, dp]
         L.oracle_corr_create.argtypes = [C.c_int64, C.c_int, C.c_int, C.c_int]
         L.oracle_corr_create.restype = C.c_void_p
+        L.oracle_corr_create_iso.argtypes = [C.c_int64, C.c_int, C.c_int, C.c_int, C.c_int]
+        L.oracle_corr_create_iso.restype = C.c_void_p
         L.oracle_corr_destroy.argtypes = [C.c_void_p]
         L.oracle_corr_push.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_double, C.c_double]
         L.oracle_corr_result.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_int, dp, dp, dp]
@@ -126,8 +128,8 @@ def stream_normal(seed, domain, step, chain, m):
 class Correlator:
     """Per-chain multi-tau correlator."""
 
-    def __init__(self, n_chains, levels=16, bins=16, groups=32):
-        self.h = lib().oracle_corr_create(n_chains, levels, bins, groups)
+    def __init__(self, n_chains, levels=16, bins=16, groups=32, components=1):
+        self.h = lib().oracle_corr_create_iso(n_chains, levels, bins, groups, components)
         self.levels, self.bins, self.groups = levels, bins, groups
 
     def push(self, chain_local, group, f, g):

@@ -374,11 +374,15 @@ static void corr_insert(oracle_corr *c, int64_t chain_local, int group, int lev,
     }
 }
 
-oracle_corr *oracle_corr_create(int64_t n_chains, int levels, int bins, int groups)
+/* n_comp = 1: the xy component only (eq 43 as printed).  n_comp = 3: xy, yz and zx each keep their own
+ * history and all feed the same sums -- the equilibrium ensemble is isotropic (eq 13 has no preferred
+ * axis), so G_xyxy = G_yzyz = G_zxzx and the average is an estimate of the same G from three times
+ * the data.  History slot of (chain k, component q) = q n_chains + k. */
+oracle_corr *oracle_corr_create_iso(int64_t n_chains, int levels, int bins, int groups, int n_comp)
 {
     oracle_corr *c = (oracle_corr *)calloc(1, sizeof(oracle_corr));
-    c->n_chains = n_chains; c->levels = levels; c->bins = bins; c->groups = groups;
-    size_t nl = (size_t)n_chains * levels;
+    c->n_chains = n_chains; c->levels = levels; c->bins = bins; c->groups = groups; c->n_comp = n_comp;
+    size_t nl = (size_t)n_chains * n_comp * levels;
     c->ring = (double *)calloc(nl * bins, sizeof(double));
     c->pos = (int *)calloc(nl, sizeof(int));
     c->filled = (int *)calloc(nl, sizeof(int));
@@ -389,6 +393,10 @@ oracle_corr *oracle_corr_create(int64_t n_chains, int levels, int bins, int grou
     c->sum_gg = (double *)calloc((size_t)groups * levels * bins, sizeof(double));
     c->count = (int64_t *)calloc((size_t)groups * levels * bins, sizeof(int64_t));
     return c;
+}
+oracle_corr *oracle_corr_create(int64_t n_chains, int levels, int bins, int groups)
+{
+    return oracle_corr_create_iso(n_chains, levels, bins, groups, 1);
 }
 void oracle_corr_destroy(oracle_corr *c)
 {
@@ -516,9 +524,11 @@ static void *worker(void *arg)
                     double *o = w->stress_sum + (size_t)idx * 12;
                     for (int t = 0; t < 6; ++t) { o[t] += sig[t]; o[6 + t] += sigv[t]; }
                 }
-                if (smp)
-                    oracle_corr_push(w->corr, k, (int)((chain / 32) % (uint64_t)w->corr->groups),   /* DESIGN.md section 7 */
-                                     sig[3], sig[3] + sigv[3]);
+                if (smp)                                         /* components 3, 4, 5 = xy, yz, zx */
+                    for (int q = 0; q < w->corr->n_comp; ++q)
+                        oracle_corr_push(w->corr, (int64_t)q * w->corr->n_chains + k,
+                                         (int)((chain / 32) % (uint64_t)w->corr->groups),
+                                         sig[3 + q], sig[3 + q] + sigv[3 + q]);
             }
         }
     }

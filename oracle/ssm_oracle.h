@@ -50,6 +50,7 @@ typedef struct {
 
 typedef struct {
     int64_t n_chains; int levels, bins, groups;
+    int n_comp;                    /* 1: xy only; 3: xy, yz, zx feed the same sums (isotropic average) */
     double *ring; int *pos, *filled; double *acc_f, *acc_g; int *acc_n;
     double *sum; int64_t *count;   /* [groups][levels][bins]: sum of f_new g_old (eq 43) */
     double *sum_gg;                /* [groups][levels][bins]: sum of g_new g_old (eq 66) */
@@ -72,6 +73,7 @@ void     oracle_init_chain(const oracle_params *p, uint64_t chain, double *R, do
 void     oracle_step_chain(const oracle_params *p, uint64_t chain, uint64_t step, double shear_rate,
                            double *R, double *A, int32_t *S, int32_t *Z, double *min_margin);
 oracle_corr *oracle_corr_create(int64_t n_chains, int levels, int bins, int groups);
+oracle_corr *oracle_corr_create_iso(int64_t n_chains, int levels, int bins, int groups, int n_comp);
 void     oracle_corr_destroy(oracle_corr *c);
 void     oracle_corr_push(oracle_corr *c, int64_t chain_local, int group, double f, double g);
 int      oracle_corr_result(const oracle_corr *c, int n_beads, double base_dt, int cap,

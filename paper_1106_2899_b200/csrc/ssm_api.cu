@@ -81,6 +81,7 @@ static bool check_params(const ssm_params *p, std::string &why)
         if (p->corr_levels < 1 || p->corr_levels > kCorrMaxLevels) { why = "corr_levels must be 1..32"; return false; }
         if (p->corr_bins < 2 || p->corr_bins > 32 || (p->corr_bins & 1)) { why = "corr_bins must be even, 2..32"; return false; }
         if (p->corr_groups < 1 || p->corr_groups > 1024) { why = "corr_groups must be 1..1024"; return false; }
+        if (!(p->corr_components == 0 || p->corr_components == 1 || p->corr_components == 3)) { why = "corr_components must be 0, 1 or 3"; return false; }
     }
     return true;
 }
@@ -95,10 +96,11 @@ static Layout make_layout(const ssm_params *p)
     L.stress = o; o = align_up(o + (size_t)p->stress_capacity * 12 * 8, 256);
     const bool corr = p->sample_every > 0;
     const size_t M = (size_t)p->n_chains;
-    L.samples = o; if (corr) o = align_up(o + (size_t)kMaxFuse * M * 8, 256);
-    L.ring = o; if (corr) o = align_up(o + (size_t)p->corr_levels * p->corr_bins * M * 4, 256);
-    L.accf = o; if (corr) o = align_up(o + (size_t)p->corr_levels * M * 4, 256);
-    L.accg = o; if (corr) o = align_up(o + (size_t)p->corr_levels * M * 4, 256);
+    const size_t Mv = M * (size_t)(p->corr_components == 3 ? 3 : 1);      // histories: one per chain and component
+    L.samples = o; if (corr) o = align_up(o + (size_t)kMaxFuse * Mv * 8, 256);
+    L.ring = o; if (corr) o = align_up(o + (size_t)p->corr_levels * p->corr_bins * Mv * 4, 256);
+    L.accf = o; if (corr) o = align_up(o + (size_t)p->corr_levels * Mv * 4, 256);
+    L.accg = o; if (corr) o = align_up(o + (size_t)p->corr_levels * Mv * 4, 256);
     // two sum arrays: f_new g_old (eq 43) and g_new g_old (eq 66)
     L.csum = o; if (corr) o = align_up(o + 2 * (size_t)p->corr_groups * p->corr_levels * p->corr_bins * 8, 256);
     // staging for host-pointer get/set state and chain stress: chunks of <= 65536 chains
@@ -185,6 +187,7 @@ extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, s
     philox_round_keys((unsigned)(p->seed & 0xFFFFFFFFull), (unsigned)(p->seed >> 32), sp.rk);
     sp.springs_on = c->springs_on ? 1 : 0;
     sp.k_attempts = p->k_attempts;
+    sp.n_comp = p->corr_components == 3 ? 3 : 1;
     sp.dt3 = (float)(3.0 * p->dt);
     const double m2ln2 = -2.0 * 0.6931471805599453;        // r^2 = -2 ln u = (-2 ln 2) log2 u
     sp.bm_noise = (float)(m2ln2 * 2.0 * p->dt);
@@ -281,6 +284,7 @@ extern "C" int ssm_step(ssm_ctx *c, int64_t n_steps, double shear_rate)
             cp.sum_gg = cp.sum + (size_t)p.corr_groups * p.corr_levels * p.corr_bins;
             cp.M = p.n_chains; cp.chain_offset = p.chain_offset;
             cp.n_samples = (int)nsmp; cp.L = p.corr_levels; cp.Pb = p.corr_bins; cp.groups = p.corr_groups;
+            cp.Mv = (long long)p.n_chains * sp.n_comp;
             std::memcpy(cp.pos, c->cpos, sizeof cp.pos); std::memcpy(cp.filled, c->cfil, sizeof cp.filled);
             std::memcpy(cp.parity, c->cpar, sizeof cp.parity);
             CK(c, launch_corr(cp, c->st));
@@ -468,7 +472,7 @@ extern "C" int ssm_gt_sums(ssm_ctx *c, double *h_sum, int64_t *h_count)
             for (int q = 0; q < p.corr_bins; ++q) {
                 const size_t i = ((size_t)g * p.corr_levels + lev) * p.corr_bins + q;
                 h_sum[i] = (double)raw[i] / 65536.0;
-                h_count[i] = c->ccount[(size_t)lev * 32 + q] * ng;
+                h_count[i] = c->ccount[(size_t)lev * 32 + q] * ng * (p.corr_components == 3 ? 3 : 1);
             }
     }
     return SSM_OK;

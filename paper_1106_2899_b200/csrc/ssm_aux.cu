@@ -166,30 +166,31 @@ cudaError_t launch_chain_stress(const unsigned char *state, float *out, int N, l
 // ---------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) ssm_corr_kernel(const __grid_constant__ CorrParams C)
 {
+    // one thread per HISTORY k = q M + chain (component q = xy, or xy / yz / zx), Mv = n_comp M of them
     const long long k0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool valid = k0 < C.M;
-    const long long k = valid ? k0 : C.M - 1;           // idle lanes of the last warp shadow a real chain and add 0
+    const bool valid = k0 < C.Mv;
+    const long long k = valid ? k0 : C.Mv - 1;          // idle lanes of the last warp shadow a real history and add 0
     const int L = C.L, Pb = C.Pb, lane = threadIdx.x & 31;
     // group = (global chain index / 32) % groups: the same for the whole warp when the local chain 0
-    // sits on a multiple of 32 (always, unless a shard starts elsewhere)
-    const int group = (int)(((C.chain_offset + (unsigned long long)k) >> 5) % (unsigned)C.groups);
+    // sits on a multiple of 32 and M is one (else the per-lane path below takes over)
+    const int group = (int)(((C.chain_offset + (unsigned long long)(k % C.M)) >> 5) % (unsigned)C.groups);
     const bool one_group = __all_sync(0xffffffffu, group == __shfl_sync(0xffffffffu, group, 0));
     long long *gsum = C.sum + (long long)group * L * Pb, *gsum2 = C.sum_gg + (long long)group * L * Pb;
     unsigned char pos[kCorrMaxLevels], fil[kCorrMaxLevels], par[kCorrMaxLevels];
     for (int lev = 0; lev < L; ++lev) { pos[lev] = C.pos[lev]; fil[lev] = C.filled[lev]; par[lev] = C.parity[lev]; }
     for (int s = 0; s < C.n_samples; ++s) {
-        const float2 fg = C.samples[(long long)s * C.M + k];
+        const float2 fg = C.samples[(long long)s * C.Mv + k];
         float f = fg.x, g = fg.y;
         for (int lev = 0; lev < L; ++lev) {              // (every bound in here is the same for all chains)
-            const long long lm = (long long)lev * C.M + k;
-            float *ring = C.ring + (long long)lev * Pb * C.M + k;
+            const long long lm = (long long)lev * C.Mv + k;
+            float *ring = C.ring + (long long)lev * Pb * C.Mv + k;
             const int p0 = pos[lev];
-            if (valid) ring[(long long)p0 * C.M] = g;
+            if (valid) ring[(long long)p0 * C.Mv] = g;
             if (fil[lev] < Pb) ++fil[lev];
             const int kmin = lev == 0 ? 0 : Pb / 2;
             for (int q = kmin; q < fil[lev]; ++q) {
                 int idx = p0 - q; if (idx < 0) idx += Pb;
-                const float old = valid ? ring[(long long)idx * C.M] : 0.0f;
+                const float old = valid ? ring[(long long)idx * C.Mv] : 0.0f;
                 // fixed point 2^-16: f_new g_old for G(t) (eq 43), g_new g_old for the virtual-stress share (eq 66)
                 const long long v = __float2ll_rn(f * old * 65536.0f), v2 = __float2ll_rn(g * old * 65536.0f);
                 if (one_group) {
@@ -224,7 +225,7 @@ __global__ void __launch_bounds__(256) ssm_corr_kernel(const __grid_constant__ C
 
 cudaError_t launch_corr(const CorrParams &c, cudaStream_t st)
 {
-    ssm_corr_kernel<<<(unsigned)((c.M + 255) / 256), 256, 0, st>>>(c);
+    ssm_corr_kernel<<<(unsigned)((c.Mv + 255) / 256), 256, 0, st>>>(c);
     return cudaGetLastError();
 }
 

@@ -41,6 +41,7 @@ constexpr int kSmZ = 12544;      // int  [32]   Z per chain
 constexpr int kSmX = 12672;      // int  [33]   exclusive prefix of Z over the warp's chains (+ total), padded to 36
 constexpr int kSmEv = 12816;     // uint [64]   construction candidates [chain][word]: bit k = attempt k passed the 16-bit test; [32 + chain] = (k << 16) | half of the chain's latest candidate
 constexpr int kSmSamp = 13072;   // int  [32]   per-chain fixed-point sum of d_x d_y over slip-springs (sample steps)
+constexpr int kSmSamp2 = 3584;   // int  [2][32] the same for d_y d_z and d_z d_x (isotropic correlator), in the spare kB after the mirror
 constexpr int kStageSteps = 8;   // recorded steps whose warp sums wait in kSmStage before they are added to the CTA sums
 constexpr int kSmStage = 13200;  // int  [8][12] warp sums of the last recorded steps (int32 fixed point)
 constexpr int kSmDm = 13584;     // uint [32]   destruction masks [chain][word]: bit j = slip-spring j was destroyed in this step
@@ -55,7 +56,8 @@ __host__ __device__ constexpr int fx_index(int bead_in_warp) { return (bead_in_w
 struct StepParams {
     unsigned char *state;             // warp tiles
     long long     *stress;            // [capacity][12] int64 fixed-point sums; slot of this launch's first record
-    float2        *samples;           // [n_sample_steps of this launch][M] (f, g) per chain, or null
+    float2        *samples;           // [n_sample_steps of this launch][n_comp][M] (f, g) per chain and component, or null
+    int            n_comp;            // 1: xy; 3: xy, yz, zx
     long long      n_chains;          // M (chains >= M in the last tile are padding)
     unsigned long long chain_offset;  // global index of local chain 0
     unsigned long long step0;         // global index of the first step of this launch
@@ -95,12 +97,14 @@ struct InitParams {
 
 constexpr int kCorrMaxLevels = 32;
 struct CorrParams {
-    const float2 *samples;     // [n_samples][M] (f, g) = (sigma_xy, sigma_xy + sigma^(v)_xy)
-    float *ring;               // [L][P][M] block-averaged g history
-    float *acc_f, *acc_g;      // [L][M] first element of the pending pair
+    const float2 *samples;     // [n_samples][Mv] (f, g) = (sigma_ab, sigma_ab + sigma^(v)_ab); Mv = n_comp M histories,
+                               // history q M + k = component q (xy, yz, zx) of chain k
+    float *ring;               // [L][P][Mv] block-averaged g history
+    float *acc_f, *acc_g;      // [L][Mv] first element of the pending pair
     long long *sum;            // [groups][L][P] int64 fixed point (2^-16): f_new g_old (eq 43)
     long long *sum_gg;         // [groups][L][P] int64 fixed point (2^-16): g_new g_old (eq 66)
-    long long M;
+    long long M;               // chains
+    long long Mv;              // histories = n_comp * M
     unsigned long long chain_offset;
     int n_samples, L, Pb, groups;
     unsigned char pos[kCorrMaxLevels], filled[kCorrMaxLevels], parity[kCorrMaxLevels];   // at launch start

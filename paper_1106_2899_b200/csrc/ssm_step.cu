@@ -58,6 +58,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     unsigned *Dm = reinterpret_cast<unsigned *>(wb + kSmDm);
     unsigned char *Map = wb + kSmMap;
     int *Samp = reinterpret_cast<int *>(wb + kSmSamp);
+    int *Samp2 = reinterpret_cast<int *>(wb + kSmSamp2);
     int *Stage = reinterpret_cast<int *>(wb + kSmStage);
     int4 *Stage4 = reinterpret_cast<int4 *>(wb + kSmStage);
     unsigned long long *acc = reinterpret_cast<unsigned long long *>(smem + kSmAcc);
@@ -67,7 +68,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     if (threadIdx.x < 20) reinterpret_cast<unsigned *>(smem + kSmKeys)[threadIdx.x] = P.rk[threadIdx.x];
     for (int i = threadIdx.x; i < kMaxFuse * 12; i += kBlockThreads) acc[i] = 0ull;
     Ev[lane] = 0u;
-    Samp[lane] = 0;
+    Samp[lane] = 0; Samp2[lane] = 0; Samp2[32 + lane] = 0;
     Dm[lane] = 0u;
     __syncthreads();
 
@@ -206,15 +207,20 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     v[5] = fmaf(b[3 * k + 2], b[3 * k], v[5]);
                 }
                 if (smp_prev) {
-                    // per-chain f = sigma_xy, g = sigma_xy + sigma^(v)_xy for the correlator (eq 43)
-                    float f = 3.0f * v[3];
+                    // per-chain f = sigma_ab, g = sigma_ab + sigma^(v)_ab for the correlator (eq 43): ab = xy, and
+                    // yz, zx as well when the isotropic average is on (history q of the chain at [smp][q][chain])
+                    for (int q = 0; q < P.n_comp; ++q) {
+                        float f = 3.0f * (q == 0 ? v[3] : (q == 1 ? v[4] : v[5]));
 #pragma unroll
-                    for (int o = G / 2; o >= 1; o >>= 1) f += __shfl_xor_sync(kFull, f, o);
-                    if (l == 0) {
-                        const int sx = Samp[cw];
-                        Samp[cw] = 0;
-                        const float g = fmaf(P.cs * (1.0f / (float)(1 << kSampleShift)), (float)sx, f);
-                        if (valid && P.samples) P.samples[(long long)smp * P.n_chains + chain_local] = make_float2(f, g);
+                        for (int o = G / 2; o >= 1; o >>= 1) f += __shfl_xor_sync(kFull, f, o);
+                        if (l == 0) {
+                            int *sp = q == 0 ? Samp + cw : Samp2 + (q - 1) * 32 + cw;
+                            const int sx = *sp;
+                            *sp = 0;
+                            const float g = fmaf(P.cs * (1.0f / (float)(1 << kSampleShift)), (float)sx, f);
+                            if (valid && P.samples)
+                                P.samples[((long long)smp * P.n_comp + q) * P.n_chains + chain_local] = make_float2(f, g);
+                        }
                     }
                     ++smp;
                 }
@@ -368,7 +374,13 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                         sv[0] = fmaf(dx, dx, sv[0]); sv[1] = fmaf(dy, dy, sv[1]); sv[2] = fmaf(dz, dz, sv[2]);
                         sv[3] = fmaf(dx, dy, sv[3]); sv[4] = fmaf(dy, dz, sv[4]); sv[5] = fmaf(dz, dx, sv[5]);
                         cnt += 1.0f;
-                        if (sample) atomicAdd(Samp + c, __float2int_rn(dx * dy * (float)(1 << kSampleShift)));
+                        if (sample) {
+                            atomicAdd(Samp + c, __float2int_rn(dx * dy * (float)(1 << kSampleShift)));
+                            if (P.n_comp == 3) {
+                                atomicAdd(Samp2 + c, __float2int_rn(dy * dz * (float)(1 << kSampleShift)));
+                                atomicAdd(Samp2 + 32 + c, __float2int_rn(dz * dx * (float)(1 << kSampleShift)));
+                            }
+                        }
                     }
                 }
                 // construction attempts (eqs 50, 51), drawn by the chain's own lanes; K = N - Z
@@ -462,7 +474,13 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                                 sv[0] = fmaf(dx, dx, sv[0]); sv[1] = fmaf(dy, dy, sv[1]); sv[2] = fmaf(dz, dz, sv[2]);
                                 sv[3] = fmaf(dx, dy, sv[3]); sv[4] = fmaf(dy, dz, sv[4]); sv[5] = fmaf(dz, dx, sv[5]);
                                 cnt += 1.0f;
-                                if (sample) atomicAdd(Samp + cw, __float2int_rn(dx * dy * (float)(1 << kSampleShift)));
+                                if (sample) {
+                                    atomicAdd(Samp + cw, __float2int_rn(dx * dy * (float)(1 << kSampleShift)));
+                                    if (P.n_comp == 3) {
+                                        atomicAdd(Samp2 + cw, __float2int_rn(dy * dz * (float)(1 << kSampleShift)));
+                                        atomicAdd(Samp2 + 32 + cw, __float2int_rn(dz * dx * (float)(1 << kSampleShift)));
+                                    }
+                                }
                             }
                         }
                         if (changed) Zs[cw] = Zn;

@@ -164,18 +164,19 @@ def test_split_runs_fusion_depth_and_ensemble_size_do_not_change_results(ssm):
     assert np.array_equal(R, R0[:, :, 128:192]) and np.array_equal(S, S0[:, 128:192])
 
 
-@pytest.mark.parametrize("M,offset", [(512, 0), (500, 7)])
-def test_correlator_matches_oracle_on_identical_trajectories(ssm, M, offset):
+@pytest.mark.parametrize("M,offset,comps", [(512, 0, 1), (500, 7, 1), (512, 0, 3), (500, 7, 3)])
+def test_correlator_matches_oracle_on_identical_trajectories(ssm, M, offset, comps):
     """Rouse limit (no forks): GPU multi-tau sums against the oracle's correlator fed by
     the oracle's own stresses of the same trajectories.  (500, 7): a ragged last warp and a
     shard that does not start on a multiple of 32, so that a warp's chains fall into two
-    groups (the per-lane path of the correlator kernel)."""
+    groups (the per-lane path of the correlator kernel).  comps = 3: the isotropic average, xy, yz and
+    zx histories feeding the same sums."""
     N, steps = 8, 2000
     e = oracle.Ensemble(N, M, n_0=0.0, seed=13, chain_offset=offset)
     g = ssm.Ensemble(N, M, n_0=0.0, seed=13, chain_offset=offset, sample_every=10, corr_levels=6, corr_bins=16,
-                     corr_groups=32)
+                     corr_groups=32, corr_components=comps)
     upload(e, g)
-    corr = oracle.Correlator(M, levels=6, bins=16, groups=32)
+    corr = oracle.Correlator(M, levels=6, bins=16, groups=32, components=comps)
     e.run(steps, sample_every=10, corr=corr)
     g.step(steps)
     t0, G0, se0 = corr.result(N, 0.1)

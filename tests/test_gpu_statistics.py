@@ -272,3 +272,32 @@ def test_virtual_stress_contribution_gpu_vs_oracle(ssm):
     r = ssm.Ensemble(8, 1024, n_0=0.0, seed=5, sample_every=10, corr_levels=3, corr_bins=16, corr_groups=32)
     r.step(600)
     assert np.allclose(r.gt_virtual()[1], 0.0, atol=1e-12)
+
+
+def test_isotropic_average_of_the_correlator(ssm):
+    """corr_components = 3: xy, yz and zx histories feed the same sums.  With
+    slip-springs on, the GPU estimate agrees with the oracle's isotropic estimate within 3 combined
+    standard errors, with the xy-only estimate of the same GPU run, and its standard error is smaller."""
+    N, steps, levels, groups = 16, 5000, 5, 32
+    e = oracle.Ensemble(N, 512, seed=401)
+    c = oracle.Correlator(512, levels=levels, bins=16, groups=groups, components=3)
+    e.run(steps, sample_every=10, corr=c, n_threads=8)
+    t0, G0, se0 = c.result(N, 0.1)
+    d0 = c.result_virtual(0.1)
+    kw = dict(sample_every=10, corr_levels=levels, corr_bins=16, corr_groups=groups)
+    g3 = ssm.Ensemble(N, 4096, seed=402, corr_components=3, **kw)
+    g1 = ssm.Ensemble(N, 4096, seed=402, corr_components=1, **kw)
+    g3.step(steps); g1.step(steps)
+    t3, G3, se3 = g3.gt()
+    t1, G1, se1 = g1.gt()
+    assert np.allclose(t0, t3) and np.allclose(t1, t3)
+    z = (G3 - G0) / np.sqrt(se0 ** 2 + se3 ** 2)
+    assert np.mean(np.abs(z) < 3.0) >= 0.97 and np.abs(z).max() < 4.5, z
+    z = (G3 - G1) / np.sqrt(se1 ** 2 + se3 ** 2)                 # same trajectories: strongly correlated, so loose
+    assert np.abs(z).max() < 3.0, z
+    assert np.median(se3 / se1) < 0.8                            # ~ 1/sqrt(3) at lags where components decorrelate
+    dv = g3.gt_virtual()
+    z = (dv[1] - d0[1]) / np.sqrt(dv[2] ** 2 + d0[2] ** 2)
+    assert np.mean(np.abs(z) < 3.0) >= 0.95 and np.abs(z).max() < 4.5, z
+    # the two runs share the dynamics: the isotropic option changes what is correlated, not the state
+    assert np.array_equal(g3.get_state()[0], g1.get_state()[0])
