@@ -41,6 +41,7 @@ constexpr int kSmZ = 12544;      // int  [32]   Z per chain
 constexpr int kSmX = 12672;      // int  [33]   exclusive prefix of Z over the warp's chains (+ total), padded to 36
 constexpr int kSmEv = 12816;     // uint [64]   construction candidates [chain][word]: bit k = attempt k passed the 16-bit test; [32 + chain] = (k << 16) | half of the chain's latest candidate
 constexpr int kSmSamp = 13072;   // int  [32]   per-chain fixed-point sum of d_x d_y over slip-springs (sample steps)
+constexpr int kSmKeys = 3840;    // uint [20]   the warp's copy of the Philox round keys (16-byte aligned)
 constexpr int kSmSamp2 = 3584;   // int  [2][32] the same for d_y d_z and d_z d_x (isotropic correlator), in the spare kB after the mirror
 constexpr int kStageSteps = 8;   // recorded steps whose warp sums wait in kSmStage before they are added to the CTA sums
 constexpr int kSmStage = 13200;  // int  [8][12] warp sums of the last recorded steps (int32 fixed point)
@@ -49,8 +50,7 @@ constexpr int kSmMap = 13712;    // uint8[128]  dealing map: byte 4 lane + it = 
                                  //             slip-spring number lane + 32 it (it = 0..3), rebuilt when some Z changes
 constexpr int kSmWarp = 13968;
 constexpr int kSmAcc = kWarpsPerBlock * kSmWarp;                          // int64 [kMaxFuse][12] per CTA
-constexpr int kSmKeys = kSmAcc + kMaxFuse * 12 * 8;                       // uint [20] Philox round keys (+ padding to 128 B)
-constexpr int kSmStep = kSmKeys + 128;                                    // 114,944 B: 2 CTAs per SM (2 x (114,944 + 1024) <= 233,472)
+constexpr int kSmStep = kSmAcc + kMaxFuse * 12 * 8;                       // 114,816 B: 2 CTAs per SM (2 x (114,816 + 1024) <= 233,472)
 __host__ __device__ constexpr int fx_index(int bead_in_warp) { return (bead_in_warp >> 3) * 28 + (bead_in_warp & 7) * 3; }
 
 struct StepParams {

@@ -64,8 +64,10 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     unsigned long long *acc = reinterpret_cast<unsigned long long *>(smem + kSmAcc);
 
     const BoxMuller bm_noise(P.bm_noise), bm_anchor(P.bm_anchor);
-    const uint4 *Keys = reinterpret_cast<const uint4 *>(smem + kSmKeys);
-    if (threadIdx.x < 20) reinterpret_cast<unsigned *>(smem + kSmKeys)[threadIdx.x] = P.rk[threadIdx.x];
+    // each warp keeps its own copy of the Philox round keys inside its region: their address is then a
+    // constant offset from the warp's base register (a CTA-wide copy costs an address computation per call)
+    const uint4 *Keys = reinterpret_cast<const uint4 *>(wb + kSmKeys);
+    if (lane < 20) reinterpret_cast<unsigned *>(wb + kSmKeys)[lane] = P.rk[lane];
     for (int i = threadIdx.x; i < kMaxFuse * 12; i += kBlockThreads) acc[i] = 0ull;
     Ev[lane] = 0u;
     Samp[lane] = 0; Samp2[lane] = 0; Samp2[32 + lane] = 0;
