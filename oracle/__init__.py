@@ -82,6 +82,10 @@ def lib():
         L.oracle_run.argtypes = [PP, C.POINTER(State), C.c_int64, C.c_double, C.c_int, dp, C.c_int,
                                  C.c_void_p, C.c_double, C.c_int]
         L.oracle_run.restype = C.c_int64
+        L.oracle_step_chain_kappa.argtypes = [PP, C.c_uint64, C.c_uint64, dp, dp, dp, i32p, i32p, dp]
+        L.oracle_run_kappa.argtypes = [PP, C.POINTER(State), C.c_int64, C.c_int64, dp, C.c_int, dp, C.c_int,
+                                       C.c_void_p, C.c_double, C.c_int]
+        L.oracle_run_kappa.restype = C.c_int64
         _lib = L
     return _lib
 
@@ -198,6 +202,24 @@ class Ensemble:
         st = self._state()
         got = lib().oracle_run(C.byref(self.p), C.byref(st), n_steps, shear_rate, stress_every, _dp(out),
                                sample_every, corr.h if corr is not None else None, guard, n_threads)
+        assert got == ns
+        self.step = st.step
+        return out[:ns]
+
+    def run_kappa(self, n_steps, kappa, chains_per_group=None, stress_every=0, sample_every=0, corr=None,
+                  guard=1e-5, n_threads=1):
+        """As run(), under a general velocity gradient (eqs 18, 21): kappa [groups][3][3] (or one [3][3]),
+        group of local chain k = k // chains_per_group (default: one group)."""
+        cpg = self.M if chains_per_group is None else int(chains_per_group)
+        kap = np.ascontiguousarray(np.asarray(kappa, dtype=np.float64).reshape(-1, 9))
+        assert kap.shape[0] == -(-self.M // cpg)
+        ns = 0
+        if stress_every > 0:
+            ns = (self.step + n_steps) // stress_every - self.step // stress_every
+        out = np.zeros((max(ns, 1), 12))
+        st = self._state()
+        got = lib().oracle_run_kappa(C.byref(self.p), C.byref(st), n_steps, cpg, _dp(kap), stress_every, _dp(out),
+                                     sample_every, corr.h if corr is not None else None, guard, n_threads)
         assert got == ns
         self.step = st.step
         return out[:ns]

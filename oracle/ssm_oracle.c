@@ -231,7 +231,10 @@ static int attempts_K(const oracle_params *p, int Z)
     return empty;                                                      /* K = N - Z: the paper's GPU choice */
 }
 
-void oracle_step_chain(const oracle_params *p, uint64_t chain, uint64_t step, double shear_rate,
+/* One time step of one chain.  kappa == NULL: simple shear kappa_xy = shear_rate (eq 60);
+ * else kappa[3a + b] = kappa_ab is the full velocity gradient tensor of eqs (18), (21)
+ * and shear_rate is ignored. */
+static void step_chain(const oracle_params *p, uint64_t chain, uint64_t step, double shear_rate, const double *kappa,
                        double *R, double *A, int32_t *S, int32_t *Zio, double *min_margin)
 {
     const int N = p->n_beads;
@@ -251,18 +254,27 @@ void oracle_step_chain(const oracle_params *p, uint64_t chain, uint64_t step, do
         int s = S[j] - 1;
         for (int c = 0; c < 3; ++c) F[3 * s + c] -= (3.0 / p->n_s) * (R[3 * s + c] - A[3 * j + c]);
     }
-    /* explicit Euler, eqs (44),(45) (reading R1); kappa_xy = shear_rate (eq 60) */
+    /* explicit Euler, eqs (44),(45) (reading R1); the affine term dt kappa . R_i, dt kappa . A_j uses the
+     * time-t positions; kappa_xy = shear_rate only (eq 60) when no tensor is given */
     double z8[8];
     for (int i = 0; i < N; ++i) {
-        double ry = R[3 * i + 1];
+        const double rx = R[3 * i], ry = R[3 * i + 1], rz = R[3 * i + 2];
         for (int c = 0; c < 3; ++c) {
             uint32_t m = (uint32_t)(3 * i + c);
             if ((m & 7) == 0) normal_call(p->seed, ORACLE_DOM_NOISE, step, chain, m >> 3, z8);
-            double flow = (c == 0) ? dt * shear_rate * ry : 0.0;
+            double flow;
+            if (kappa) flow = dt * (kappa[3 * c] * rx + kappa[3 * c + 1] * ry + kappa[3 * c + 2] * rz);
+            else flow = (c == 0) ? dt * shear_rate * ry : 0.0;
             R[3 * i + c] = R[3 * i + c] + dt * F[3 * i + c] + flow + sqrt(2.0 * dt) * z8[m & 7];
         }
     }
-    for (int j = 0; j < Z; ++j) A[3 * j] = A[3 * j] + dt * shear_rate * A[3 * j + 1];
+    for (int j = 0; j < Z; ++j) {
+        if (kappa) {
+            const double ax = A[3 * j], ay = A[3 * j + 1], az = A[3 * j + 2];
+            for (int c = 0; c < 3; ++c)
+                A[3 * j + c] = A[3 * j + c] + dt * (kappa[3 * c] * ax + kappa[3 * c + 1] * ay + kappa[3 * c + 2] * az);
+        } else A[3 * j] = A[3 * j] + dt * shear_rate * A[3 * j + 1];
+    }
     free(F);
 
     /* ---- substep 2: hop, one uniform per slip-spring, cumulative intervals
@@ -336,6 +348,19 @@ void oracle_step_chain(const oracle_params *p, uint64_t chain, uint64_t step, do
     }
     for (int j = Zs; j < oracle_zmax(p); ++j) { S[j] = 0; A[3 * j] = A[3 * j + 1] = A[3 * j + 2] = 0.0; }
     *Zio = Zs;
+}
+
+void oracle_step_chain(const oracle_params *p, uint64_t chain, uint64_t step, double shear_rate,
+                       double *R, double *A, int32_t *S, int32_t *Zio, double *min_margin)
+{
+    step_chain(p, chain, step, shear_rate, NULL, R, A, S, Zio, min_margin);
+}
+
+/* the same step under a general velocity gradient tensor kappa[3a + b] = kappa_ab (eqs 18, 21) */
+void oracle_step_chain_kappa(const oracle_params *p, uint64_t chain, uint64_t step, const double kappa[9],
+                             double *R, double *A, int32_t *S, int32_t *Zio, double *min_margin)
+{
+    step_chain(p, chain, step, 0.0, kappa, R, A, S, Zio, min_margin);
 }
 
 /* ------------------------------------------------------------------------- */
@@ -496,6 +521,7 @@ typedef struct {
     const oracle_params *p; oracle_state *st; int64_t k0, k1; int64_t n_steps; double shear_rate;
     int stress_every; double *stress_sum; /* [n_samples][12] partial */
     int sample_every; oracle_corr *corr; double guard;
+    const double *kappa; int64_t chains_per_group;   /* kappa of local chain k: kappa + 9 (k / chains_per_group), or NULL */
 } work_t;
 
 static void *worker(void *arg)
@@ -510,7 +536,8 @@ static void *worker(void *arg)
         for (int64_t n = 0; n < w->n_steps; ++n) {
             const uint64_t step = (uint64_t)(st->step + n);
             double margin = INFINITY;
-            oracle_step_chain(p, chain, step, w->shear_rate, R, A, S, &st->Z[k], &margin);
+            step_chain(p, chain, step, w->shear_rate, w->kappa ? w->kappa + 9 * (k / w->chains_per_group) : NULL,
+                       R, A, S, &st->Z[k], &margin);
             if (margin < st->min_margin[k]) st->min_margin[k] = margin;
             if (margin < w->guard && st->first_fragile_step[k] < 0) st->first_fragile_step[k] = (int64_t)step;
             const int64_t done = st->step + n + 1;          /* sample after the n-th step: t = n dt (R17) */
@@ -537,7 +564,8 @@ static void *worker(void *arg)
 
 /* stress_out: [n_samples][12] ensemble MEANS (eq 54); n_samples = number of multiples
  * of stress_every in (step, step+n_steps].  Returns n_samples. */
-int64_t oracle_run(const oracle_params *p, oracle_state *st, int64_t n_steps, double shear_rate,
+static int64_t run(const oracle_params *p, oracle_state *st, int64_t n_steps, double shear_rate,
+                   const double *kappa, int64_t chains_per_group,
                    int stress_every, double *stress_out, int sample_every, oracle_corr *corr,
                    double guard, int n_threads)
 {
@@ -558,6 +586,7 @@ int64_t oracle_run(const oracle_params *p, oracle_state *st, int64_t n_steps, do
         w[t].n_steps = n_steps; w[t].shear_rate = shear_rate; w[t].stress_every = stress_every;
         w[t].stress_sum = n_samples ? (double *)calloc((size_t)n_samples * 12, sizeof(double)) : NULL;
         w[t].sample_every = sample_every; w[t].corr = corr; w[t].guard = guard;
+        w[t].kappa = kappa; w[t].chains_per_group = chains_per_group;
         if (priv) {
             priv[t] = *corr;
             priv[t].sum = (double *)calloc(nsum, sizeof(double));
@@ -589,4 +618,21 @@ int64_t oracle_run(const oracle_params *p, oracle_state *st, int64_t n_steps, do
     free(w); free(th);
     st->step += n_steps;
     return n_samples;
+}
+
+int64_t oracle_run(const oracle_params *p, oracle_state *st, int64_t n_steps, double shear_rate,
+                   int stress_every, double *stress_out, int sample_every, oracle_corr *corr,
+                   double guard, int n_threads)
+{
+    return run(p, st, n_steps, shear_rate, NULL, 1, stress_every, stress_out, sample_every, corr, guard, n_threads);
+}
+
+/* As oracle_run, with one velocity gradient tensor per block of chains_per_group consecutive local chains
+ * (eqs 18, 21; the embedding of P:L17): kappa [ceil(M / chains_per_group)][9], row-major kappa_ab. */
+int64_t oracle_run_kappa(const oracle_params *p, oracle_state *st, int64_t n_steps, int64_t chains_per_group,
+                         const double *kappa, int stress_every, double *stress_out, int sample_every,
+                         oracle_corr *corr, double guard, int n_threads)
+{
+    if (chains_per_group < 1 || !kappa) return -1;
+    return run(p, st, n_steps, 0.0, kappa, chains_per_group, stress_every, stress_out, sample_every, corr, guard, n_threads);
 }

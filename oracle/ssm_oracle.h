@@ -72,6 +72,8 @@ void     oracle_poisson_thresholds(const oracle_params *p, int64_t *tcdf);
 void     oracle_init_chain(const oracle_params *p, uint64_t chain, double *R, double *A, int32_t *S, int32_t *Z);
 void     oracle_step_chain(const oracle_params *p, uint64_t chain, uint64_t step, double shear_rate,
                            double *R, double *A, int32_t *S, int32_t *Z, double *min_margin);
+void     oracle_step_chain_kappa(const oracle_params *p, uint64_t chain, uint64_t step, const double kappa[9],
+                                 double *R, double *A, int32_t *S, int32_t *Z, double *min_margin);
 oracle_corr *oracle_corr_create(int64_t n_chains, int levels, int bins, int groups);
 oracle_corr *oracle_corr_create_iso(int64_t n_chains, int levels, int bins, int groups, int n_comp);
 void     oracle_corr_destroy(oracle_corr *c);
@@ -83,6 +85,9 @@ int      oracle_corr_result_virtual(const oracle_corr *c, double base_dt, int ca
 int64_t  oracle_run(const oracle_params *p, oracle_state *st, int64_t n_steps, double shear_rate,
                     int stress_every, double *stress_out, int sample_every, oracle_corr *corr,
                     double guard, int n_threads);
+int64_t  oracle_run_kappa(const oracle_params *p, oracle_state *st, int64_t n_steps, int64_t chains_per_group,
+                          const double *kappa, int stress_every, double *stress_out, int sample_every,
+                          oracle_corr *corr, double guard, int n_threads);
 
 #ifdef __cplusplus
 }
