@@ -30,7 +30,9 @@
  *                                                                            -> A[(c*zmax+j)*M+k]
  *                         The anchor's x is A[0] + A[3]: under shear the library advects it as a
  *                         compensated sum (eq 45 adds the same increment every step, which a plain
- *                         fp32 sum would round the same way every step).  A[3] = 0 is a valid input.
+ *                         fp32 sum would round the same way every step).  A[3] = 0 is a valid input,
+ *                         and what ssm_get_state returns after ssm_step_kappa (whose low parts are
+ *                         kept in another encoding, below one ulp of each coordinate).
  *    S[j][k]     uint8    bead index 1..N of slip-spring j, 0 = empty slot   -> S[j*M+k]
  *  The occupied slots of a chain are always the first Z_k ones (the paper's "indices run
  *  from 1 to Z"); zmax = N (the paper's Z <= N).
@@ -97,6 +99,26 @@ int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, size_t works
  * after every step whose (1-based) global index is a multiple of stress_every; correlator
  * samples likewise with sample_every.  SSM_ERANGE if the stress buffer would overflow. */
 int ssm_step(ssm_ctx *ctx, int64_t n_steps, double shear_rate);
+
+/* As ssm_step, under a general velocity gradient tensor (eqs 18, 21; eqs 44, 45 add
+ * dt kappa . R_i and dt kappa . A_j), one tensor per GROUP of chains -- the embedding in a flow solver the
+ * paper aims at: group g holds the local chains [g chains_per_group, (g+1) chains_per_group),
+ * h_kappa (host) [n_groups][9], n_groups = ceil(n_chains / chains_per_group), row-major kappa_ab =
+ * d v_a / d r_b in 1/tau0, constant during the call (the host array may be reused after the call returns).
+ * chains_per_group >= n_chains means one group; otherwise it must be a multiple of 256 / n_beads (the
+ * chains of one warp share a tensor), else SSM_EINVAL.  Asynchronous; stress and correlator samples are
+ * recorded as by ssm_step (over the whole ensemble; ssm_group_stress reads the groups).  Anchors are advected
+ * as compensated sums in all three coordinates (10 extra bits each, kept in the fourth word of the anchor);
+ * that word restarts from zero (a change below one ulp of the anchor) when the flow changes between this
+ * call and simple shear, and after ssm_set_state. */
+int ssm_step_kappa(ssm_ctx *ctx, int64_t n_steps, int64_t chains_per_group, const double *h_kappa);
+
+/* Means over each group of chains_per_group consecutive local chains (any value >= 1; >= n_chains = one
+ * group) of the stress of the CURRENT state and of the number of slip-springs: h_out (host)
+ * [n_groups][13] = sigma xx,yy,zz,xy,yz,zx (eq 16), sigma_v likewise (eq 76), <Z> (eq 10 at equilibrium;
+ * its steady-state value under flow is what P:L428 prints).  Exact integer sums on the device
+ * (deterministic).  Synchronises the stream. */
+int ssm_group_stress(ssm_ctx *ctx, int64_t chains_per_group, double *h_out);
 
 /* Number of stress samples recorded since init / the last reset. */
 int64_t ssm_stress_count(const ssm_ctx *ctx);

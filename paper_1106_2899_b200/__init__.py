@@ -18,7 +18,7 @@ EXPORTS = ["ssm_workspace_bytes", "ssm_init", "ssm_step", "ssm_stress_count", "s
            "ssm_stress_sums_device", "ssm_chain_stress", "ssm_gt", "ssm_gt_sums", "ssm_get_state", "ssm_set_state",
            "ssm_reset_accumulators", "ssm_launch_count", "ssm_set_fusion", "ssm_set_grid", "ssm_destroy", "ssm_last_error",
            "ssm_moduli", "ssm_eta0", "ssm_tau_d", "ssm_issue_rates",
-           "ssm_gt_virtual", "ssm_gt_sums_virtual"]
+           "ssm_gt_virtual", "ssm_gt_sums_virtual", "ssm_step_kappa", "ssm_group_stress"]
 
 
 class Params(C.Structure):
@@ -68,6 +68,8 @@ def lib():
     L.ssm_issue_rates.argtypes = [vp, dp]; L.ssm_issue_rates.restype = C.c_int
     L.ssm_gt_virtual.argtypes = [vp, C.POINTER(C.c_int32), dp, dp, dp]; L.ssm_gt_virtual.restype = C.c_int
     L.ssm_gt_sums_virtual.argtypes = [vp, dp]; L.ssm_gt_sums_virtual.restype = C.c_int
+    L.ssm_step_kappa.argtypes = [vp, C.c_int64, C.c_int64, dp]; L.ssm_step_kappa.restype = C.c_int
+    L.ssm_group_stress.argtypes = [vp, C.c_int64, dp]; L.ssm_group_stress.restype = C.c_int
     L.ssm_moduli.argtypes = [C.c_int32, dp, dp, C.c_int32, dp, dp, dp]; L.ssm_moduli.restype = C.c_int
     L.ssm_eta0.argtypes = [C.c_int32, dp, dp, dp]; L.ssm_eta0.restype = C.c_int
     L.ssm_tau_d.argtypes = [C.c_int32, dp, dp, C.c_double, C.c_double, dp]; L.ssm_tau_d.restype = C.c_int
@@ -152,6 +154,23 @@ class Ensemble:
     def step(self, n_steps, shear_rate=0.0):
         with self._torch.cuda.device(self.device):
             self._ck(lib().ssm_step(self.h, n_steps, shear_rate))
+
+    def step_kappa(self, n_steps, kappa, chains_per_group=None):
+        """ssm_step_kappa: kappa [groups][3][3] (or one [3][3]); group of local chain k = k // chains_per_group."""
+        cpg = self.M if chains_per_group is None else int(chains_per_group)
+        kap = np.ascontiguousarray(np.asarray(kappa, dtype=np.float64).reshape(-1, 9))
+        if kap.shape[0] != -(-self.M // min(cpg, self.M)):
+            raise SsmError(SSM_EINVAL, "kappa must hold one tensor per group")
+        with self._torch.cuda.device(self.device):
+            self._ck(lib().ssm_step_kappa(self.h, n_steps, cpg, kap.ctypes.data_as(C.POINTER(C.c_double))))
+
+    def group_stress(self, chains_per_group=None):
+        """ssm_group_stress: [groups][13] = means of sigma[6], sigma_v[6] and Z over each group, current state."""
+        cpg = self.M if chains_per_group is None else min(int(chains_per_group), self.M)
+        out = np.zeros((-(-self.M // cpg), 13))
+        with self._torch.cuda.device(self.device):
+            self._ck(lib().ssm_group_stress(self.h, cpg, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out
 
     def stress_count(self):
         return lib().ssm_stress_count(self.h)

@@ -20,7 +20,10 @@ cudaError_t launch_step(int n_beads, const StepParams &p, int grid, cudaStream_t
 cudaError_t launch_init(const InitParams &p, cudaStream_t st);
 cudaError_t measure_rates(unsigned *d_scratch, int blocks, cudaStream_t st, double cycles[4]);
 cudaError_t launch_xfer(bool do_export, unsigned char *state, float *R, float *A, unsigned char *S, int N,
-                        long long k0, long long nk, long long pitch, cudaStream_t st);
+                        long long k0, long long nk, long long pitch, int hide_low, cudaStream_t st);
+cudaError_t launch_clear_low(unsigned char *state, long long n_tiles, cudaStream_t st);
+cudaError_t launch_group_stress(const unsigned char *state, long long *out, int N, long long M, long long cpg, float cs,
+                                cudaStream_t st);
 cudaError_t launch_chain_stress(const unsigned char *state, float *out, int N, long long M, float cs, cudaStream_t st);
 cudaError_t launch_corr(const CorrParams &c, cudaStream_t st);
 }  // namespace ssm
@@ -30,7 +33,7 @@ using namespace ssm;
 static thread_local std::string g_err;   // errors without a ctx
 
 struct Layout {
-    size_t state, stress, samples, ring, accf, accg, csum, stage, total;
+    size_t state, stress, kappa, samples, ring, accf, accg, csum, stage, total;
     long long n_tiles, stage_chains;
 };
 
@@ -44,10 +47,13 @@ struct ssm_ctx {
     int fuse, grid, grid_default;
     long long launches;
     bool springs_on;
+    int low_mode;            // encoding of the anchors' fourth word: 0 all zero, 1 fp32 low part of x (simple shear),
+                             // 2 three packed 10-bit low parts (general tensor)
     StepParams sp;           // constant part filled at init
     // correlator schedule (identical for all chains) and product counts, host side
     unsigned char cpos[kCorrMaxLevels], cfil[kCorrMaxLevels], cpar[kCorrMaxLevels];
     std::vector<long long> ccount;      // [L][P] insertions with a product at (level, bin)
+    std::vector<float> kappa_host;      // dt kappa of the last ssm_step_kappa call, [groups][9]
     std::string err;
 };
 
@@ -94,6 +100,7 @@ static Layout make_layout(const ssm_params *p)
     size_t o = 0;
     L.state = o; o = align_up(o + (size_t)L.n_tiles * kTileBytes, 256);
     L.stress = o; o = align_up(o + (size_t)p->stress_capacity * 12 * 8, 256);
+    L.kappa = o; o = align_up(o + (size_t)L.n_tiles * 9 * 4, 256);        // dt kappa per group (at most one group per tile)
     const bool corr = p->sample_every > 0;
     const size_t M = (size_t)p->n_chains;
     const size_t Mv = M * (size_t)(p->corr_components == 3 ? 3 : 1);      // histories: one per chain and component
@@ -164,7 +171,7 @@ extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, s
     ssm_ctx *c = new (std::nothrow) ssm_ctx();
     if (!c) return fail(nullptr, SSM_ENOMEM, "host allocation failed");
     c->p = *p; c->lay = lay; c->ws = (unsigned char *)d_workspace; c->st = (cudaStream_t)cuda_stream;
-    c->step = 0; c->n_records = 0; c->fuse = kMaxFuse; c->launches = 0;
+    c->step = 0; c->n_records = 0; c->fuse = kMaxFuse; c->launches = 0; c->low_mode = 0;
     c->springs_on = p->n_0 > 0.0 && std::isfinite(p->n_0);
     corr_clear(c);
 
@@ -206,7 +213,7 @@ extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, s
     InitParams ip;
     std::memset(&ip, 0, sizeof ip);
     ip.state = c->ws + lay.state;
-    ip.n_chains_padded = lay.n_tiles * chains_per_warp(p->n_beads);
+    ip.n_chains_padded = lay.n_tiles * chains_per_warp(p->n_beads); ip.n_chains = p->n_chains;
     ip.chain_offset = p->chain_offset; std::memcpy(ip.rk, sp.rk, sizeof ip.rk);
     ip.n_beads = p->n_beads; ip.springs_on = sp.springs_on;
     ip.bm_bond = (float)(m2ln2 / 3.0); ip.bm_anchor = sp.bm_anchor;
@@ -244,18 +251,27 @@ static void corr_schedule_sample(ssm_ctx *c)
     }
 }
 
-extern "C" int ssm_step(ssm_ctx *c, int64_t n_steps, double shear_rate)
+// advance n_steps under simple shear (d_kappa null) or under the device table of tensors d_kappa
+static int step_impl(ssm_ctx *c, int64_t n_steps, double shear_rate, const float *d_kappa, long long tiles_per_group)
 {
-    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
-    if (n_steps < 0) return fail(c, SSM_EINVAL, "n_steps < 0");
-    if (!std::isfinite(shear_rate)) return fail(c, SSM_EINVAL, "shear_rate is not finite");
     const ssm_params &p = c->p;
     if (p.stress_every > 0) {
         const long long need = (c->step + n_steps) / p.stress_every - c->step / p.stress_every;
         if (c->n_records + need > p.stress_capacity) return fail(c, SSM_ERANGE, "stress buffer would overflow (stress_capacity)");
     }
     StepParams sp = c->sp;
-    sp.gdt = (float)(shear_rate * p.dt);
+    sp.gdt = d_kappa ? 0.0f : (float)(shear_rate * p.dt);
+    sp.kappa = d_kappa; sp.tiles_per_group = (int)tiles_per_group;
+    // the fourth word of an anchor is the low part of its compensated advection; simple shear and the
+    // general tensor encode it differently, so it restarts from zero when the kind of flow changes
+    const int want = d_kappa ? 2 : (sp.gdt != 0.0f ? 1 : 0);
+    if (n_steps > 0 && want != 0 && c->springs_on) {
+        if (c->low_mode != 0 && c->low_mode != want) {
+            CK(c, launch_clear_low(c->ws + c->lay.state, c->lay.n_tiles, c->st));
+            c->launches += 1;
+        }
+        c->low_mode = want;
+    }
     long long left = n_steps;
     while (left > 0) {
         const int T = (int)(left < c->fuse ? left : c->fuse);
@@ -294,6 +310,66 @@ extern "C" int ssm_step(ssm_ctx *c, int64_t n_steps, double shear_rate)
         c->n_records += nrec;
         c->step += T;
         left -= T;
+    }
+    return SSM_OK;
+}
+
+extern "C" int ssm_step(ssm_ctx *c, int64_t n_steps, double shear_rate)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (n_steps < 0) return fail(c, SSM_EINVAL, "n_steps < 0");
+    if (!std::isfinite(shear_rate)) return fail(c, SSM_EINVAL, "shear_rate is not finite");
+    return step_impl(c, n_steps, shear_rate, nullptr, 1);
+}
+
+// number of groups and tiles per group for blocks of chains_per_group local chains; false if a warp tile
+// would hold chains of two groups
+static bool group_geometry(const ssm_ctx *c, int64_t cpg, long long *n_groups, long long *tiles_per_group)
+{
+    const long long M = c->p.n_chains, cpw = chains_per_warp(c->p.n_beads);
+    if (cpg < 1) return false;
+    if (cpg >= M) { *n_groups = 1; *tiles_per_group = c->lay.n_tiles; return true; }
+    if (cpg % cpw != 0) return false;
+    *n_groups = (M + cpg - 1) / cpg; *tiles_per_group = cpg / cpw;
+    return true;
+}
+
+extern "C" int ssm_step_kappa(ssm_ctx *c, int64_t n_steps, int64_t chains_per_group, const double *h_kappa)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (n_steps < 0) return fail(c, SSM_EINVAL, "n_steps < 0");
+    if (!h_kappa) return fail(c, SSM_EINVAL, "h_kappa is NULL");
+    long long ng = 0, tpg = 0;
+    if (!group_geometry(c, chains_per_group, &ng, &tpg))
+        return fail(c, SSM_EINVAL, "chains_per_group must be >= n_chains (one group) or a multiple of 256 / n_beads (the chains of a warp share one tensor)");
+    c->kappa_host.resize((size_t)ng * 9);
+    for (size_t i = 0; i < (size_t)ng * 9; ++i) {
+        if (!std::isfinite(h_kappa[i])) return fail(c, SSM_EINVAL, "kappa is not finite");
+        c->kappa_host[i] = (float)(h_kappa[i] * c->p.dt);
+    }
+    float *d_kappa = reinterpret_cast<float *>(c->ws + c->lay.kappa);
+    CK(c, cudaMemcpyAsync(d_kappa, c->kappa_host.data(), (size_t)ng * 9 * 4, cudaMemcpyHostToDevice, c->st));
+    return step_impl(c, n_steps, 0.0, d_kappa, tpg);
+}
+
+extern "C" int ssm_group_stress(ssm_ctx *c, int64_t chains_per_group, double *h_out)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (!h_out) return fail(c, SSM_EINVAL, "h_out is NULL");
+    if (chains_per_group < 1) return fail(c, SSM_EINVAL, "chains_per_group must be >= 1");
+    const long long M = c->p.n_chains, cpg = chains_per_group < M ? chains_per_group : M, ng = (M + cpg - 1) / cpg;
+    if ((size_t)ng * 13 * 8 > c->lay.total - c->lay.stage) return fail(c, SSM_ENOMEM, "staging area too small for this many groups");
+    long long *d = reinterpret_cast<long long *>(c->ws + c->lay.stage);
+    CK(c, cudaMemsetAsync(d, 0, (size_t)ng * 13 * 8, c->st));
+    CK(c, launch_group_stress(c->ws + c->lay.state, d, c->p.n_beads, M, cpg, c->sp.cs, c->st));
+    c->launches += 1;
+    std::vector<long long> raw((size_t)ng * 13);
+    CK(c, cudaMemcpyAsync(raw.data(), d, (size_t)ng * 13 * 8, cudaMemcpyDeviceToHost, c->st));
+    CK(c, cudaStreamSynchronize(c->st));
+    for (long long g = 0; g < ng; ++g) {
+        const long long n = (g + 1) * cpg <= M ? cpg : M - g * cpg;
+        for (int t = 0; t < 13; ++t)
+            h_out[g * 13 + t] = (double)raw[(size_t)g * 13 + t] / ((double)(1 << kStressShift) * (double)n);
     }
     return SSM_OK;
 }
@@ -361,8 +437,9 @@ static int xfer_state(ssm_ctx *c, bool do_export, float *R, float *A, uint8_t *S
 {
     const int N = c->p.n_beads; const long long M = c->p.n_chains;
     unsigned char *state = c->ws + c->lay.state;
+    const int hide = c->low_mode == 2 ? 1 : 0;       // packed low parts are not a float: exported as 0
     if (dev) {
-        CK(c, launch_xfer(do_export, state, R, A, S, N, 0, M, M, c->st));
+        CK(c, launch_xfer(do_export, state, R, A, S, N, 0, M, M, hide, c->st));
         c->launches += do_export ? 1 : 2;
         return SSM_OK;
     }
@@ -373,7 +450,7 @@ static int xfer_state(ssm_ctx *c, bool do_export, float *R, float *A, uint8_t *S
     for (long long k0 = 0; k0 < M; k0 += chunk) {
         const long long nk = M - k0 < chunk ? M - k0 : chunk;
         if (do_export) {
-            CK(c, launch_xfer(true, state, dR, dA, dS, N, k0, nk, chunk, c->st));
+            CK(c, launch_xfer(true, state, dR, dA, dS, N, k0, nk, chunk, hide, c->st));
             CK(c, cudaMemcpy2DAsync(R + k0, (size_t)M * 4, dR, (size_t)chunk * 4, (size_t)nk * 4, (size_t)3 * N, cudaMemcpyDeviceToHost, c->st));
             CK(c, cudaMemcpy2DAsync(A + k0, (size_t)M * 4, dA, (size_t)chunk * 4, (size_t)nk * 4, (size_t)4 * N, cudaMemcpyDeviceToHost, c->st));
             CK(c, cudaMemcpy2DAsync(S + k0, (size_t)M, dS, (size_t)chunk, (size_t)nk, (size_t)N, cudaMemcpyDeviceToHost, c->st));
@@ -382,7 +459,7 @@ static int xfer_state(ssm_ctx *c, bool do_export, float *R, float *A, uint8_t *S
             CK(c, cudaMemcpy2DAsync(dR, (size_t)chunk * 4, R + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)3 * N, cudaMemcpyHostToDevice, c->st));
             CK(c, cudaMemcpy2DAsync(dA, (size_t)chunk * 4, A + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)4 * N, cudaMemcpyHostToDevice, c->st));
             CK(c, cudaMemcpy2DAsync(dS, (size_t)chunk, S + k0, (size_t)M, (size_t)nk, (size_t)N, cudaMemcpyHostToDevice, c->st));
-            CK(c, launch_xfer(false, state, dR, dA, dS, N, k0, nk, chunk, c->st));
+            CK(c, launch_xfer(false, state, dR, dA, dS, N, k0, nk, chunk, 0, c->st));
             c->launches += 2;
         }
     }
@@ -404,7 +481,7 @@ extern "C" int ssm_set_state(ssm_ctx *c, const float *R, const float *A, const u
     if (!R || !A || !S) return fail(c, SSM_EINVAL, "NULL state pointer");
     if (global_step < 0) return fail(c, SSM_EINVAL, "global_step < 0");
     int rc = xfer_state(c, false, const_cast<float *>(R), const_cast<float *>(A), const_cast<uint8_t *>(S), dev);
-    if (rc == SSM_OK) c->step = global_step;
+    if (rc == SSM_OK) { c->step = global_step; c->low_mode = 1; }      // A[3] of the caller is the fp32 low part of x
     return rc;
 }
 

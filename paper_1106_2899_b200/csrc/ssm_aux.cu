@@ -35,8 +35,10 @@ __global__ void __launch_bounds__(128) ssm_init_kernel(const __grid_constant__ I
     for (int i = 0; i < N; ++i)
         for (int c = 0; c < 3; ++c) *reinterpret_cast<float *>(st + off_R(k, N, i, c)) = R[3 * i + c];
 
+    // the chains that pad the last warp tile never carry slip-springs (the step kernel gives them no
+    // construction attempts either), so that the warp's slot phase only ever sees real ones
     int Z = 0;
-    if (P.springs_on) {
+    if (P.springs_on && k < P.n_chains) {
         uint32_t w[4];
         stream_call(sk, P.rk, DOM_INIT_Z, chain, 0u, w);
         const uint32_t code = code23(w[0]);
@@ -73,7 +75,7 @@ cudaError_t launch_init(const InitParams &p, cudaStream_t st)
 // ---------------------------------------------------------------------------------------
 template <bool EXPORT>
 __global__ void __launch_bounds__(256) ssm_xfer_kernel(unsigned char *state, float *R, float *A, unsigned char *S,
-                                                       int N, long long k0, long long nk, long long pitch)
+                                                       int N, long long k0, long long nk, long long pitch, int hide_low)
 {
     const long long kk = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (kk >= nk) return;
@@ -86,7 +88,8 @@ __global__ void __launch_bounds__(256) ssm_xfer_kernel(unsigned char *state, flo
     } else if (row < 7 * N) {
         const int rr = row - 3 * N, c = rr / N, j = rr % N;
         float *p = reinterpret_cast<float *>(state + off_A(k, N, j, c));
-        if (EXPORT) A[(long long)rr * pitch + kk] = *p; else *p = A[(long long)rr * pitch + kk];
+        // (hide_low: the fourth word holds the packed low parts of ssm_step_kappa, not a float; export 0)
+        if (EXPORT) A[(long long)rr * pitch + kk] = (hide_low && c == 3) ? 0.0f : *p; else *p = A[(long long)rr * pitch + kk];
     } else {
         const int j = row - 7 * N;
         unsigned char *p = state + off_S(k, N, j);
@@ -106,12 +109,12 @@ __global__ void __launch_bounds__(256) ssm_count_z_kernel(unsigned char *state, 
 }
 
 cudaError_t launch_xfer(bool do_export, unsigned char *state, float *R, float *A, unsigned char *S, int N,
-                        long long k0, long long nk, long long pitch, cudaStream_t st)
+                        long long k0, long long nk, long long pitch, int hide_low, cudaStream_t st)
 {
     dim3 grid((unsigned)((nk + 255) / 256), (unsigned)(8 * N));
-    if (do_export) ssm_xfer_kernel<true><<<grid, 256, 0, st>>>(state, R, A, S, N, k0, nk, pitch);
+    if (do_export) ssm_xfer_kernel<true><<<grid, 256, 0, st>>>(state, R, A, S, N, k0, nk, pitch, hide_low);
     else {
-        ssm_xfer_kernel<false><<<grid, 256, 0, st>>>(state, R, A, S, N, k0, nk, pitch);
+        ssm_xfer_kernel<false><<<grid, 256, 0, st>>>(state, R, A, S, N, k0, nk, pitch, 0);
         ssm_count_z_kernel<<<(unsigned)((nk + 255) / 256), 256, 0, st>>>(state, N, k0, nk);
     }
     return cudaGetLastError();
@@ -150,6 +153,75 @@ __global__ void __launch_bounds__(128) ssm_chain_stress_kernel(const unsigned ch
 cudaError_t launch_chain_stress(const unsigned char *state, float *out, int N, long long M, float cs, cudaStream_t st)
 {
     ssm_chain_stress_kernel<<<(unsigned)((M + 127) / 128), 128, 0, st>>>(state, out, N, M, cs);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------
+// Clear the fourth word of every anchor (the low part(s) of the compensated advection): run when
+// the flow changes between simple shear and a general tensor, whose encodings of that word differ.
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) ssm_clear_low_kernel(unsigned char *state, long long n_tiles)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;      // (tile, slot of the warp)
+    if (i >= n_tiles * 256) return;
+    reinterpret_cast<float4 *>(state + (i >> 8) * kTileBytes + kTileA)[i & 255].w = 0.0f;
+}
+
+cudaError_t launch_clear_low(unsigned char *state, long long n_tiles, cudaStream_t st)
+{
+    ssm_clear_low_kernel<<<(unsigned)((n_tiles * 256 + 255) / 256), 256, 0, st>>>(state, n_tiles);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------
+// Stress of the current state per GROUP of chains_per_group consecutive local chains (eqs 16, 76
+// averaged by eq 54 over each group) and the groups' slip-spring counts: what a flow solver that
+// gives every group its own velocity gradient reads back.  One thread per chain;
+// out[group][13] int64 fixed point 2^-kStressShift: sigma[6], sigma_v[6], Z.  Integer sums, so the
+// result does not depend on the order of the atomics.
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) ssm_group_stress_kernel(const unsigned char *state, long long *out, int N,
+                                                               long long M, long long cpg, float cs)
+{
+    const long long k0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool valid = k0 < M;
+    const long long k = valid ? k0 : M - 1;
+    float sg[6] = {0, 0, 0, 0, 0, 0}, sv[6] = {0, 0, 0, 0, 0, 0};
+    float p[3], q[3];
+    for (int c = 0; c < 3; ++c) p[c] = *reinterpret_cast<const float *>(state + off_R(k, N, 0, c));
+    for (int i = 1; i < N; ++i) {
+        float b[3];
+        for (int c = 0; c < 3; ++c) { q[c] = *reinterpret_cast<const float *>(state + off_R(k, N, i, c)); b[c] = q[c] - p[c]; p[c] = q[c]; }
+        sg[0] += fmaf(3.f * b[0], b[0], -1.f); sg[1] += fmaf(3.f * b[1], b[1], -1.f); sg[2] += fmaf(3.f * b[2], b[2], -1.f);
+        sg[3] = fmaf(3.f * b[0], b[1], sg[3]); sg[4] = fmaf(3.f * b[1], b[2], sg[4]); sg[5] = fmaf(3.f * b[2], b[0], sg[5]);
+    }
+    sg[0] -= 1.f; sg[1] -= 1.f; sg[2] -= 1.f;                 // 3 sum b^2 - N = sum (3 b^2 - 1) - 1
+    const int Z = *reinterpret_cast<const int *>(state + off_Z(k, N));
+    for (int j = 0; j < Z; ++j) {
+        const int s = state[off_S(k, N, j)] - 1;
+        float d[3];
+        for (int c = 0; c < 3; ++c)
+            d[c] = *reinterpret_cast<const float *>(state + off_R(k, N, s, c)) - *reinterpret_cast<const float *>(state + off_A(k, N, j, c));
+        sv[0] += fmaf(cs * d[0], d[0], -1.f); sv[1] += fmaf(cs * d[1], d[1], -1.f); sv[2] += fmaf(cs * d[2], d[2], -1.f);
+        sv[3] = fmaf(cs * d[0], d[1], sv[3]); sv[4] = fmaf(cs * d[1], d[2], sv[4]); sv[5] = fmaf(cs * d[2], d[0], sv[5]);
+    }
+    const long long group = k / cpg;
+    const bool one_group = __all_sync(0xffffffffu, group == __shfl_sync(0xffffffffu, group, 0));
+    constexpr float scale = (float)(1 << kStressShift);
+    for (int t = 0; t < 13; ++t) {
+        long long v = t < 6 ? __float2ll_rn(sg[t] * scale) : (t < 12 ? __float2ll_rn(sv[t - 6] * scale) : (long long)Z << kStressShift);
+        if (!valid) v = 0;
+        if (one_group) {
+            for (int o = 16; o >= 1; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+            if ((threadIdx.x & 31) == 0) atomicAdd(reinterpret_cast<unsigned long long *>(out + group * 13 + t), (unsigned long long)v);
+        } else if (valid) atomicAdd(reinterpret_cast<unsigned long long *>(out + group * 13 + t), (unsigned long long)v);
+    }
+}
+
+cudaError_t launch_group_stress(const unsigned char *state, long long *out, int N, long long M, long long cpg, float cs,
+                                cudaStream_t st)
+{
+    ssm_group_stress_kernel<<<(unsigned)((M + 127) / 128), 128, 0, st>>>(state, out, N, M, cpg, cs);
     return cudaGetLastError();
 }
 

@@ -10,7 +10,11 @@
 //                                lane = coordinate (f%3) of the lane's bead f/3
 //   bytes [3072,7168)  A image : [chain in warp][slot 0..N-1] float4 = (A_x, A_y, A_z, A_x low part);
 //                                A_x + low part is the anchor's x, kept as a compensated sum so
-//                                that the affine advection of eq (45) does not drift in fp32
+//                                that the affine advection of eq (45) does not drift in fp32.
+//                                Under a general tensor (ssm_step_kappa) the fourth word holds three
+//                                signed 10-bit low parts instead, bits [10c, 10c + 10) for coordinate c
+//                                in units of ulp(A_c) / 1024 (advect_packed in ssm_step.cu); the host
+//                                tracks which encoding is current and clears the word on a change
 //   bytes [7168,7424)  S image : [chain in warp][slot] uint8, 0 = empty, 1..N
 //   bytes [7424,7552)  Z       : [chain in warp] int32 (32 entries, CPW used)
 #pragma once
@@ -42,6 +46,7 @@ constexpr int kSmX = 12672;      // int  [33]   exclusive prefix of Z over the w
 constexpr int kSmEv = 12816;     // uint [64]   construction candidates [chain][word]: bit k = attempt k passed the 16-bit test; [32 + chain] = (k << 16) | half of the chain's latest candidate
 constexpr int kSmSamp = 13072;   // int  [32]   per-chain fixed-point sum of d_x d_y over slip-springs (sample steps)
 constexpr int kSmKeys = 3840;    // uint [20]   the warp's copy of the Philox round keys (16-byte aligned)
+constexpr int kSmKap = 3920;     // float[9]   dt kappa of the warp's group of chains (general flow only), up to 3956
 constexpr int kSmSamp2 = 3584;   // int  [2][32] the same for d_y d_z and d_z d_x (isotropic correlator), in the spare kB after the mirror
 constexpr int kStageSteps = 8;   // recorded steps whose warp sums wait in kSmStage before they are added to the CTA sums
 constexpr int kSmStage = 13200;  // int  [8][12] warp sums of the last recorded steps (int32 fixed point)
@@ -73,6 +78,8 @@ struct StepParams {
     float bm_noise;   // -2 ln2 * 2 dt: r^2 = bm * log2(u) gives sqrt(2 dt) * N(0,1)  (eqs 44, 46, 47)
     float bm_anchor;  // -2 ln2 * N_s/3: anchor offsets of new slip-springs (eq 52)
     float gdt;        // shear_rate * dt      (eq 44, 45 with kappa_xy of eq 60)
+    const float *kappa;               // null, or [groups][9] dt kappa_ab row-major (eqs 18, 21): general flow
+    int   tiles_per_group;            // group of a warp tile = tile / tiles_per_group
     float fx_scale;   // dt * (3/N_s) * 2^kFxShift
     float q2l;        // 2 * (3/(4 N_s)) * log2(e): exponent scale of 1 - tanh(x) = 2/(1+e^{2x})
     float h2;         // 2 dt/zeta_s
@@ -86,6 +93,7 @@ struct StepParams {
 struct InitParams {
     unsigned char *state;
     long long      n_chains_padded;   // n_tiles * CPW
+    long long      n_chains;          // M
     unsigned long long chain_offset;
     unsigned       rk[20];            // Philox round keys
     int            n_beads;

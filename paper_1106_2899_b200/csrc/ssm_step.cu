@@ -34,9 +34,32 @@ __device__ __forceinline__ float mufu_ex2(float x)
 
 constexpr unsigned kFull = 0xffffffffu;
 
-template <int G, bool SHEAR>
+// Anchor advection under a general velocity gradient (eq 45 with the tensor of eq 21), one coordinate.
+// Eq (45) adds nearly the same small increment every step, which a plain fp32 sum rounds the same way
+// every step (or drops altogether when it is below half an ulp), so each coordinate is advanced as a
+// compensated sum whose low part is kept as a signed 10-bit integer q in units of ulp(hi)/1024 =
+// 2^(e - 160), e = biased exponent of hi (three of them share the fourth word of the anchor; layout
+// in ssm_common.h).  hi: coordinate, inc: dt (kappa . A) of this coordinate, q: low part in; returns
+// the new coordinate and the new low part in q.
+__device__ __forceinline__ float advect_packed(float hi, float inc, int &q)
+{
+    const int e = (__float_as_int(hi) >> 23) & 0xFF;
+    const float unit = __int_as_float(max(e - 33, 0) << 23);
+    const float t = fmaf((float)q, unit, inc);
+    const float sum = hi + t;
+    const float bb = sum - hi;
+    const float low = (hi - (sum - bb)) + (t - bb);          // hi + t = sum + low exactly (two-sum)
+    const int e2 = (__float_as_int(sum) >> 23) & 0xFF;
+    const float inv = __int_as_float((287 - max(e2, 34)) << 23);                    // 2^(160 - e2)
+    q = e2 >= 34 ? max(-512, min(511, __float2int_rn(low * inv))) : 0;
+    return sum;
+}
+
+// FLOW: 0 = no flow, 1 = simple shear kappa_xy (eq 60), 2 = one full tensor per group of chains (eqs 18, 21)
+template <int G, int FLOW>
 __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid_constant__ StepParams P)
 {
+    constexpr bool SHEAR = FLOW == 1;
     constexpr int N = kBPL * G, CPW = 32 / G, LG = Log2<G>::v, LN = LG + 3, WPC = (N + 31) / 32;
     extern __shared__ __align__(16) unsigned char smem[];
 
@@ -59,6 +82,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     unsigned char *Map = wb + kSmMap;
     int *Samp = reinterpret_cast<int *>(wb + kSmSamp);
     int *Samp2 = reinterpret_cast<int *>(wb + kSmSamp2);
+    float *Kap = reinterpret_cast<float *>(wb + kSmKap);
     int *Stage = reinterpret_cast<int *>(wb + kSmStage);
     int4 *Stage4 = reinterpret_cast<int4 *>(wb + kSmStage);
     unsigned long long *acc = reinterpret_cast<unsigned long long *>(smem + kSmAcc);
@@ -153,6 +177,8 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
             for (int v = 0; v < 8; ++v) A4[v * 32 + lane] = gA[v * 32 + lane];
             reinterpret_cast<uint2 *>(Sb)[lane] = reinterpret_cast<const uint2 *>(tp + kTileS)[lane];
             Zs[lane] = reinterpret_cast<const int *>(tp + kTileZ)[lane];
+            // dt kappa of the group this warp's chains belong to (a tile never straddles two groups)
+            if (FLOW == 2 && lane < 9) Kap[lane] = P.kappa[(long long)(tile / P.tiles_per_group) * 9 + lane];
 #pragma unroll
             for (int v = 0; v < 6; ++v) Rf4[lane * 7 + v] = make_float4(r[4 * v], r[4 * v + 1], r[4 * v + 2], r[4 * v + 3]);
         }
@@ -281,6 +307,11 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
             const int Z0 = Zs[cw];
 
             // ================= bead phase: substep 1 (eq 44) =================
+            float kap[9], ox = 0.f, oy = 0.f, oz = 0.f;       // FLOW 2: dt kappa, and the time-t position of the bead in hand
+            if (FLOW == 2) {
+#pragma unroll
+                for (int i = 0; i < 9; ++i) kap[i] = Kap[i];
+            }
 #pragma unroll
             for (int q = 0; q < 3; ++q) {
                 float z8[8];
@@ -297,6 +328,11 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                         float inc = fmaf(P.dt3, lap, z8[4 * h + e]);
                         inc = fmaf((float)fxa[e], 1.0f / (float)(1 << kFxShift), inc);
                         if (SHEAR && c == 0) inc = fmaf(P.gdt, r[f + 1], inc);
+                        if (FLOW == 2) {
+                            // dt (kappa . R_i)_c from the time-t position (x, y, z of a bead are updated in this order)
+                            if (c == 0) { ox = r[f]; oy = r[f + 1]; oz = r[f + 2]; }
+                            inc = fmaf(kap[3 * c], ox, fmaf(kap[3 * c + 1], oy, fmaf(kap[3 * c + 2], oz, inc)));
+                        }
                         r[f] += inc;
                     }
                 }
@@ -333,6 +369,19 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                         const float bb = sum - a.x;
                         a.w = (a.x - (sum - bb)) + (t - bb);
                         a.x = sum;
+                        if (act) A4[sx] = a;
+                    }
+                    if (FLOW == 2) {
+                        // eq 45 with the full tensor; the fourth word holds the three packed low parts
+                        const int pw = __float_as_int(a.w);
+                        int q0 = (pw << 22) >> 22, q1 = (pw << 12) >> 22, q2 = (pw << 2) >> 22;
+                        const float ix = fmaf(Kap[0], a.x, fmaf(Kap[1], a.y, Kap[2] * a.z));
+                        const float iy = fmaf(Kap[3], a.x, fmaf(Kap[4], a.y, Kap[5] * a.z));
+                        const float iz = fmaf(Kap[6], a.x, fmaf(Kap[7], a.y, Kap[8] * a.z));
+                        a.x = advect_packed(a.x, ix, q0);
+                        a.y = advect_packed(a.y, iy, q1);
+                        a.z = advect_packed(a.z, iz, q2);
+                        a.w = __int_as_float((q0 & 0x3FF) | ((q1 & 0x3FF) << 10) | ((q2 & 0x3FF) << 20));
                         if (act) A4[sx] = a;
                     }
                     // Glauber hop (eqs 23, 24 with the cap of eqs 48, 49):
@@ -524,32 +573,34 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
 // ---------------------------------------------------------------------------------------
 // host-side launcher
 // ---------------------------------------------------------------------------------------
-template <int G, bool SHEAR>
+template <int G, int FLOW>
 static cudaError_t launch_gs(const StepParams &p, int grid, cudaStream_t st)
 {
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(ssm_step_kernel<G, SHEAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmStep);
+        cudaError_t e = cudaFuncSetAttribute(ssm_step_kernel<G, FLOW>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmStep);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    ssm_step_kernel<G, SHEAR><<<grid, kBlockThreads, kSmStep, st>>>(p);
+    ssm_step_kernel<G, FLOW><<<grid, kBlockThreads, kSmStep, st>>>(p);
     return cudaGetLastError();
 }
 
-// the affine term of eqs 44, 45 is compiled in only when a velocity gradient is applied
+// the affine term of eqs 44, 45 is compiled in only when a velocity gradient is applied: the full tensor
+// when a table of tensors is given, else kappa_xy when the shear rate is not zero
 template <int G>
 static cudaError_t launch_g(const StepParams &p, int grid, cudaStream_t st)
 {
-    return p.gdt != 0.0f ? launch_gs<G, true>(p, grid, st) : launch_gs<G, false>(p, grid, st);
+    if (p.kappa) return launch_gs<G, 2>(p, grid, st);
+    return p.gdt != 0.0f ? launch_gs<G, 1>(p, grid, st) : launch_gs<G, 0>(p, grid, st);
 }
 
 template <int G>
 static cudaError_t occupancy_g(int *blocks_per_sm)
 {
-    cudaError_t e = cudaFuncSetAttribute(ssm_step_kernel<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmStep);
+    cudaError_t e = cudaFuncSetAttribute(ssm_step_kernel<G, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmStep);
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, ssm_step_kernel<G, true>, kBlockThreads, kSmStep);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, ssm_step_kernel<G, 2>, kBlockThreads, kSmStep);
 }
 
 cudaError_t step_occupancy(int n_beads, int *blocks_per_sm)

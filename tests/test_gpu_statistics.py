@@ -192,6 +192,12 @@ def test_edge_cases(ssm):
         g.step(40)
         n, _ = compare_state(e, g)
         assert n >= M - 1
+        # the ensemble stress of a ragged tile counts the real chains only (the chains that pad the
+        # tile carry no slip-springs); one chain, no averaging: tolerance of DESIGN.md section 8.3
+        first = e.first_fragile[e.first_fragile >= 0]
+        clean = int(first.min()) if first.size else 40
+        ok, w = close(g.stress()[:clean], want[:clean], 2e-5 * np.sqrt(N / 8.0))
+        assert ok, (N, M, w)
     # zero steps is a no-op; stress before any sample is a range error, not a crash
     g = ssm.Ensemble(32, 64, seed=3, stress_every=1, stress_capacity=4)
     R0, A0, S0, st0 = g.get_state()
