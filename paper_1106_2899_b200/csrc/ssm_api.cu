@@ -74,7 +74,7 @@ static bool check_params(const ssm_params *p, std::string &why)
 {
     if (!p) { why = "params is NULL"; return false; }
     const int N = p->n_beads;
-    if (!(N == 8 || N == 16 || N == 32 || N == 64 || N == 128)) { why = "n_beads must be 8, 16, 32, 64 or 128"; return false; }
+    if (N < 2 || N > 128) { why = "n_beads must be 2..128"; return false; }
     if (p->n_chains < 1) { why = "n_chains must be >= 1"; return false; }
     if (p->chain_offset + (uint64_t)p->n_chains + 16 > 0xFFFFFFFFull) { why = "global chain index must fit 32 bits"; return false; }
     if (!(p->dt > 0.0) || !(p->dt < 1.0 / 6.0)) { why = "dt must be in (0, 1/6): the Euler map needs 12 dt < 2"; return false; }
@@ -95,7 +95,7 @@ static bool check_params(const ssm_params *p, std::string &why)
 static Layout make_layout(const ssm_params *p)
 {
     Layout L{};
-    const int cpw = chains_per_warp(p->n_beads);
+    const int npad = padded_beads(p->n_beads), cpw = chains_per_warp(npad);
     L.n_tiles = (p->n_chains + cpw - 1) / cpw;
     size_t o = 0;
     L.state = o; o = align_up(o + (size_t)L.n_tiles * kTileBytes, 256);
@@ -113,7 +113,7 @@ static Layout make_layout(const ssm_params *p)
     // staging for host-pointer get/set state and chain stress: chunks of <= 65536 chains
     L.stage_chains = p->n_chains < 65536 ? p->n_chains : 65536;
     // (at least 1 MB, so that the issue-rate probe's scratch of 2 kB per SM fits any ensemble)
-    size_t stage_bytes = (size_t)L.stage_chains * (size_t)(29 * p->n_beads > 48 ? 29 * p->n_beads : 48);
+    size_t stage_bytes = (size_t)L.stage_chains * (size_t)(29 * npad > 48 ? 29 * npad : 48);
     if (stage_bytes < ((size_t)1 << 20)) stage_bytes = (size_t)1 << 20;
     L.stage = o; o = align_up(o + stage_bytes, 256);
     L.total = o;
@@ -177,7 +177,7 @@ extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, s
 
     int dev = 0, n_sm = 0, bps = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess || (e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess
-        || (e = step_occupancy(p->n_beads, &bps)) != cudaSuccess) {
+        || (e = step_occupancy(padded_beads(p->n_beads), &bps)) != cudaSuccess) {
         int rc = cuda_fail(nullptr, e, "device query"); delete c; return rc;
     }
     if (bps < 1) { delete c; return fail(nullptr, SSM_ECUDA, "step kernel does not fit on an SM"); }
@@ -194,6 +194,7 @@ extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, s
     philox_round_keys((unsigned)(p->seed & 0xFFFFFFFFull), (unsigned)(p->seed >> 32), sp.rk);
     sp.springs_on = c->springs_on ? 1 : 0;
     sp.k_attempts = p->k_attempts;
+    sp.n_act = p->n_beads;
     sp.n_comp = p->corr_components == 3 ? 3 : 1;
     sp.dt3 = (float)(3.0 * p->dt);
     const double m2ln2 = -2.0 * 0.6931471805599453;        // r^2 = -2 ln u = (-2 ln 2) log2 u
@@ -213,7 +214,8 @@ extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, s
     InitParams ip;
     std::memset(&ip, 0, sizeof ip);
     ip.state = c->ws + lay.state;
-    ip.n_chains_padded = lay.n_tiles * chains_per_warp(p->n_beads); ip.n_chains = p->n_chains;
+    ip.n_chains_padded = lay.n_tiles * chains_per_warp(padded_beads(p->n_beads)); ip.n_chains = p->n_chains;
+    ip.n_pad = padded_beads(p->n_beads);
     ip.chain_offset = p->chain_offset; std::memcpy(ip.rk, sp.rk, sizeof ip.rk);
     ip.n_beads = p->n_beads; ip.springs_on = sp.springs_on;
     ip.bm_bond = (float)(m2ln2 / 3.0); ip.bm_anchor = sp.bm_anchor;
@@ -287,7 +289,7 @@ static int step_impl(ssm_ctx *c, int64_t n_steps, double shear_rate, const float
         sp.n_rec = (int)nrec;
         sp.stress = reinterpret_cast<long long *>(c->ws + c->lay.stress) + c->n_records * 12;
         sp.samples = nsmp > 0 ? reinterpret_cast<float2 *>(c->ws + c->lay.samples) : nullptr;
-        CK(c, launch_step(p.n_beads, sp, c->grid, c->st));
+        CK(c, launch_step(padded_beads(p.n_beads), sp, c->grid, c->st));
         c->launches += 1;
         if (nsmp > 0) {
             CorrParams cp;
@@ -326,7 +328,7 @@ extern "C" int ssm_step(ssm_ctx *c, int64_t n_steps, double shear_rate)
 // would hold chains of two groups
 static bool group_geometry(const ssm_ctx *c, int64_t cpg, long long *n_groups, long long *tiles_per_group)
 {
-    const long long M = c->p.n_chains, cpw = chains_per_warp(c->p.n_beads);
+    const long long M = c->p.n_chains, cpw = chains_per_warp(padded_beads(c->p.n_beads));
     if (cpg < 1) return false;
     if (cpg >= M) { *n_groups = 1; *tiles_per_group = c->lay.n_tiles; return true; }
     if (cpg % cpw != 0) return false;
@@ -341,7 +343,7 @@ extern "C" int ssm_step_kappa(ssm_ctx *c, int64_t n_steps, int64_t chains_per_gr
     if (!h_kappa) return fail(c, SSM_EINVAL, "h_kappa is NULL");
     long long ng = 0, tpg = 0;
     if (!group_geometry(c, chains_per_group, &ng, &tpg))
-        return fail(c, SSM_EINVAL, "chains_per_group must be >= n_chains (one group) or a multiple of 256 / n_beads (the chains of a warp share one tensor)");
+        return fail(c, SSM_EINVAL, "chains_per_group must be >= n_chains (one group) or a multiple of the chains per warp, 256 / (n_beads rounded up to 8, 16, 32, 64 or 128)");
     c->kappa_host.resize((size_t)ng * 9);
     for (size_t i = 0; i < (size_t)ng * 9; ++i) {
         if (!std::isfinite(h_kappa[i])) return fail(c, SSM_EINVAL, "kappa is not finite");

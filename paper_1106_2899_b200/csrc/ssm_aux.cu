@@ -19,7 +19,7 @@ __global__ void __launch_bounds__(128) ssm_init_kernel(const __grid_constant__ I
 {
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= P.n_chains_padded) return;
-    const int N = P.n_beads, zmax = N;
+    const int N = P.n_beads, NP = P.n_pad, zmax = N;
     const uint32_t chain = (uint32_t)(P.chain_offset + (unsigned long long)k);
     const StreamKey sk = make_stream(0ull, P.rk);
     const BoxMuller bm_bond(P.bm_bond), bm_anchor(P.bm_anchor);
@@ -33,7 +33,7 @@ __global__ void __launch_bounds__(128) ssm_init_kernel(const __grid_constant__ I
         R[m + 3] = R[m] + z8[m & 7];
     }
     for (int i = 0; i < N; ++i)
-        for (int c = 0; c < 3; ++c) *reinterpret_cast<float *>(st + off_R(k, N, i, c)) = R[3 * i + c];
+        for (int c = 0; c < 3; ++c) *reinterpret_cast<float *>(st + off_R(k, NP, i, c)) = R[3 * i + c];
 
     // the chains that pad the last warp tile never carry slip-springs (the step kernel gives them no
     // construction attempts either), so that the warp's slot phase only ever sees real ones
@@ -44,7 +44,7 @@ __global__ void __launch_bounds__(128) ssm_init_kernel(const __grid_constant__ I
         const uint32_t code = code23(w[0]);
         while (Z < zmax && code >= P.t_cdf[Z]) ++Z;
     }
-    *reinterpret_cast<int *>(st + off_Z(k, N)) = Z;
+    *reinterpret_cast<int *>(st + off_Z(k, NP)) = Z;
     for (int j = 0; j < zmax; ++j) {
         int s = 0; float a[4] = {0.f, 0.f, 0.f, 0.f};
         if (j < Z) {
@@ -55,8 +55,8 @@ __global__ void __launch_bounds__(128) ssm_init_kernel(const __grid_constant__ I
             anchor_normals(sk, P.rk, DOM_INIT_ANCHOR, chain, (uint32_t)j, bm_anchor, z3);
             for (int c = 0; c < 3; ++c) a[c] = R[3 * (s - 1) + c] + z3[c];
         }
-        st[off_S(k, N, j)] = (unsigned char)s;
-        for (int c = 0; c < 4; ++c) *reinterpret_cast<float *>(st + off_A(k, N, j, c)) = a[c];
+        st[off_S(k, NP, j)] = (unsigned char)s;
+        for (int c = 0; c < 4; ++c) *reinterpret_cast<float *>(st + off_A(k, NP, j, c)) = a[c];
     }
 }
 
@@ -75,7 +75,7 @@ cudaError_t launch_init(const InitParams &p, cudaStream_t st)
 // ---------------------------------------------------------------------------------------
 template <bool EXPORT>
 __global__ void __launch_bounds__(256) ssm_xfer_kernel(unsigned char *state, float *R, float *A, unsigned char *S,
-                                                       int N, long long k0, long long nk, long long pitch, int hide_low)
+                                                       int N, int NP, long long k0, long long nk, long long pitch, int hide_low)
 {
     const long long kk = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (kk >= nk) return;
@@ -83,39 +83,40 @@ __global__ void __launch_bounds__(256) ssm_xfer_kernel(unsigned char *state, flo
     const int row = blockIdx.y;                         // 0 .. 8N-1
     if (row < 3 * N) {
         const int c = row / N, i = row % N;
-        float *p = reinterpret_cast<float *>(state + off_R(k, N, i, c));
+        float *p = reinterpret_cast<float *>(state + off_R(k, NP, i, c));
         if (EXPORT) R[(long long)row * pitch + kk] = *p; else *p = R[(long long)row * pitch + kk];
     } else if (row < 7 * N) {
         const int rr = row - 3 * N, c = rr / N, j = rr % N;
-        float *p = reinterpret_cast<float *>(state + off_A(k, N, j, c));
+        float *p = reinterpret_cast<float *>(state + off_A(k, NP, j, c));
         // (hide_low: the fourth word holds the packed low parts of ssm_step_kappa, not a float; export 0)
         if (EXPORT) A[(long long)rr * pitch + kk] = (hide_low && c == 3) ? 0.0f : *p; else *p = A[(long long)rr * pitch + kk];
     } else {
         const int j = row - 7 * N;
-        unsigned char *p = state + off_S(k, N, j);
+        unsigned char *p = state + off_S(k, NP, j);
         if (EXPORT) S[(long long)j * pitch + kk] = *p; else *p = S[(long long)j * pitch + kk];
     }
 }
 
 // after an import: Z_k = number of occupied slots (they must be the leading ones)
-__global__ void __launch_bounds__(256) ssm_count_z_kernel(unsigned char *state, int N, long long k0, long long nk)
+__global__ void __launch_bounds__(256) ssm_count_z_kernel(unsigned char *state, int N, int NP, long long k0, long long nk)
 {
     const long long kk = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (kk >= nk) return;
     const long long k = k0 + kk;
     int Z = 0;
-    while (Z < N && state[off_S(k, N, Z)] != 0) ++Z;
-    *reinterpret_cast<int *>(state + off_Z(k, N)) = Z;
+    while (Z < N && state[off_S(k, NP, Z)] != 0) ++Z;
+    *reinterpret_cast<int *>(state + off_Z(k, NP)) = Z;
 }
 
 cudaError_t launch_xfer(bool do_export, unsigned char *state, float *R, float *A, unsigned char *S, int N,
                         long long k0, long long nk, long long pitch, int hide_low, cudaStream_t st)
 {
+    const int NP = padded_beads(N);
     dim3 grid((unsigned)((nk + 255) / 256), (unsigned)(8 * N));
-    if (do_export) ssm_xfer_kernel<true><<<grid, 256, 0, st>>>(state, R, A, S, N, k0, nk, pitch, hide_low);
+    if (do_export) ssm_xfer_kernel<true><<<grid, 256, 0, st>>>(state, R, A, S, N, NP, k0, nk, pitch, hide_low);
     else {
-        ssm_xfer_kernel<false><<<grid, 256, 0, st>>>(state, R, A, S, N, k0, nk, pitch, 0);
-        ssm_count_z_kernel<<<(unsigned)((nk + 255) / 256), 256, 0, st>>>(state, N, k0, nk);
+        ssm_xfer_kernel<false><<<grid, 256, 0, st>>>(state, R, A, S, N, NP, k0, nk, pitch, 0);
+        ssm_count_z_kernel<<<(unsigned)((nk + 255) / 256), 256, 0, st>>>(state, N, NP, k0, nk);
     }
     return cudaGetLastError();
 }
@@ -128,22 +129,23 @@ __global__ void __launch_bounds__(128) ssm_chain_stress_kernel(const unsigned ch
 {
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= M) return;
+    const int NP = padded_beads(N);
     float sg[6] = {0, 0, 0, 0, 0, 0}, sv[6] = {0, 0, 0, 0, 0, 0};
     float p[3], q[3];
-    for (int c = 0; c < 3; ++c) p[c] = *reinterpret_cast<const float *>(state + off_R(k, N, 0, c));
+    for (int c = 0; c < 3; ++c) p[c] = *reinterpret_cast<const float *>(state + off_R(k, NP, 0, c));
     for (int i = 1; i < N; ++i) {
         float b[3];
-        for (int c = 0; c < 3; ++c) { q[c] = *reinterpret_cast<const float *>(state + off_R(k, N, i, c)); b[c] = q[c] - p[c]; p[c] = q[c]; }
+        for (int c = 0; c < 3; ++c) { q[c] = *reinterpret_cast<const float *>(state + off_R(k, NP, i, c)); b[c] = q[c] - p[c]; p[c] = q[c]; }
         sg[0] += fmaf(3.f * b[0], b[0], -1.f); sg[1] += fmaf(3.f * b[1], b[1], -1.f); sg[2] += fmaf(3.f * b[2], b[2], -1.f);
         sg[3] = fmaf(3.f * b[0], b[1], sg[3]); sg[4] = fmaf(3.f * b[1], b[2], sg[4]); sg[5] = fmaf(3.f * b[2], b[0], sg[5]);
     }
     sg[0] -= 1.f; sg[1] -= 1.f; sg[2] -= 1.f;                 // 3 sum b^2 - N = sum (3 b^2 - 1) - 1
-    const int Z = *reinterpret_cast<const int *>(state + off_Z(k, N));
+    const int Z = *reinterpret_cast<const int *>(state + off_Z(k, NP));
     for (int j = 0; j < Z; ++j) {
-        const int s = state[off_S(k, N, j)] - 1;
+        const int s = state[off_S(k, NP, j)] - 1;
         float d[3];
         for (int c = 0; c < 3; ++c)
-            d[c] = *reinterpret_cast<const float *>(state + off_R(k, N, s, c)) - *reinterpret_cast<const float *>(state + off_A(k, N, j, c));
+            d[c] = *reinterpret_cast<const float *>(state + off_R(k, NP, s, c)) - *reinterpret_cast<const float *>(state + off_A(k, NP, j, c));
         sv[0] += fmaf(cs * d[0], d[0], -1.f); sv[1] += fmaf(cs * d[1], d[1], -1.f); sv[2] += fmaf(cs * d[2], d[2], -1.f);
         sv[3] = fmaf(cs * d[0], d[1], sv[3]); sv[4] = fmaf(cs * d[1], d[2], sv[4]); sv[5] = fmaf(cs * d[2], d[0], sv[5]);
     }
@@ -186,22 +188,23 @@ __global__ void __launch_bounds__(128) ssm_group_stress_kernel(const unsigned ch
     const long long k0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = k0 < M;
     const long long k = valid ? k0 : M - 1;
+    const int NP = padded_beads(N);
     float sg[6] = {0, 0, 0, 0, 0, 0}, sv[6] = {0, 0, 0, 0, 0, 0};
     float p[3], q[3];
-    for (int c = 0; c < 3; ++c) p[c] = *reinterpret_cast<const float *>(state + off_R(k, N, 0, c));
+    for (int c = 0; c < 3; ++c) p[c] = *reinterpret_cast<const float *>(state + off_R(k, NP, 0, c));
     for (int i = 1; i < N; ++i) {
         float b[3];
-        for (int c = 0; c < 3; ++c) { q[c] = *reinterpret_cast<const float *>(state + off_R(k, N, i, c)); b[c] = q[c] - p[c]; p[c] = q[c]; }
+        for (int c = 0; c < 3; ++c) { q[c] = *reinterpret_cast<const float *>(state + off_R(k, NP, i, c)); b[c] = q[c] - p[c]; p[c] = q[c]; }
         sg[0] += fmaf(3.f * b[0], b[0], -1.f); sg[1] += fmaf(3.f * b[1], b[1], -1.f); sg[2] += fmaf(3.f * b[2], b[2], -1.f);
         sg[3] = fmaf(3.f * b[0], b[1], sg[3]); sg[4] = fmaf(3.f * b[1], b[2], sg[4]); sg[5] = fmaf(3.f * b[2], b[0], sg[5]);
     }
     sg[0] -= 1.f; sg[1] -= 1.f; sg[2] -= 1.f;                 // 3 sum b^2 - N = sum (3 b^2 - 1) - 1
-    const int Z = *reinterpret_cast<const int *>(state + off_Z(k, N));
+    const int Z = *reinterpret_cast<const int *>(state + off_Z(k, NP));
     for (int j = 0; j < Z; ++j) {
-        const int s = state[off_S(k, N, j)] - 1;
+        const int s = state[off_S(k, NP, j)] - 1;
         float d[3];
         for (int c = 0; c < 3; ++c)
-            d[c] = *reinterpret_cast<const float *>(state + off_R(k, N, s, c)) - *reinterpret_cast<const float *>(state + off_A(k, N, j, c));
+            d[c] = *reinterpret_cast<const float *>(state + off_R(k, NP, s, c)) - *reinterpret_cast<const float *>(state + off_A(k, NP, j, c));
         sv[0] += fmaf(cs * d[0], d[0], -1.f); sv[1] += fmaf(cs * d[1], d[1], -1.f); sv[2] += fmaf(cs * d[2], d[2], -1.f);
         sv[3] = fmaf(cs * d[0], d[1], sv[3]); sv[4] = fmaf(cs * d[1], d[2], sv[4]); sv[5] = fmaf(cs * d[2], d[0], sv[5]);
     }

@@ -1,8 +1,11 @@
 // ssm_common.h -- internal layout and launch-parameter structs of libssm (host + device).
 //
-// Mapping: a chain of N = 8G beads is owned by G consecutive lanes of
-// one warp (G = 1, 2, 4, 8, 16), 8 consecutive beads per lane, so a warp owns CPW = 32/G
-// = 256/N chains (256 beads, up to 256 slip-spring slots) and never talks to another warp.
+// Mapping: a chain of N beads is owned by G consecutive lanes of one warp,
+// G = 1, 2, 4, 8, 16 the smallest with 8G >= N, 8 consecutive beads per lane, so a warp owns
+// CPW = 32/G chains (256 bead places, up to 256 slip-spring slots) and never talks to another
+// warp.  When N < 8G (the paper's N = 10, 20, 40, 80) the places N..8G-1 of a chain are padding:
+// no bond reaches them, no slip-spring sits on them, they are kept at the origin.  Every
+// "n_beads" argument of the layout helpers below is the PADDED count 8G.
 // The unit of state in HBM is the "warp tile": the register / shared-memory image of one
 // warp's chains, laid out so that a warp loads and stores it with coalesced 16-byte accesses:
 //
@@ -73,6 +76,7 @@ struct StepParams {
     int            n_rec;             // popcount(rec_mask)
     int            springs_on;
     int            k_attempts;        // 0: K = N - Z (GPU); k > 0: K = min(k, N - Z)
+    int            n_act;             // N, the number of beads of a chain (<= 8G, the places a chain occupies)
     unsigned rk[20];  // Philox round keys: (k0 + r W0, k1 + r W1), r = 0..9
     float dt3;        // 3 dt                 (Rouse spring constant 3kT/b^2, eq 1)
     float bm_noise;   // -2 ln2 * 2 dt: r^2 = bm * log2(u) gives sqrt(2 dt) * N(0,1)  (eqs 44, 46, 47)
@@ -96,7 +100,8 @@ struct InitParams {
     long long      n_chains;          // M
     unsigned long long chain_offset;
     unsigned       rk[20];            // Philox round keys
-    int            n_beads;
+    int            n_beads;           // N
+    int            n_pad;             // 8G: bead places per chain in the tiles
     int            springs_on;
     float          bm_bond;           // -2 ln2 / 3:     bond components N(0, 1/3)    (eq 6)
     float          bm_anchor;         // -2 ln2 N_s / 3: anchor offsets N(0, N_s/3)  (eq 15)
@@ -119,6 +124,7 @@ struct CorrParams {
 };
 
 // address of bead coordinate / slot entry inside the tiled state (host and device)
+__host__ __device__ inline int padded_beads(int n) { int g = kBPL; while (g < n) g <<= 1; return g; }
 __host__ __device__ inline int chains_per_warp(int n_beads) { return 256 / n_beads; }
 __host__ __device__ inline long long off_R(long long chain, int n_beads, int bead, int c)
 {

@@ -65,6 +65,11 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int l = lane & (G - 1), cw = lane >> LG;
+    // NA = the chain's number of beads; N = 8G places (NA < N: the places NA..N-1 are padding at the origin)
+    const int NA = P.n_act;
+    const bool ragged = NA != N;
+    const int real_here = min(kBPL, max(0, NA - kBPL * l));          // real beads among this lane's 8 places
+    const float bonds_here = (float)min(kBPL, max(0, NA - 1 - kBPL * l));   // bonds i -> i+1 that start in this lane
     unsigned char *wb = smem + warp * kSmWarp;
     // mirror of the bead positions: the lane's 24 register floats as they are (6 x 16 bytes,
     // 28 floats per lane: the same index as Fx), read by the slot phase as three scalars per bead
@@ -221,6 +226,13 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
 #pragma unroll
                 for (int k = 0; k < 8; ++k) b[3 * k + c] = (k == 7 ? rt : r[3 * (k + 1) + c]) - r[3 * k + c];
             }
+            if (ragged) {
+                // free end at bead NA (eq 1): no bond leaves the last real bead, none touches a padding place
+#pragma unroll
+                for (int k = 0; k < 8; ++k)
+                    if (k >= NA - 1 - kBPL * l) { b[3 * k] = 0.f; b[3 * k + 1] = 0.f; b[3 * k + 2] = 0.f; }
+                if (real_here == 0) { bl[0] = 0.f; bl[1] = 0.f; bl[2] = 0.f; }
+            }
 
             // ---- observables of the state after step n-1 (eqs 16, 76) and ensemble sums (eq 54)
             if (rec_prev || smp_prev) {
@@ -258,7 +270,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     // (scaled by 2^kStressShift here, a power of two: the products are the same numbers)
                     constexpr float scale = (float)(1 << kStressShift);
                     const float s3 = valid ? 3.0f * scale : 0.0f, css = P.cs * scale;
-                    const float nb = valid ? ((l == G - 1) ? 7.0f * scale : 8.0f * scale) : 0.0f;
+                    const float nb = valid ? bonds_here * scale : 0.0f;
                     const float cnts = cnt * scale;
                     float t[12];
                     t[0] = fmaf(s3, v[0], -nb); t[1] = fmaf(s3, v[1], -nb); t[2] = fmaf(s3, v[2], -nb);
@@ -337,6 +349,11 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     }
                 }
             }
+            if (ragged) {
+#pragma unroll
+                for (int f = 0; f < 24; ++f)
+                    if (f >= 3 * real_here) r[f] = 0.0f;
+            }
 #pragma unroll
             for (int v = 0; v < 6; ++v) Rf4[lane * 7 + v] = make_float4(r[4 * v], r[4 * v + 1], r[4 * v + 2], r[4 * v + 3]);
             __syncwarp();
@@ -391,7 +408,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     // neighbours along the chain are 3 floats away, 7 across a lane boundary (4 floats of padding)
                     const int fi = fx_index(b0), kb = b0 & 7;
                     const float4 r0 = bead(fi);
-                    const float4 rp = bead(fi + (s < N ? (kb == 7 ? 7 : 3) : 0));
+                    const float4 rp = bead(fi + (s < NA ? (kb == 7 ? 7 : 3) : 0));
                     const float4 rm = bead(fi - (s > 1 ? (kb == 0 ? 7 : 3) : 0));
                     const float d0x = r0.x - a.x, d0y = r0.y - a.y, d0z = r0.z - a.z;
                     const float dpx = rp.x - a.x, dpy = rp.y - a.y, dpz = rp.z - a.z;
@@ -401,13 +418,13 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     const float em = fmaf(dmz, dmz, fmaf(dmy, dmy, dmx * dmx));
                     float pp = fminf(__fdividef(P.h2, 1.0f + mufu_ex2(P.q2l * (ep - e0))), 0.5f);
                     float pm = fminf(__fdividef(P.h2, 1.0f + mufu_ex2(P.q2l * (em - e0))), 0.5f);
-                    if (s == N) pp = 0.0f;
+                    if (s == NA) pp = 0.0f;
                     if (s == 1) pm = 0.0f;
                     const float uu = u23(w_hop);
                     const bool up = uu < pp, dn = !up && uu < pp + pm;
                     const int sn = s + (up ? 1 : 0) - (dn ? 1 : 0);
                     // destruction at the ends (eq 53), integer-domain comparison
-                    const bool destroyed = (sn == 1 || sn == N) && code23(w_end) < P.t_destroy;
+                    const bool destroyed = (sn == 1 || sn == NA) && code23(w_end) < P.t_destroy;
                     const bool live = act && !destroyed;
                     if (act && sn != s) Sb[sx] = (unsigned char)sn;
                     if (act && destroyed) {
@@ -440,7 +457,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                 // chain's K <= 8G attempts; e comes from the ANCHOR call, which only a candidate
                 // (h <= (T(2 p_c) - 1) >> 7, about 2e-3 per attempt) ever evaluates.
                 {
-                    const int empty = N - Z0;
+                    const int empty = NA - Z0;
                     int K = P.k_attempts > 0 ? (P.k_attempts < empty ? P.k_attempts : empty) : empty;
                     if (!valid) K = 0;
                     if (8 * l < K) {
@@ -486,7 +503,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                                 A4[base + Zn] = make_float4(0.f, 0.f, 0.f, 0.f);
                             }
                         }
-                        const int K0 = P.k_attempts > 0 ? min(P.k_attempts, N - Z0) : N - Z0;
+                        const int K0 = P.k_attempts > 0 ? min(P.k_attempts, NA - Z0) : NA - Z0;
 #pragma unroll
                         for (int wd = 0; wd < WPC; ++wd) {
                             unsigned m = Ev[cw * WPC + wd];
@@ -507,7 +524,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                                 }
                                 const unsigned code = (h << 7) | (wa[2] >> 25);
                                 if (code >= P.t_c2[K0]) continue;
-                                const int snew = code < P.t_c1[K0] ? 1 : N;
+                                const int snew = code < P.t_c1[K0] ? 1 : NA;
                                 float z3[3], unused;
                                 bm_anchor(wa[0], z3[0], z3[1]);                                       // eq 52
                                 bm_anchor(wa[1], z3[2], unused);

@@ -143,3 +143,58 @@ def test_split_calls_and_fusion_depth_do_not_change_results(ssm):
     b.step_kappa(33, KAPPA); b.step_kappa(37, KAPPA)
     Ra, Aa, Sa, _ = a.get_state(); Rb, Ab, Sb, _ = b.get_state()
     assert np.array_equal(Ra, Rb) and np.array_equal(Aa, Ab) and np.array_equal(Sa, Sb)
+
+
+# ----------------------------------------------------------------------------- any N (the paper's 10, 20, 40, 80)
+@pytest.mark.parametrize("N,M,steps", [(2, 70, 200), (3, 70, 200), (9, 50, 300), (10, 300, 1000), (20, 100, 1000),
+                                       (40, 50, 500), (80, 19, 200), (127, 9, 100)])
+def test_bead_numbers_that_do_not_fill_the_lanes(ssm, N, M, steps):
+    """The paper runs N = 10, 20, 40, 80 (Figs 1-6); a chain occupies 8, 16, 32, 64 or 128 bead places and the
+    places beyond N are padding.  Device init (a0) and the step (a1-a8) against the oracle, as for the full sizes."""
+    from parity_util import from_external
+    e = oracle.Ensemble(N, M, seed=9)
+    g = ssm.Ensemble(N, M, seed=9, stress_every=1, stress_capacity=steps + 1)
+    Rg, Ag, Sg, Zg = from_external(*g.get_state()[:3])
+    assert np.array_equal(Sg, e.S) and np.array_equal(Zg, e.Z)
+    ok, w = close(Rg, e.R, 3e-6 if N <= 32 else 8e-6)
+    assert ok, w
+    upload(e, g)
+    want = e.run(steps, shear_rate=0.05, stress_every=1, guard=GUARD)
+    g.step(steps, 0.05)
+    n, worst = compare_state(e, g)
+    assert n >= _min_unflagged(M, N, steps), n
+    first = e.first_fragile[e.first_fragile >= 0]
+    clean = int(first.min()) if first.size else steps
+    ok, w = close(g.stress()[:clean], want[:clean], max(TOL, 3e-5 * np.sqrt(max(N, 8) / 8.0) / np.sqrt(M)))
+    assert ok, "ensemble stress off by %.3g over the first %d steps" % (w, clean)
+    # per-chain and per-group stresses of the final state on the chains that cannot have forked
+    cs = g.chain_stress()
+    sel = e.first_fragile < 0
+    want_c = np.array([np.concatenate(e.chain_stress(k)) for k in np.nonzero(sel)[0]])
+    good, w = close(cs.T[sel], want_c, 2e-5 * np.sqrt(max(N, 8) / 8.0))
+    assert good, w
+    assert abs(g.group_stress()[0, 12] - e.Z.mean()) < (1e-9 if sel.all() else 1.0)
+
+
+def test_mean_slipspring_number_under_shear_n80(ssm, golden_dir):
+    """P:L428 (Fig 5): N = 80, <Z>_eq = 20; under steady shear <Z> = 4.2 at gamma_dot = 0.1 and 1.6 at
+    gamma_dot = 1 8.7 at gamma_dot = 0.01 (the paper's CPU scheme, K = 1).  The oracle affords only gamma_dot = 1
+    (tests/test_oracle_dynamics.py); the slower rates need 1e6 - 1e7 steps and are run here."""
+    import os
+    vals = {}
+    for line in open(os.path.join(golden_dir, "paper_printed_values.txt")):
+        if line.strip() and not line.startswith("#"):
+            k, v, tol = line.split()[:3]
+            vals[k] = (float(v), float(tol))
+    N, M = 80, 512
+    for rate, key, settle in ((1.0, "Z_shear_N80_rate1", 340000), (0.1, "Z_shear_N80_rate0.1", 1500000),
+                              (0.01, "Z_shear_N80_rate0.01", 8000000)):
+        g = ssm.Ensemble(N, M, seed=71, k_attempts=1)
+        assert abs(g.group_stress()[0, 12] - 20.0) < 4 * np.sqrt(20.0 / M)
+        g.step(settle, rate)
+        zs = []
+        for _ in range(30):
+            g.step(2000, rate)
+            zs.append(g.group_stress()[0, 12])
+        want, tol = vals[key]
+        assert abs(np.mean(zs) - want) < tol, (rate, np.mean(zs), want)
