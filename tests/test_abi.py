@@ -61,7 +61,9 @@ def test_workspace_bytes_and_parameter_checks():
     assert n >= 125 * 7552 + 10 * 96
     assert m.workspace_bytes(_params(n_chains=2000)) > n
     assert m.workspace_bytes(_params(sample_every=10)) > n + 1000 * 16 * 16 * 4
-    for bad in (dict(n_beads=12), dict(n_beads=256), dict(n_chains=0), dict(dt=0.0), dict(dt=0.2), dict(n_s=0.0),
+    # any bead number 2..128 is accepted: N = 20 takes the 32 bead places per chain of N = 32
+    assert m.workspace_bytes(_params(n_beads=20)) == n
+    for bad in (dict(n_beads=1), dict(n_beads=129), dict(n_beads=256), dict(n_chains=0), dict(dt=0.0), dict(dt=0.2), dict(n_s=0.0),
                 dict(zeta_s=-1.0), dict(stress_capacity=0), dict(sample_every=10, corr_bins=15),
                 dict(sample_every=10, corr_levels=0), dict(chain_offset=2**32), dict(k_attempts=-1),
                 dict(sample_every=10, corr_components=2)):
