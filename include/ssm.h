@@ -59,7 +59,9 @@ typedef struct ssm_ctx ssm_ctx;   /* opaque, host side */
 
 /* Parameters of the model as the paper states them plus bookkeeping. */
 typedef struct {
-    int32_t  n_beads;         /* N: 8, 16, 32, 64 or 128 (8 beads per lane, N/8 lanes per chain)  */
+    int32_t  n_beads;         /* N, 2..128.  A chain takes 8, 16, 32, 64 or 128 bead places (the   */
+                              /* smallest that holds N; 8 places per lane): N = 10, 20, 40, 80 of   */
+                              /* the paper run at the speed of 16, 32, 64, 128                      */
     int64_t  n_chains;        /* M >= 1                                                           */
     double   n_s;             /* slip-spring strength N_s (eq 1)                           */
     double   n_0;             /* beads per slip-spring N_0 (eq 10); <= 0 or inf: no slip-  */
@@ -105,8 +107,8 @@ int ssm_step(ssm_ctx *ctx, int64_t n_steps, double shear_rate);
  * paper aims at: group g holds the local chains [g chains_per_group, (g+1) chains_per_group),
  * h_kappa (host) [n_groups][9], n_groups = ceil(n_chains / chains_per_group), row-major kappa_ab =
  * d v_a / d r_b in 1/tau0, constant during the call (the host array may be reused after the call returns).
- * chains_per_group >= n_chains means one group; otherwise it must be a multiple of 256 / n_beads (the
- * chains of one warp share a tensor), else SSM_EINVAL.  Asynchronous; stress and correlator samples are
+ * chains_per_group >= n_chains means one group; otherwise it must be a multiple of the chains per warp,
+ * 256 / (bead places per chain) (the chains of one warp share a tensor), else SSM_EINVAL.  Asynchronous; stress and correlator samples are
  * recorded as by ssm_step (over the whole ensemble; ssm_group_stress reads the groups).  Anchors are advected
  * as compensated sums in all three coordinates (10 extra bits each, kept in the fourth word of the anchor);
  * that word restarts from zero (a change below one ulp of the anchor) when the flow changes between this
