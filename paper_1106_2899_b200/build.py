@@ -13,9 +13,11 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libssm.so")
 SOURCES = ["ssm_step.cu", "ssm_aux.cu", "ssm_api.cu", "ssm_rheo.cu"]
+STEP_G = [1, 2, 4, 8, 16]       # ssm_step.cu is also compiled once per G (-DSSM_G): the kernels of 8G bead places
+OBJ = os.path.join(_HERE, "build")
 HEADERS = ["ssm_common.h", "ssm_rng.cuh", os.path.join("..", "..", "include", "ssm.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "--fmad=true", "-Xcompiler", "-fPIC", "-shared", "-cudart", "shared"]
+              "--fmad=true", "-Xcompiler", "-fPIC", "-cudart", "shared"]
 
 
 def nvcc():
@@ -37,13 +39,28 @@ def build(force=False, verbose=False):
     """Compile csrc/*.cu into libssm.so; returns its path."""
     if not force and not stale():
         return LIB
-    cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-          ["-o", LIB] + [os.path.join(CSRC, f) for f in SOURCES]
+    from concurrent.futures import ThreadPoolExecutor
+    os.makedirs(OBJ, exist_ok=True)
+    exe = nvcc()
+    units = [(f, [], os.path.join(OBJ, f[:-3] + ".o")) for f in SOURCES]
+    units += [("ssm_step.cu", ["-DSSM_G=%d" % g], os.path.join(OBJ, "ssm_step_g%d.o" % g)) for g in STEP_G]
+
+    def compile_one(u):
+        src, defs, obj = u
+        cmd = [exe] + NVCC_FLAGS + defs + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, os.path.join(CSRC, src)]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + r.stdout + r.stderr)
+        return r.stderr
+
+    with ThreadPoolExecutor(max_workers=min(len(units), os.cpu_count() or 1)) as ex:
+        logs = list(ex.map(compile_one, units))
+    cmd = [exe] + NVCC_FLAGS + ["-shared", "-o", LIB] + [u[2] for u in units]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
-        raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + r.stdout + r.stderr)
+        raise RuntimeError("nvcc link failed:\n" + " ".join(cmd) + "\n" + r.stdout + r.stderr)
     if verbose:
-        sys.stderr.write(r.stderr)
+        sys.stderr.write("".join(logs))
     return LIB
 
 

@@ -18,6 +18,11 @@
 
 namespace ssm {
 
+#define SSM_CAT2(a, b) a##b
+#define SSM_CAT(a, b) SSM_CAT2(a, b)
+
+#ifdef SSM_G   // ---- the kernels of one G (this file is compiled once per G, and once without for the dispatcher)
+
 template <int G> struct Log2;
 template <> struct Log2<1> { static constexpr int v = 0; };
 template <> struct Log2<2> { static constexpr int v = 1; };
@@ -56,7 +61,8 @@ __device__ __forceinline__ float advect_packed(float hi, float inc, int &q)
 }
 
 // FLOW: 0 = no flow, 1 = simple shear kappa_xy (eq 60), 2 = one full tensor per group of chains (eqs 18, 21)
-template <int G, int FLOW>
+// RAGGED: the chain has fewer beads than the 8G places it occupies (ssm_common.h)
+template <int G, int FLOW, bool RAGGED>
 __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid_constant__ StepParams P)
 {
     constexpr bool SHEAR = FLOW == 1;
@@ -66,8 +72,8 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int l = lane & (G - 1), cw = lane >> LG;
     // NA = the chain's number of beads; N = 8G places (NA < N: the places NA..N-1 are padding at the origin)
-    const int NA = P.n_act;
-    const bool ragged = NA != N;
+    const int NA = RAGGED ? P.n_act : N;
+    constexpr bool ragged = RAGGED;
     const int real_here = min(kBPL, max(0, NA - kBPL * l));          // real beads among this lane's 8 places
     const float bonds_here = (float)min(kBPL, max(0, NA - 1 - kBPL * l));   // bonds i -> i+1 that start in this lane
     unsigned char *wb = smem + warp * kSmWarp;
@@ -588,60 +594,71 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
 }
 
 // ---------------------------------------------------------------------------------------
-// host-side launcher
+// host-side launcher.  This file is compiled once per G with -DSSM_G=<G> (the kernels of that G:
+// 3 flows x full / ragged) and once without (the dispatcher), so that the build runs in parallel.
 // ---------------------------------------------------------------------------------------
-template <int G, int FLOW>
-static cudaError_t launch_gs(const StepParams &p, int grid, cudaStream_t st)
+template <int G, int FLOW, bool RAGGED>
+static cudaError_t launch_gfr(const StepParams &p, int grid, cudaStream_t st)
 {
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(ssm_step_kernel<G, FLOW>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmStep);
+        cudaError_t e = cudaFuncSetAttribute(ssm_step_kernel<G, FLOW, RAGGED>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmStep);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    ssm_step_kernel<G, FLOW><<<grid, kBlockThreads, kSmStep, st>>>(p);
+    ssm_step_kernel<G, FLOW, RAGGED><<<grid, kBlockThreads, kSmStep, st>>>(p);
     return cudaGetLastError();
+}
+
+template <int G, int FLOW>
+static cudaError_t launch_gf(const StepParams &p, int grid, cudaStream_t st)
+{
+    return p.n_act != kBPL * G ? launch_gfr<G, FLOW, true>(p, grid, st) : launch_gfr<G, FLOW, false>(p, grid, st);
 }
 
 // the affine term of eqs 44, 45 is compiled in only when a velocity gradient is applied: the full tensor
 // when a table of tensors is given, else kappa_xy when the shear rate is not zero
-template <int G>
-static cudaError_t launch_g(const StepParams &p, int grid, cudaStream_t st)
+cudaError_t SSM_CAT(launch_step_g, SSM_G)(const StepParams &p, int grid, cudaStream_t st)
 {
-    if (p.kappa) return launch_gs<G, 2>(p, grid, st);
-    return p.gdt != 0.0f ? launch_gs<G, 1>(p, grid, st) : launch_gs<G, 0>(p, grid, st);
+    if (p.kappa) return launch_gf<SSM_G, 2>(p, grid, st);
+    return p.gdt != 0.0f ? launch_gf<SSM_G, 1>(p, grid, st) : launch_gf<SSM_G, 0>(p, grid, st);
 }
 
-template <int G>
-static cudaError_t occupancy_g(int *blocks_per_sm)
+cudaError_t SSM_CAT(step_occupancy_g, SSM_G)(int *blocks_per_sm)
 {
-    cudaError_t e = cudaFuncSetAttribute(ssm_step_kernel<G, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmStep);
+    cudaError_t e = cudaFuncSetAttribute(ssm_step_kernel<SSM_G, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmStep);
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, ssm_step_kernel<G, 2>, kBlockThreads, kSmStep);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, ssm_step_kernel<SSM_G, 2, true>, kBlockThreads, kSmStep);
 }
 
-cudaError_t step_occupancy(int n_beads, int *blocks_per_sm)
+#else   // the dispatcher over the bead places per chain, 8G
+
+#define SSM_DECL(g) cudaError_t launch_step_g##g(const StepParams &, int, cudaStream_t); cudaError_t step_occupancy_g##g(int *);
+SSM_DECL(1) SSM_DECL(2) SSM_DECL(4) SSM_DECL(8) SSM_DECL(16)
+
+cudaError_t step_occupancy(int n_places, int *blocks_per_sm)
 {
-    switch (n_beads) {
-        case 8: return occupancy_g<1>(blocks_per_sm);
-        case 16: return occupancy_g<2>(blocks_per_sm);
-        case 32: return occupancy_g<4>(blocks_per_sm);
-        case 64: return occupancy_g<8>(blocks_per_sm);
-        case 128: return occupancy_g<16>(blocks_per_sm);
+    switch (n_places) {
+        case 8: return step_occupancy_g1(blocks_per_sm);
+        case 16: return step_occupancy_g2(blocks_per_sm);
+        case 32: return step_occupancy_g4(blocks_per_sm);
+        case 64: return step_occupancy_g8(blocks_per_sm);
+        case 128: return step_occupancy_g16(blocks_per_sm);
     }
     return cudaErrorInvalidValue;
 }
 
-cudaError_t launch_step(int n_beads, const StepParams &p, int grid, cudaStream_t st)
+cudaError_t launch_step(int n_places, const StepParams &p, int grid, cudaStream_t st)
 {
-    switch (n_beads) {
-        case 8: return launch_g<1>(p, grid, st);
-        case 16: return launch_g<2>(p, grid, st);
-        case 32: return launch_g<4>(p, grid, st);
-        case 64: return launch_g<8>(p, grid, st);
-        case 128: return launch_g<16>(p, grid, st);
+    switch (n_places) {
+        case 8: return launch_step_g1(p, grid, st);
+        case 16: return launch_step_g2(p, grid, st);
+        case 32: return launch_step_g4(p, grid, st);
+        case 64: return launch_step_g8(p, grid, st);
+        case 128: return launch_step_g16(p, grid, st);
     }
     return cudaErrorInvalidValue;
 }
+#endif
 
 }  // namespace ssm
