@@ -198,3 +198,40 @@ def test_mean_slipspring_number_under_shear_n80(ssm, golden_dir):
             zs.append(g.group_stress()[0, 12])
         want, tol = vals[key]
         assert abs(np.mean(zs) - want) < tol, (rate, np.mean(zs), want)
+
+
+def test_steady_shear_viscosity_at_low_rate_is_the_integral_of_gt(ssm):
+    """eqs (59), (61), (62): eta(gamma_dot) = <sigma_xy>/gamma_dot at the plateau tends to eta_0 = int G(t) dt as
+    gamma_dot -> 0 (linear response; at low rates this is also the Cox-Merz value, eq 63).  Both sides are
+    the GPU's: G(t) from the equilibrium correlator -> ssm_eta0, and the plateau of a sheared copy, at the paper's
+    N = 10.  The eq (43) estimator correlates sigma with sigma + sigma_v and the plateau stress is sigma alone.
+    Measured: eta_0 = 0.609 +- 0.0005 (0.618 with the correlator fed every 10 steps: the trapezoidal rule of P:L392
+    over-counts the Rouse modes faster than the sampling interval), plateau 0.597 +- 0.002 at gamma_dot = 0.01 - 0.05:
+    2 % apart, the order of the time-discretisation error of the three-substep scheme at dt / zeta_s = 0.1 (for the
+    Rouse part alone the Euler map gives a ratio 1 - k_p dt / 2 per mode); hence the 3 % allowance."""
+    N, M, dt, rate = 10, 65536, 0.01, 0.02
+    g = ssm.Ensemble(N, M, seed=55, sample_every=2, corr_levels=10, corr_bins=16, corr_groups=32)
+    g.step(2000)
+    g.reset_accumulators()
+    g.step(60000)
+    t, G, se = g.gt()
+    keep = t <= 40.0                                     # G has decayed to noise long before (tau_d of a few tau0)
+    eta0 = ssm.eta0(t[keep], G[keep])
+    w = np.gradient(t[keep])                             # trapezoid-like weights, for the error bar only
+    eta0_se = float(np.sqrt(np.sum((w * se[keep]) ** 2)))
+    h = ssm.Ensemble(N, M, seed=56, stress_every=10, stress_capacity=4000)
+    h.step(5000, rate)                                   # t = 50: plateau
+    h.reset_accumulators()
+    h.step(30000, rate)
+    sxy = h.stress()[:, 3]
+    eta = sxy.mean() / (N * rate)                        # sigma = (rho_0 / N) <sigma_chain>  (eq 16, c_0 = rho_0 / N)
+    blocks = sxy[: len(sxy) // 30 * 30].reshape(30, -1).mean(1)
+    eta_se = blocks.std(ddof=1) / np.sqrt(30) / (N * rate)
+    assert 0.3 < eta0 < 3.0
+    assert abs(eta - eta0) < 4.0 * np.hypot(eta_se, eta0_se) + 0.03 * eta0, (eta, eta_se, eta0, eta0_se)
+    # and shear thinning at a high rate (Fig 5): the plateau viscosity falls well below eta_0
+    h2 = ssm.Ensemble(N, M, seed=57, stress_every=10, stress_capacity=1000)
+    h2.step(3000, 2.0)
+    h2.reset_accumulators()
+    h2.step(5000, 2.0)
+    assert h2.stress()[:, 3].mean() / (N * 2.0) < 0.8 * eta0
