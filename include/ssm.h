@@ -84,6 +84,10 @@ typedef struct {
                               /* zx each keep their own history and feed the same sums -- the equilibrium   */
                               /* ensemble is isotropic, so this is the same G(t) from three times the data  */
                               /* (meaningful without flow only)                                             */
+    int64_t  stage_chains;    /* chains per chunk of the staging area that ssm_get_state / ssm_set_state use for    */
+                              /* HOST pointers (29 x bead places bytes each): 0 = 65536.  n_chains makes a state    */
+                              /* transfer three copies and one kernel, which is what lets it overlap the stepping   */
+                              /* of another ctx on another stream                                                   */
 } ssm_params;
 
 /* Bytes of device workspace ssm_init() needs for these parameters (0 on bad parameters). */

@@ -27,7 +27,7 @@ class Params(C.Structure):
                 ("zeta_s", C.c_double), ("dt", C.c_double), ("seed", C.c_uint64), ("chain_offset", C.c_uint64),
                 ("stress_every", C.c_int32), ("stress_capacity", C.c_int64), ("sample_every", C.c_int32),
                 ("corr_levels", C.c_int32), ("corr_bins", C.c_int32), ("corr_groups", C.c_int32),
-                ("k_attempts", C.c_int32), ("corr_components", C.c_int32)]
+                ("k_attempts", C.c_int32), ("corr_components", C.c_int32), ("stage_chains", C.c_int64)]
 
 
 class SsmError(RuntimeError):
@@ -124,14 +124,15 @@ class Ensemble:
 
     def __init__(self, n_beads, n_chains, n_s=0.5, n_0=4.0, zeta_s=0.1, dt=0.01, seed=1, chain_offset=0,
                  stress_every=0, stress_capacity=0, sample_every=0, corr_levels=16, corr_bins=16,
-                 corr_groups=32, k_attempts=0, corr_components=1, device="cuda:0", stream=None):
+                 corr_groups=32, k_attempts=0, corr_components=1, stage_chains=0, device="cuda:0", stream=None):
         import torch
         if not torch.cuda.is_available():
             raise SsmError(SSM_ECUDA, "no CUDA device: libssm has no CPU fallback")
         self._torch = torch
         self.device = torch.device(device)
         self.p = Params(n_beads, n_chains, n_s, n_0, zeta_s, dt, seed, chain_offset, stress_every,
-                        stress_capacity, sample_every, corr_levels, corr_bins, corr_groups, k_attempts, corr_components)
+                        stress_capacity, sample_every, corr_levels, corr_bins, corr_groups, k_attempts, corr_components,
+                        stage_chains)
         self.N, self.M = n_beads, n_chains
         L = lib()
         nbytes = L.ssm_workspace_bytes(C.byref(self.p))

@@ -81,6 +81,7 @@ static bool check_params(const ssm_params *p, std::string &why)
     if (!(p->n_s > 0.0)) { why = "n_s must be > 0"; return false; }
     if (!(p->zeta_s > 0.0)) { why = "zeta_s must be > 0"; return false; }
     if (p->k_attempts < 0) { why = "k_attempts must be >= 0"; return false; }
+    if (p->stage_chains < 0) { why = "stage_chains must be >= 0"; return false; }
     if (p->stress_every < 0 || p->sample_every < 0 || p->stress_capacity < 0) { why = "negative sampling parameter"; return false; }
     if (p->stress_every > 0 && p->stress_capacity < 1) { why = "stress_capacity must be >= 1 when stress_every > 0"; return false; }
     if (p->sample_every > 0) {
@@ -111,7 +112,8 @@ static Layout make_layout(const ssm_params *p)
     // two sum arrays: f_new g_old (eq 43) and g_new g_old (eq 66)
     L.csum = o; if (corr) o = align_up(o + 2 * (size_t)p->corr_groups * p->corr_levels * p->corr_bins * 8, 256);
     // staging for host-pointer get/set state and chain stress: chunks of <= 65536 chains
-    L.stage_chains = p->n_chains < 65536 ? p->n_chains : 65536;
+    const long long want_stage = p->stage_chains > 0 ? p->stage_chains : 65536;
+    L.stage_chains = p->n_chains < want_stage ? p->n_chains : want_stage;
     // (at least 1 MB, so that the issue-rate probe's scratch of 2 kB per SM fits any ensemble)
     size_t stage_bytes = (size_t)L.stage_chains * (size_t)(29 * npad > 48 ? 29 * npad : 48);
     if (stage_bytes < ((size_t)1 << 20)) stage_bytes = (size_t)1 << 20;

@@ -32,7 +32,7 @@ def test_params_struct_matches_header_layout():
     assert [f[0] for f in p._fields_] == ["n_beads", "n_chains", "n_s", "n_0", "zeta_s", "dt", "seed",
                                           "chain_offset", "stress_every", "stress_capacity", "sample_every",
                                           "corr_levels", "corr_bins", "corr_groups", "k_attempts",
-                                          "corr_components"]
+                                          "corr_components", "stage_chains"]
     # ask the C compiler what the header says
     import subprocess
     import tempfile
@@ -50,7 +50,7 @@ def test_params_struct_matches_header_layout():
 def _params(**kw):
     d = dict(n_beads=32, n_chains=1000, n_s=0.5, n_0=4.0, zeta_s=0.1, dt=0.01, seed=1, chain_offset=0,
              stress_every=1, stress_capacity=10, sample_every=0, corr_levels=16, corr_bins=16, corr_groups=32,
-             k_attempts=0, corr_components=1)
+             k_attempts=0, corr_components=1, stage_chains=0)
     d.update(kw)
     return m.Params(**d)
 
@@ -66,7 +66,7 @@ def test_workspace_bytes_and_parameter_checks():
     for bad in (dict(n_beads=1), dict(n_beads=129), dict(n_beads=256), dict(n_chains=0), dict(dt=0.0), dict(dt=0.2), dict(n_s=0.0),
                 dict(zeta_s=-1.0), dict(stress_capacity=0), dict(sample_every=10, corr_bins=15),
                 dict(sample_every=10, corr_levels=0), dict(chain_offset=2**32), dict(k_attempts=-1),
-                dict(sample_every=10, corr_components=2)):
+                dict(sample_every=10, corr_components=2), dict(stage_chains=-1)):
         assert m.workspace_bytes(_params(**bad)) == 0, bad
         assert len(m.lib().ssm_last_error(None)) > 0
 

@@ -46,6 +46,12 @@ def test_set_get_state_roundtrip_is_bit_exact(ssm):
     R2, A2, S2, step = g.get_state()
     assert step == 123
     assert np.array_equal(R, R2) and np.array_equal(A, A2) and np.array_equal(S, S2)
+    # the staging chunk of host-pointer transfers does not matter: many small chunks, or one for everything
+    for chunk in (5, 37, 1000):
+        h = ssm.Ensemble(32, 37, seed=5, stage_chains=chunk)
+        h.set_state(R, A, S, 7)
+        R3, A3, S3, step = h.get_state()
+        assert step == 7 and np.array_equal(R, R3) and np.array_equal(A, A3) and np.array_equal(S, S3)
 
 
 def test_device_init_matches_oracle_init(ssm):
