@@ -126,6 +126,13 @@ int ssm_step_kappa(ssm_ctx *ctx, int64_t n_steps, int64_t chains_per_group, cons
  * (deterministic).  Synchronises the stream. */
 int ssm_group_stress(ssm_ctx *ctx, int64_t chains_per_group, double *h_out);
 
+/* The same two calls for a flow solver that lives on the GPU: d_kappa (device) [n_groups][9] double is read, and
+ * d_out (device) [n_groups][13] double is written, by kernels on the ctx's stream; neither call synchronises, so
+ * a coupling loop (tensors in, n micro steps, group stresses out) can be queued without the host in it.  Values
+ * are those of the host variants bit for bit.  Non-finite tensors are not checked here. */
+int ssm_step_kappa_device(ssm_ctx *ctx, int64_t n_steps, int64_t chains_per_group, const double *d_kappa);
+int ssm_group_stress_device(ssm_ctx *ctx, int64_t chains_per_group, double *d_out);
+
 /* Number of stress samples recorded since init / the last reset. */
 int64_t ssm_stress_count(const ssm_ctx *ctx);
 

@@ -18,7 +18,8 @@ EXPORTS = ["ssm_workspace_bytes", "ssm_init", "ssm_step", "ssm_stress_count", "s
            "ssm_stress_sums_device", "ssm_chain_stress", "ssm_gt", "ssm_gt_sums", "ssm_get_state", "ssm_set_state",
            "ssm_reset_accumulators", "ssm_launch_count", "ssm_set_fusion", "ssm_set_grid", "ssm_destroy", "ssm_last_error",
            "ssm_moduli", "ssm_eta0", "ssm_tau_d", "ssm_issue_rates",
-           "ssm_gt_virtual", "ssm_gt_sums_virtual", "ssm_step_kappa", "ssm_group_stress"]
+           "ssm_gt_virtual", "ssm_gt_sums_virtual", "ssm_step_kappa", "ssm_group_stress",
+           "ssm_step_kappa_device", "ssm_group_stress_device"]
 
 
 class Params(C.Structure):
@@ -70,6 +71,8 @@ def lib():
     L.ssm_gt_sums_virtual.argtypes = [vp, dp]; L.ssm_gt_sums_virtual.restype = C.c_int
     L.ssm_step_kappa.argtypes = [vp, C.c_int64, C.c_int64, dp]; L.ssm_step_kappa.restype = C.c_int
     L.ssm_group_stress.argtypes = [vp, C.c_int64, dp]; L.ssm_group_stress.restype = C.c_int
+    L.ssm_step_kappa_device.argtypes = [vp, C.c_int64, C.c_int64, vp]; L.ssm_step_kappa_device.restype = C.c_int
+    L.ssm_group_stress_device.argtypes = [vp, C.c_int64, vp]; L.ssm_group_stress_device.restype = C.c_int
     L.ssm_moduli.argtypes = [C.c_int32, dp, dp, C.c_int32, dp, dp, dp]; L.ssm_moduli.restype = C.c_int
     L.ssm_eta0.argtypes = [C.c_int32, dp, dp, dp]; L.ssm_eta0.restype = C.c_int
     L.ssm_tau_d.argtypes = [C.c_int32, dp, dp, C.c_double, C.c_double, dp]; L.ssm_tau_d.restype = C.c_int
@@ -164,6 +167,25 @@ class Ensemble:
             raise SsmError(SSM_EINVAL, "kappa must hold one tensor per group")
         with self._torch.cuda.device(self.device):
             self._ck(lib().ssm_step_kappa(self.h, n_steps, cpg, kap.ctypes.data_as(C.POINTER(C.c_double))))
+
+    def step_kappa_device(self, n_steps, kappa, chains_per_group=None):
+        """ssm_step_kappa_device: kappa = CUDA float64 tensor [groups][3][3]; asynchronous."""
+        cpg = self.M if chains_per_group is None else int(chains_per_group)
+        assert kappa.is_cuda and kappa.dtype == self._torch.float64 and kappa.is_contiguous()
+        assert kappa.numel() == 9 * -(-self.M // min(cpg, self.M))
+        with self._torch.cuda.device(self.device):
+            self._ck(lib().ssm_step_kappa_device(self.h, n_steps, cpg, C.c_void_p(kappa.data_ptr())))
+
+    def group_stress_device(self, chains_per_group=None, out=None):
+        """ssm_group_stress_device: fills / returns a CUDA float64 tensor [groups][13]; asynchronous."""
+        cpg = self.M if chains_per_group is None else min(int(chains_per_group), self.M)
+        ng = -(-self.M // cpg)
+        if out is None:
+            out = self._torch.empty((ng, 13), dtype=self._torch.float64, device=self.device)
+        assert out.is_cuda and out.dtype == self._torch.float64 and out.is_contiguous() and out.numel() == ng * 13
+        with self._torch.cuda.device(self.device):
+            self._ck(lib().ssm_group_stress_device(self.h, cpg, C.c_void_p(out.data_ptr())))
+        return out
 
     def group_stress(self, chains_per_group=None):
         """ssm_group_stress: [groups][13] = means of sigma[6], sigma_v[6] and Z over each group, current state."""

@@ -24,6 +24,9 @@ cudaError_t launch_xfer(bool do_export, unsigned char *state, float *R, float *A
 cudaError_t launch_clear_low(unsigned char *state, long long n_tiles, cudaStream_t st);
 cudaError_t launch_group_stress(const unsigned char *state, long long *out, int N, long long M, long long cpg, float cs,
                                 cudaStream_t st);
+cudaError_t launch_kappa(const double *d_kappa, float *out, long long n, double dt, cudaStream_t st);
+cudaError_t launch_group_mean(const long long *sums, double *out, long long n_groups, long long M, long long cpg,
+                              cudaStream_t st);
 cudaError_t launch_chain_stress(const unsigned char *state, float *out, int N, long long M, float cs, cudaStream_t st);
 cudaError_t launch_corr(const CorrParams &c, cudaStream_t st);
 }  // namespace ssm
@@ -354,6 +357,35 @@ extern "C" int ssm_step_kappa(ssm_ctx *c, int64_t n_steps, int64_t chains_per_gr
     float *d_kappa = reinterpret_cast<float *>(c->ws + c->lay.kappa);
     CK(c, cudaMemcpyAsync(d_kappa, c->kappa_host.data(), (size_t)ng * 9 * 4, cudaMemcpyHostToDevice, c->st));
     return step_impl(c, n_steps, 0.0, d_kappa, tpg);
+}
+
+extern "C" int ssm_step_kappa_device(ssm_ctx *c, int64_t n_steps, int64_t chains_per_group, const double *d_kappa)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (n_steps < 0) return fail(c, SSM_EINVAL, "n_steps < 0");
+    if (!d_kappa) return fail(c, SSM_EINVAL, "d_kappa is NULL");
+    long long ng = 0, tpg = 0;
+    if (!group_geometry(c, chains_per_group, &ng, &tpg))
+        return fail(c, SSM_EINVAL, "chains_per_group must be >= n_chains (one group) or a multiple of the chains per warp, 256 / (n_beads rounded up to 8, 16, 32, 64 or 128)");
+    float *d_table = reinterpret_cast<float *>(c->ws + c->lay.kappa);
+    CK(c, launch_kappa(d_kappa, d_table, ng * 9, c->p.dt, c->st));
+    c->launches += 1;
+    return step_impl(c, n_steps, 0.0, d_table, tpg);
+}
+
+extern "C" int ssm_group_stress_device(ssm_ctx *c, int64_t chains_per_group, double *d_out)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (!d_out) return fail(c, SSM_EINVAL, "d_out is NULL");
+    if (chains_per_group < 1) return fail(c, SSM_EINVAL, "chains_per_group must be >= 1");
+    const long long M = c->p.n_chains, cpg = chains_per_group < M ? chains_per_group : M, ng = (M + cpg - 1) / cpg;
+    if ((size_t)ng * 13 * 8 > c->lay.total - c->lay.stage) return fail(c, SSM_ENOMEM, "staging area too small for this many groups");
+    long long *d = reinterpret_cast<long long *>(c->ws + c->lay.stage);
+    CK(c, cudaMemsetAsync(d, 0, (size_t)ng * 13 * 8, c->st));
+    CK(c, launch_group_stress(c->ws + c->lay.state, d, c->p.n_beads, M, cpg, c->sp.cs, c->st));
+    CK(c, launch_group_mean(d, d_out, ng, M, cpg, c->st));
+    c->launches += 2;
+    return SSM_OK;
 }
 
 extern "C" int ssm_group_stress(ssm_ctx *c, int64_t chains_per_group, double *h_out)

@@ -221,6 +221,36 @@ __global__ void __launch_bounds__(128) ssm_group_stress_kernel(const unsigned ch
     }
 }
 
+// dt kappa as the step kernel reads it (float) from a device table of tensors in double
+__global__ void __launch_bounds__(256) ssm_kappa_kernel(const double *kappa, float *out, long long n, double dt)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = (float)(kappa[i] * dt);
+}
+
+cudaError_t launch_kappa(const double *d_kappa, float *out, long long n, double dt, cudaStream_t st)
+{
+    ssm_kappa_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_kappa, out, n, dt);
+    return cudaGetLastError();
+}
+
+// group means from the fixed-point sums of ssm_group_stress_kernel: out[g][t] = sum / (2^kStressShift * chains in g)
+__global__ void __launch_bounds__(256) ssm_group_mean_kernel(const long long *sums, double *out, long long n_groups,
+                                                             long long M, long long cpg)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_groups * 13) return;
+    const long long g = i / 13, n = (g + 1) * cpg <= M ? cpg : M - g * cpg;
+    out[i] = (double)sums[i] / ((double)(1 << kStressShift) * (double)n);
+}
+
+cudaError_t launch_group_mean(const long long *sums, double *out, long long n_groups, long long M, long long cpg,
+                              cudaStream_t st)
+{
+    ssm_group_mean_kernel<<<(unsigned)((n_groups * 13 + 255) / 256), 256, 0, st>>>(sums, out, n_groups, M, cpg);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_group_stress(const unsigned char *state, long long *out, int N, long long M, long long cpg, float cs,
                                 cudaStream_t st)
 {

@@ -127,6 +127,24 @@ def test_groups_with_their_own_tensors_and_group_stress(ssm):
     assert g5.shape == (3, 13) and abs(g5[2, 12] - Z[80:].mean()) < 1e-9
 
 
+def test_device_variants_of_the_group_calls_equal_the_host_ones(ssm):
+    """A coupling loop queued without the host in it: tensors from a CUDA tensor, group stresses into one."""
+    import torch
+    N, M, cpg = 16, 128, 32
+    kap = np.stack([KAPPA, 0.5 * KAPPA, np.zeros((3, 3)), -KAPPA.T])
+    a = ssm.Ensemble(N, M, seed=6); b = ssm.Ensemble(N, M, seed=6)
+    dk = torch.tensor(kap, dtype=torch.float64, device="cuda")
+    out = torch.empty((4, 13), dtype=torch.float64, device="cuda")
+    for _ in range(3):                                      # three macro steps of 20 micro steps
+        a.step_kappa(20, kap, chains_per_group=cpg)
+        b.step_kappa_device(20, dk, chains_per_group=cpg)
+        b.group_stress_device(cpg, out)
+        torch.cuda.synchronize()
+        assert np.array_equal(a.group_stress(cpg), out.cpu().numpy())
+    Ra, Aa, Sa, _ = a.get_state(); Rb, Ab, Sb, _ = b.get_state()
+    assert np.array_equal(Ra, Rb) and np.array_equal(Aa, Ab) and np.array_equal(Sa, Sb)
+
+
 def test_bad_group_size_is_rejected(ssm):
     g = ssm.Ensemble(32, 96, seed=1)
     with pytest.raises(ssm.SsmError) as ei:
