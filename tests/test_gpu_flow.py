@@ -254,3 +254,40 @@ def test_steady_shear_viscosity_at_low_rate_is_the_integral_of_gt(ssm):
     h2.reset_accumulators()
     h2.step(5000, 2.0)
     assert h2.stress()[:, 3].mean() / (N * 2.0) < 0.8 * eta0
+
+
+def test_viscosity_and_relaxation_time_scaling_printed_in_the_paper(ssm, golden_dir):
+    """Figs 1-3 as far as the paper PRINTS numbers: plateau modulus about 0.1 rho_0 kT,
+    eta_0 ~ (N-1)^3.40 and tau_d ~ (N-1)^3.48 for large N.  Whole pipeline on the GPU at the paper's N = 40 and 80:
+    step kernel (short-chain variant) -> isotropic multi-tau correlator -> ssm_gt -> ssm_eta0 / ssm_tau_d.
+    (Measured with twice the chains and 1.7 times the steps: eta_0 = 25.47 +- 0.03 and 290.4 +- 0.6, exponent 3.45;
+    tau_d = 338 and 4430, exponent 3.65; 20 -> 40 gives 2.93 and 3.29: still in the crossover.)"""
+    import os
+    vals = {}
+    for line in open(os.path.join(golden_dir, "paper_printed_values.txt")):
+        if line.strip() and not line.startswith("#"):
+            k, v, tol = line.split()[:3]
+            vals[k] = (float(v), float(tol))
+    out = {}
+    for N, M, steps, levels in ((40, 4096, 1500000, 14), (80, 4096, 6000000, 16)):
+        g = ssm.Ensemble(N, M, seed=100 + N, sample_every=10, corr_levels=levels, corr_bins=16, corr_groups=32,
+                         corr_components=3)
+        g.step(steps // 10)
+        g.reset_accumulators()
+        g.step(steps)
+        t, G, se = g.gt()
+        bad = np.nonzero(G < 2 * se)[0]
+        cut = int(bad[0]) if len(bad) else len(t)                  # beyond the first G < 2 SE the table is noise
+        i0 = int(np.searchsorted(t, 0.2 * t[cut - 1]))
+        out[N] = (ssm.eta0(t[:cut], G[:cut]), ssm.tau_d(t[:cut], G[:cut], t[i0], t[cut - 1]), t, G)
+    lr = np.log(79.0 / 39.0)
+    x_eta = np.log(out[80][0] / out[40][0]) / lr
+    x_tau = np.log(out[80][1] / out[40][1]) / lr
+    want, tol = vals["eta0_exponent_large_N"]
+    assert abs(x_eta - want) < tol, (x_eta, out[40][0], out[80][0])
+    want, tol = vals["tau_d_exponent_large_N"]
+    assert abs(x_tau - want) < tol, (x_tau, out[40][1], out[80][1])
+    want, tol = vals["plateau_modulus"]
+    t, G = out[80][2], out[80][3]
+    plateau = G[(t >= 10.0) & (t <= 30.0)]
+    assert len(plateau) >= 3 and np.all(np.abs(plateau - want) < tol), plateau
