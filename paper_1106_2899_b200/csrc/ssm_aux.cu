@@ -269,6 +269,22 @@ cudaError_t launch_group_stress(const unsigned char *state, long long *out, int 
 // values at the start of the launch.  Sums are int64 fixed point (2^-16) so that the
 // result does not depend on the order of the atomics.
 // ---------------------------------------------------------------------------------------
+// One round of a warp-wide transposing sum: every lane holds 2H partial sums v[0..2H); lanes whose bit o is set
+// keep the upper H and send the lower H to their partner (lane ^ o), the others the other way round; afterwards
+// v[0..H) are sums over twice as many lanes.  Five rounds (H = 16, 8, 4, 2, 1 with o = 16, 8, 4, 2, 1) turn 32
+// values per lane into ONE total per lane, value number = lane: 31 shuffles instead of 32 warp reductions.
+template <int H>
+__device__ __forceinline__ void transpose_sum_round(int (&v)[32], int o, int lane)
+{
+    const bool up = (lane & o) != 0;
+#pragma unroll
+    for (int i = 0; i < H; ++i) {
+        const int send = up ? v[i] : v[i + H];
+        const int keep = up ? v[i + H] : v[i];
+        v[i] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+    }
+}
+
 __global__ void __launch_bounds__(256) ssm_corr_kernel(const __grid_constant__ CorrParams C)
 {
     // one thread per HISTORY k = q M + chain (component q = xy, or xy / yz / zx), Mv = n_comp M of them
@@ -292,28 +308,68 @@ __global__ void __launch_bounds__(256) ssm_corr_kernel(const __grid_constant__ C
             const int p0 = pos[lev];
             if (valid) ring[(long long)p0 * C.Mv] = g;
             if (fil[lev] < Pb) ++fil[lev];
-            const int kmin = lev == 0 ? 0 : Pb / 2;
-            for (int q = kmin; q < fil[lev]; ++q) {
-                int idx = p0 - q; if (idx < 0) idx += Pb;
-                const float old = valid ? ring[(long long)idx * C.Mv] : 0.0f;
-                // fixed point 2^-16: f_new g_old for G(t) (eq 43), g_new g_old for the virtual-stress share (eq 66)
-                const long long v = __float2ll_rn(f * old * 65536.0f), v2 = __float2ll_rn(g * old * 65536.0f);
-                if (one_group) {
-                    // exact warp sums of the 64-bit values as two 32-bit integer reductions each:
-                    // v = hi 2^20 + lo, 0 <= lo < 2^20 (|v| < 2^46 keeps the sum of 32 hi's in 32 bits)
-                    const int hi = __reduce_add_sync(0xffffffffu, (int)(v >> 20));
-                    const int lo = __reduce_add_sync(0xffffffffu, (int)(v & 0xFFFFF));
-                    const int hi2 = __reduce_add_sync(0xffffffffu, (int)(v2 >> 20));
-                    const int lo2 = __reduce_add_sync(0xffffffffu, (int)(v2 & 0xFFFFF));
-                    if (lane == 0) {
-                        atomicAdd(reinterpret_cast<unsigned long long *>(gsum + lev * Pb + q),
-                                  (unsigned long long)(((long long)hi << 20) + (long long)lo));
-                        atomicAdd(reinterpret_cast<unsigned long long *>(gsum2 + lev * Pb + q),
-                                  (unsigned long long)(((long long)hi2 << 20) + (long long)lo2));
+            const int kmin = lev == 0 ? 0 : Pb / 2, kfil = fil[lev];
+            // the bins of this insertion, 16 at a time: products in fixed point 2^-16, f_new g_old for G(t)
+            // (eq 43) at even places and g_new g_old for the virtual-stress share (eq 66) at odd places
+            for (int q0 = kmin; q0 < kfil; q0 += 16) {
+                const int nb = kfil - q0 < 16 ? kfil - q0 : 16;
+                float pf[16], pg[16], big = 0.0f;
+#pragma unroll
+                for (int b = 0; b < 16; ++b) {
+                    int idx = p0 - (q0 + b); if (idx < 0) idx += Pb;
+                    const float old = (valid && b < nb) ? ring[(long long)idx * C.Mv] : 0.0f;
+                    pf[b] = f * old * 65536.0f; pg[b] = g * old * 65536.0f;
+                    big = fmaxf(big, fmaxf(fabsf(pf[b]), fabsf(pg[b])));
+                }
+                if (one_group && !__any_sync(0xffffffffu, !(big < 3.3e7f))) {
+                    // every |product| < 2^25, so the sum over the warp's 32 chains fits 32 bits: one transposing
+                    // sum gives lane i the warp's total of value i, and the 32 lanes add their totals at once
+                    int v[32];
+#pragma unroll
+                    for (int b = 0; b < 16; ++b) { v[2 * b] = __float2int_rn(pf[b]); v[2 * b + 1] = __float2int_rn(pg[b]); }
+                    int mine_bin, total;
+                    if (nb > 8) {
+                        transpose_sum_round<16>(v, 16, lane); transpose_sum_round<8>(v, 8, lane);
+                        transpose_sum_round<4>(v, 4, lane); transpose_sum_round<2>(v, 2, lane);
+                        transpose_sum_round<1>(v, 1, lane);
+                        total = v[0]; mine_bin = lane >> 1;
+                    } else {
+                        // 16 values only (the upper levels): four rounds leave value number lane >> 1 in the two
+                        // lanes of a pair, which share the bin's two sums between them
+                        transpose_sum_round<8>(v, 16, lane); transpose_sum_round<4>(v, 8, lane);
+                        transpose_sum_round<2>(v, 4, lane); transpose_sum_round<1>(v, 2, lane);
+                        total = v[0] + __shfl_xor_sync(0xffffffffu, v[0], 1);
+                        mine_bin = (lane >> 2) | ((lane & 1) ? 16 : 0);      // the odd lane of a pair stays idle
                     }
-                } else if (valid) {
-                    atomicAdd(reinterpret_cast<unsigned long long *>(gsum + lev * Pb + q), (unsigned long long)v);
-                    atomicAdd(reinterpret_cast<unsigned long long *>(gsum2 + lev * Pb + q), (unsigned long long)v2);
+                    const bool gg = nb > 8 ? (lane & 1) != 0 : (lane & 2) != 0;
+                    if (mine_bin < nb && total != 0)
+                        atomicAdd(reinterpret_cast<unsigned long long *>((gg ? gsum2 : gsum) + lev * Pb + q0 + mine_bin),
+                                  (unsigned long long)(long long)total);
+                } else {
+                    for (int b = 0; b < nb; ++b) {
+                        float pfb = 0.f, pgb = 0.f;
+#pragma unroll
+                        for (int e = 0; e < 16; ++e) if (e == b) { pfb = pf[e]; pgb = pg[e]; }
+                        const long long v = __float2ll_rn(pfb), v2 = __float2ll_rn(pgb);
+                        const int q = q0 + b;
+                        if (one_group) {
+                            // exact warp sums of the 64-bit values as two 32-bit integer reductions each:
+                            // v = hi 2^20 + lo, 0 <= lo < 2^20 (|v| < 2^46 keeps the sum of 32 hi's in 32 bits)
+                            const int hi = __reduce_add_sync(0xffffffffu, (int)(v >> 20));
+                            const int lo = __reduce_add_sync(0xffffffffu, (int)(v & 0xFFFFF));
+                            const int hi2 = __reduce_add_sync(0xffffffffu, (int)(v2 >> 20));
+                            const int lo2 = __reduce_add_sync(0xffffffffu, (int)(v2 & 0xFFFFF));
+                            if (lane == 0) {
+                                atomicAdd(reinterpret_cast<unsigned long long *>(gsum + lev * Pb + q),
+                                          (unsigned long long)(((long long)hi << 20) + (long long)lo));
+                                atomicAdd(reinterpret_cast<unsigned long long *>(gsum2 + lev * Pb + q),
+                                          (unsigned long long)(((long long)hi2 << 20) + (long long)lo2));
+                            }
+                        } else if (valid) {
+                            atomicAdd(reinterpret_cast<unsigned long long *>(gsum + lev * Pb + q), (unsigned long long)v);
+                            atomicAdd(reinterpret_cast<unsigned long long *>(gsum2 + lev * Pb + q), (unsigned long long)v2);
+                        }
+                    }
                 }
             }
             pos[lev] = (unsigned char)((p0 + 1) % Pb);
