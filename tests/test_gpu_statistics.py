@@ -307,3 +307,30 @@ def test_isotropic_average_of_the_correlator(ssm):
     assert np.mean(np.abs(z) < 3.0) >= 0.95 and np.abs(z).max() < 4.5, z
     # the two runs share the dynamics: the isotropic option changes what is correlated, not the state
     assert np.array_equal(g3.get_state()[0], g1.get_state()[0])
+
+
+def test_large_ensemble_needs_64_bit_offsets(ssm):
+    """33.5 million chains of N = 32 (1.07e9 beads, 31.7 GB of warp tiles: byte offsets far beyond 32 bits; B200 holds
+    180 GB).  Philox is keyed by the global chain index, so the first and the last 256 chains of the big ensemble must
+    equal, bit for bit, two small ensembles placed at those indices."""
+    import torch
+    N, M, steps, n = 32, 1 << 25, 40, 256
+    big = ssm.Ensemble(N, M, seed=12, stress_every=10, stress_capacity=8)
+    big.step(steps)
+    out = torch.empty((12, M), dtype=torch.float32, device="cuda")
+    big.chain_stress(out)
+    torch.cuda.synchronize()
+    got_first, got_last = out[:, :n].cpu().numpy(), out[:, M - n:].cpu().numpy()
+    mean_big = big.stress()
+    del big, out
+    torch.cuda.empty_cache()
+    for off, got in ((0, got_first), (M - n, got_last)):
+        small = ssm.Ensemble(N, n, seed=12, chain_offset=off)
+        small.step(steps)
+        assert np.array_equal(small.chain_stress(), got), off
+    # the ensemble means of 3.4e7 chains (1.3e8 lane shares per sample in the exact integer reduction): no flow, so
+    # the off-diagonal means vanish within a few standard errors (per chain sigma_xy has variance N - 1: SE = 1e-3,
+    # sigma_v_xy has variance <Z>: SE = 5e-4) and the three diagonal components agree with each other
+    assert mean_big.shape == (4, 12) and np.all(np.isfinite(mean_big))
+    assert np.all(np.abs(mean_big[:, 3:6]) < 5e-3) and np.all(np.abs(mean_big[:, 9:12]) < 2.5e-3)
+    assert np.all(np.ptp(mean_big[:, 0:3], axis=1) < 0.01) and np.all(np.ptp(mean_big[:, 6:9], axis=1) < 0.004)
