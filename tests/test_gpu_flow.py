@@ -291,3 +291,23 @@ def test_viscosity_and_relaxation_time_scaling_printed_in_the_paper(ssm, golden_
     t, G = out[80][2], out[80][3]
     plateau = G[(t >= 10.0) & (t <= 30.0)]
     assert len(plateau) >= 3 and np.all(np.abs(plateau - want) < tol), plateau
+
+
+def test_rouse_chains_under_general_kappa_reach_the_lyapunov_stress_on_the_gpu(ssm):
+    """The closed form that pins the oracle (tests/test_oracle_flow.py: stationary covariance of each normal mode's
+    Euler map from its discrete Lyapunov equation), here against the GPU directly with 65,536 chains: the ensemble
+    mean of every stress component within 5 standard errors (about 1e-3 of the normal stresses)."""
+    from test_oracle_flow import KAPPA as K, _rouse_stationary_stress
+    N, M, dt = 8, 65536, 0.01
+    want = _rouse_stationary_stress(N, dt, K)
+    g = ssm.Ensemble(N, M, n_0=0.0, dt=dt, seed=5, stress_every=50, stress_capacity=64)
+    g.step_kappa(1000, K)                                       # > 9 Rouse times
+    g.reset_accumulators()
+    g.step_kappa(2000, K)                                       # 40 samples, 0.5 tau0 apart (tau_R = 1.09)
+    s = g.stress()[:, :6]
+    mean = s.mean(0)
+    per_chain = g.chain_stress()[:6].astype(np.float64)         # spread of one sample over chains
+    se = per_chain.std(1, ddof=1) / np.sqrt(M) / np.sqrt(len(s) / 3.0)     # samples 0.5 tau0 apart: ~ every third independent
+    comp = [(0, 0), (1, 1), (2, 2), (0, 1), (1, 2), (2, 0)]
+    for t, (a, b) in enumerate(comp):
+        assert abs(mean[t] - want[a, b]) < 5.0 * se[t] + 2e-4, (t, mean[t], want[a, b], se[t])
