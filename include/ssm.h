@@ -133,6 +133,14 @@ int ssm_group_stress(ssm_ctx *ctx, int64_t chains_per_group, double *h_out);
 int ssm_step_kappa_device(ssm_ctx *ctx, int64_t n_steps, int64_t chains_per_group, const double *d_kappa);
 int ssm_group_stress_device(ssm_ctx *ctx, int64_t chains_per_group, double *d_out);
 
+/* Translate every chain so that its first bead is at the origin, anchors with it.  Nothing observable changes
+ * (the model depends on R_i - R_j and R_S - A only: bonds, hop energies, both stresses); under a flow with a
+ * stretching direction the chain's centre drifts as exp(kappa t), and a long run (steady elongation) has to call
+ * this every few hundred steps to keep the coordinates within fp32's reach.  The anchors' compensation words
+ * restart from zero.  Asynchronous.  (The trajectory after the call differs from the uncentred one by fp32
+ * rounding only, but is no longer bit-identical to it.) */
+int ssm_recenter(ssm_ctx *ctx);
+
 /* Number of stress samples recorded since init / the last reset. */
 int64_t ssm_stress_count(const ssm_ctx *ctx);
 

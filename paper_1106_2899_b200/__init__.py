@@ -19,7 +19,7 @@ EXPORTS = ["ssm_workspace_bytes", "ssm_init", "ssm_step", "ssm_stress_count", "s
            "ssm_reset_accumulators", "ssm_launch_count", "ssm_set_fusion", "ssm_set_grid", "ssm_destroy", "ssm_last_error",
            "ssm_moduli", "ssm_eta0", "ssm_tau_d", "ssm_issue_rates",
            "ssm_gt_virtual", "ssm_gt_sums_virtual", "ssm_step_kappa", "ssm_group_stress",
-           "ssm_step_kappa_device", "ssm_group_stress_device"]
+           "ssm_step_kappa_device", "ssm_group_stress_device", "ssm_recenter"]
 
 
 class Params(C.Structure):
@@ -73,6 +73,7 @@ def lib():
     L.ssm_group_stress.argtypes = [vp, C.c_int64, dp]; L.ssm_group_stress.restype = C.c_int
     L.ssm_step_kappa_device.argtypes = [vp, C.c_int64, C.c_int64, vp]; L.ssm_step_kappa_device.restype = C.c_int
     L.ssm_group_stress_device.argtypes = [vp, C.c_int64, vp]; L.ssm_group_stress_device.restype = C.c_int
+    L.ssm_recenter.argtypes = [vp]; L.ssm_recenter.restype = C.c_int
     L.ssm_moduli.argtypes = [C.c_int32, dp, dp, C.c_int32, dp, dp, dp]; L.ssm_moduli.restype = C.c_int
     L.ssm_eta0.argtypes = [C.c_int32, dp, dp, dp]; L.ssm_eta0.restype = C.c_int
     L.ssm_tau_d.argtypes = [C.c_int32, dp, dp, C.c_double, C.c_double, dp]; L.ssm_tau_d.restype = C.c_int
@@ -186,6 +187,10 @@ class Ensemble:
         with self._torch.cuda.device(self.device):
             self._ck(lib().ssm_group_stress_device(self.h, cpg, C.c_void_p(out.data_ptr())))
         return out
+
+    def recenter(self):
+        with self._torch.cuda.device(self.device):
+            self._ck(lib().ssm_recenter(self.h))
 
     def group_stress(self, chains_per_group=None):
         """ssm_group_stress: [groups][13] = means of sigma[6], sigma_v[6] and Z over each group, current state."""

@@ -24,6 +24,7 @@ cudaError_t launch_xfer(bool do_export, unsigned char *state, float *R, float *A
 cudaError_t launch_clear_low(unsigned char *state, long long n_tiles, cudaStream_t st);
 cudaError_t launch_group_stress(const unsigned char *state, long long *out, int N, long long M, long long cpg, float cs,
                                 cudaStream_t st);
+cudaError_t launch_recenter(unsigned char *state, int N, long long M, cudaStream_t st);
 cudaError_t launch_kappa(const double *d_kappa, float *out, long long n, double dt, cudaStream_t st);
 cudaError_t launch_group_mean(const long long *sums, double *out, long long n_groups, long long M, long long cpg,
                               cudaStream_t st);
@@ -371,6 +372,15 @@ extern "C" int ssm_step_kappa_device(ssm_ctx *c, int64_t n_steps, int64_t chains
     CK(c, launch_kappa(d_kappa, d_table, ng * 9, c->p.dt, c->st));
     c->launches += 1;
     return step_impl(c, n_steps, 0.0, d_table, tpg);
+}
+
+extern "C" int ssm_recenter(ssm_ctx *c)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    CK(c, launch_recenter(c->ws + c->lay.state, c->p.n_beads, c->p.n_chains, c->st));
+    c->launches += 1;
+    c->low_mode = 0;                       // every low word is zero again
+    return SSM_OK;
 }
 
 extern "C" int ssm_group_stress_device(ssm_ctx *c, int64_t chains_per_group, double *d_out)

@@ -221,6 +221,35 @@ __global__ void __launch_bounds__(128) ssm_group_stress_kernel(const unsigned ch
     }
 }
 
+// ---------------------------------------------------------------------------------------
+// Translate every chain so that its first bead sits at the origin (beads and anchors alike).  Forces,
+// hop probabilities and both stresses depend on differences R_i - R_j and R_S - A only, so nothing
+// observable changes; under a flow with a stretching direction the absolute coordinates (the chain's
+// centre drifts as exp(kappa t)) would otherwise use up the fp32 mantissa.  The anchors' low words
+// are cleared (their unit is tied to the coordinate's exponent).
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) ssm_recenter_kernel(unsigned char *state, int N, long long M)
+{
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= M) return;
+    const int NP = padded_beads(N);
+    float o[3];
+    for (int c = 0; c < 3; ++c) o[c] = *reinterpret_cast<const float *>(state + off_R(k, NP, 0, c));
+    for (int i = 0; i < N; ++i)
+        for (int c = 0; c < 3; ++c) *reinterpret_cast<float *>(state + off_R(k, NP, i, c)) -= o[c];
+    const int Z = *reinterpret_cast<const int *>(state + off_Z(k, NP));
+    for (int j = 0; j < Z; ++j) {
+        for (int c = 0; c < 3; ++c) *reinterpret_cast<float *>(state + off_A(k, NP, j, c)) -= o[c];
+        *reinterpret_cast<float *>(state + off_A(k, NP, j, 3)) = 0.0f;
+    }
+}
+
+cudaError_t launch_recenter(unsigned char *state, int N, long long M, cudaStream_t st)
+{
+    ssm_recenter_kernel<<<(unsigned)((M + 127) / 128), 128, 0, st>>>(state, N, M);
+    return cudaGetLastError();
+}
+
 // dt kappa as the step kernel reads it (float) from a device table of tensors in double
 __global__ void __launch_bounds__(256) ssm_kappa_kernel(const double *kappa, float *out, long long n, double dt)
 {

@@ -311,3 +311,42 @@ def test_rouse_chains_under_general_kappa_reach_the_lyapunov_stress_on_the_gpu(s
     comp = [(0, 0), (1, 1), (2, 2), (0, 1), (1, 2), (2, 0)]
     for t, (a, b) in enumerate(comp):
         assert abs(mean[t] - want[a, b]) < 5.0 * se[t] + 2e-4, (t, mean[t], want[a, b], se[t])
+
+
+def test_recentring_changes_nothing_observable_and_keeps_elongation_finite(ssm):
+    """ssm_recenter: the model depends on differences of positions only (pin P8: translation invariance).  (i) GPU and
+    oracle, both translated chain by chain, stay in parity; stresses before = after.  (ii) Uniaxial elongation at
+    rate 0.1 for t = 400 (N = 8: below the coil-stretch rate k_1 = 0.46 of the Hookean chain, so a steady state
+    exists): the chain centres would have drifted by exp(40); with a call every 500 steps the run stays finite and
+    stationary."""
+    N, M = 16, 128
+    e = oracle.Ensemble(N, M, seed=19)
+    g = ssm.Ensemble(N, M, seed=19)
+    upload(e, g)
+    k = 0.25 * KAPPA
+    e.run_kappa(150, k, guard=GUARD); g.step_kappa(150, k)
+    before = g.chain_stress()
+    g.recenter()
+    origin = e.R[:, :1, :].copy()
+    e.R -= origin
+    e.A[e.S > 0] -= np.broadcast_to(origin, e.A.shape)[e.S > 0]
+    after = g.chain_stress()
+    assert np.allclose(before, after, rtol=0, atol=2e-5 * np.maximum(1.0, np.abs(before)).max())
+    R, A, S, _ = g.get_state()
+    assert np.all(R[:, 0, :] == 0.0)
+    e.run_kappa(150, k, guard=GUARD); g.step_kappa(150, k)
+    n, worst = compare_state(e, g)
+    assert n >= _min_unflagged(M, N, 300)
+    # (ii)
+    ext = np.diag([0.1, -0.05, -0.05])
+    h = ssm.Ensemble(8, 16384, seed=20, stress_every=100, stress_capacity=500)
+    for _ in range(80):
+        h.step_kappa(500, ext)
+        h.recenter()
+    s = h.stress()
+    assert np.all(np.isfinite(s))
+    n1 = s[:, 0] - s[:, 1]                                     # first normal stress difference, stationary and positive
+    late, later = n1[200:300].mean(), n1[300:400].mean()
+    assert late > 0.3 and abs(late - later) < 0.05 * late, (late, later)
+    R, A, S, _ = h.get_state()
+    assert np.abs(R).max() < 1e3                                 # without the calls: exp(0.1 * 5) per 500 steps, 1e17 overall
