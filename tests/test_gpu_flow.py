@@ -350,3 +350,30 @@ def test_recentring_changes_nothing_observable_and_keeps_elongation_finite(ssm):
     assert late > 0.3 and abs(late - later) < 0.05 * late, (late, later)
     R, A, S, _ = h.get_state()
     assert np.abs(R).max() < 1e3                                 # without the calls: exp(0.1 * 5) per 500 steps, 1e17 overall
+
+
+def test_trouton_ratio_at_low_elongation_rate(ssm):
+    """Linear response under the diagonal tensor kappa = diag(e, -e/2, -e/2): the steady uniaxial elongational
+    viscosity (sigma_xx - sigma_yy) / e tends to 3 eta_0 (Trouton) with eta_0 = int G(t) dt of eq (59) from the GPU's own
+    correlator.  Together with the shear test above this covers diagonal and off-diagonal entries of eq (18)'s tensor
+    against the equilibrium fluctuations.  Allowance as there (time-discretisation offset of about 2 %)."""
+    N, M, rate = 10, 65536, 0.02
+    g = ssm.Ensemble(N, M, seed=61, sample_every=2, corr_levels=10, corr_bins=16, corr_groups=32, corr_components=3)
+    g.step(2000)
+    g.reset_accumulators()
+    g.step(40000)
+    t, G, se = g.gt()
+    keep = t <= 40.0
+    eta0 = ssm.eta0(t[keep], G[keep])
+    w = np.gradient(t[keep]); eta0_se = float(np.sqrt(np.sum((w * se[keep]) ** 2)))
+    h = ssm.Ensemble(N, M, seed=62, stress_every=10, stress_capacity=4000)
+    ext = np.diag([rate, -rate / 2, -rate / 2])
+    h.step_kappa(5000, ext)
+    h.reset_accumulators()
+    h.step_kappa(30000, ext)
+    s = h.stress()
+    n1 = s[:, 0] - 0.5 * (s[:, 1] + s[:, 2])
+    eta_e = n1.mean() / (N * rate)
+    blocks = n1[: len(n1) // 30 * 30].reshape(30, -1).mean(1)
+    eta_e_se = blocks.std(ddof=1) / np.sqrt(30) / (N * rate)
+    assert abs(eta_e - 3.0 * eta0) < 4.0 * np.hypot(eta_e_se, 3.0 * eta0_se) + 0.04 * 3.0 * eta0, (eta_e, eta_e_se, eta0, eta0_se)
