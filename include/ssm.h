@@ -112,8 +112,9 @@ int ssm_step(ssm_ctx *ctx, int64_t n_steps, double shear_rate);
  * h_kappa (host) [n_groups][9], n_groups = ceil(n_chains / chains_per_group), row-major kappa_ab =
  * d v_a / d r_b in 1/tau0, constant during the call (the host array may be reused after the call returns).
  * chains_per_group >= n_chains means one group; otherwise it must be a multiple of the chains per warp,
- * 256 / (bead places per chain) (the chains of one warp share a tensor), else SSM_EINVAL.  Asynchronous; stress and correlator samples are
- * recorded as by ssm_step (over the whole ensemble; ssm_group_stress reads the groups).  Anchors are advected
+ * 256 / (bead places per chain) (the chains of one warp share a tensor), else SSM_EINVAL.  Asynchronous; stress
+ * and correlator samples are recorded as by ssm_step (over the whole ensemble; ssm_group_stress reads the
+ * groups).  Anchors are advected
  * as compensated sums in all three coordinates (10 extra bits each, kept in the fourth word of the anchor);
  * that word restarts from zero (a change below one ulp of the anchor) when the flow changes between this
  * call and simple shear, and after ssm_set_state. */
