@@ -1,7 +1,12 @@
-"""GPU parity under a general velocity gradient tensor, one per group of chains (
-eqs 18, 21, 44, 45): ssm_step_kappa and ssm_group_stress through the C ABI against the fp64 oracle on the
-same seeded inputs.  Acceptance as in test_gpu_parity.py: indices bit-exact up to a chain's first fragile
-hop decision, positions, anchors and stresses within 1e-5 relative."""
+"""GPU tests of what was built beyond the hot path's rows, through the C ABI:
+ - a general velocity gradient tensor, one per group of chains (eqs 18, 21, 44, 45): ssm_step_kappa / ssm_group_stress
+   (and their device-pointer variants, ssm_recenter) against the fp64 oracle on the same seeded inputs, acceptance as in
+   test_gpu_parity.py (indices bit-exact up to a chain's first fragile hop decision, positions, anchors and stresses
+   within 1e-5 relative), and against closed forms (Lyapunov stress of the Rouse chain, Trouton ratio);
+ - any bead number 2..128 (the paper's N = 10, 20, 40, 80) against the oracle;
+ - the numbers the paper PRINTS about its figures, reproduced by the whole GPU pipeline: <Z> under steady shear at
+   N = 80, eta_0 and tau_d exponents and the plateau modulus, steady-shear viscosity
+   against the integral of G(t) (eqs 59, 61-63)."""
 import numpy as np
 import pytest
 
