@@ -51,6 +51,8 @@ def parse():
     ap.add_argument("--cpu-seconds", type=float, default=20.0)
     ap.add_argument("--table1", action="store_true",
                     help="context only: the paper's Table 1 shapes (65,536 beads, 1e4 steps) timed on this GPU")
+    ap.add_argument("--configs", action="store_true",
+                    help="context only: the other BASELINE.json configs (C2, C3, C5 shapes) timed on this GPU, device-resident")
     return ap.parse_args()
 
 
@@ -194,12 +196,40 @@ def run_table1():
     print(json.dumps({"workload": "PAPER.md Table 1 (context)", "rows": rows}))
 
 
+def run_configs():
+    """BASELINE.json configs[1], [2], [4] (C2, C3, C5 of SURVEY 8d) as they are run in production: same kernels as
+    the bench line, their own shapes, sampling and flow; CUDA events around a few thousand steps after a warm-up.
+    Context beside the bench line (which is configs[3]); parity of these shapes is tests/test_gpu_statistics.py."""
+    import torch
+    import paper_1106_2899_b200 as ssm
+    cases = [("C2 equilibrium G(t)", dict(n_beads=16, n_chains=65536, stress_every=10, sample_every=10), 0.0, 6400),
+             ("C2 without the correlator", dict(n_beads=16, n_chains=65536, stress_every=10), 0.0, 6400),
+             ("C3 start-up shear", dict(n_beads=32, n_chains=262144, stress_every=10), 0.1, 2560),
+             ("C5 long chains, G(t)", dict(n_beads=128, n_chains=131072, dt=0.005, stress_every=10, sample_every=10), 0.0, 1280),
+             ("C5 long chains, steady shear", dict(n_beads=128, n_chains=131072, dt=0.005, stress_every=10), 1e-3, 1280)]
+    rows = []
+    for name, kw, rate, steps in cases:
+        g = ssm.Ensemble(seed=2, stress_capacity=steps // 5, **kw)
+        g.step(steps // 5, rate)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); g.step(steps, rate); e1.record(); torch.cuda.synchronize()
+        t = e0.elapsed_time(e1) * 1e-3
+        rows.append({"config": name, "n_beads": kw["n_beads"], "n_chains": kw["n_chains"], "shear_rate": rate, "steps": steps,
+                     "seconds": t, "bead_updates_per_s": kw["n_beads"] * kw["n_chains"] * steps / t,
+                     "ms_per_32_steps": 1e3 * t / steps * 32})
+        del g
+    print(json.dumps({"workload": "BASELINE.json configs[1], [2], [4] (context)", "rows": rows}))
+
+
 def main():
     a = parse()
     if a.impl == "reference":
         return run_reference(a)
     if a.table1:
         return run_table1()
+    if a.configs:
+        return run_configs()
 
     import torch
     import torch.distributed as dist
