@@ -37,7 +37,7 @@ using namespace ssm;
 static thread_local std::string g_err;   // errors without a ctx
 
 struct Layout {
-    size_t state, stress, kappa, samples, ring, accf, accg, csum, stage, total;
+    size_t state, stress, kappa, counter, samples, ring, accf, accg, csum, stage, total;
     long long n_tiles, stage_chains;
 };
 
@@ -106,6 +106,7 @@ static Layout make_layout(const ssm_params *p)
     L.state = o; o = align_up(o + (size_t)L.n_tiles * kTileBytes, 256);
     L.stress = o; o = align_up(o + (size_t)p->stress_capacity * 12 * 8, 256);
     L.kappa = o; o = align_up(o + (size_t)L.n_tiles * 9 * 4, 256);        // dt kappa per group (at most one group per tile)
+    L.counter = o; o = align_up(o + 2 * sizeof(int), 256);                 // tile counters of the step kernel
     const bool corr = p->sample_every > 0;
     const size_t M = (size_t)p->n_chains;
     const size_t Mv = M * (size_t)(p->corr_components == 3 ? 3 : 1);      // histories: one per chain and component
@@ -234,7 +235,9 @@ extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, s
             ip.t_cdf[z] = threshold23(cdf);
         }
     }
-    if ((e = cudaMemsetAsync(c->ws + lay.state, 0, (size_t)lay.n_tiles * kTileBytes, c->st)) != cudaSuccess
+    sp.tile_counter = reinterpret_cast<int *>(c->ws + lay.counter); sp.counter_slot = 0;
+    if ((e = cudaMemsetAsync(c->ws + lay.counter, 0, 2 * sizeof(int), c->st)) != cudaSuccess
+        || (e = cudaMemsetAsync(c->ws + lay.state, 0, (size_t)lay.n_tiles * kTileBytes, c->st)) != cudaSuccess
         || (e = launch_init(ip, c->st)) != cudaSuccess) {
         int rc = cuda_fail(nullptr, e, "ssm_init launch"); delete c; return rc;
     }
@@ -295,7 +298,9 @@ static int step_impl(ssm_ctx *c, int64_t n_steps, double shear_rate, const float
         sp.n_rec = (int)nrec;
         sp.stress = reinterpret_cast<long long *>(c->ws + c->lay.stress) + c->n_records * 12;
         sp.samples = nsmp > 0 ? reinterpret_cast<float2 *>(c->ws + c->lay.samples) : nullptr;
+        sp.counter_slot = c->sp.counter_slot;
         CK(c, launch_step(padded_beads(p.n_beads), sp, c->grid, c->st));
+        c->sp.counter_slot ^= 1;
         c->launches += 1;
         if (nsmp > 0) {
             CorrParams cp;

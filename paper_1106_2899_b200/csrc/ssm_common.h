@@ -70,6 +70,8 @@ struct StepParams {
     unsigned long long chain_offset;  // global index of local chain 0
     unsigned long long step0;         // global index of the first step of this launch
     int            n_tiles;
+    int           *tile_counter;      // [2] in the workspace: tiles handed out beyond each warp's first; slot counter_slot is
+    int            counter_slot;      // this launch's (zero on entry), the other one is zeroed for the next launch
     int            n_fuse;            // steps in this launch (<= kMaxFuse)
     unsigned       rec_mask;          // bit n: the ensemble stress is recorded after step n of this launch
     unsigned       smp_mask;          // bit n: the correlator is fed after step n of this launch

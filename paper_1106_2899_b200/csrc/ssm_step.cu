@@ -164,8 +164,13 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
         __syncwarp();
     };
 
+    // tiles: every warp starts on its own, the rest are handed out first come, first served (a counter in the
+    // workspace), so that a small ensemble, whose tiles per warp are 1 or 2, keeps every SM busy to the end;
+    // results do not depend on which warp runs a tile.  This launch's counter was zeroed by the previous one.
     const int nwarps = gridDim.x * kWarpsPerBlock;
-    for (int tile = blockIdx.x * kWarpsPerBlock + warp; tile < P.n_tiles; tile += nwarps) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) P.tile_counter[1 - P.counter_slot] = 0;
+    int tile = blockIdx.x * kWarpsPerBlock + warp;
+    for (; tile < P.n_tiles; tile = nwarps + __shfl_sync(kFull, lane == 0 ? atomicAdd(P.tile_counter + P.counter_slot, 1) : 0, 0)) {
         unsigned char *tp = P.state + (long long)tile * kTileBytes;
         const long long chain_local = (long long)tile * CPW + cw;
         const uint32_t chain0 = (uint32_t)(P.chain_offset + (unsigned long long)tile * CPW);
