@@ -69,7 +69,7 @@ def ncu_traffic(n_beads, n_chains):
     from the committed `ncu --set full` capture of this workload; None for other workloads."""
     if (n_beads, n_chains) != (32, 1 << 20):
         return None
-    path = os.path.join(ROOT, "profiles", "r1_v7_step_kernel_metrics.csv")
+    path = os.path.join(ROOT, "profiles", "r1_v8_step_kernel_metrics.csv")
     try:
         import csv
         tot = 0.0
