@@ -47,6 +47,8 @@ def parse():
     ap.add_argument("--beads", type=int, default=32)
     ap.add_argument("--inner", type=int, default=128, help="time steps per bench step")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-contexts", type=int, default=2, help="contexts (streams, host threads) of the e2e leg")
+    ap.add_argument("--e2e-steps", type=int, default=0, help="e2e steps per context (0: min(steps, 4), at least 2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=20.0)
     ap.add_argument("--table1", action="store_true",
@@ -300,21 +302,29 @@ def main():
         pin = [torch.from_numpy(x).pin_memory() for x in (R, A, S)]
         Rp, Ap, Sp = [p.numpy() for p in pin]
         h2d = Rp.nbytes + Ap.nbytes + Sp.nbytes
-        ke = max(2, min(K, 4))
+        ke = a.e2e_steps if a.e2e_steps > 0 else max(2, min(K, 4))
+        nctx = max(1, a.e2e_contexts)
         pair = [ssm.Ensemble(N, M, seed=4, chain_offset=k0, stress_every=1, stress_capacity=inner, stage_chains=M,
-                             device="cuda:%d" % local_rank, stream=torch.cuda.Stream(dev)) for _ in range(2)]
-        outs = [None, None]
+                             device="cuda:%d" % local_rank, stream=torch.cuda.Stream(dev)) for _ in range(nctx)]
+        outs = [None] * nctx
 
-        def e2e_steps(i, n):
+        # context i starts when context i-1 has uploaded its first batch (inside the timed region), so that the
+        # contexts do not begin in phase (all uploading, then all stepping) but as a pipeline
+        def e2e_steps(i, n, uploaded=None):
             torch.cuda.set_device(local_rank)
-            for _ in range(n):
+            if uploaded is not None and i > 0:
+                uploaded[i - 1].wait()
+            for k in range(n):
                 pair[i].reset_accumulators()
                 pair[i].set_state(Rp, Ap, Sp, step)
+                if uploaded is not None and k == 0:
+                    uploaded[i].set()
                 pair[i].step(inner)
                 outs[i] = pair[i].stress()
 
         def e2e_run(n):
-            th = [threading.Thread(target=e2e_steps, args=(i, n)) for i in range(2)]
+            uploaded = [threading.Event() for _ in range(nctx)]
+            th = [threading.Thread(target=e2e_steps, args=(i, n, uploaded)) for i in range(nctx)]
             for x in th:
                 x.start()
             for x in th:
@@ -331,15 +341,16 @@ def main():
         e2e_steps(0, 2)                                         # one context alone: copies and stepping in series
         barrier()
         dt_serial = (time.perf_counter() - t1) / 2
-        assert np.array_equal(outs[0], outs[1])                 # same input, same seed: same samples
+        assert all(np.array_equal(outs[0], o) for o in outs[1:])    # same input, same seed: same samples
         t = torch.tensor([dt], dtype=torch.float64, device=dev)
         if world > 1:
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e = {"value": float(M) * N * inner * 2 * ke * world / float(t.item()), "unit": "bead-updates/s",
+        e2e = {"value": float(M) * N * inner * nctx * ke * world / float(t.item()), "unit": "bead-updates/s",
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(outs[0].nbytes),
-               "steps": 2 * ke, "serial_value": float(M) * N * inner / dt_serial,
-               "what": "ssm_set_state(host pinned) + ssm_step(%d) + ssm_stress(host) per step; two contexts on two "
-                       "streams, one host thread each (serial_value: one context alone)" % inner}
+               "steps": nctx * ke, "contexts": nctx, "serial_value": float(M) * N * inner / dt_serial,
+               "what": "ssm_set_state(host pinned) + ssm_step(%d) + ssm_stress(host) per step; %d contexts on as many "
+                       "streams, one host thread each, started one upload apart (serial_value: one context "
+                       "alone)" % (inner, nctx)}
         del pair
 
     if rank != 0:

@@ -491,7 +491,7 @@ static int xfer_state(ssm_ctx *c, bool do_export, float *R, float *A, uint8_t *S
     const int hide = c->low_mode == 2 ? 1 : 0;       // packed low parts are not a float: exported as 0
     if (dev) {
         CK(c, launch_xfer(do_export, state, R, A, S, N, 0, M, M, hide, c->st));
-        c->launches += do_export ? 1 : 2;
+        c->launches += 1;
         return SSM_OK;
     }
     const long long chunk = c->lay.stage_chains;
@@ -507,11 +507,17 @@ static int xfer_state(ssm_ctx *c, bool do_export, float *R, float *A, uint8_t *S
             CK(c, cudaMemcpy2DAsync(S + k0, (size_t)M, dS, (size_t)chunk, (size_t)nk, (size_t)N, cudaMemcpyDeviceToHost, c->st));
             c->launches += 1;
         } else {
-            CK(c, cudaMemcpy2DAsync(dR, (size_t)chunk * 4, R + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)3 * N, cudaMemcpyHostToDevice, c->st));
-            CK(c, cudaMemcpy2DAsync(dA, (size_t)chunk * 4, A + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)4 * N, cudaMemcpyHostToDevice, c->st));
-            CK(c, cudaMemcpy2DAsync(dS, (size_t)chunk, S + k0, (size_t)M, (size_t)nk, (size_t)N, cudaMemcpyHostToDevice, c->st));
+            if (chunk == M) {      // the staging rows are the caller's rows: three plain copies
+                CK(c, cudaMemcpyAsync(dR, R, (size_t)M * 4 * 3 * N, cudaMemcpyHostToDevice, c->st));
+                CK(c, cudaMemcpyAsync(dA, A, (size_t)M * 4 * 4 * N, cudaMemcpyHostToDevice, c->st));
+                CK(c, cudaMemcpyAsync(dS, S, (size_t)M * N, cudaMemcpyHostToDevice, c->st));
+            } else {
+                CK(c, cudaMemcpy2DAsync(dR, (size_t)chunk * 4, R + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)3 * N, cudaMemcpyHostToDevice, c->st));
+                CK(c, cudaMemcpy2DAsync(dA, (size_t)chunk * 4, A + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)4 * N, cudaMemcpyHostToDevice, c->st));
+                CK(c, cudaMemcpy2DAsync(dS, (size_t)chunk, S + k0, (size_t)M, (size_t)nk, (size_t)N, cudaMemcpyHostToDevice, c->st));
+            }
             CK(c, launch_xfer(false, state, dR, dA, dS, N, k0, nk, chunk, 0, c->st));
-            c->launches += 2;
+            c->launches += 1;
         }
     }
     CK(c, cudaStreamSynchronize(c->st));
