@@ -48,7 +48,7 @@ def parse():
     ap.add_argument("--inner", type=int, default=128, help="time steps per bench step")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-contexts", type=int, default=2, help="contexts (streams, host threads) of the e2e leg")
-    ap.add_argument("--e2e-steps", type=int, default=0, help="e2e steps per context (0: min(steps, 4), at least 2)")
+    ap.add_argument("--e2e-steps", type=int, default=0, help="e2e steps per context (0: min(steps, 10), at least 2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=20.0)
     ap.add_argument("--table1", action="store_true",
@@ -302,7 +302,7 @@ def main():
         pin = [torch.from_numpy(x).pin_memory() for x in (R, A, S)]
         Rp, Ap, Sp = [p.numpy() for p in pin]
         h2d = Rp.nbytes + Ap.nbytes + Sp.nbytes
-        ke = a.e2e_steps if a.e2e_steps > 0 else max(2, min(K, 4))
+        ke = a.e2e_steps if a.e2e_steps > 0 else max(2, min(K, 10))
         nctx = max(1, a.e2e_contexts)
         pair = [ssm.Ensemble(N, M, seed=4, chain_offset=k0, stress_every=1, stress_capacity=inner, stage_chains=M,
                              device="cuda:%d" % local_rank, stream=torch.cuda.Stream(dev)) for _ in range(nctx)]

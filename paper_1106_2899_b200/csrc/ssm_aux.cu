@@ -97,27 +97,33 @@ __global__ void __launch_bounds__(256) ssm_xfer_kernel(unsigned char *state, flo
     else
         for (int i = threadIdx.x; i < n16; i += 256) i4[i] = make_uint4(0u, 0u, 0u, 0u);     // the tiles' unused tail bytes
     __syncthreads();
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const long long k = cb + lane, kk = k - k0;
-    const bool in = k >= k0 && k < k0 + nk;
-    if (in) {
-        for (int row = warp; row < 8 * N; row += 8) {
+    // a warp request covers 4 external rows x 8 chains (four whole 32-byte sectors); in the image the 8 chains
+    // of a row are a multiple of 32 words apart in A, so 8 lanes per row (not 32) keeps the bank conflicts short
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, sub = lane >> 3, ch8 = lane & 7;
+    for (int row = warp * 4 + sub; row < 8 * N; row += 32) {
+#pragma unroll
+        for (int ps = 0; ps < 4; ++ps) {
+            const int cl = ch8 + 8 * ps;
+            const long long kk = cb + cl - k0;
+            if (kk < 0 || kk >= nk) continue;
             if (row < 3 * N) {
                 const int c = row / N, i = row % N;
-                float *p = reinterpret_cast<float *>(img + off_R(lane, NP, i, c));
+                float *p = reinterpret_cast<float *>(img + off_R(cl, NP, i, c));
                 if (EXPORT) R[(long long)row * pitch + kk] = *p; else *p = R[(long long)row * pitch + kk];
             } else if (row < 7 * N) {
                 const int rr = row - 3 * N, c = rr / N, j = rr % N;
-                float *p = reinterpret_cast<float *>(img + off_A(lane, NP, j, c));
+                float *p = reinterpret_cast<float *>(img + off_A(cl, NP, j, c));
                 // (hide_low: the fourth word holds the packed low parts of ssm_step_kappa, not a float; export 0)
                 if (EXPORT) A[(long long)rr * pitch + kk] = (hide_low && c == 3) ? 0.0f : *p; else *p = A[(long long)rr * pitch + kk];
             } else {
                 const int j = row - 7 * N;
-                unsigned char *p = img + off_S(lane, NP, j);
+                unsigned char *p = img + off_S(cl, NP, j);
                 if (EXPORT) S[(long long)j * pitch + kk] = *p; else *p = S[(long long)j * pitch + kk];
             }
         }
     }
+    const long long k = cb + lane;
+    const bool in = k >= k0 && k < k0 + nk;
     if (!EXPORT) {
         __syncthreads();
         if (warp == 0 && in) {
