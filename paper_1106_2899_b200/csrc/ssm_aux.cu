@@ -99,26 +99,43 @@ __global__ void __launch_bounds__(256) ssm_xfer_kernel(unsigned char *state, flo
     __syncthreads();
     // a warp request covers 4 external rows x 8 chains (four whole 32-byte sectors); in the image the 8 chains
     // of a row are a multiple of 32 words apart in A, so 8 lanes per row (not 32) keeps the bank conflicts short
+    // (offsets inside the image as off_R / off_A / off_S of ssm_common.h, with the chain's part, tile and place
+    // in the tile, split off so that a row's own part is computed once: G and the chains per tile are powers of two)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, sub = lane >> 3, ch8 = lane & 7;
+    const int sh = __ffs(cpw) - 1;
     for (int row = warp * 4 + sub; row < 8 * N; row += 32) {
+        int row_off, cw_stride;
+        float *gf = nullptr;
+        unsigned char *gb = nullptr;
+        bool zero = false;
+        if (row < 3 * N) {
+            const int c = row / N, i = row - c * N, f = (i & (kBPL - 1)) * 3 + c;
+            row_off = kTileR + (((f >> 2) * 32 + (i >> 3)) * 4 + (f & 3)) * 4;
+            cw_stride = G * 16;
+            gf = R + (long long)row * pitch;
+        } else if (row < 7 * N) {
+            const int rr = row - 3 * N, c = rr / N, j = rr - c * N;
+            row_off = kTileA + (j * 4 + c) * 4;
+            cw_stride = NP * 16;
+            gf = A + (long long)rr * pitch;
+            // (hide_low: the fourth word holds the packed low parts of ssm_step_kappa, not a float; export 0)
+            zero = EXPORT && hide_low && c == 3;
+        } else {
+            row_off = kTileS + (row - 7 * N);
+            cw_stride = NP;
+            gb = S + (long long)(row - 7 * N) * pitch;
+        }
 #pragma unroll
         for (int ps = 0; ps < 4; ++ps) {
             const int cl = ch8 + 8 * ps;
             const long long kk = cb + cl - k0;
             if (kk < 0 || kk >= nk) continue;
-            if (row < 3 * N) {
-                const int c = row / N, i = row % N;
-                float *p = reinterpret_cast<float *>(img + off_R(cl, NP, i, c));
-                if (EXPORT) R[(long long)row * pitch + kk] = *p; else *p = R[(long long)row * pitch + kk];
-            } else if (row < 7 * N) {
-                const int rr = row - 3 * N, c = rr / N, j = rr % N;
-                float *p = reinterpret_cast<float *>(img + off_A(cl, NP, j, c));
-                // (hide_low: the fourth word holds the packed low parts of ssm_step_kappa, not a float; export 0)
-                if (EXPORT) A[(long long)rr * pitch + kk] = (hide_low && c == 3) ? 0.0f : *p; else *p = A[(long long)rr * pitch + kk];
+            unsigned char *p = img + (cl >> sh) * kTileBytes + (cl & (cpw - 1)) * cw_stride + row_off;
+            if (gf) {
+                float *pf = reinterpret_cast<float *>(p);
+                if (EXPORT) gf[kk] = zero ? 0.0f : *pf; else *pf = gf[kk];
             } else {
-                const int j = row - 7 * N;
-                unsigned char *p = img + off_S(cl, NP, j);
-                if (EXPORT) S[(long long)j * pitch + kk] = *p; else *p = S[(long long)j * pitch + kk];
+                if (EXPORT) gb[kk] = *p; else *p = gb[kk];
             }
         }
     }
