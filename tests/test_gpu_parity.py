@@ -54,6 +54,29 @@ def test_set_get_state_roundtrip_is_bit_exact(ssm):
         assert step == 7 and np.array_equal(R, R3) and np.array_equal(A, A3) and np.array_equal(S, S3)
 
 
+def test_state_import_export_every_shape_and_chunk(ssm):
+    """a10: the import / export kernel moves 32 chains (G whole tiles) per CTA through an image of the tiles; chunks
+    that start and end inside a tile, ragged bead numbers (N < 8G) and every G must give the same bytes back, and the
+    import must count Z (read back as the mean of Z over all chains, exact in int64)."""
+    for N, M in ((8, 203), (16, 77), (20, 131), (32, 300), (80, 45), (128, 70)):
+        e = oracle.Ensemble(N, M, seed=11)
+        e.round_to_fp32()
+        R, A, S = to_external(e)
+        for chunk in (0, 7, 33, 64, M):
+            g = ssm.Ensemble(N, M, seed=99, stage_chains=chunk)       # another seed: every byte must come from the import
+            g.set_state(R, A, S, 5)
+            R2, A2, S2, step = g.get_state()
+            assert step == 5 and np.array_equal(R, R2) and np.array_equal(A, A2) and np.array_equal(S, S2), (N, M, chunk)
+            assert abs(g.group_stress()[0, 12] * M - float((S != 0).sum())) < 1e-6, (N, M, chunk)
+        # device pointers: one launch for the whole ensemble
+        import torch
+        g = ssm.Ensemble(N, M, seed=98)
+        dR, dA, dS = [torch.from_numpy(x).cuda() for x in (R, A, S)]
+        g.set_state(dR, dA, dS, 6)
+        R2, A2, S2, step = g.get_state()
+        assert np.array_equal(R, R2) and np.array_equal(A, A2) and np.array_equal(S, S2), (N, M, "device")
+
+
 def test_device_init_matches_oracle_init(ssm):
     """a0: Z and S bit-exact (integer-domain sampling), R and A to fp32 rounding."""
     for N, M in ((8, 300), (32, 130), (128, 20)):
