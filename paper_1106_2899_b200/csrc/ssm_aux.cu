@@ -73,10 +73,10 @@ cudaError_t launch_init(const InitParams &p, cudaStream_t st)
 // rows 0..3N-1 of R, then 4N rows of A (x, y, z, low part of x), then N rows of S; chains
 // [k0, k0+nk), external element (row, k) at row*pitch + (k - k0).
 // A CTA owns 32 consecutive chains = G whole tiles and transposes them through an image of those
-// tiles in shared memory: the external rows are read / written 128 bytes per warp (lane = chain),
-// the tiles 16 bytes per thread, so both sides of the copy move whole sectors.  (One thread per
-// element writing straight into the tiles, as before, touched a 32-byte sector per 4-byte word:
-// 6.7 ms for the 1 GB of config 4 against the 17.5 ms of its PCIe copy.)  On import the CTA also
+// tiles in shared memory: the external rows are read / written 32 bytes (8 chains) per row and four
+// rows per warp request, the tiles 16 bytes per thread, so both sides of the copy move whole
+// sectors.  (One thread per element writing straight into the tiles, as at first, touched a 32-byte
+// sector per 4-byte word: 6.7 ms for the 1 GB of config 4 against the 17.5 ms of its PCIe copy.)  On import the CTA also
 // counts Z_k = number of occupied slots (they must be the leading ones).
 // ---------------------------------------------------------------------------------------
 template <bool EXPORT>
@@ -89,7 +89,7 @@ __global__ void __launch_bounds__(256) ssm_xfer_kernel(unsigned char *state, flo
     const long long t0 = cb / cpw, t_last = (k0 + nk - 1) / cpw;
     const int nt = (int)(t_last - t0 + 1 < (long long)G ? t_last - t0 + 1 : (long long)G);    // tiles that exist
     // an import that covers every byte the kernels read of these tiles needs no copy of the old image
-    const bool full = cb >= k0 && cb + 32 <= k0 + nk && N == NP;
+    const bool full = cb >= k0 && cb + 32 <= k0 + nk;
     uint4 *g4 = reinterpret_cast<uint4 *>(state + t0 * kTileBytes), *i4 = reinterpret_cast<uint4 *>(img);
     const int n16 = nt * (kTileBytes / 16);
     if (EXPORT || !full)
@@ -97,47 +97,58 @@ __global__ void __launch_bounds__(256) ssm_xfer_kernel(unsigned char *state, flo
     else
         for (int i = threadIdx.x; i < n16; i += 256) i4[i] = make_uint4(0u, 0u, 0u, 0u);     // the tiles' unused tail bytes
     __syncthreads();
-    // a warp request covers 4 external rows x 8 chains (four whole 32-byte sectors); in the image the 8 chains
-    // of a row are a multiple of 32 words apart in A, so 8 lanes per row (not 32) keeps the bank conflicts short
-    // (offsets inside the image as off_R / off_A / off_S of ssm_common.h, with the chain's part, tile and place
-    // in the tile, split off so that a row's own part is computed once: G and the chains per tile are powers of two)
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, sub = lane >> 3, ch8 = lane & 7;
-    const int sh = __ffs(cpw) - 1;
-    for (int row = warp * 4 + sub; row < 8 * N; row += 32) {
-        int row_off, cw_stride;
-        float *gf = nullptr;
-        unsigned char *gb = nullptr;
-        bool zero = false;
-        if (row < 3 * N) {
-            const int c = row / N, i = row - c * N, f = (i & (kBPL - 1)) * 3 + c;
-            row_off = kTileR + (((f >> 2) * 32 + (i >> 3)) * 4 + (f & 3)) * 4;
-            cw_stride = G * 16;
-            gf = R + (long long)row * pitch;
-        } else if (row < 7 * N) {
-            const int rr = row - 3 * N, c = rr / N, j = rr - c * N;
-            row_off = kTileA + (j * 4 + c) * 4;
-            cw_stride = NP * 16;
-            gf = A + (long long)rr * pitch;
-            // (hide_low: the fourth word holds the packed low parts of ssm_step_kappa, not a float; export 0)
-            zero = EXPORT && hide_low && c == 3;
-        } else {
-            row_off = kTileS + (row - 7 * N);
-            cw_stride = NP;
-            gb = S + (long long)(row - 7 * N) * pitch;
-        }
+    // Every thread moves one 16-byte word of the image (one float4 of a lane's beads, one anchor, four bytes of S)
+    // and gathers / scatters its four elements from / to four external rows; the lanes of a warp are laid so that
+    // the image side is (nearly) free of bank conflicts and an external request still covers whole 32-byte sectors
+    // (8 consecutive chains of a row).  Places and slots beyond N (N < 8G) are written as zero on import.
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int sh = __ffs(cpw) - 1, lg = 5 - sh;
+    // beads: unit (tile T, float4 v of the 6 a lane holds); lane = the lane of the step kernel, cw * G + g
+    for (int u = warp; u < nt * 6; u += 8) {
+        const int T = u / 6, v = u - 6 * T, cw = lane >> lg, g = lane & (G - 1);
+        const long long kk = cb + T * cpw + cw - k0;
+        if (kk < 0 || kk >= nk) continue;
+        float4 *p = reinterpret_cast<float4 *>(img + T * kTileBytes + kTileR) + v * 32 + lane;
+        float w[4];
+        if (EXPORT) { const float4 t = *p; w[0] = t.x; w[1] = t.y; w[2] = t.z; w[3] = t.w; }
 #pragma unroll
-        for (int ps = 0; ps < 4; ++ps) {
-            const int cl = ch8 + 8 * ps;
-            const long long kk = cb + cl - k0;
-            if (kk < 0 || kk >= nk) continue;
-            unsigned char *p = img + (cl >> sh) * kTileBytes + (cl & (cpw - 1)) * cw_stride + row_off;
-            if (gf) {
-                float *pf = reinterpret_cast<float *>(p);
-                if (EXPORT) gf[kk] = zero ? 0.0f : *pf; else *pf = gf[kk];
-            } else {
-                if (EXPORT) gb[kk] = *p; else *p = gb[kk];
-            }
+        for (int e = 0; e < 4; ++e) {
+            const int f = 4 * v + e, i = kBPL * g + f / 3, c = f % 3;
+            float *q = R + (long long)(c * N + i) * pitch + kk;
+            if (EXPORT) { if (i < N) *q = w[e]; } else w[e] = i < N ? *q : 0.0f;
         }
+        if (!EXPORT) *p = make_float4(w[0], w[1], w[2], w[3]);
+    }
+    // anchors: unit (8 chains cg, 4 slots jb); lane = 4 * chain + slot
+    for (int u = warp; u < NP; u += 8) {
+        const int cl = (u & 3) * 8 + (lane >> 2), j = (u >> 2) * 4 + (lane & 3);
+        const long long kk = cb + cl - k0;
+        if (kk < 0 || kk >= nk) continue;
+        float4 *p = reinterpret_cast<float4 *>(img + (cl >> sh) * kTileBytes + kTileA) + (cl & (cpw - 1)) * NP + j;
+        float w[4];
+        if (EXPORT) { const float4 t = *p; w[0] = t.x; w[1] = t.y; w[2] = t.z; w[3] = t.w; }
+        // (hide_low: the fourth word holds the packed low parts of ssm_step_kappa, not a float; export 0)
+        if (EXPORT && hide_low) w[3] = 0.0f;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            float *q = A + (long long)(c * N + j) * pitch + kk;
+            if (EXPORT) { if (j < N) *q = w[c]; } else w[c] = j < N ? *q : 0.0f;
+        }
+        if (!EXPORT) *p = make_float4(w[0], w[1], w[2], w[3]);
+    }
+    // bead indices: unit (8 chains, 4 groups of 4 slots); a thread packs the bytes of 4 consecutive slots
+    for (int u = warp; u < 4 * ((NP + 15) / 16); u += 8) {
+        const int cl = (u & 3) * 8 + (lane >> 2), j0 = ((u >> 2) * 4 + (lane & 3)) * 4;
+        const long long kk = cb + cl - k0;
+        if (kk < 0 || kk >= nk || j0 >= NP) continue;
+        unsigned *p = reinterpret_cast<unsigned *>(img + (cl >> sh) * kTileBytes + kTileS + (cl & (cpw - 1)) * NP + j0);
+        unsigned w = EXPORT ? *p : 0u;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            unsigned char *q = S + (long long)(j0 + e) * pitch + kk;
+            if (EXPORT) { if (j0 + e < N) *q = (unsigned char)(w >> (8 * e)); } else w |= (j0 + e < N ? (unsigned)*q : 0u) << (8 * e);
+        }
+        if (!EXPORT) *p = w;
     }
     const long long k = cb + lane;
     const bool in = k >= k0 && k < k0 + nk;
