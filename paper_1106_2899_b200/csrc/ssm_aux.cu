@@ -80,7 +80,7 @@ cudaError_t launch_init(const InitParams &p, cudaStream_t st)
 // counts Z_k = number of occupied slots (they must be the leading ones).
 // ---------------------------------------------------------------------------------------
 template <bool EXPORT>
-__global__ void __launch_bounds__(256) ssm_xfer_kernel(unsigned char *state, float *R, float *A, unsigned char *S,
+__global__ void __launch_bounds__(256, 6) ssm_xfer_kernel(unsigned char *state, float *R, float *A, unsigned char *S,
                                                        int N, int NP, long long k0, long long nk, long long pitch, int hide_low)
 {
     extern __shared__ __align__(16) unsigned char img[];
