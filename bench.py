@@ -293,8 +293,8 @@ def main():
 
     # ---- end to end through the public API with HOST buffers (pinned): every step uploads its input
     # state (ssm_set_state, host pointers), steps, and reads the stress samples back (ssm_stress, host
-    # pointers).  Two contexts on two streams, one host thread each (ctypes releases the GIL), so that the
-    # upload of one batch overlaps the stepping of the other; every batch still pays its own copies.
+    # pointers).  --e2e-contexts (2) contexts on as many streams, one host thread each (ctypes releases the GIL),
+    # so that the upload of one batch overlaps the stepping of the other; every batch still pays its own copies.
     e2e = None
     if not a.no_e2e:
         import threading
