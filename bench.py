@@ -307,6 +307,7 @@ def main():
         pair = [ssm.Ensemble(N, M, seed=4, chain_offset=k0, stress_every=1, stress_capacity=inner, stage_chains=M,
                              device="cuda:%d" % local_rank, stream=torch.cuda.Stream(dev)) for _ in range(nctx)]
         outs = [None] * nctx
+        errs = []
 
         # context i starts when context i-1 has uploaded its first batch (inside the timed region), so that the
         # contexts do not begin in phase (all uploading, then all stepping) but as a pipeline
@@ -314,13 +315,19 @@ def main():
             torch.cuda.set_device(local_rank)
             if uploaded is not None and i > 0:
                 uploaded[i - 1].wait()
-            for k in range(n):
-                pair[i].reset_accumulators()
-                pair[i].set_state(Rp, Ap, Sp, step)
-                if uploaded is not None and k == 0:
-                    uploaded[i].set()
-                pair[i].step(inner)
-                outs[i] = pair[i].stress()
+            try:
+                for k in range(n):
+                    pair[i].reset_accumulators()
+                    pair[i].set_state(Rp, Ap, Sp, step)
+                    if uploaded is not None and k == 0:
+                        uploaded[i].set()
+                    pair[i].step(inner)
+                    outs[i] = pair[i].stress()
+            except BaseException as exc:                       # re-raised by e2e_run: a failed leg must not pass
+                errs.append(exc)
+            finally:
+                if uploaded is not None:
+                    uploaded[i].set()                          # never leave the next context waiting
 
         def e2e_run(n):
             uploaded = [threading.Event() for _ in range(nctx)]
@@ -329,6 +336,8 @@ def main():
                 x.start()
             for x in th:
                 x.join()
+            if errs:
+                raise errs[0]
 
         e2e_run(1)
         barrier()
@@ -339,6 +348,8 @@ def main():
         barrier()
         t1 = time.perf_counter()
         e2e_steps(0, 2)                                         # one context alone: copies and stepping in series
+        if errs:
+            raise errs[0]
         barrier()
         dt_serial = (time.perf_counter() - t1) / 2
         assert all(np.array_equal(outs[0], o) for o in outs[1:])    # same input, same seed: same samples
