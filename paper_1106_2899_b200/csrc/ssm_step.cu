@@ -374,7 +374,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
             for (int t = 0; t < 6; ++t) sv[t] = 0.0f;
             cnt = 0.0f;
             if (P.springs_on) {
-                bool event = false, cand = false;
+                bool event = false;
                 // one slip-spring per lane per pass: number f = lane + 32 it of the warp.  (Two or three
                 // per lane in one straight-line pass were measured slower: 8.2 and 9.1 ms against 7.7 ms
                 // per launch; the extra predicated-off pass costs more than the overlap of the chains wins.)
@@ -485,14 +485,12 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                                     atomicOr(Ev + cw * WPC + (k >> 5), 1u << (k & 31));
                                     Ev[32 + cw] = ((unsigned)k << 16) | (unsigned)h;   // the chain's latest candidate and its half
                                     event = true;
-                                    cand = true;
                                 }
                             }
                         }
                     }
                 }
                 if (__any_sync(kFull, event)) {
-                    const bool any_cand = __any_sync(kFull, cand);
                     __syncwarp();
                     int Zn = Z0;
                     if (l == 0) {
@@ -517,7 +515,6 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                             }
                         }
                         const int K0 = P.k_attempts > 0 ? min(P.k_attempts, NA - Z0) : NA - Z0;
-                        if (any_cand)       // warp-uniform: a warp-step with destructions only never looks at the candidates
 #pragma unroll
                         for (int wd = 0; wd < WPC; ++wd) {
                             unsigned m = Ev[cw * WPC + wd];
