@@ -36,7 +36,8 @@ def build(force=False):
 class Params(C.Structure):
     _fields_ = [("n_beads", C.c_int32), ("n_chains", C.c_int64), ("z_max", C.c_int32),
                 ("n_s", C.c_double), ("n_0", C.c_double), ("zeta_s", C.c_double), ("dt", C.c_double),
-                ("seed", C.c_uint64), ("k_mode", C.c_int32), ("chain_offset", C.c_uint64)]
+                ("seed", C.c_uint64), ("k_mode", C.c_int32), ("chain_offset", C.c_uint64),
+                ("noise_bits", C.c_int32)]
 
 
 class State(C.Structure):
@@ -61,6 +62,7 @@ def lib():
         L.oracle_u23.argtypes = [C.c_uint32]; L.oracle_u23.restype = C.c_double
         L.oracle_threshold23.argtypes = [C.c_double]; L.oracle_threshold23.restype = C.c_int64
         L.oracle_box_muller.argtypes = [C.c_uint32, dp]
+        L.oracle_box_muller23.argtypes = [C.c_uint32, C.c_uint32, dp]
         L.oracle_stream_normal.argtypes = [C.c_uint64, C.c_int, C.c_uint64, C.c_uint64, C.c_uint32]
         L.oracle_stream_normal.restype = C.c_double
         L.oracle_zmax.argtypes = [PP]; L.oracle_zmax.restype = C.c_int
@@ -125,6 +127,13 @@ def box_muller(w):
     return z[0], z[1]
 
 
+def box_muller23(wa, wb):
+    """Two normals from two Philox words at 23-bit resolution (the oracle's noise_bits = 23 law)."""
+    z = (C.c_double * 2)()
+    lib().oracle_box_muller23(wa, wb, z)
+    return z[0], z[1]
+
+
 def stream_normal(seed, domain, step, chain, m):
     return lib().oracle_stream_normal(seed, domain, step, chain, m)
 
@@ -163,8 +172,10 @@ class Ensemble:
     """M chains held as numpy fp64 arrays R[M][N][3], A[M][zmax][3], S[M][zmax], Z[M]."""
 
     def __init__(self, n_beads, n_chains, n_s=0.5, n_0=4.0, zeta_s=0.1, dt=0.01, seed=1,
-                 z_max=0, k_mode=K_EMPTY, chain_offset=0, init=True):
-        self.p = Params(n_beads, n_chains, z_max, n_s, n_0, zeta_s, dt, seed, k_mode, chain_offset)
+                 z_max=0, k_mode=K_EMPTY, chain_offset=0, init=True, noise_bits=16):
+        # noise_bits = 23: the full-resolution noise law (no GPU counterpart; the A/B pin of DESIGN.md reading R24)
+        assert noise_bits in (16, 23)
+        self.p = Params(n_beads, n_chains, z_max, n_s, n_0, zeta_s, dt, seed, k_mode, chain_offset, noise_bits)
         self.N, self.M = n_beads, n_chains
         self.zmax = lib().oracle_zmax(C.byref(self.p))
         self.R = np.zeros((n_chains, n_beads, 3)); self.A = np.zeros((n_chains, self.zmax, 3))

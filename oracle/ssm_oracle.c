@@ -98,6 +98,18 @@ void oracle_box_muller(uint32_t w, double z[2])
     z[1] = r * sin(th);
 }
 
+/* The same transform at the full resolution of the decision uniforms (P:L307 fixes no resolution): two
+ * words give one pair, u_a, u_b = (k + 1/2) 2^-23; |z| <= sqrt(48 ln 2) = 5.77.  Used only when
+ * oracle_params.noise_bits = 23 (the A/B pin of reading R24); the contract with the GPU is the 16-bit form. */
+void oracle_box_muller23(uint32_t wa, uint32_t wb, double z[2])
+{
+    double ua = oracle_u23(wa), ub = oracle_u23(wb);
+    double r = sqrt(-2.0 * log(ua));
+    double th = 6.283185307179586476925286766559 * (ub - 0.5);
+    z[0] = r * cos(th);
+    z[1] = r * sin(th);
+}
+
 /* Normal number m of the stream (domain, step, chain): Philox call q = m>>3 gives the
  * eight normals z_{8q+2e}, z_{8q+2e+1} from word e = 0..3. */
 static void normal_call(uint64_t seed, int domain, uint64_t step, uint64_t chain, uint32_t q,
@@ -261,11 +273,23 @@ static void step_chain(const oracle_params *p, uint64_t chain, uint64_t step, do
         const double rx = R[3 * i], ry = R[3 * i + 1], rz = R[3 * i + 2];
         for (int c = 0; c < 3; ++c) {
             uint32_t m = (uint32_t)(3 * i + c);
-            if ((m & 7) == 0) normal_call(p->seed, ORACLE_DOM_NOISE, step, chain, m >> 3, z8);
+            double w;                                   /* w_i of eqs (46), (47) */
+            if (p->noise_bits == 23) {                  /* full-resolution law (A/B pin of reading R24 only) */
+                if ((m & 3) == 0) {
+                    uint32_t wd[4];
+                    oracle_stream(p->seed, ORACLE_DOM_NOISE, step, chain, m >> 2, wd);
+                    oracle_box_muller23(wd[0], wd[1], z8);
+                    oracle_box_muller23(wd[2], wd[3], z8 + 2);
+                }
+                w = z8[m & 3];
+            } else {
+                if ((m & 7) == 0) normal_call(p->seed, ORACLE_DOM_NOISE, step, chain, m >> 3, z8);
+                w = z8[m & 7];
+            }
             double flow;
             if (kappa) flow = dt * (kappa[3 * c] * rx + kappa[3 * c + 1] * ry + kappa[3 * c + 2] * rz);
             else flow = (c == 0) ? dt * shear_rate * ry : 0.0;
-            R[3 * i + c] = R[3 * i + c] + dt * F[3 * i + c] + flow + sqrt(2.0 * dt) * z8[m & 7];
+            R[3 * i + c] = R[3 * i + c] + dt * F[3 * i + c] + flow + sqrt(2.0 * dt) * w;
         }
     }
     for (int j = 0; j < Z; ++j) {

@@ -36,6 +36,13 @@ typedef struct {
     uint64_t seed;
     int32_t  k_mode;
     uint64_t chain_offset; /* global index of local chain 0 (Philox is keyed by the global index) */
+    int32_t  noise_bits;   /* resolution of the Box-Muller inputs behind the bead noise w_i (eqs 46, 47; DESIGN.md
+                              reading R24).  0 or 16: the RNG contract shared with the GPU (16-bit codes, one word per
+                              pair of normals, eight normals per call).  23: the full-resolution law this oracle was
+                              first written with (23-bit uniforms, two words per pair, four normals per call: normal
+                              m = 3*bead + axis is normal m&3 of call m>>2).  23 has no GPU counterpart; it exists so
+                              that the tests can show that the dynamics do not depend on the narrowing (the A/B pin
+                              of tests/test_oracle_noise_law.py) */
 } oracle_params;
 
 typedef struct {
@@ -62,6 +69,7 @@ uint32_t oracle_code23(uint32_t w);
 double   oracle_u23(uint32_t w);
 int64_t  oracle_threshold23(double p);
 void     oracle_box_muller(uint32_t w, double z[2]);
+void     oracle_box_muller23(uint32_t wa, uint32_t wb, double z[2]);
 double   oracle_stream_normal(uint64_t seed, int domain, uint64_t step, uint64_t chain, uint32_t m);
 int      oracle_zmax(const oracle_params *p);
 void     oracle_hop_probabilities(const oracle_params *p, const double *R, const double *A, int s,
