@@ -155,11 +155,29 @@ int ssm_stress(ssm_ctx *ctx, int64_t first_sample, int64_t n_samples, double *h_
  * sum over local chains of (component + delta_ab) * 2^18 rounded per lane. */
 int ssm_stress_sums(ssm_ctx *ctx, int64_t first_sample, int64_t n_samples, int64_t *h_out);
 
+/* The means of ssm_stress from raw sums and the TOTAL number of chains behind them (no ctx, no device work): what a
+ * sharded run calls on the all-reduced sums of all its ranks.  h_sums (host) [n_samples][12] int64, h_out (host)
+ * [n_samples][12]: sum / (2^18 n_chains_total), the diagonal components of sigma minus 1 (eq 16's -N, of which the
+ * sums hold N - 1).  For one context ssm_stress_from_sums(ssm_stress_sums(...), n_chains) == ssm_stress(...). */
+int ssm_stress_from_sums(const int64_t *h_sums, int64_t n_samples, int64_t n_chains_total, double *h_out);
+
 /* Device address of those sums for samples [first_sample, first_sample + n_samples): *d_ptr
  * (device) int64 [n_samples][12] inside the caller's workspace, so that a multi-GPU run can
  * all-reduce them in place (NCCL) without a copy.  Work queued on the ctx's stream must be
- * ordered before any use on another stream by the caller. */
+ * ordered before any use on another stream: ssm_stream_wait_ctx / ssm_ctx_wait_stream below do that
+ * without blocking the host.  After an in-place all-reduce the sums are those of ALL ranks: ssm_stress
+ * (which divides by the local chain count) no longer applies to those samples -- use ssm_stress_from_sums
+ * with the global chain count. */
 int ssm_stress_sums_device(ssm_ctx *ctx, int64_t first_sample, int64_t n_samples, int64_t **d_ptr);
+
+/* Cross-stream ordering for the exchange above, with CUDA events (no host synchronisation):
+ *  ssm_stream_wait_ctx: work queued LATER on cuda_stream (e.g. NCCL's) waits for everything queued so far on the
+ *                       ctx's stream (the step kernels that produce the sums);
+ *  ssm_ctx_wait_stream: work queued LATER on the ctx's stream (the next steps, ssm_stress_sums) waits for
+ *                       everything queued so far on cuda_stream (the all-reduce).
+ * cuda_stream = cudaStream_t cast to void* (NULL = the legacy default stream). */
+int ssm_stream_wait_ctx(ssm_ctx *ctx, void *cuda_stream);
+int ssm_ctx_wait_stream(ssm_ctx *ctx, void *cuda_stream);
 
 /* Per-chain stresses of the CURRENT state: out [12][M] float32 (component-major, chain
  * fastest), host or device. */
@@ -180,7 +198,7 @@ int ssm_gt(ssm_ctx *ctx, int32_t *n_lags, double *h_lag_time, double *h_G, doubl
 int ssm_gt_virtual(ssm_ctx *ctx, int32_t *n_lags, double *h_lag_time, double *h_dgv, double *h_se);
 int ssm_gt_sums_virtual(ssm_ctx *ctx, double *h_sum_gg);
 
-/* Diagnostic for the roofline: measured cycles per warp instruction per
+/* DIAGNOSTIC, not part of the hot path (bench.py prints it beside the roofline): measured cycles per warp instruction per
  * scheduler, at the step kernel's residency (4 warps per scheduler), of h_cycles[0] FFMA,
  * [1] LOP3/IADD3/SHF, [2] IMAD, [3] IMAD.WIDE (the 32 x 32 -> 64-bit multiply of Philox).
  * Runs four short kernels on the ctx's stream, uses the workspace's staging area (nothing of
@@ -191,8 +209,10 @@ int ssm_issue_rates(ssm_ctx *ctx, double *h_cycles);
  * h_t[n_lags] strictly increasing lag times >= 0 (as ssm_gt returns them), h_G[n_lags].  All (host).
  *  ssm_moduli : storage and loss moduli, eqs (55), (56), by the trapezoidal rule the paper names
  *               (P:L392), the integral truncated at the last lag: h_storage[q] = G'(h_omega[q]),
- *               h_loss[q] = G''(h_omega[q]); the dynamic viscosity of eq (64) is
- *               sqrt(G'^2 + G''^2).
+ *               h_loss[q] = G''(h_omega[q]).
+ *  ssm_eta_star : dynamic viscosity of eq (64) for the Cox-Merz comparison of eq (63):
+ *               h_eta_star[q] = sqrt(G'^2 + G''^2) / w at w = h_omega[q] > 0.  (The printed eq (64) lacks the
+ *               1/w; eq (63) cannot hold without it -- for w -> 0 only sqrt(..)/w tends to eta_0.)
  *  ssm_eta0   : zero-shear viscosity, eq (59), trapezoidal rule.
  *  ssm_tau_d  : longest relaxation time, eq (58): -1 / slope of the least-squares line through
  *               ln G(t) over t_lo <= t <= t_hi (points with G <= 0 skipped); SSM_ERANGE if the
@@ -200,6 +220,8 @@ int ssm_issue_rates(ssm_ctx *ctx, double *h_cycles);
  * SSM_EINVAL on NULL pointers, n_lags < 2, lag times not increasing, negative frequencies. */
 int ssm_moduli(int32_t n_lags, const double *h_t, const double *h_G, int32_t n_omega, const double *h_omega,
                double *h_storage, double *h_loss);
+int ssm_eta_star(int32_t n_lags, const double *h_t, const double *h_G, int32_t n_omega, const double *h_omega,
+                 double *h_eta_star);
 int ssm_eta0(int32_t n_lags, const double *h_t, const double *h_G, double *h_eta0);
 int ssm_tau_d(int32_t n_lags, const double *h_t, const double *h_G, double t_lo, double t_hi, double *h_tau_d);
 
@@ -212,6 +234,9 @@ int ssm_gt_sums(ssm_ctx *ctx, double *h_sum, int64_t *h_count);
  * global_step (host) may be NULL on get.  State + global_step = exact resume. */
 int ssm_get_state(ssm_ctx *ctx, float *R, float *A, uint8_t *S, int64_t *global_step,
                   int pointers_are_device);
+/* ssm_set_state checks S on the device: a chain's occupied slots must be its leading ones and hold bead indices
+ * 1..n_beads.  Otherwise it returns SSM_EINVAL; the chain then keeps its valid leading slots only (the state
+ * stays safe to step).  It synchronises the stream (also with device pointers) to report that. */
 int ssm_set_state(ssm_ctx *ctx, const float *R, const float *A, const uint8_t *S,
                   int64_t global_step, int pointers_are_device);
 

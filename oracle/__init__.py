@@ -77,6 +77,7 @@ def lib():
         L.oracle_corr_create_iso.restype = C.c_void_p
         L.oracle_corr_destroy.argtypes = [C.c_void_p]
         L.oracle_corr_push.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_double, C.c_double]
+        L.oracle_corr_sums.argtypes = [C.c_void_p, dp, dp, i64p]
         L.oracle_corr_result.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_int, dp, dp, dp]
         L.oracle_corr_result.restype = C.c_int
         L.oracle_corr_result_virtual.argtypes = [C.c_void_p, C.c_double, C.c_int, dp, dp, dp]
@@ -147,6 +148,13 @@ class Correlator:
 
     def push(self, chain_local, group, f, g):
         lib().oracle_corr_push(self.h, chain_local, group, f, g)
+
+    def sums(self):
+        """Raw accumulators [groups][levels][bins]: (sum f_new g_old, sum g_new g_old, product counts)."""
+        shape = (self.groups, self.levels, self.bins)
+        s = np.zeros(shape); gg = np.zeros(shape); c = np.zeros(shape, dtype=np.int64)
+        lib().oracle_corr_sums(self.h, _dp(s), _dp(gg), c.ctypes.data_as(C.POINTER(C.c_int64)))
+        return s, gg, c
 
     def result(self, n_beads, base_dt):
         cap = self.levels * self.bins

@@ -5,7 +5,7 @@ section 4.1 written out as the definitions, in numpy fp64.  Shares no code with 
   zero-shear viscosity   eq (59)
   longest relaxation     eq (58): 1/tau_d = -lim ln G(t)/t, read on a finite table as the
                          least-squares slope of ln G over a window
-  dynamic viscosity      eq (64)
+  dynamic viscosity      eq (64), with the 1/w eq (63) needs (reading R25)
 
 Pinned in tests/test_rheology.py by closed forms: a Maxwell mode G = g exp(-t/tau) has
 G' = g w^2 tau^2/(1 + w^2 tau^2), G'' = g w tau/(1 + w^2 tau^2), eta0 = g tau, tau_d = tau;
@@ -36,5 +36,7 @@ def tau_d(t, G, t_lo, t_hi):
     return -1.0 / slope
 
 
-def dynamic_viscosity(g1, g2):
-    return np.sqrt(np.asarray(g1) ** 2 + np.asarray(g2) ** 2)
+def dynamic_viscosity(g1, g2, omega):
+    """eq (64) as the Cox-Merz rule of eq (63) needs it: |eta*|(w) = sqrt(G'^2 + G''^2) / w (the printed formula
+    lacks the 1/w; reading R25)."""
+    return np.sqrt(np.asarray(g1) ** 2 + np.asarray(g2) ** 2) / np.asarray(omega, dtype=np.float64)

@@ -457,6 +457,16 @@ void oracle_corr_push(oracle_corr *c, int64_t chain_local, int group, double f, 
 {
     corr_insert(c, chain_local, group, 0, f, g);
 }
+/* raw accumulators [groups][levels][bins] (sum of f_new g_old, of g_new g_old, product counts), so that a test can
+ * compare another correlator's sums bin by bin */
+void oracle_corr_sums(const oracle_corr *c, double *sum, double *sum_gg, int64_t *count)
+{
+    const size_t n = (size_t)c->groups * c->levels * c->bins;
+    memcpy(sum, c->sum, n * sizeof(double));
+    memcpy(sum_gg, c->sum_gg, n * sizeof(double));
+    memcpy(count, c->count, n * sizeof(int64_t));
+}
+
 /* distinct lags in increasing order: level 0 bins 0..P-1, level l>0 bins P/2..P-1.
  * G/(rho0 kT) = sum/(count N) (reading R13); se = std over groups / sqrt(groups). */
 int oracle_corr_result(const oracle_corr *c, int n_beads, double base_dt, int cap,

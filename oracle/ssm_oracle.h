@@ -86,6 +86,7 @@ oracle_corr *oracle_corr_create(int64_t n_chains, int levels, int bins, int grou
 oracle_corr *oracle_corr_create_iso(int64_t n_chains, int levels, int bins, int groups, int n_comp);
 void     oracle_corr_destroy(oracle_corr *c);
 void     oracle_corr_push(oracle_corr *c, int64_t chain_local, int group, double f, double g);
+void     oracle_corr_sums(const oracle_corr *c, double *sum, double *sum_gg, int64_t *count);
 int      oracle_corr_result(const oracle_corr *c, int n_beads, double base_dt, int cap,
                             double *lag_time, double *G, double *se);
 int      oracle_corr_result_virtual(const oracle_corr *c, double base_dt, int cap,

@@ -19,7 +19,8 @@ EXPORTS = ["ssm_workspace_bytes", "ssm_init", "ssm_step", "ssm_stress_count", "s
            "ssm_reset_accumulators", "ssm_launch_count", "ssm_set_fusion", "ssm_set_grid", "ssm_destroy", "ssm_last_error",
            "ssm_moduli", "ssm_eta0", "ssm_tau_d", "ssm_issue_rates",
            "ssm_gt_virtual", "ssm_gt_sums_virtual", "ssm_step_kappa", "ssm_group_stress",
-           "ssm_step_kappa_device", "ssm_group_stress_device", "ssm_recenter"]
+           "ssm_step_kappa_device", "ssm_group_stress_device", "ssm_recenter",
+           "ssm_eta_star", "ssm_stress_from_sums", "ssm_stream_wait_ctx", "ssm_ctx_wait_stream"]
 
 
 class Params(C.Structure):
@@ -76,6 +77,10 @@ def lib():
     L.ssm_recenter.argtypes = [vp]; L.ssm_recenter.restype = C.c_int
     L.ssm_moduli.argtypes = [C.c_int32, dp, dp, C.c_int32, dp, dp, dp]; L.ssm_moduli.restype = C.c_int
     L.ssm_eta0.argtypes = [C.c_int32, dp, dp, dp]; L.ssm_eta0.restype = C.c_int
+    L.ssm_eta_star.argtypes = [C.c_int32, dp, dp, C.c_int32, dp, dp]; L.ssm_eta_star.restype = C.c_int
+    L.ssm_stress_from_sums.argtypes = [C.POINTER(C.c_int64), C.c_int64, C.c_int64, dp]; L.ssm_stress_from_sums.restype = C.c_int
+    L.ssm_stream_wait_ctx.argtypes = [vp, vp]; L.ssm_stream_wait_ctx.restype = C.c_int
+    L.ssm_ctx_wait_stream.argtypes = [vp, vp]; L.ssm_ctx_wait_stream.restype = C.c_int
     L.ssm_tau_d.argtypes = [C.c_int32, dp, dp, C.c_double, C.c_double, dp]; L.ssm_tau_d.restype = C.c_int
     _lib = L
     return L
@@ -105,6 +110,23 @@ def moduli(t, G, omega):
     g1 = np.zeros(len(w)); g2 = np.zeros(len(w))
     _ck0(lib().ssm_moduli(len(t), tp, Gp, len(w), wp, _d(g1)[1], _d(g2)[1]), "ssm_moduli: bad arguments")
     return g1, g2
+
+
+def eta_star(t, G, omega):
+    """ssm_eta_star: dynamic viscosity sqrt(G'^2 + G''^2) / omega, eq 64 (for the Cox-Merz rule, eq 63)."""
+    t, tp = _d(t); G, Gp = _d(G); w, wp = _d(omega)
+    out = np.zeros(len(w))
+    _ck0(lib().ssm_eta_star(len(t), tp, Gp, len(w), wp, _d(out)[1]), "ssm_eta_star: bad arguments")
+    return out
+
+
+def stress_from_sums(sums, n_chains_total):
+    """ssm_stress_from_sums: ensemble means [n][12] from (all-reduced) fixed-point sums [n][12] int64."""
+    a = np.ascontiguousarray(sums, dtype=np.int64).reshape(-1, 12)
+    out = np.zeros((max(len(a), 1), 12))
+    _ck0(lib().ssm_stress_from_sums(a.ctypes.data_as(C.POINTER(C.c_int64)), len(a), int(n_chains_total),
+                                    out.ctypes.data_as(C.POINTER(C.c_double))), "ssm_stress_from_sums: bad arguments")
+    return out[:len(a)]
 
 
 def eta0(t, G):
@@ -156,6 +178,10 @@ class Ensemble:
         if rc != SSM_OK:
             raise SsmError(rc, lib().ssm_last_error(self.h).decode())
 
+    def _dev(self):
+        """Every call of the C ABI runs with the context's device current (its kernels and copies go there)."""
+        return self._torch.cuda.device(self.device)
+
     def step(self, n_steps, shear_rate=0.0):
         with self._torch.cuda.device(self.device):
             self._ck(lib().ssm_step(self.h, n_steps, shear_rate))
@@ -204,16 +230,18 @@ class Ensemble:
         return lib().ssm_stress_count(self.h)
 
     def stress(self, first=0, n=None):
-        n = self.stress_count() - first if n is None else n
-        out = np.zeros((max(n, 1), 12))
-        self._ck(lib().ssm_stress(self.h, first, n, out.ctypes.data_as(C.POINTER(C.c_double))))
-        return out[:n]
+        with self._dev():
+            n = self.stress_count() - first if n is None else n
+            out = np.zeros((max(n, 1), 12))
+            self._ck(lib().ssm_stress(self.h, first, n, out.ctypes.data_as(C.POINTER(C.c_double))))
+            return out[:n]
 
     def stress_sums(self, first=0, n=None):
-        n = self.stress_count() - first if n is None else n
-        out = np.zeros((max(n, 1), 12), dtype=np.int64)
-        self._ck(lib().ssm_stress_sums(self.h, first, n, out.ctypes.data_as(C.POINTER(C.c_int64))))
-        return out[:n]
+        with self._dev():
+            n = self.stress_count() - first if n is None else n
+            out = np.zeros((max(n, 1), 12), dtype=np.int64)
+            self._ck(lib().ssm_stress_sums(self.h, first, n, out.ctypes.data_as(C.POINTER(C.c_int64))))
+            return out[:n]
 
     def stress_sums_device(self, first=0, n=None):
         """int64 CUDA tensor [n][12] aliasing the fixed-point sums inside the workspace."""
@@ -225,69 +253,76 @@ class Ensemble:
 
     def chain_stress(self, out=None):
         """[12][M] float32: numpy (host) by default, or fill a given CUDA tensor."""
-        if out is None:
-            a = np.zeros((12, self.M), dtype=np.float32)
-            self._ck(lib().ssm_chain_stress(self.h, C.c_void_p(a.ctypes.data), 0))
-            return a
-        self._ck(lib().ssm_chain_stress(self.h, C.c_void_p(out.data_ptr()), 1))
-        return out
+        with self._dev():
+            if out is None:
+                a = np.zeros((12, self.M), dtype=np.float32)
+                self._ck(lib().ssm_chain_stress(self.h, C.c_void_p(a.ctypes.data), 0))
+                return a
+            self._ck(lib().ssm_chain_stress(self.h, C.c_void_p(out.data_ptr()), 1))
+            return out
 
     def gt_virtual(self):
         """ssm_gt_virtual: (lag times, dGv(t) of eq 66, standard error)."""
-        cap = self.p.corr_levels * self.p.corr_bins
-        n = C.c_int32(cap)
-        t = np.zeros(cap); d = np.zeros(cap); se = np.zeros(cap)
-        dd = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
-        self._ck(lib().ssm_gt_virtual(self.h, C.byref(n), dd(t), dd(d), dd(se)))
-        return t[:n.value].copy(), d[:n.value].copy(), se[:n.value].copy()
+        with self._dev():
+            cap = self.p.corr_levels * self.p.corr_bins
+            n = C.c_int32(cap)
+            t = np.zeros(cap); d = np.zeros(cap); se = np.zeros(cap)
+            dd = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+            self._ck(lib().ssm_gt_virtual(self.h, C.byref(n), dd(t), dd(d), dd(se)))
+            return t[:n.value].copy(), d[:n.value].copy(), se[:n.value].copy()
 
     def gt(self):
-        cap = self.p.corr_levels * self.p.corr_bins
-        n = C.c_int32(cap)
-        t = np.zeros(cap); G = np.zeros(cap); se = np.zeros(cap)
-        d = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
-        self._ck(lib().ssm_gt(self.h, C.byref(n), d(t), d(G), d(se)))
-        return t[:n.value].copy(), G[:n.value].copy(), se[:n.value].copy()
+        with self._dev():
+            cap = self.p.corr_levels * self.p.corr_bins
+            n = C.c_int32(cap)
+            t = np.zeros(cap); G = np.zeros(cap); se = np.zeros(cap)
+            d = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+            self._ck(lib().ssm_gt(self.h, C.byref(n), d(t), d(G), d(se)))
+            return t[:n.value].copy(), G[:n.value].copy(), se[:n.value].copy()
 
     def gt_sums(self):
-        shape = (self.p.corr_groups, self.p.corr_levels, self.p.corr_bins)
-        s = np.zeros(shape); c = np.zeros(shape, dtype=np.int64)
-        self._ck(lib().ssm_gt_sums(self.h, s.ctypes.data_as(C.POINTER(C.c_double)),
-                                   c.ctypes.data_as(C.POINTER(C.c_int64))))
-        return s, c
+        with self._dev():
+            shape = (self.p.corr_groups, self.p.corr_levels, self.p.corr_bins)
+            s = np.zeros(shape); c = np.zeros(shape, dtype=np.int64)
+            self._ck(lib().ssm_gt_sums(self.h, s.ctypes.data_as(C.POINTER(C.c_double)),
+                                       c.ctypes.data_as(C.POINTER(C.c_int64))))
+            return s, c
 
     def get_state(self, R=None, A=None, S=None):
         """External SoA layout: R[3][N][M], A[4][N][M] float32 (x, y, z, low part of x), S[N][M] uint8.  Host numpy
         arrays by default; pass CUDA tensors (all three) to stay on the device."""
-        step = C.c_int64()
-        if R is None:
-            R = np.zeros((3, self.N, self.M), dtype=np.float32); A = np.zeros((4, self.N, self.M), dtype=np.float32)
-            S = np.zeros((self.N, self.M), dtype=np.uint8)
-            self._ck(lib().ssm_get_state(self.h, C.c_void_p(R.ctypes.data), C.c_void_p(A.ctypes.data),
-                                         C.c_void_p(S.ctypes.data), C.byref(step), 0))
-        elif isinstance(R, np.ndarray):
-            self._ck(lib().ssm_get_state(self.h, C.c_void_p(R.ctypes.data), C.c_void_p(A.ctypes.data),
-                                         C.c_void_p(S.ctypes.data), C.byref(step), 0))
-        else:
-            dev = 1 if R.is_cuda else 0
-            self._ck(lib().ssm_get_state(self.h, C.c_void_p(R.data_ptr()), C.c_void_p(A.data_ptr()),
-                                         C.c_void_p(S.data_ptr()), C.byref(step), dev))
-        return R, A, S, step.value
+        with self._dev():
+            step = C.c_int64()
+            if R is None:
+                R = np.zeros((3, self.N, self.M), dtype=np.float32); A = np.zeros((4, self.N, self.M), dtype=np.float32)
+                S = np.zeros((self.N, self.M), dtype=np.uint8)
+                self._ck(lib().ssm_get_state(self.h, C.c_void_p(R.ctypes.data), C.c_void_p(A.ctypes.data),
+                                             C.c_void_p(S.ctypes.data), C.byref(step), 0))
+            elif isinstance(R, np.ndarray):
+                self._ck(lib().ssm_get_state(self.h, C.c_void_p(R.ctypes.data), C.c_void_p(A.ctypes.data),
+                                             C.c_void_p(S.ctypes.data), C.byref(step), 0))
+            else:
+                dev = 1 if R.is_cuda else 0
+                self._ck(lib().ssm_get_state(self.h, C.c_void_p(R.data_ptr()), C.c_void_p(A.data_ptr()),
+                                             C.c_void_p(S.data_ptr()), C.byref(step), dev))
+            return R, A, S, step.value
 
     def set_state(self, R, A, S, global_step):
-        if isinstance(R, np.ndarray):
-            assert R.dtype == np.float32 and A.dtype == np.float32 and S.dtype == np.uint8
-            assert R.flags.c_contiguous and A.flags.c_contiguous and S.flags.c_contiguous
-            assert R.shape == (3, self.N, self.M) and A.shape == (4, self.N, self.M) and S.shape == (self.N, self.M)
-            self._ck(lib().ssm_set_state(self.h, C.c_void_p(R.ctypes.data), C.c_void_p(A.ctypes.data),
-                                         C.c_void_p(S.ctypes.data), global_step, 0))
-        else:
-            dev = 1 if R.is_cuda else 0
-            self._ck(lib().ssm_set_state(self.h, C.c_void_p(R.data_ptr()), C.c_void_p(A.data_ptr()),
-                                         C.c_void_p(S.data_ptr()), global_step, dev))
+        with self._dev():
+            if isinstance(R, np.ndarray):
+                assert R.dtype == np.float32 and A.dtype == np.float32 and S.dtype == np.uint8
+                assert R.flags.c_contiguous and A.flags.c_contiguous and S.flags.c_contiguous
+                assert R.shape == (3, self.N, self.M) and A.shape == (4, self.N, self.M) and S.shape == (self.N, self.M)
+                self._ck(lib().ssm_set_state(self.h, C.c_void_p(R.ctypes.data), C.c_void_p(A.ctypes.data),
+                                             C.c_void_p(S.ctypes.data), global_step, 0))
+            else:
+                dev = 1 if R.is_cuda else 0
+                self._ck(lib().ssm_set_state(self.h, C.c_void_p(R.data_ptr()), C.c_void_p(A.data_ptr()),
+                                             C.c_void_p(S.data_ptr()), global_step, dev))
 
     def reset_accumulators(self):
-        self._ck(lib().ssm_reset_accumulators(self.h))
+        with self._dev():
+            self._ck(lib().ssm_reset_accumulators(self.h))
 
     def launch_count(self):
         return lib().ssm_launch_count(self.h)
@@ -301,6 +336,16 @@ class Ensemble:
         with self._torch.cuda.device(self.device):
             self._ck(lib().ssm_issue_rates(self.h, out.ctypes.data_as(C.POINTER(C.c_double))))
         return {"ffma": out[0], "alu": out[1], "imad": out[2], "imad_wide": out[3]}
+
+    def stream_wait_ctx(self, stream):
+        """ssm_stream_wait_ctx: later work on `stream` (a torch.cuda.Stream) waits for this context's queued work."""
+        with self._dev():
+            self._ck(lib().ssm_stream_wait_ctx(self.h, C.c_void_p(stream.cuda_stream)))
+
+    def ctx_wait_stream(self, stream):
+        """ssm_ctx_wait_stream: this context's later work waits for what is queued on `stream` so far."""
+        with self._dev():
+            self._ck(lib().ssm_ctx_wait_stream(self.h, C.c_void_p(stream.cuda_stream)))
 
     def set_grid(self, blocks):
         self._ck(lib().ssm_set_grid(self.h, blocks))

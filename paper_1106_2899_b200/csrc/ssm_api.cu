@@ -20,7 +20,7 @@ cudaError_t launch_step(int n_beads, const StepParams &p, int grid, cudaStream_t
 cudaError_t launch_init(const InitParams &p, cudaStream_t st);
 cudaError_t measure_rates(unsigned *d_scratch, int blocks, cudaStream_t st, double cycles[4]);
 cudaError_t launch_xfer(bool do_export, unsigned char *state, float *R, float *A, unsigned char *S, int N,
-                        long long k0, long long nk, long long pitch, int hide_low, cudaStream_t st);
+                        long long k0, long long nk, long long pitch, int hide_low, int *bad_state, cudaStream_t st);
 cudaError_t launch_clear_low(unsigned char *state, long long n_tiles, cudaStream_t st);
 cudaError_t launch_group_stress(const unsigned char *state, long long *out, int N, long long M, long long cpg, float cs,
                                 cudaStream_t st);
@@ -106,7 +106,7 @@ static Layout make_layout(const ssm_params *p)
     L.state = o; o = align_up(o + (size_t)L.n_tiles * kTileBytes, 256);
     L.stress = o; o = align_up(o + (size_t)p->stress_capacity * 12 * 8, 256);
     L.kappa = o; o = align_up(o + (size_t)L.n_tiles * 9 * 4, 256);        // dt kappa per group (at most one group per tile)
-    L.counter = o; o = align_up(o + 2 * sizeof(int), 256);                 // tile counters of the step kernel
+    L.counter = o; o = align_up(o + 3 * sizeof(int), 256);                 // tile counters of the step kernel [0], [1]; [2] = "the imported state was malformed"
     const bool corr = p->sample_every > 0;
     const size_t M = (size_t)p->n_chains;
     const size_t Mv = M * (size_t)(p->corr_components == 3 ? 3 : 1);      // histories: one per chain and component
@@ -236,7 +236,7 @@ extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, s
         }
     }
     sp.tile_counter = reinterpret_cast<int *>(c->ws + lay.counter); sp.counter_slot = 0;
-    if ((e = cudaMemsetAsync(c->ws + lay.counter, 0, 2 * sizeof(int), c->st)) != cudaSuccess
+    if ((e = cudaMemsetAsync(c->ws + lay.counter, 0, 3 * sizeof(int), c->st)) != cudaSuccess
         || (e = cudaMemsetAsync(c->ws + lay.state, 0, (size_t)lay.n_tiles * kTileBytes, c->st)) != cudaSuccess
         || (e = launch_init(ip, c->st)) != cudaSuccess) {
         int rc = cuda_fail(nullptr, e, "ssm_init launch"); delete c; return rc;
@@ -448,6 +448,30 @@ extern "C" int ssm_stress_sums_device(ssm_ctx *c, int64_t first, int64_t n, int6
     return SSM_OK;
 }
 
+static int order_streams(ssm_ctx *c, cudaStream_t first, cudaStream_t then)
+{
+    if (first == then) return SSM_OK;
+    cudaEvent_t ev;
+    CK(c, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+    cudaError_t e = cudaEventRecord(ev, first);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(then, ev, 0);
+    cudaEventDestroy(ev);                       // released once the wait has been satisfied
+    if (e != cudaSuccess) return cuda_fail(c, e, "stream ordering");
+    return SSM_OK;
+}
+
+extern "C" int ssm_stream_wait_ctx(ssm_ctx *c, void *cuda_stream)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    return order_streams(c, c->st, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int ssm_ctx_wait_stream(ssm_ctx *c, void *cuda_stream)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    return order_streams(c, (cudaStream_t)cuda_stream, c->st);
+}
+
 extern "C" int ssm_stress(ssm_ctx *c, int64_t first, int64_t n, double *h_out)
 {
     if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
@@ -457,10 +481,8 @@ extern "C" int ssm_stress(ssm_ctx *c, int64_t first, int64_t n, double *h_out)
     if (rc != SSM_OK) return rc;
     // sums hold sum_bonds (3 b_a b_b - delta_ab) and sum_j ((3/N_s) d_a d_b - delta_ab):
     // sigma_aa = 3 sum b_a^2 - N needs one more -1 per chain (eq 16); sigma^(v) needs none (eq 76)
-    const double scale = 1.0 / ((double)(1 << kStressShift) * (double)c->p.n_chains);
-    for (int64_t i = 0; i < n; ++i)
-        for (int t = 0; t < 12; ++t)
-            h_out[i * 12 + t] = (double)raw[(size_t)i * 12 + t] * scale - (t < 3 ? 1.0 : 0.0);
+    static_assert(kStressShift == 18, "ssm_stress_from_sums (ssm_rheo.cu) divides by 2^18");
+    if (ssm_stress_from_sums(raw.data(), n, c->p.n_chains, h_out) != SSM_OK) return fail(c, SSM_EINVAL, "bad sample range");
     return SSM_OK;
 }
 
@@ -489,8 +511,9 @@ static int xfer_state(ssm_ctx *c, bool do_export, float *R, float *A, uint8_t *S
     const int N = c->p.n_beads; const long long M = c->p.n_chains;
     unsigned char *state = c->ws + c->lay.state;
     const int hide = c->low_mode == 2 ? 1 : 0;       // packed low parts are not a float: exported as 0
+    int *bad = reinterpret_cast<int *>(c->ws + c->lay.counter) + 2;
     if (dev) {
-        CK(c, launch_xfer(do_export, state, R, A, S, N, 0, M, M, hide, c->st));
+        CK(c, launch_xfer(do_export, state, R, A, S, N, 0, M, M, hide, bad, c->st));
         c->launches += 1;
         return SSM_OK;
     }
@@ -501,7 +524,7 @@ static int xfer_state(ssm_ctx *c, bool do_export, float *R, float *A, uint8_t *S
     for (long long k0 = 0; k0 < M; k0 += chunk) {
         const long long nk = M - k0 < chunk ? M - k0 : chunk;
         if (do_export) {
-            CK(c, launch_xfer(true, state, dR, dA, dS, N, k0, nk, chunk, hide, c->st));
+            CK(c, launch_xfer(true, state, dR, dA, dS, N, k0, nk, chunk, hide, bad, c->st));
             CK(c, cudaMemcpy2DAsync(R + k0, (size_t)M * 4, dR, (size_t)chunk * 4, (size_t)nk * 4, (size_t)3 * N, cudaMemcpyDeviceToHost, c->st));
             CK(c, cudaMemcpy2DAsync(A + k0, (size_t)M * 4, dA, (size_t)chunk * 4, (size_t)nk * 4, (size_t)4 * N, cudaMemcpyDeviceToHost, c->st));
             CK(c, cudaMemcpy2DAsync(S + k0, (size_t)M, dS, (size_t)chunk, (size_t)nk, (size_t)N, cudaMemcpyDeviceToHost, c->st));
@@ -516,7 +539,7 @@ static int xfer_state(ssm_ctx *c, bool do_export, float *R, float *A, uint8_t *S
                 CK(c, cudaMemcpy2DAsync(dA, (size_t)chunk * 4, A + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)4 * N, cudaMemcpyHostToDevice, c->st));
                 CK(c, cudaMemcpy2DAsync(dS, (size_t)chunk, S + k0, (size_t)M, (size_t)nk, (size_t)N, cudaMemcpyHostToDevice, c->st));
             }
-            CK(c, launch_xfer(false, state, dR, dA, dS, N, k0, nk, chunk, 0, c->st));
+            CK(c, launch_xfer(false, state, dR, dA, dS, N, k0, nk, chunk, 0, bad, c->st));
             c->launches += 1;
         }
     }
@@ -538,8 +561,19 @@ extern "C" int ssm_set_state(ssm_ctx *c, const float *R, const float *A, const u
     if (!R || !A || !S) return fail(c, SSM_EINVAL, "NULL state pointer");
     if (global_step < 0) return fail(c, SSM_EINVAL, "global_step < 0");
     int rc = xfer_state(c, false, const_cast<float *>(R), const_cast<float *>(A), const_cast<uint8_t *>(S), dev);
-    if (rc == SSM_OK) { c->step = global_step; c->low_mode = 1; }      // A[3] of the caller is the fp32 low part of x
-    return rc;
+    if (rc != SSM_OK) return rc;
+    c->step = global_step; c->low_mode = 1;                            // A[3] of the caller is the fp32 low part of x
+    // the import kernel flags a chain whose S is not "bead indices 1..N in the leading slots, 0 after them"
+    int bad = 0;
+    int *d_bad = reinterpret_cast<int *>(c->ws + c->lay.counter) + 2;
+    CK(c, cudaMemcpyAsync(&bad, d_bad, sizeof bad, cudaMemcpyDeviceToHost, c->st));
+    CK(c, cudaStreamSynchronize(c->st));
+    if (bad) {
+        CK(c, cudaMemsetAsync(d_bad, 0, sizeof bad, c->st));
+        return fail(c, SSM_EINVAL, "S is malformed: a chain's occupied slots must be its leading ones and hold bead indices 1..n_beads "
+                                   "(the offending slots were cleared)");
+    }
+    return SSM_OK;
 }
 
 extern "C" int ssm_reset_accumulators(ssm_ctx *c)

@@ -81,7 +81,8 @@ cudaError_t launch_init(const InitParams &p, cudaStream_t st)
 // ---------------------------------------------------------------------------------------
 template <bool EXPORT>
 __global__ void __launch_bounds__(256, 6) ssm_xfer_kernel(unsigned char *state, float *R, float *A, unsigned char *S,
-                                                       int N, int NP, long long k0, long long nk, long long pitch, int hide_low)
+                                                       int N, int NP, long long k0, long long nk, long long pitch, int hide_low,
+                                                       int *bad_state)
 {
     extern __shared__ __align__(16) unsigned char img[];
     const int G = NP / kBPL, cpw = 32 / G;
@@ -155,8 +156,15 @@ __global__ void __launch_bounds__(256, 6) ssm_xfer_kernel(unsigned char *state, 
     if (!EXPORT) {
         __syncthreads();
         if (warp == 0 && in) {
+            // Z = the leading occupied slots.  A caller's S must hold bead indices 1..N there and 0 after
+            // them; anything else would send the step kernel's scatter outside the chain.  Such a chain keeps its
+            // valid leading slots only, the rest is cleared, and the flag makes ssm_set_state fail.
             int Z = 0;
-            while (Z < N && img[off_S(lane, NP, Z)] != 0) ++Z;
+            while (Z < N && img[off_S(lane, NP, Z)] != 0 && img[off_S(lane, NP, Z)] <= N) ++Z;
+            bool bad = false;
+            for (int j = Z; j < NP; ++j)
+                if (img[off_S(lane, NP, j)] != 0) { bad = true; img[off_S(lane, NP, j)] = 0; }
+            if (bad) atomicExch(bad_state, 1);
             *reinterpret_cast<int *>(img + off_Z(lane, NP)) = Z;
         }
         __syncthreads();
@@ -165,7 +173,7 @@ __global__ void __launch_bounds__(256, 6) ssm_xfer_kernel(unsigned char *state, 
 }
 
 cudaError_t launch_xfer(bool do_export, unsigned char *state, float *R, float *A, unsigned char *S, int N,
-                        long long k0, long long nk, long long pitch, int hide_low, cudaStream_t st)
+                        long long k0, long long nk, long long pitch, int hide_low, int *bad_state, cudaStream_t st)
 {
     if (nk <= 0) return cudaSuccess;
     const int NP = padded_beads(N);
@@ -174,10 +182,10 @@ cudaError_t launch_xfer(bool do_export, unsigned char *state, float *R, float *A
     cudaError_t e;
     if (do_export) {
         if ((e = cudaFuncSetAttribute(ssm_xfer_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-        ssm_xfer_kernel<true><<<grid, 256, smem, st>>>(state, R, A, S, N, NP, k0, nk, pitch, hide_low);
+        ssm_xfer_kernel<true><<<grid, 256, smem, st>>>(state, R, A, S, N, NP, k0, nk, pitch, hide_low, bad_state);
     } else {
         if ((e = cudaFuncSetAttribute(ssm_xfer_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-        ssm_xfer_kernel<false><<<grid, 256, smem, st>>>(state, R, A, S, N, NP, k0, nk, pitch, 0);
+        ssm_xfer_kernel<false><<<grid, 256, smem, st>>>(state, R, A, S, N, NP, k0, nk, pitch, 0, bad_state);
     }
     return cudaGetLastError();
 }

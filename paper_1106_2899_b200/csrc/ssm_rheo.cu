@@ -42,6 +42,37 @@ extern "C" int ssm_moduli(int32_t n_lags, const double *h_t, const double *h_G, 
     return SSM_OK;
 }
 
+// eq (64): dynamic viscosity eta*(w) = sqrt(G'^2 + G''^2) / w for the Cox-Merz comparison of eq (63), eta(rate) ~
+// eta*(w = rate).  (P:L424 prints the square root without the 1/w; eq (63) needs it: for w -> 0, G'' -> eta_0 w, so
+// only sqrt(G'^2 + G''^2) / w tends to eta_0 = eta(rate -> 0).  DESIGN.md reading R25.)
+extern "C" int ssm_eta_star(int32_t n_lags, const double *h_t, const double *h_G, int32_t n_omega, const double *h_omega,
+                            double *h_eta_star)
+{
+    if (n_omega < 0 || (n_omega > 0 && (!h_omega || !h_eta_star))) return SSM_EINVAL;
+    for (int32_t q = 0; q < n_omega; ++q)
+        if (!(h_omega[q] > 0.0) || !std::isfinite(h_omega[q])) return SSM_EINVAL;
+    for (int32_t q = 0; q < n_omega; ++q) {
+        double g1 = 0.0, g2 = 0.0;
+        const int rc = ssm_moduli(n_lags, h_t, h_G, 1, h_omega + q, &g1, &g2);
+        if (rc != SSM_OK) return rc;
+        h_eta_star[q] = std::sqrt(g1 * g1 + g2 * g2) / h_omega[q];
+    }
+    return SSM_OK;
+}
+
+// Ensemble means (eq 54) of sigma (eq 16) and sigma^(v) (eq 76) from the raw fixed-point sums of ssm_stress_sums /
+// ssm_stress_sums_device -- summed over every rank of a sharded ensemble -- and the TOTAL number of chains behind
+// them: value = sum / (2^18 M); sigma_aa = 3 sum b_a^2 - N, of which the sums hold N - 1 of the N (one per bond), so
+// the three diagonal components of sigma take one more -1 per chain (ssm_stress does the same for one context).
+extern "C" int ssm_stress_from_sums(const int64_t *h_sums, int64_t n_samples, int64_t n_chains_total, double *h_out)
+{
+    if (n_samples < 0 || n_chains_total < 1 || (n_samples > 0 && (!h_sums || !h_out))) return SSM_EINVAL;
+    const double scale = 1.0 / (262144.0 * (double)n_chains_total);
+    for (int64_t i = 0; i < n_samples; ++i)
+        for (int t = 0; t < 12; ++t) h_out[i * 12 + t] = (double)h_sums[i * 12 + t] * scale - (t < 3 ? 1.0 : 0.0);
+    return SSM_OK;
+}
+
 // eq (59): eta_0 = int_0^inf G(t) dt, trapezoidal rule, truncated at the last lag
 extern "C" int ssm_eta0(int32_t n_lags, const double *h_t, const double *h_G, double *h_eta0)
 {

@@ -13,6 +13,8 @@
 // Mapping and layouts: ssm_common.h and DESIGN.md section 6.
 #include <cuda_runtime.h>
 
+#include <atomic>
+
 #include "ssm_common.h"
 #include "ssm_rng.cuh"
 
@@ -605,11 +607,15 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
 template <int G, int FLOW, bool RAGGED>
 static cudaError_t launch_gfr(const StepParams &p, int grid, cudaStream_t st)
 {
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(ssm_step_kernel<G, FLOW, RAGGED>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmStep);
+    // the attribute belongs to the (function, device) pair: remember per device where it has been set
+    static std::atomic<unsigned long long> configured{0ull};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev >= 64 || !((configured.load(std::memory_order_relaxed) >> dev) & 1ull)) {
+        e = cudaFuncSetAttribute(ssm_step_kernel<G, FLOW, RAGGED>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmStep);
         if (e != cudaSuccess) return e;
-        configured = true;
+        if (dev < 64) configured.fetch_or(1ull << dev, std::memory_order_relaxed);
     }
     ssm_step_kernel<G, FLOW, RAGGED><<<grid, kBlockThreads, kSmStep, st>>>(p);
     return cudaGetLastError();

@@ -31,22 +31,27 @@ def weak_range(n_chains_per_rank, rank):
     return k0, k0 + int(n_chains_per_rank)
 
 
-def allreduce_sums(t, group=None):
+def allreduce_sums(t, group=None, ctx=None):
     """In-place sum over ranks of an int64 tensor of fixed-point sums (stress samples
-    [n][12] or correlator sums).  NCCL on device tensors, gloo on CPU tensors."""
+    [n][12] or correlator sums).  NCCL on device tensors, gloo on CPU tensors.
+    ctx: the Ensemble whose workspace t aliases (ssm_stress_sums_device).  torch orders the collective
+    with torch's CURRENT stream; when the context runs on a stream of its own, the two are ordered with
+    events (ssm_stream_wait_ctx before, ssm_ctx_wait_stream after) -- no host synchronisation."""
     import torch
     import torch.distributed as dist
     assert t.dtype == torch.int64
     if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+        cur = torch.cuda.current_stream(t.device) if (ctx is not None and t.is_cuda) else None
+        if cur is not None:
+            ctx.stream_wait_ctx(cur)
         dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+        if cur is not None:
+            ctx.ctx_wait_stream(cur)
     return t
 
 
-def stress_means(sums, n_chains_total, shift=18):
-    """Ensemble means (eq 54) from the all-reduced fixed-point sums [n][12]: value =
-    sum / (2^shift M) and the remaining -1 of the three diagonal bond-stress components
-    (eq 16: -N kT 1, of which N-1 are folded into the sums; see ssm_stress in ssm.h)."""
-    import numpy as np
-    a = np.asarray(sums, dtype=np.float64) / (float(1 << shift) * float(n_chains_total))
-    a[:, :3] -= 1.0
-    return a
+def stress_means(sums, n_chains_total):
+    """Ensemble means (eq 54) from the all-reduced fixed-point sums [n][12]: ssm_stress_from_sums of the C ABI
+    (the fixed point and the remaining -1 of eq 16's diagonal are the library's business, not this module's)."""
+    from . import stress_from_sums
+    return stress_from_sums(sums, n_chains_total)

@@ -59,3 +59,18 @@ def compare_state(e, g, upto_step=None):
     good, worst_a = close(Ag[ok][occ], e.A[ok][occ])
     assert good, "anchors off by %.3g" % worst_a
     return int(ok.sum()), max(worst, worst_a)
+
+
+def compare_chain_stress_sums(e, g):
+    """North_star: "per-step stress within 1e-5 relative over the first 1000 steps".  With slip-springs on, a chain
+    that has met a fragile hop decision may have forked, so the recorded ENSEMBLE stress cannot be compared beyond the
+    first fragile step of any chain.  What can be compared at any step is the same sum restricted to the chains that
+    cannot have forked yet: the mean over those chains of the oracle's per-chain sigma, sigma^(v) (eqs 16, 76) against
+    the mean over the SAME chains of the GPU's ssm_chain_stress.  Returns (chains compared, worst ratio)."""
+    cs = g.chain_stress()                                   # [12][M] of the GPU's current state
+    ok = np.nonzero((e.first_fragile < 0) | (e.first_fragile >= e.step))[0]
+    want = np.array([np.concatenate(e.chain_stress(int(k))) for k in ok])
+    got = cs.T[ok].astype(np.float64)
+    good, worst = close(got.mean(0), want.mean(0))
+    assert good, "stress summed over the %d unforked chains off by %.3g (tolerance %.1g)" % (len(ok), worst, TOL)
+    return len(ok), worst

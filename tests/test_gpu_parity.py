@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 
 import oracle
-from parity_util import GUARD, TOL, close, compare_state, from_external, to_external, upload
+from parity_util import GUARD, TOL, close, compare_chain_stress_sums, compare_state, from_external, to_external, upload
 
 pytestmark = pytest.mark.gpu
 
@@ -123,6 +123,9 @@ def test_c1_tiny_equilibrium_ensemble(ssm):
         n, worst = compare_state(e, g)
         # expected cut-short chains ~ hop decisions x 2 x 2 GUARD ~ 20 per 1000 steps; more is a bug
         assert n >= M - (3 + upto // 20), (upto, n)
+        # the stress at this step, summed over the chains that cannot have forked, within 1e-5
+        ns, _ = compare_chain_stress_sums(e, g)
+        assert ns == n
     want = np.concatenate(wants)
     got = g.stress()
     first = e.first_fragile[e.first_fragile >= 0]
@@ -134,13 +137,22 @@ def test_c1_tiny_equilibrium_ensemble(ssm):
     assert np.abs(got - want).max() < 0.5
 
 
-@pytest.mark.parametrize("N,M,steps", [(16, 200, 300), (32, 100, 1000), (64, 33, 200), (128, 19, 200)])
-def test_slipspring_chains_all_sizes(ssm, N, M, steps):
+@pytest.mark.parametrize("N,M", [(16, 200), (32, 100), (64, 65), (128, 97)])
+def test_slipspring_chains_all_sizes(ssm, N, M):
+    """Every kernel size (G = 2, 4, 8, 16; ragged last tiles) over north_star's full window of 1000 steps, with
+    dumps at 1, 10, 100, 1000: S, Z bit-exact and R, A within 1e-5 on every chain up to its first fragile step,
+    and the stress summed over those chains within 1e-5 at every dump."""
+    steps = 1000
     e, g = _pair(ssm, N, M, steps, seed=7)
-    e.run(steps, guard=GUARD)
-    g.step(steps)
-    n, worst = compare_state(e, g)
-    assert n >= _min_unflagged(M, N, steps)
+    done = 0
+    for upto in (1, 10, 100, 1000):
+        e.run(upto - done, guard=GUARD)
+        g.step(upto - done)
+        done = upto
+        n, worst = compare_state(e, g)
+        assert n >= _min_unflagged(M, N, upto), (upto, n)
+        ns, _ = compare_chain_stress_sums(e, g)
+        assert ns == n
     # per-chain stresses of the final state on the chains that cannot have forked
     cs = g.chain_stress()
     ok = (e.first_fragile < 0)
@@ -158,6 +170,7 @@ def test_shear_flow(ssm):
     g.step(steps, shear_rate=0.1)
     n, worst = compare_state(e, g)
     assert n >= _min_unflagged(M, N, steps)
+    compare_chain_stress_sums(e, g)
     first = e.first_fragile[e.first_fragile >= 0]
     clean = int(first.min()) if first.size else steps
     ok, w = close(g.stress()[:clean], want[:clean])
@@ -211,8 +224,21 @@ def test_correlator_matches_oracle_on_identical_trajectories(ssm, M, offset, com
     t0, G0, se0 = corr.result(N, 0.1)
     t1, G1, se1 = g.gt()
     assert np.allclose(t0, t1)
-    assert np.allclose(G1, G0, rtol=0, atol=2e-4 * np.abs(G0).max())
     assert np.allclose(se1, se0, rtol=0.02, atol=1e-6)
+    # the raw sums, group by group and lag by lag, each against a bound of ITS OWN size: a product f g carries the
+    # fp32 error of the two stresses (relative 1e-5 of sqrt(<f^2><g^2>) at worst, TOL) and the 2^-16 fixed point
+    # of its sum; the errors of a bin's n products are independent in sign, so the bin's sum is good to
+    # TOL |sum| + 4 sqrt(n) (TOL <f g>_0 + 2^-17), <f g>_0 = the lag-0 mean product
+    so, sgo, co = corr.sums()
+    sg, cg = g.gt_sums()
+    assert np.array_equal(cg, co)                          # the host-side schedule counts the same products
+    used = co > 0
+    fg0 = so[:, 0, 0].sum() / co[:, 0, 0].sum()
+    bound = TOL * np.abs(so) + 4.0 * np.sqrt(co) * (TOL * fg0 + 2.0 ** -17)
+    assert np.all(np.abs(sg - so)[used] <= bound[used]), float((np.abs(sg - so)[used] / bound[used]).max())
+    # and G(t) itself lag by lag: the same bound summed over the groups
+    n_lag = co.sum(0)[co.sum(0) > 0]
+    assert np.all(np.abs(G1 - G0) <= TOL * np.abs(G0) + 4.0 * (TOL * fg0 + 2.0 ** -17) / (np.sqrt(n_lag) * N))
 
 
 def test_device_view_of_the_stress_sums_is_what_the_exchange_reduces(ssm):
@@ -243,3 +269,93 @@ def test_issue_rate_probe(ssm):
     R, A, S, step = g.get_state()          # the probe used the staging area only
     g2 = ssm.Ensemble(8, 64, seed=1)
     assert np.array_equal(R, g2.get_state()[0]) and np.array_equal(S, g2.get_state()[2])
+
+
+def test_set_state_rejects_malformed_slip_spring_indices(ssm):
+    """The checkpoint-restore path validates S on the device: occupied slots must be the leading ones and
+    hold bead indices 1..N.  A bad chain keeps its valid leading slots only, the call fails with SSM_EINVAL, and the
+    ensemble can still be stepped (no out-of-range scatter)."""
+    N, M = 20, 70                                          # ragged: 20 beads in 32 places
+    e = oracle.Ensemble(N, M, seed=3)
+    e.round_to_fp32()
+    R, A, S = to_external(e)
+    g = ssm.Ensemble(N, M, seed=3)
+    g.set_state(R, A, S, 0)                                # well-formed: accepted
+    for what in ("gap", "range"):
+        S2 = S.copy()
+        k = int(np.argmax(e.Z >= 2))
+        if what == "gap":
+            S2[e.Z[k] + 1, k] = 3                          # an occupied slot after an empty one
+        else:
+            S2[1, k] = N + 1                               # a bead index beyond the chain
+        with pytest.raises(ssm.SsmError) as err:
+            g.set_state(R, A, S2, 0)
+        assert err.value.code == ssm.SSM_EINVAL
+        Rb, Ab, Sb, _ = g.get_state()
+        want = S.copy()
+        if what == "range":
+            want[1:, k] = 0                                # the valid leading slot survives
+        assert np.array_equal(Sb, want)
+        g.step(40)                                         # still safe to step
+        assert g.get_state()[2].max() <= N
+        g.set_state(R, A, S, 0)                            # and a good state is accepted again
+
+
+def test_two_contexts_on_two_devices_in_one_process(ssm):
+    """The dynamic shared-memory attribute of the step kernel is per device: a second context on cuda:1 (first use
+    of FLOW 0 / 1 and of the non-ragged kernels there) must launch, and every call must run on its own device."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    out = []
+    for dev in ("cuda:0", "cuda:1"):
+        g = ssm.Ensemble(32, 300, seed=5, stress_every=1, stress_capacity=64, sample_every=10, corr_levels=3, device=dev)
+        g.step(20)
+        g.step(20, shear_rate=0.1)
+        out.append((g.get_state(), g.stress_sums(), g.gt_sums()[0], g.chain_stress()))
+    for a, b in zip(out[0][0][:3], out[1][0][:3]):
+        assert np.array_equal(a, b)
+    assert np.array_equal(out[0][1], out[1][1]) and np.array_equal(out[0][2], out[1][2]) and np.array_equal(out[0][3], out[1][3])
+
+
+def _nccl_rank(rank, world, port, q):
+    import os
+    import torch
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world), LOCAL_RANK=str(rank))
+    torch.cuda.set_device(rank)
+    dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", rank))
+    import paper_1106_2899_b200 as m
+    from paper_1106_2899_b200 import shard
+    M, N, steps = 1000, 16, 48
+    k0, k1 = shard.strong_range(M, rank, world)
+    st = torch.cuda.Stream()                                # the context's own stream, NOT the one NCCL syncs with
+    g = m.Ensemble(N, k1 - k0, seed=41, chain_offset=k0, stress_every=1, stress_capacity=steps, device="cuda:%d" % rank, stream=st)
+    g.step(steps)
+    sums = g.stress_sums_device(0, steps)
+    shard.allreduce_sums(sums, ctx=g)                       # orders the two streams with events (ssm_stream_wait_ctx)
+    out = g.stress_sums()                                   # on the ctx's stream, after the exchange
+    dist.destroy_process_group()
+    q.put((rank, out))
+
+
+def test_nccl_allreduce_of_two_shards_equals_the_single_gpu_sums(ssm):
+    """two NCCL ranks, each a contiguous shard of the global chain index on its own GPU and its own
+    stream; the in-place all-reduce of ssm_stress_sums_device gives, on both ranks, exactly the int64 sums of the
+    single-GPU run of the whole ensemble."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    ps = [ctx.Process(target=_nccl_rank, args=(r, 2, 29541, q)) for r in range(2)]
+    for p in ps:
+        p.start()
+    got = dict(q.get(timeout=300) for _ in ps)
+    for p in ps:
+        p.join(60)
+    ref = ssm.Ensemble(16, 1000, seed=41, stress_every=1, stress_capacity=48)
+    ref.step(48)
+    want = ref.stress_sums()
+    assert np.array_equal(got[0], want) and np.array_equal(got[1], want)

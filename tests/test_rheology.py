@@ -27,7 +27,9 @@ def test_oracle_against_maxwell_closed_forms():
     assert np.allclose(g2, g * x / (1 + x * x), rtol=2e-5, atol=1e-9)
     assert abs(ref.eta0(t, G) - g * tau) < 1e-6
     assert abs(ref.tau_d(t, G, 10.0, 60.0) - tau) < 1e-9
-    assert np.allclose(ref.dynamic_viscosity(g1, g2), g * x / np.sqrt(1 + x * x), rtol=2e-5)
+    # |eta*|(w) = g tau / sqrt(1 + w^2 tau^2): tends to eta0 = g tau as w -> 0 (what the Cox-Merz rule, eq 63, needs)
+    assert np.allclose(ref.dynamic_viscosity(g1, g2, w), g * tau / np.sqrt(1 + x * x), rtol=2e-5)
+    assert abs(ref.dynamic_viscosity(g1, g2, w)[0] - ref.eta0(t, G)) < 1e-3 * g * tau
 
 
 def test_oracle_against_the_rouse_spectrum():
@@ -57,6 +59,9 @@ def test_library_equals_oracle_on_the_multitau_grid():
     b1, b2 = ref.moduli(t, G, w)
     assert np.allclose(a1, b1, rtol=1e-12, atol=1e-14) and np.allclose(a2, b2, rtol=1e-12, atol=1e-14)
     assert abs(ssm.eta0(t, G) - ref.eta0(t, G)) < 1e-12
+    assert np.allclose(ssm.eta_star(t, G, w), ref.dynamic_viscosity(b1, b2, w), rtol=1e-12)
+    with pytest.raises(ssm.SsmError):
+        ssm.eta_star(t, G, [0.0])
     assert abs(ssm.tau_d(t, G, 100.0, 600.0) - ref.tau_d(t, G, 100.0, 600.0)) < 1e-9 * 150.0
     # ragged input: two lags; a window whose points are all non-positive
     assert abs(ssm.eta0([0.0, 2.0], [1.0, 0.5]) - 1.5) < 1e-15
@@ -78,3 +83,16 @@ def test_library_rejects_bad_tables():
         ssm.eta0([0.0], [1.0])
     with pytest.raises(ssm.SsmError):
         ssm.tau_d(t, G, 5.0, 1.0)
+
+
+def test_stress_from_sums_is_the_mean_with_the_diagonal_constant():
+    """ssm_stress_from_sums: value = sum / (2^18 M), sigma_aa one more -1 (eq 16: -N, the sums hold N - 1)."""
+    sums = np.arange(24, dtype=np.int64).reshape(2, 12) * (1 << 18) * 5
+    out = ssm.stress_from_sums(sums, 5)
+    want = np.arange(24, dtype=np.float64).reshape(2, 12)
+    want[:, :3] -= 1.0
+    assert np.array_equal(out, want)
+    from paper_1106_2899_b200 import shard
+    assert np.array_equal(shard.stress_means(sums, 5), want)
+    with pytest.raises(ssm.SsmError):
+        ssm.stress_from_sums(sums, 0)
