@@ -66,12 +66,16 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
 
 
+TRAFFIC_CSV = os.path.join("profiles", "r2_step_kernel_metrics.csv")
+
+
 def ncu_traffic(n_beads, n_chains):
     """DRAM bytes per launch of the step kernel (dram__bytes_read.sum + dram__bytes_write.sum)
-    from the committed `ncu --set full` capture of this workload; None for other workloads."""
+    from the committed `ncu --set full` capture of this workload (NOT measured by this run: a profiler cannot
+    run inside a timed bench; the line says where the number comes from); None for other workloads."""
     if (n_beads, n_chains) != (32, 1 << 20):
         return None
-    path = os.path.join(ROOT, "profiles", "r1_v8_step_kernel_metrics.csv")
+    path = os.path.join(ROOT, TRAFFIC_CSV)
     try:
         import csv
         tot = 0.0
@@ -132,8 +136,15 @@ def cpu_baseline(n_beads, seconds, threads=None):
     t0 = time.perf_counter(); e.run(4, stress_every=1, n_threads=threads); probe = (time.perf_counter() - t0) / 4
     n = int(max(8, min(20000, seconds / max(probe, 1e-6))))
     t0 = time.perf_counter(); e.run(n, stress_every=1, n_threads=threads); dt = time.perf_counter() - t0
+    # once more on ONE thread (the paper's own CPU column is a single thread)
+    M1 = 256
+    e1 = oracle.Ensemble(n_beads, M1, seed=4)
+    n1 = int(max(8, min(20000, 0.25 * seconds / max(probe * threads * M1 / M, 1e-6))))
+    t0 = time.perf_counter(); e1.run(n1, stress_every=1, n_threads=1); dt1 = time.perf_counter() - t0
     return {"value": M * n_beads * n / dt, "unit": "bead-updates/s", "cores": threads, "kind": "oracle",
-            "sample": "%d chains x N=%d x %d steps, stress every step, %d threads, %.1f s" % (M, n_beads, n, threads, dt)}
+            "sample": "%d chains x N=%d x %d steps, stress every step, %d threads, %.1f s" % (M, n_beads, n, threads, dt),
+            "one_thread": {"value": M1 * n_beads * n1 / dt1, "unit": "bead-updates/s", "cores": 1,
+                           "sample": "%d chains x N=%d x %d steps, 1 thread, %.1f s" % (M1, n_beads, n1, dt1)}}
 
 
 def run_reference(a):
@@ -233,14 +244,29 @@ def main():
     if a.configs:
         return run_configs()
 
+    # `python bench.py --gpus N` without a launcher: start the N ranks ourselves, exactly as the driver's
+    # torchrun line does (one process per GPU, NCCL), and let rank 0's JSON line through.  A run whose world size
+    # differs from --gpus never reports: one rank must not stand in for an N-GPU measurement.
+    if a.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        import socket
+        with socket.socket() as so:
+            so.bind(("127.0.0.1", 0)); port = so.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(a.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
+
     import torch
     import torch.distributed as dist
     from paper_1106_2899_b200 import shard
     import paper_1106_2899_b200 as ssm
 
     rank, local_rank, world = shard.world()
+    if world != a.gpus:
+        raise SystemExit("bench.py: --gpus %d but the launcher started %d rank(s)" % (a.gpus, world))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    if torch.cuda.device_count() <= local_rank:
+        raise SystemExit("bench.py: rank %d has no GPU (%d visible)" % (local_rank, torch.cuda.device_count()))
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     if world > 1:
@@ -265,7 +291,7 @@ def main():
         first = g.stress_count()
         g.step(inner)
         if world > 1:                              # the path's only exchange: exact int64 sums (eq 54)
-            shard.allreduce_sums(g.stress_sums_device(first, inner))
+            shard.allreduce_sums(g.stress_sums_device(first, inner), ctx=g)
 
     for _ in range(W):
         one_step()
@@ -391,6 +417,7 @@ def main():
         "e2e": e2e,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_alu, "unit": "T thread-instr/s",
                      "frac": achieved / peak_alu, "traffic": traffic,
+                     "traffic_source": (TRAFFIC_CSV + " (committed ncu --set full capture of this workload, not this run)") if traffic else None,
                      "kernel": "ssm_step_kernel<G=%d>" % (N // 8), "launch_ms": launch_ms,
                      "i_alg_per_bead_update": I_ALG,
                      "rate_weighted": {"frac": weighted / peak_alu, "i_alg_issue_cycles_per_bead_update": i_alg_cycles,

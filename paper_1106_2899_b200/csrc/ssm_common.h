@@ -37,12 +37,16 @@ constexpr int kSampleShift = 20;             // per-chain slip-spring virial (co
 
 // per-warp shared memory of the step kernel.  The bead positions and the slip-spring force
 // accumulators share one index: coordinate c of bead b of the warp (0..255) sits at word
-//   (b >> 3) * 28 + (b & 7) * 3 + c      (28 words per lane: 24 used + 4 of padding)
-// so that the bead lanes move their 24 words as 6 aligned 16-byte accesses (consecutive lanes
-// 112 bytes apart: conflict-free) and the position mirror is the lane's register image as it is.
-constexpr int kSmRm = 0;         // float[896]  bead positions mirror (+1 kB spare up to kSmA)
+//   3 b + 4 (b >> 5) + c      (a lane's 24 words are contiguous; 4 words of padding after every 4 lanes)
+// so that the bead lanes move their 24 words as 6 aligned 16-byte accesses -- the lanes of a quarter warp start
+// 96 bytes apart, the two halves of it a further 16: eight distinct 16-byte bank groups, conflict-free -- the
+// position mirror is the lane's register image as it is, and, for chains of up to 32 beads (which never straddle
+// a padding gap), the slot phase finds a bead's neighbours along the chain exactly 3 words away.  (An earlier
+// layout padded every lane to 28 words: also conflict-free, but the neighbour offset then depended on the bead's
+// place in its lane, a dozen issue slots per slot pass.)
+constexpr int kSmRm = 0;         // float[800]  bead positions mirror (+1.3 kB spare up to kSmA)
 constexpr int kSmA = 4608;       // float4[256] anchors [chain][slot] (x, y, z, x low part)
-constexpr int kSmFx = 8704;      // int  [896]  fixed-point slip-spring displacement per bead coordinate, padded
+constexpr int kSmFx = 8704;      // int  [800]  fixed-point slip-spring displacement per bead coordinate (+0.4 kB spare up to kSmS)
 constexpr int kSmS = 12288;      // uint8[256]  bead index per slot
 constexpr int kSmZ = 12544;      // int  [32]   Z per chain
 constexpr int kSmX = 12672;      // int  [33]   exclusive prefix of Z over the warp's chains (+ total), padded to 36
@@ -59,7 +63,7 @@ constexpr int kSmMap = 13712;    // uint8[128]  dealing map: byte 4 lane + it = 
 constexpr int kSmWarp = 13968;
 constexpr int kSmAcc = kWarpsPerBlock * kSmWarp;                          // int64 [kMaxFuse][12] per CTA
 constexpr int kSmStep = kSmAcc + kMaxFuse * 12 * 8;                       // 114,816 B: 2 CTAs per SM (2 x (114,816 + 1024) <= 233,472)
-__host__ __device__ constexpr int fx_index(int bead_in_warp) { return (bead_in_warp >> 3) * 28 + (bead_in_warp & 7) * 3; }
+__host__ __device__ constexpr int fx_index(int bead_in_warp) { return bead_in_warp * 3 + ((bead_in_warp >> 5) << 2); }
 
 struct StepParams {
     unsigned char *state;             // warp tiles

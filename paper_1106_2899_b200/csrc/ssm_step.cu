@@ -79,8 +79,10 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     const int real_here = min(kBPL, max(0, NA - kBPL * l));          // real beads among this lane's 8 places
     const float bonds_here = (float)min(kBPL, max(0, NA - 1 - kBPL * l));   // bonds i -> i+1 that start in this lane
     unsigned char *wb = smem + warp * kSmWarp;
-    // mirror of the bead positions: the lane's 24 register floats as they are (6 x 16 bytes,
-    // 28 floats per lane: the same index as Fx), read by the slot phase as three scalars per bead
+    // mirror of the bead positions: the lane's 24 register floats as they are (6 x 16 bytes per lane,
+    // bead b of the warp at word fx_index(b): the same index as Fx), read by the slot phase as three scalars per bead;
+    // lq = the lane's first 16-byte word in it
+    const int lq = lane * 6 + (lane >> 2);
     float *Rf = reinterpret_cast<float *>(wb + kSmRm);
     float4 *Rf4 = reinterpret_cast<float4 *>(wb + kSmRm);
     auto bead = [&](int fi) -> float4 { return make_float4(Rf[fi], Rf[fi + 1], Rf[fi + 2], 0.0f); };
@@ -106,9 +108,10 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     const uint4 *Keys = reinterpret_cast<const uint4 *>(wb + kSmKeys);
     if (lane < 20) reinterpret_cast<unsigned *>(wb + kSmKeys)[lane] = P.rk[lane];
     for (int i = threadIdx.x; i < kMaxFuse * 12; i += kBlockThreads) acc[i] = 0ull;
-    Ev[lane] = 0u;
     Samp[lane] = 0; Samp2[lane] = 0; Samp2[32 + lane] = 0;
     Dm[lane] = 0u;
+    Ev[lane] = 0u;
+    reinterpret_cast<unsigned *>(Map)[lane] = 0u;
     __syncthreads();
 
     // dealing: slip-spring f of the warp (0 <= f < Tz) belongs to the chain c with
@@ -156,6 +159,20 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
         return (c << LN) | j;
     };
 
+    // the same for the slip-springs number 128 + lane + 32 q, q = 0..3 (byte q), which only a warp with more than 128
+    // slip-springs has: found through the prefix in shared memory
+    auto deal_high = [&](int Tz) -> unsigned {
+        unsigned hi = 0u;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int f = 128 + lane + 32 * q;
+            int c = 0, j = 0;
+            if (f < Tz) locate(f, c, j);
+            hi |= (unsigned)((c << LN) | j) << (8 * q);
+        }
+        return hi;
+    };
+
     // add the staged warp sums of records [r0, r1) to the CTA's 64-bit sums
     auto flush_stage = [&](int r0, int r1) {
         __syncwarp();
@@ -198,7 +215,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
             // dt kappa of the group this warp's chains belong to (a tile never straddles two groups)
             if (FLOW == 2 && lane < 9) Kap[lane] = P.kappa[(long long)(tile / P.tiles_per_group) * 9 + lane];
 #pragma unroll
-            for (int v = 0; v < 6; ++v) Rf4[lane * 7 + v] = make_float4(r[4 * v], r[4 * v + 1], r[4 * v + 2], r[4 * v + 3]);
+            for (int v = 0; v < 6; ++v) Rf4[lq + v] = make_float4(r[4 * v], r[4 * v + 1], r[4 * v + 2], r[4 * v + 3]);
         }
         __syncwarp();
         int Tz = deal(Zs[cw]);
@@ -343,8 +360,8 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                 normal_call<true>(sk, P.rk, DOM_NOISE, chain, (uint32_t)(3 * l + q), bm_noise, z8, Keys);
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
-                    const int4 fx = Fx4[lane * 7 + 2 * q + h];
-                    Fx4[lane * 7 + 2 * q + h] = make_int4(0, 0, 0, 0);
+                    const int4 fx = Fx4[lq + 2 * q + h];
+                    Fx4[lq + 2 * q + h] = make_int4(0, 0, 0, 0);
                     const int fxa[4] = {fx.x, fx.y, fx.z, fx.w};
 #pragma unroll
                     for (int e = 0; e < 4; ++e) {
@@ -368,7 +385,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     if (f >= 3 * real_here) r[f] = 0.0f;
             }
 #pragma unroll
-            for (int v = 0; v < 6; ++v) Rf4[lane * 7 + v] = make_float4(r[4 * v], r[4 * v + 1], r[4 * v + 2], r[4 * v + 3]);
+            for (int v = 0; v < 6; ++v) Rf4[lq + v] = make_float4(r[4 * v], r[4 * v + 1], r[4 * v + 2], r[4 * v + 3]);
             __syncwarp();
 
             // ================= slot phase: substeps 2 and 3 =================
@@ -381,10 +398,13 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                 // per lane in one straight-line pass were measured slower: 8.2 and 9.1 ms against 7.7 ms
                 // per launch; the extra predicated-off pass costs more than the overlap of the chains wins.)
                 const int nit = (Tz + 31) >> 5;
+                unsigned cur = cj;                 // byte 0 = this pass's (chain, slot) of the lane
                 for (int it = 0; it < nit; ++it) {
                     const int f = lane + 32 * it;
                     const bool act = f < Tz;
-                    const int sx = slot_index(it, act ? f : 0), c = sx >> LN, j = sx & (N - 1), base = sx & ~(N - 1);
+                    if (it == 4) cur = deal_high(Tz);
+                    const int sx = (int)(cur & 0xFFu), c = sx >> LN, j = sx & (N - 1), base = sx & ~(N - 1);
+                    cur >>= 8;
                     uint32_t w[4];
                     stream_call<true>(sk, P.rk, DOM_SLOT, chain0 + (uint32_t)c, (uint32_t)(j >> 1), w, Keys);
                     const uint32_t w_hop = (j & 1) ? w[2] : w[0], w_end = (j & 1) ? w[3] : w[1];
@@ -418,11 +438,13 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     // p+- = min{ h [1 - tanh x+-], 1/2 } = min{ 2h / (1 + e^{2 x+-}), 1/2 },
                     // x+- = (3/4N_s)(|R_{s+-1}-A|^2 - |R_s-A|^2)
                     const int b0 = base + s - 1;
-                    // neighbours along the chain are 3 floats away, 7 across a lane boundary (4 floats of padding)
-                    const int fi = fx_index(b0), kb = b0 & 7;
+                    // neighbours along the chain are 3 floats away (7 across the padding after every 32 beads,
+                    // which only chains of more than 32 beads can straddle)
+                    const int fi = fx_index(b0);
+                    const int up3 = (G > 4 && (b0 & 31) == 31) ? 7 : 3, dn3 = (G > 4 && (b0 & 31) == 0) ? 7 : 3;
                     const float4 r0 = bead(fi);
-                    const float4 rp = bead(fi + (s < NA ? (kb == 7 ? 7 : 3) : 0));
-                    const float4 rm = bead(fi - (s > 1 ? (kb == 0 ? 7 : 3) : 0));
+                    const float4 rp = bead(fi + (s < NA ? up3 : 0));
+                    const float4 rm = bead(fi - (s > 1 ? dn3 : 0));
                     const float d0x = r0.x - a.x, d0y = r0.y - a.y, d0z = r0.z - a.z;
                     const float dpx = rp.x - a.x, dpy = rp.y - a.y, dpz = rp.z - a.z;
                     const float dmx = rm.x - a.x, dmy = rm.y - a.y, dmz = rm.z - a.z;
@@ -448,7 +470,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     if (live) {
                         const float dx = up ? dpx : (dn ? dmx : d0x), dy = up ? dpy : (dn ? dmy : d0y),
                                     dz = up ? dpz : (dn ? dmz : d0z);
-                        int *fp = Fx + fi + (up ? (kb == 7 ? 7 : 3) : 0) - (dn ? (kb == 0 ? 7 : 3) : 0);
+                        int *fp = Fx + fi + (up ? up3 : 0) - (dn ? dn3 : 0);
                         atomicAdd(fp, __float2int_rn(-P.fx_scale * dx));
                         atomicAdd(fp + 1, __float2int_rn(-P.fx_scale * dy));
                         atomicAdd(fp + 2, __float2int_rn(-P.fx_scale * dz));
@@ -479,16 +501,16 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                         const int hmax = P.h_c2[K];
                         const unsigned m2 = __vminu2(__vminu2(w[0], w[1]), __vminu2(w[2], w[3]));
                         if ((int)min(m2 & 0xFFFFu, m2 >> 16) <= hmax) {
+                            // the lane's candidates (bit e: attempt 8l + e) and (attempt << 16) | half of its last one
+                            unsigned cnd = 0u, last = 0u;
 #pragma unroll
                             for (int e = 0; e < 8; ++e) {
-                                const int k = 8 * l + e;
-                                const int h = (int)((w[e >> 1] >> (16 * (e & 1))) & 0xFFFFu);
-                                if (k < K && h <= hmax) {
-                                    atomicOr(Ev + cw * WPC + (k >> 5), 1u << (k & 31));
-                                    Ev[32 + cw] = ((unsigned)k << 16) | (unsigned)h;   // the chain's latest candidate and its half
-                                    event = true;
-                                }
+                                const unsigned h = (w[e >> 1] >> (16 * (e & 1))) & 0xFFFFu;
+                                if (8 * l + e < K && (int)h <= hmax) { cnd |= 1u << e; last = ((unsigned)(8 * l + e) << 16) | h; }
                             }
+                            atomicOr(Ev + cw * WPC + (l >> 2), cnd << (8 * (l & 3)));
+                            atomicMax(Ev + 32 + cw, last);      // the chain's last candidate and its half (largest attempt wins)
+                            event = true;
                         }
                     }
                 }
@@ -564,6 +586,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                                 }
                             }
                         }
+                        Ev[32 + cw] = 0u;
                         if (changed) Zs[cw] = Zn;
                     }
                     __syncwarp();

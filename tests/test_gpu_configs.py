@@ -60,8 +60,9 @@ def test_c2_equilibrium_gt_full_size_and_depth(ssm):
     z = _z_report("C2", t_g, G_g, se_g, t_o, G_o, se_o)
     assert z.size >= 16 + 9 * 8
     assert np.mean(np.abs(z) < 3.0) >= 0.95 and np.abs(z).max() < 4.5, z
-    # pin P7: N G(0) = <s_xy (s_xy + sv_xy)> = N - 1 up to the O(dt) bias of the Euler map
-    assert abs(G_g[0] * N - (N - 1)) < 0.06 * (N - 1)
+    # pin P7 with the Euler map's O(dt) bias: N G(0) = <s_xy (s_xy + sv_xy)> = sum_p 1/(1 - k_p dt/2)^2 = 15.964
+    # (N - 1 = 15 in the limit dt -> 0; the slip-springs leave the equal-time value alone, eq 13)
+    assert abs(G_g[0] * N - 15.964) < 0.02 * 15.964, G_g[0] * N
     # G(t) has decayed to noise at the longest lags: the deep levels hold what the schedule says they hold
     s, c = g.gt_sums()
     n_samples = 100000
@@ -124,29 +125,34 @@ def test_c3_startup_shear_four_rates_full_size(ssm):
         assert np.mean(np.abs(z) < 3.0) >= 0.95 and np.abs(z).max() < 6.0, (rate, np.abs(z).max())
 
     # ---- 1e-3, 1e-4: common-random-number differencing against the twin, and linear response
-    keep = G_c > -1.0
+    # int_0^t G by the trapezoidal rule on the correlator's lags.  Two O(dt) effects bound how closely eta+ can follow
+    # it, both properties of the explicit Euler scheme the paper uses, not of either program: the scheme's
+    # stationary law is not the Boltzmann one, so the equal-time correlation N G(0) = sum_p 1/(1 - k_p dt/2)^2 sits
+    # 3 % above the true response to a strain step, 3 <sum b_y^2> = sum_p 1/(1 - k_p dt/2); and the
+    # lags are 10 dt apart where G falls from 1.04 to 0.45 within the first one.  Tolerance: 6 % of int G beyond
+    # t = 3 tau0, 12 % before, plus the statistical error.
     cum = np.concatenate([[0.0], np.cumsum(0.5 * (G_c[1:] + G_c[:-1]) * np.diff(t_c))])        # int_0^t G, trapezoid
-    eta_lr = np.interp(t, t_c[keep], cum[keep])
+    eta_lr = np.interp(t, t_c, cum)
     eta0 = cum[-1]
+    tau_c = 25.0                                                       # correlation time of the ensemble stress ~ tau_d
     for rate in (1e-3, 1e-4):
         eta = (curves[rate] - curves[0.0]) / (N * rate)
-        # (i) while the twin trajectories still coincide the difference is nearly noise-free: the first 2 tau0 pin
-        # the whole linear-response pipeline sharply (leaving sigma^(v) out of eq 43 would be off by 25 %)
-        early = slice(0, 20)
-        rel = np.abs(eta[early] - eta_lr[early]) / eta_lr[early]
-        # (ii) later the twins decorrelate (hop decisions fork) and the difference carries the noise of two
-        # independent ensembles: its size is read off the stationary tail, where eta+ has reached eta0
-        tail = slice(steps // every // 2, None)
-        noise = eta[tail].std()
-        z = (eta - eta_lr) / noise
-        print("C3 rate %g (CRN): early |eta+ - int G| / int G max %.3f; eta+ tail mean %.3f vs eta0 = int G = %.3f; "
-              "tail noise per sample %.3f; |z| < 3 on %.1f %%"
-              % (rate, rel.max(), eta[tail].mean(), eta0, noise, 100.0 * np.mean(np.abs(z) < 3.0)))
-        assert rel.max() < 0.05, (rate, rel)
-        assert np.mean(np.abs(z) < 3.0) >= 0.97
-        # the plateau: the mean over the tail (1e4 samples, correlated over ~ tau_d) against eta0
-        n_eff = (t[-1] - t[tail][0]) / 40.0                            # ~ independent stretches of 2 tau_d
-        assert abs(eta[tail].mean() - eta0) < 0.05 * eta0 + 4.0 * noise / math.sqrt(n_eff), (rate, eta[tail].mean(), eta0)
+        # (i) the first 3 tau0: most twin chains still coincide, the difference is nearly noise-free and pins the whole
+        # linear-response pipeline (leaving sigma^(v) out of eq 43 would be off by 25 %)
+        early = slice(4, 30)
+        r_early = eta[early].mean() / eta_lr[early].mean()
+        # (ii) later the twins decorrelate (hop decisions fork) and the difference carries the noise of two independent
+        # ensembles, correlated over ~ tau_d: windows of growing length, each against its own standard error
+        rows = []
+        for a, b in ((30, 100), (100, 300), (300, 1000), (1000, 3000), (3000, 10000), (10000, 20000)):
+            w = eta[a:b]
+            se = w.std() * math.sqrt(min(1.0, 2.0 * tau_c / ((b - a) * every * 0.01)))
+            rows.append((t[a], t[b - 1], w.mean(), eta_lr[a:b].mean(), se))
+        print("C3 rate %g (CRN): eta+ / int G over 0.5 <= t <= 3: %.3f; windows (t0, t1, eta+, int G, SE): %s; eta0 = %.3f"
+              % (rate, r_early, [tuple(round(float(x), 3) for x in r) for r in rows], eta0))
+        assert abs(r_early - 1.0) < 0.12, (rate, r_early)
+        for t0, t1, m, lr, se in rows:
+            assert abs(m - lr) < 0.06 * lr + 4.0 * se, (rate, t0, t1, m, lr, se)
     # shear thinning and overshoot at the fast rate, Newtonian plateau at the slow ones (Fig 4)
     e1 = curves[1e-1] / (N * 1e-1)
     assert e1.max() > 1.1 * e1[-2000:].mean() and e1[-2000:].mean() < 0.8 * eta0
@@ -168,7 +174,7 @@ def test_c5_long_chains_gt_and_shear(ssm):
     z = _z_report("C5", t_g, G_g, se_g, t_o, G_o, se_o)
     assert z.size >= 16 + 8 * 8
     assert np.mean(np.abs(z) < 3.0) >= 0.95 and np.abs(z).max() < 4.5, z
-    assert abs(G_g[0] * N - (N - 1)) < 0.04 * (N - 1)                # pin P7 (Euler bias 1.5 % at dt = 0.005)
+    assert abs(G_g[0] * N - 130.943) < 0.02 * 130.943, G_g[0] * N    # pin P7 with the Euler bias at dt = 0.005
     # entangled plateau: G(t) ~ 0.1 rho0 kT for large N at intermediate times
     mid = (t_g > 20.0) & (t_g < 60.0)
     print("C5 plateau: G(20 < t < 60) = %s" % np.round(G_g[mid], 3))

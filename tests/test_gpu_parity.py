@@ -137,16 +137,19 @@ def test_c1_tiny_equilibrium_ensemble(ssm):
     assert np.abs(got - want).max() < 0.5
 
 
-@pytest.mark.parametrize("N,M", [(16, 200), (32, 100), (64, 65), (128, 97)])
+@pytest.mark.parametrize("N,M", [(16, 1003), (32, 1001), (64, 1001), (128, 1031)])
 def test_slipspring_chains_all_sizes(ssm, N, M):
     """Every kernel size (G = 2, 4, 8, 16; ragged last tiles) over north_star's full window of 1000 steps, with
     dumps at 1, 10, 100, 1000: S, Z bit-exact and R, A within 1e-5 on every chain up to its first fragile step,
-    and the stress summed over those chains within 1e-5 at every dump."""
+    and the stress summed over those chains within 1e-5 at every dump.  (A thousand chains, as in the Rouse-limit
+    test: the stress is an ensemble quantity, eq 54 -- one chain's 3 sum b_a b_b carries the fp32 rounding of
+    its N - 1 bonds, ~1e-4 at N = 128, and it is the mean over the ensemble that north_star
+    bounds; at N = 128 a quarter of the chains are still unforked at step 1000.)"""
     steps = 1000
     e, g = _pair(ssm, N, M, steps, seed=7)
     done = 0
     for upto in (1, 10, 100, 1000):
-        e.run(upto - done, guard=GUARD)
+        e.run(upto - done, guard=GUARD, n_threads=8)
         g.step(upto - done)
         done = upto
         n, worst = compare_state(e, g)
