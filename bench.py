@@ -31,8 +31,9 @@ if ROOT not in sys.path:
 # (DESIGN.md section 9.2).  The roofline numerator is I_ALG x bead-updates/s, NOT the number
 # of instructions the kernel happens to execute, so padding cannot raise the fraction.
 I_ALG = 95.0
-# of which 32 x 32 -> 64-bit multiplies (IMAD.WIDE) of Philox: 0.594 calls x 20.  They are not full-rate
-# instructions on B200; ssm_issue_rates() measures their cost live for the rate-weighted fraction.
+# of which 32 x 32 -> 64-bit multiplies (IMAD.WIDE) of Philox: 0.594 calls x 20.  On B200 each of them holds the issue
+# port for about three cycles beyond its own slot (other instructions do not overlap it: profiles/r2_issue_model.md);
+# ssm_issue_rates() measures that cost live for the rate-weighted fraction.
 I_ALG_WIDE = 0.59375 * 20.0
 N_SM, SMSP_PER_SM, LANES = 148, 4, 32
 

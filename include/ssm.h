@@ -198,18 +198,21 @@ int ssm_gt(ssm_ctx *ctx, int32_t *n_lags, double *h_lag_time, double *h_G, doubl
 int ssm_gt_virtual(ssm_ctx *ctx, int32_t *n_lags, double *h_lag_time, double *h_dgv, double *h_se);
 int ssm_gt_sums_virtual(ssm_ctx *ctx, double *h_sum_gg);
 
-/* DIAGNOSTIC, not part of the hot path (bench.py prints it beside the roofline): measured cycles per warp instruction per
- * scheduler, at the step kernel's residency (4 warps per scheduler), of h_cycles[0] FFMA,
- * [1] LOP3/IADD3/SHF, [2] IMAD, [3] IMAD.WIDE (the 32 x 32 -> 64-bit multiply of Philox).
- * Runs four short kernels on the ctx's stream, uses the workspace's staging area (nothing of
- * the ensemble is touched) and synchronises.  h_cycles (host)[4]. */
+/* DIAGNOSTIC, not part of the hot path (bench.py prints it beside the roofline): cycles per
+ * group of instructions per scheduler, measured at the step kernel's residency (4 warps per scheduler):
+ * h_cycles (host)[8] = [0] FFMA, [1] LOP3 (ALU pipe), [2] IMAD, [3] IMAD.WIDE + the LOP3 folding its halves,
+ * [4] the same + 4 FFMA (they do not hide under the multiply: it holds the issue port), [5] MUFU, [6] I2FP + F2I,
+ * [7] the instructions of one Philox round (2 multiplies, 2 LOP3).  Runs short kernels on the ctx's stream, uses the workspace's staging
+ * area (nothing of the ensemble is touched) and synchronises. */
 int ssm_issue_rates(ssm_ctx *ctx, double *h_cycles);
 
 /* Host post-processing of a tabulated G(t) (section 4.1); no device work, no ctx.
  * h_t[n_lags] strictly increasing lag times >= 0 (as ssm_gt returns them), h_G[n_lags].  All (host).
  *  ssm_moduli : storage and loss moduli, eqs (55), (56), by the trapezoidal rule the paper names
  *               (P:L392), the integral truncated at the last lag: h_storage[q] = G'(h_omega[q]),
- *               h_loss[q] = G''(h_omega[q]).
+ *               h_loss[q] = G''(h_omega[q]).  (On the lags of ssm_gt, whose spacing doubles from level to level, the
+ *               rule follows sin(w t), cos(w t) only while w times the spacing is small at the lags where G still
+ *               matters: w up to about 0.1 / tau0 for the entangled chains of the paper.)
  *  ssm_eta_star : dynamic viscosity of eq (64) for the Cox-Merz comparison of eq (63):
  *               h_eta_star[q] = sqrt(G'^2 + G''^2) / w at w = h_omega[q] > 0.  (The printed eq (64) lacks the
  *               1/w; eq (63) cannot hold without it -- for w -> 0 only sqrt(..)/w tends to eta_0.)

@@ -22,13 +22,20 @@ K_EMPTY, K_ONE = 0, 1
 
 
 def build(force=False):
-    """Compile the oracle with gcc (no fast-math, no FMA contraction)."""
+    """Compile the oracle with gcc (no fast-math, no FMA contraction).  ORACLE_SANITIZE=1 in the environment builds
+    it with -fsanitize=address,undefined into a library of its own (run the tests with libasan preloaded:
+    LD_PRELOAD=$(gcc -print-file-name=libasan.so) ORACLE_SANITIZE=1 python -m pytest tests -m "not gpu" -k oracle)."""
+    global _LIB
+    san = os.environ.get("ORACLE_SANITIZE") == "1"
+    if san:
+        _LIB = os.path.join(_HERE, "liboracle_ssm_san.so")
     if (not force and os.path.exists(_LIB)
             and os.path.getmtime(_LIB) >= max(os.path.getmtime(_SRC),
                                               os.path.getmtime(os.path.join(_HERE, "ssm_oracle.h")))):
         return _LIB
-    cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fPIC", "-shared", "-pthread",
-           "-o", _LIB, _SRC, "-lm"]
+    cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fPIC", "-shared", "-pthread"] \
+        + (["-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"] if san else []) \
+        + ["-o", _LIB, _SRC, "-lm"]
     subprocess.check_call(cmd)
     return _LIB
 

@@ -46,7 +46,8 @@ def lib():
     global _lib
     if _lib is not None:
         return _lib
-    path = _build.build()
+    # SSM_LIB=check in the environment loads libssm_check.so: the same library with device-side assertions
+    path = _build.build(check=os.environ.get("SSM_LIB") == "check")
     L = C.CDLL(path)
     PP, vp, dp, fp = C.POINTER(Params), C.c_void_p, C.POINTER(C.c_double), C.c_void_p
     L.ssm_workspace_bytes.argtypes = [PP]; L.ssm_workspace_bytes.restype = C.c_size_t
@@ -331,11 +332,14 @@ class Ensemble:
         self._ck(lib().ssm_set_fusion(self.h, steps_per_launch))
 
     def issue_rates(self):
-        """ssm_issue_rates: cycles per warp instruction per scheduler of FFMA, LOP3-class, IMAD, IMAD.WIDE."""
-        out = np.zeros(4)
-        with self._torch.cuda.device(self.device):
+        """ssm_issue_rates (diagnostic): cycles per instruction group per scheduler; imad_wide = the issue cycles one
+        32 x 32 -> 64-bit multiply occupies inside a Philox round (the round's cycles minus one slot for each of its
+        two LOP3, halved)."""
+        out = np.zeros(8)
+        with self._dev():
             self._ck(lib().ssm_issue_rates(self.h, out.ctypes.data_as(C.POINTER(C.c_double))))
-        return {"ffma": out[0], "alu": out[1], "imad": out[2], "imad_wide": out[3]}
+        return {"ffma": out[0], "alu": out[1], "imad": out[2], "imad_wide": 0.5 * (out[7] - 2.0), "wide_lop3": out[3],
+                "wide_lop3_4ffma": out[4], "mufu": out[5], "i2f_f2i": out[6], "philox_round": out[7]}
 
     def stream_wait_ctx(self, stream):
         """ssm_stream_wait_ctx: later work on `stream` (a torch.cuda.Stream) waits for this context's queued work."""

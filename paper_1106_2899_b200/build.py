@@ -1,6 +1,6 @@
 """Build libssm.so (the C-ABI library of include/ssm.h) in-tree with nvcc for sm_100a.
 
-    python -m paper_1106_2899_b200.build [--force]
+    python -m paper_1106_2899_b200.build [--force] [--check]
 
 nvcc cross-compiles without a GPU.  The .so is git-ignored but travels with gpurun.
 """
@@ -12,6 +12,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libssm.so")
+LIB_CHECK = os.path.join(_HERE, "libssm_check.so")       # the same sources with -DSSM_CHECK: device-side assertions on
 SOURCES = ["ssm_step.cu", "ssm_aux.cu", "ssm_api.cu", "ssm_rheo.cu"]
 STEP_G = [1, 2, 4, 8, 16]       # ssm_step.cu is also compiled once per G (-DSSM_G): the kernels of 8G bead places
 OBJ = os.path.join(_HERE, "build")
@@ -27,23 +28,28 @@ def nvcc():
     return exe
 
 
-def stale():
-    if not os.path.exists(LIB):
+def stale(lib=None):
+    lib = lib or LIB
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
+    t = os.path.getmtime(lib)
     deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.abspath(__file__)]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force=False, verbose=False):
-    """Compile csrc/*.cu into libssm.so; returns its path."""
-    if not force and not stale():
-        return LIB
+def build(force=False, verbose=False, check=False):
+    """Compile csrc/*.cu into libssm.so (check=True: into libssm_check.so with the device-side assertions of
+    ssm_common.h compiled in); returns its path."""
+    lib = LIB_CHECK if check else LIB
+    if not force and not stale(lib):
+        return lib
     from concurrent.futures import ThreadPoolExecutor
-    os.makedirs(OBJ, exist_ok=True)
+    obj = OBJ + ("_check" if check else "")
+    os.makedirs(obj, exist_ok=True)
     exe = nvcc()
-    units = [(f, [], os.path.join(OBJ, f[:-3] + ".o")) for f in SOURCES]
-    units += [("ssm_step.cu", ["-DSSM_G=%d" % g], os.path.join(OBJ, "ssm_step_g%d.o" % g)) for g in STEP_G]
+    extra = ["-DSSM_CHECK"] if check else []
+    units = [(f, extra, os.path.join(obj, f[:-3] + ".o")) for f in SOURCES]
+    units += [("ssm_step.cu", extra + ["-DSSM_G=%d" % g], os.path.join(obj, "ssm_step_g%d.o" % g)) for g in STEP_G]
 
     def compile_one(u):
         src, defs, obj = u
@@ -55,14 +61,14 @@ def build(force=False, verbose=False):
 
     with ThreadPoolExecutor(max_workers=min(len(units), os.cpu_count() or 1)) as ex:
         logs = list(ex.map(compile_one, units))
-    cmd = [exe] + NVCC_FLAGS + ["-shared", "-o", LIB] + [u[2] for u in units]
+    cmd = [exe] + NVCC_FLAGS + ["-shared", "-o", lib] + [u[2] for u in units]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError("nvcc link failed:\n" + " ".join(cmd) + "\n" + r.stdout + r.stderr)
     if verbose:
         sys.stderr.write("".join(logs))
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose=True))
+    print(build(force="--force" in sys.argv, verbose=True, check="--check" in sys.argv))

@@ -18,7 +18,7 @@ namespace ssm {
 cudaError_t step_occupancy(int n_beads, int *blocks_per_sm);
 cudaError_t launch_step(int n_beads, const StepParams &p, int grid, cudaStream_t st);
 cudaError_t launch_init(const InitParams &p, cudaStream_t st);
-cudaError_t measure_rates(unsigned *d_scratch, int blocks, cudaStream_t st, double cycles[4]);
+cudaError_t measure_rates(unsigned *d_scratch, int blocks, cudaStream_t st, double cycles[8]);
 cudaError_t launch_xfer(bool do_export, unsigned char *state, float *R, float *A, unsigned char *S, int N,
                         long long k0, long long nk, long long pitch, int hide_low, int *bad_state, cudaStream_t st);
 cudaError_t launch_clear_low(unsigned char *state, long long n_tiles, cudaStream_t st);
@@ -285,7 +285,11 @@ static int step_impl(ssm_ctx *c, int64_t n_steps, double shear_rate, const float
     }
     long long left = n_steps;
     while (left > 0) {
-        const int T = (int)(left < c->fuse ? left : c->fuse);
+        int T = (int)(left < c->fuse ? left : c->fuse);
+        // a launch never crosses a multiple of 2^32 steps: the kernel forms the part of its Philox calls that depends
+        // on the step's high bits once per tile (ssm_rng.cuh, stream_prefix)
+        const long long to_wrap = 0x100000000ll - (c->step & 0xFFFFFFFFll);
+        if (T > to_wrap) T = (int)to_wrap;
         sp.step0 = (unsigned long long)c->step; sp.n_fuse = T;
         long long nrec = 0, nsmp = 0;
         if (p.stress_every > 0) nrec = (c->step + T) / p.stress_every - c->step / p.stress_every;
@@ -599,10 +603,7 @@ extern "C" int ssm_issue_rates(ssm_ctx *c, double *h_cycles)
     CK(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     const size_t need = (size_t)(1 + sms * 512) * sizeof(unsigned);
     if (need > c->lay.total - c->lay.stage) return fail(c, SSM_ENOMEM, "staging area too small for the issue-rate probe");
-    double raw[4];
-    CK(c, measure_rates(reinterpret_cast<unsigned *>(c->ws + c->lay.stage), sms, c->st, raw));
-    h_cycles[0] = raw[0]; h_cycles[1] = raw[1]; h_cycles[2] = raw[2];
-    h_cycles[3] = 2.0 * raw[3] - raw[1];          // the probe's pair is IMAD.WIDE + LOP3
+    CK(c, measure_rates(reinterpret_cast<unsigned *>(c->ws + c->lay.stage), sms, c->st, h_cycles));
     return SSM_OK;
 }
 

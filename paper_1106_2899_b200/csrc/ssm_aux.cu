@@ -110,6 +110,7 @@ __global__ void __launch_bounds__(256, 6) ssm_xfer_kernel(unsigned char *state, 
         const long long kk = cb + T * cpw + cw - k0;
         if (kk < 0 || kk >= nk) continue;
         float4 *p = reinterpret_cast<float4 *>(img + T * kTileBytes + kTileR) + v * 32 + lane;
+        SSM_ASSERT(T < nt && cw < cpw);
         float w[4];
         if (EXPORT) { const float4 t = *p; w[0] = t.x; w[1] = t.y; w[2] = t.z; w[3] = t.w; }
 #pragma unroll
@@ -126,6 +127,7 @@ __global__ void __launch_bounds__(256, 6) ssm_xfer_kernel(unsigned char *state, 
         const long long kk = cb + cl - k0;
         if (kk < 0 || kk >= nk) continue;
         float4 *p = reinterpret_cast<float4 *>(img + (cl >> sh) * kTileBytes + kTileA) + (cl & (cpw - 1)) * NP + j;
+        SSM_ASSERT((cl >> sh) < nt && j < NP);
         float w[4];
         if (EXPORT) { const float4 t = *p; w[0] = t.x; w[1] = t.y; w[2] = t.z; w[3] = t.w; }
         // (hide_low: the fourth word holds the packed low parts of ssm_step_kappa, not a float; export 0)
@@ -404,6 +406,7 @@ __global__ void __launch_bounds__(256) ssm_corr_kernel(const __grid_constant__ C
             const long long lm = (long long)lev * C.Mv + k;
             float *ring = C.ring + (long long)lev * Pb * C.Mv + k;
             const int p0 = pos[lev];
+            SSM_ASSERT(p0 >= 0 && p0 < Pb && k >= 0 && k < C.Mv && group >= 0 && group < C.groups);
             if (valid) ring[(long long)p0 * C.Mv] = g;
             if (fil[lev] < Pb) ++fil[lev];
             const int kmin = lev == 0 ? 0 : Pb / 2, kfil = fil[lev];
@@ -492,57 +495,85 @@ cudaError_t launch_corr(const CorrParams &c, cudaStream_t st)
 
 namespace ssm {
 // ---------------------------------------------------------------------------------------
-// Issue-rate probe: cycles per warp instruction per scheduler for the
-// instruction classes of the step kernel, measured with 4 warps per scheduler (the step
-// kernel's residency) and 4 independent chains per lane.  OP 0: FFMA, 1: LOP3/IADD3/SHF,
-// 2: IMAD, 3: IMAD.WIDE (+ one LOP3, subtracted on the host with the rate of OP 1).
+// Issue-rate probe (DIAGNOSTIC): cycles per group of instructions per scheduler, measured
+// at the step kernel's residency (4 warps per scheduler) with 4 independent chains per lane.  A group is
+//   NW x [IMAD.WIDE.U32 + the LOP3 that folds its two halves]  (the Philox round's pattern),
+//   NL x LOP3 (ALU pipe), NF x FFMA, NM x MUFU.EX2, NI x IMAD (low half), NY x [I2FP + F2I].
+// What the step kernel's roofline needs from it: the ALU pipe takes 2 cycles per LOP3-class instruction; IMAD 2;
+// the 32 x 32 -> 64-bit multiply holds the ISSUE port, not just its pipe -- FFMAs put beside it do not hide
+// (group of one multiply + n FFMA = multiply + n cycles), so each one costs ~3 issue cycles beyond its own slot.
 // ---------------------------------------------------------------------------------------
-template <int OP>
+template <int NW, int NL, int NF, int NM, int NI, int NY>
 __global__ void __launch_bounds__(512) ssm_rate_kernel(unsigned *out, int iters, unsigned seed)
 {
     constexpr int ILP = 4;
-    unsigned a[ILP], b[ILP]; float f[ILP], g[ILP];
+    unsigned a[ILP], l[ILP][4], im[ILP][2]; float f[ILP][4], m[ILP];
 #pragma unroll
-    for (int i = 0; i < ILP; ++i) { a[i] = seed + threadIdx.x * 7u + i; b[i] = seed * 3u + i; f[i] = a[i] * 1e-3f; g[i] = 1.0001f + i; }
+    for (int i = 0; i < ILP; ++i) {
+        a[i] = seed + threadIdx.x * 7u + i; m[i] = 0.5f + 1e-3f * threadIdx.x;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { l[i][j] = seed + 11u * j + i + threadIdx.x; f[i][j] = 1.0f + 1e-3f * (j + i + threadIdx.x); }
+        im[i][0] = seed + threadIdx.x; im[i][1] = seed * 5u + threadIdx.x;
+    }
     const long long t0 = clock64();
     for (int n = 0; n < iters; ++n) {
 #pragma unroll
         for (int i = 0; i < ILP; ++i) {
-            if (OP == 0) f[i] = fmaf(f[i], g[i], 0.5f);
-            if (OP == 1) { a[i] = (a[i] ^ b[i]) + 0x9E3779B9u; a[i] ^= a[i] >> 7; }
-            if (OP == 2) a[i] = a[i] * 0xD2511F53u + b[i];
-            if (OP == 3) { const unsigned long long p = (unsigned long long)a[i] * 0xD2511F53u; a[i] = (unsigned)(p >> 32) ^ (unsigned)p; }
+#pragma unroll
+            for (int w = 0; w < NW; ++w) a[i] = __umulhi(a[i], 0xD2511F53u) ^ (a[i] * 0xD2511F53u);
+#pragma unroll
+            for (int j = 0; j < NL; ++j) asm volatile("lop3.b32 %0, %0, %1, 0x9E3779B9, 0x96;" : "+r"(l[i][j & 3]) : "r"(l[i][(j + 1) & 3]));
+#pragma unroll
+            for (int j = 0; j < NF; ++j) asm volatile("fma.rn.f32 %0, %0, %1, %1;" : "+f"(f[i][j & 3]) : "f"(f[i][(j + 1) & 3]));
+#pragma unroll
+            for (int j = 0; j < NM; ++j) asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(m[i]));
+#pragma unroll
+            for (int j = 0; j < NI; ++j) asm volatile("mad.lo.u32 %0, %0, 0xCD9E8D57, %1;" : "+r"(im[i][j & 1]) : "r"(im[i][(j + 1) & 1]));
+#pragma unroll
+            for (int j = 0; j < NY; ++j) { float t; asm volatile("cvt.rn.f32.s32 %0, %1;" : "=f"(t) : "r"(l[i][j & 3])); asm volatile("cvt.rni.s32.f32 %0, %1;" : "=r"(l[i][j & 3]) : "f"(t)); }
         }
     }
     const long long t1 = clock64();
     unsigned r = 0;
 #pragma unroll
-    for (int i = 0; i < ILP; ++i) r += a[i] + b[i] + __float_as_uint(f[i]);
+    for (int i = 0; i < ILP; ++i) {
+        r += a[i] + __float_as_uint(m[i]) + im[i][0] + im[i][1];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) r += l[i][j] + __float_as_uint(f[i][j]);
+    }
     out[1 + blockIdx.x * blockDim.x + threadIdx.x] = r;
-    if (threadIdx.x == 0 && blockIdx.x == 0) out[0] = (unsigned)(t1 - t0);
+    if ((threadIdx.x & 31) == 0) atomicMax(out, (unsigned)(t1 - t0));      // the slowest warp of the grid
 }
 
-// out: device scratch of at least (1 + blocks * 512) words; cycles[4] as described above (raw,
-// per warp instruction of the loop body: 1, 4, 1 and 2 instructions per chain and iteration)
-cudaError_t measure_rates(unsigned *d_scratch, int blocks, cudaStream_t st, double cycles[4])
+template <int NW, int NL, int NF, int NM, int NI, int NY>
+static cudaError_t rate_one(unsigned *d_scratch, int blocks, cudaStream_t st, double *cycles_per_group)
 {
-    const int iters = 4000, ilp = 4, warps_per_smsp = 4;
-    const int per_iter[4] = {1, 4, 1, 2};
-    for (int op = 0; op < 4; ++op) {
-        for (int rep = 0; rep < 2; ++rep) {                      // first launch warms the instruction cache
-            switch (op) {
-                case 0: ssm_rate_kernel<0><<<blocks, 512, 0, st>>>(d_scratch, iters, 1u); break;
-                case 1: ssm_rate_kernel<1><<<blocks, 512, 0, st>>>(d_scratch, iters, 1u); break;
-                case 2: ssm_rate_kernel<2><<<blocks, 512, 0, st>>>(d_scratch, iters, 1u); break;
-                default: ssm_rate_kernel<3><<<blocks, 512, 0, st>>>(d_scratch, iters, 1u); break;
-            }
-        }
-        unsigned cyc = 0;
-        cudaError_t e = cudaMemcpyAsync(&cyc, d_scratch, sizeof cyc, cudaMemcpyDeviceToHost, st);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-        if (e != cudaSuccess) return e;
-        cycles[op] = (double)cyc / ((double)iters * ilp * per_iter[op] * warps_per_smsp);
-    }
+    const int iters = 2000, ilp = 4, warps_per_smsp = 4;
+    ssm_rate_kernel<NW, NL, NF, NM, NI, NY><<<blocks, 512, 0, st>>>(d_scratch, iters, 1u);      // warms the instruction cache
+    cudaError_t e = cudaMemsetAsync(d_scratch, 0, sizeof(unsigned), st);
+    if (e != cudaSuccess) return e;
+    ssm_rate_kernel<NW, NL, NF, NM, NI, NY><<<blocks, 512, 0, st>>>(d_scratch, iters, 1u);
+    unsigned cyc = 0;
+    e = cudaMemcpyAsync(&cyc, d_scratch, sizeof cyc, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return e;
+    *cycles_per_group = (double)cyc / ((double)iters * ilp * warps_per_smsp);
     return cudaGetLastError();
+}
+
+// out: device scratch of at least (1 + blocks * 512) words; cycles[8] = cycles per group of
+// [0] FFMA, [1] LOP3, [2] IMAD, [3] IMAD.WIDE + LOP3, [4] IMAD.WIDE + LOP3 + 4 FFMA, [5] MUFU, [6] I2FP + F2I,
+// [7] 2 x (IMAD.WIDE + LOP3): the instructions of one Philox round
+cudaError_t measure_rates(unsigned *d_scratch, int blocks, cudaStream_t st, double cycles[8])
+{
+    cudaError_t e;
+    if ((e = rate_one<0, 0, 1, 0, 0, 0>(d_scratch, blocks, st, cycles + 0)) != cudaSuccess) return e;
+    if ((e = rate_one<0, 1, 0, 0, 0, 0>(d_scratch, blocks, st, cycles + 1)) != cudaSuccess) return e;
+    if ((e = rate_one<0, 0, 0, 0, 1, 0>(d_scratch, blocks, st, cycles + 2)) != cudaSuccess) return e;
+    if ((e = rate_one<1, 0, 0, 0, 0, 0>(d_scratch, blocks, st, cycles + 3)) != cudaSuccess) return e;
+    if ((e = rate_one<1, 0, 4, 0, 0, 0>(d_scratch, blocks, st, cycles + 4)) != cudaSuccess) return e;
+    if ((e = rate_one<0, 0, 0, 1, 0, 0>(d_scratch, blocks, st, cycles + 5)) != cudaSuccess) return e;
+    if ((e = rate_one<0, 0, 0, 0, 0, 1>(d_scratch, blocks, st, cycles + 6)) != cudaSuccess) return e;
+    return rate_one<2, 0, 0, 0, 0, 0>(d_scratch, blocks, st, cycles + 7);
 }
 }  // namespace ssm

@@ -23,6 +23,16 @@
 #pragma once
 #include <cstdint>
 
+// Device-side assertions of the checked build (python -m paper_1106_2899_b200.build --check -> libssm_check.so,
+// loaded with SSM_LIB=check): every index the kernels form into the warp's shared memory and into the tiles is
+// tested against its bounds, and a violation traps (the next CUDA call on the stream fails).  Compiled out of the
+// product library.  (compute-sanitizer is closed on the B200 pool this was developed on; profiles/r2_sanitizers.md.)
+#ifdef SSM_CHECK
+#define SSM_ASSERT(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define SSM_ASSERT(cond) do { } while (0)
+#endif
+
 namespace ssm {
 
 constexpr int kBPL = 8;                      // beads per lane
@@ -54,6 +64,8 @@ constexpr int kSmEv = 12816;     // uint [64]   construction candidates [chain][
 constexpr int kSmSamp = 13072;   // int  [32]   per-chain fixed-point sum of d_x d_y over slip-springs (sample steps)
 constexpr int kSmKeys = 3840;    // uint [20]   the warp's copy of the Philox round keys (16-byte aligned)
 constexpr int kSmKap = 3920;     // float[9]   dt kappa of the warp's group of chains (general flow only), up to 3956
+constexpr int kSmPre = 3968;     // uint4[3][8] what rounds 1, 2 of Philox make of (domain, chain) for the NOISE, SLOT and ATTEMPT domains
+                                 //             (ssm_rng.cuh, stream_prefix), chains per warp <= 8 only; up to 4352
 constexpr int kSmSamp2 = 3584;   // int  [2][32] the same for d_y d_z and d_z d_x (isotropic correlator), in the spare kB after the mirror
 constexpr int kStageSteps = 8;   // recorded steps whose warp sums wait in kSmStage before they are added to the CTA sums
 constexpr int kSmStage = 13200;  // int  [8][12] warp sums of the last recorded steps (int32 fixed point)

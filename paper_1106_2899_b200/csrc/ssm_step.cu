@@ -106,6 +106,9 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     // each warp keeps its own copy of the Philox round keys inside its region: their address is then a
     // constant offset from the warp's base register (a CTA-wide copy costs an address computation per call)
     const uint4 *Keys = reinterpret_cast<const uint4 *>(wb + kSmKeys);
+    // the launch-constant part of the Philox calls of this tile's chains (ssm_rng.cuh, stream_prefix): [domain][chain]
+    constexpr bool PRE = CPW <= 8;
+    uint4 *Pre = reinterpret_cast<uint4 *>(wb + kSmPre);
     if (lane < 20) reinterpret_cast<unsigned *>(wb + kSmKeys)[lane] = P.rk[lane];
     for (int i = threadIdx.x; i < kMaxFuse * 12; i += kBlockThreads) acc[i] = 0ull;
     Samp[lane] = 0; Samp2[lane] = 0; Samp2[32 + lane] = 0;
@@ -149,6 +152,14 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
         }
         __syncwarp();
         cj = reinterpret_cast<const unsigned *>(Map)[lane];
+        SSM_ASSERT(z >= 0 && z <= N && total <= 256);
+#ifdef SSM_CHECK
+        for (int it = 0; it < 4; ++it)
+            if (lane + 32 * it < total) {
+                const int e = (int)((cj >> (8 * it)) & 0xFFu);
+                SSM_ASSERT((e >> LN) < CPW && (e & (N - 1)) < Zs[e >> LN] && Xp[e >> LN] + (e & (N - 1)) == lane + 32 * it);
+            }
+#endif
         return total;
     };
     // (c << LN) | j of slip-spring number f = lane + 32 it of the warp (f < Tz)
@@ -212,6 +223,11 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
             for (int v = 0; v < 8; ++v) A4[v * 32 + lane] = gA[v * 32 + lane];
             reinterpret_cast<uint2 *>(Sb)[lane] = reinterpret_cast<const uint2 *>(tp + kTileS)[lane];
             Zs[lane] = reinterpret_cast<const int *>(tp + kTileZ)[lane];
+            if (PRE && lane < 3 * CPW) {
+                const StreamKey sk0 = make_stream(P.step0, P.rk);
+                const int dom = lane / CPW, c = lane - dom * CPW;
+                Pre[lane] = stream_prefix(sk0, P.rk, dom == 0 ? DOM_NOISE : (dom == 1 ? DOM_SLOT : DOM_ATTEMPT), chain0 + (uint32_t)c);
+            }
             // dt kappa of the group this warp's chains belong to (a tile never straddles two groups)
             if (FLOW == 2 && lane < 9) Kap[lane] = P.kappa[(long long)(tile / P.tiles_per_group) * 9 + lane];
 #pragma unroll
@@ -288,6 +304,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                             const int sx = *sp;
                             *sp = 0;
                             const float g = fmaf(P.cs * (1.0f / (float)(1 << kSampleShift)), (float)sx, f);
+                            SSM_ASSERT(smp < kMaxFuse);
                             if (valid && P.samples)
                                 P.samples[((long long)smp * P.n_comp + q) * P.n_chains + chain_local] = make_float2(f, g);
                         }
@@ -310,6 +327,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     // |off-diagonal| <= half the sum of two diagonals, so the two traces bound all
                     // 12 shares by 256, and a 32-lane sum of shares * 2^18 fits 32 bits
                     const bool big = !(3.0f * (v[0] + v[1] + v[2]) < 240.0f && P.cs * (sv[0] + sv[1] + sv[2]) < 240.0f);
+                    SSM_ASSERT(rec < kMaxFuse && rec - stage_base >= 0 && rec - stage_base < kStageSteps && rec < P.n_rec);
                     int4 *row = Stage4 + (rec - stage_base) * 3;
                     if (__any_sync(kFull, big)) {
                         // rare (strongly stretched chains): sum the shares as two 32-bit halves and add
@@ -357,7 +375,12 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
 #pragma unroll
             for (int q = 0; q < 3; ++q) {
                 float z8[8];
-                normal_call<true>(sk, P.rk, DOM_NOISE, chain, (uint32_t)(3 * l + q), bm_noise, z8, Keys);
+                if (PRE) {
+                    uint32_t w[4];
+                    stream_call_pre(sk, Pre[cw], (uint32_t)(3 * l + q), w, Keys);
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) bm_noise(w[e], z8[2 * e], z8[2 * e + 1]);
+                } else normal_call<true>(sk, P.rk, DOM_NOISE, chain, (uint32_t)(3 * l + q), bm_noise, z8, Keys);
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
                     const int4 fx = Fx4[lq + 2 * q + h];
@@ -406,8 +429,10 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     const int sx = (int)(cur & 0xFFu), c = sx >> LN, j = sx & (N - 1), base = sx & ~(N - 1);
                     cur >>= 8;
                     uint32_t w[4];
-                    stream_call<true>(sk, P.rk, DOM_SLOT, chain0 + (uint32_t)c, (uint32_t)(j >> 1), w, Keys);
+                    if (PRE) stream_call_pre(sk, Pre[CPW + c], (uint32_t)(j >> 1), w, Keys);
+                    else stream_call<true>(sk, P.rk, DOM_SLOT, chain0 + (uint32_t)c, (uint32_t)(j >> 1), w, Keys);
                     const uint32_t w_hop = (j & 1) ? w[2] : w[0], w_end = (j & 1) ? w[3] : w[1];
+                    SSM_ASSERT(!act || (c < CPW && j < Zs[c] && Sb[sx] >= 1 && Sb[sx] <= NA));
                     const int s = max((int)Sb[sx], 1);       // 1..N (an idle lane may look at an empty slot: any bead will do)
                     float4 a = A4[sx];
                     if (SHEAR) {
@@ -441,6 +466,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     // neighbours along the chain are 3 floats away (7 across the padding after every 32 beads,
                     // which only chains of more than 32 beads can straddle)
                     const int fi = fx_index(b0);
+                    SSM_ASSERT(b0 >= base && b0 < base + N && fi >= 0 && fi + 2 < 800);
                     const int up3 = (G > 4 && (b0 & 31) == 31) ? 7 : 3, dn3 = (G > 4 && (b0 & 31) == 0) ? 7 : 3;
                     const float4 r0 = bead(fi);
                     const float4 rp = bead(fi + (s < NA ? up3 : 0));
@@ -471,6 +497,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                         const float dx = up ? dpx : (dn ? dmx : d0x), dy = up ? dpy : (dn ? dmy : d0y),
                                     dz = up ? dpz : (dn ? dmz : d0z);
                         int *fp = Fx + fi + (up ? up3 : 0) - (dn ? dn3 : 0);
+                        SSM_ASSERT(sn >= 1 && sn <= NA && fp == Fx + fx_index(base + sn - 1));
                         atomicAdd(fp, __float2int_rn(-P.fx_scale * dx));
                         atomicAdd(fp + 1, __float2int_rn(-P.fx_scale * dy));
                         atomicAdd(fp + 2, __float2int_rn(-P.fx_scale * dz));
@@ -495,9 +522,11 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     const int empty = NA - Z0;
                     int K = P.k_attempts > 0 ? (P.k_attempts < empty ? P.k_attempts : empty) : empty;
                     if (!valid) K = 0;
+                    SSM_ASSERT(K >= 0 && K <= NA && Z0 >= 0 && Z0 <= NA);
                     if (8 * l < K) {
                         uint32_t w[4];
-                        stream_call<true>(sk, P.rk, DOM_ATTEMPT, chain, (uint32_t)l, w, Keys);
+                        if (PRE) stream_call_pre(sk, Pre[2 * CPW + cw], (uint32_t)l, w, Keys);
+                        else stream_call<true>(sk, P.rk, DOM_ATTEMPT, chain, (uint32_t)l, w, Keys);
                         const int hmax = P.h_c2[K];
                         const unsigned m2 = __vminu2(__vminu2(w[0], w[1]), __vminu2(w[2], w[3]));
                         if ((int)min(m2 & 0xFFFFu, m2 >> 16) <= hmax) {
@@ -533,6 +562,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                                 m &= ~(1u << bit);
                                 const int j = 32 * wd + bit;
                                 --Zn;
+                                SSM_ASSERT(Zn >= 0 && j <= Zn && j < N);
                                 if (j != Zn) { Sb[base + j] = Sb[base + Zn]; A4[base + j] = A4[base + Zn]; }
                                 Sb[base + Zn] = 0;
                                 A4[base + Zn] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -565,6 +595,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                                 bm_anchor(wa[1], z3[2], unused);
                                 const float4 rb = bead(fx_index(base + snew - 1));
                                 const float4 a = make_float4(rb.x + z3[0], rb.y + z3[1], rb.z + z3[2], 0.0f);
+                                SSM_ASSERT(Zn >= 0 && Zn < NA && k < K0);
                                 Sb[base + Zn] = (unsigned char)snew;
                                 A4[base + Zn] = a;
                                 ++Zn;

@@ -262,13 +262,17 @@ def test_device_view_of_the_stress_sums_is_what_the_exchange_reduces(ssm):
 
 
 def test_issue_rate_probe(ssm):
-    """ssm_issue_rates: plain ALU and FP32 instructions issue about once per
-    cycle per scheduler, IMAD at half rate, and the 32 x 32 -> 64-bit multiply of Philox slower still."""
+    """ssm_issue_rates: FP32 issues once per cycle per scheduler, the ALU pipe (LOP3) and
+    IMAD every second cycle, the special-function unit every eighth, and the 32 x 32 -> 64-bit multiply of Philox
+    holds the issue port for about three cycles beyond its own -- FFMAs beside it do not hide."""
     g = ssm.Ensemble(8, 64, seed=1)
     r = g.issue_rates()
-    assert 0.9 < r["ffma"] < 1.6 and 0.9 < r["alu"] < 1.6
-    assert 1.7 < r["imad"] < 2.6
-    assert 3.0 < r["imad_wide"] < 6.0
+    assert 0.9 < r["ffma"] < 1.6
+    assert 1.7 < r["alu"] < 2.6 and 1.7 < r["imad"] < 2.6
+    assert 7.0 < r["mufu"] < 9.5 and 7.0 < r["i2f_f2i"] < 9.5
+    assert 2.5 < r["imad_wide"] < 5.0
+    assert r["wide_lop3_4ffma"] - r["wide_lop3"] > 3.0            # four FFMA cost four more cycles: no overlap
+    assert 7.0 < r["philox_round"] < 10.5
     R, A, S, step = g.get_state()          # the probe used the staging area only
     g2 = ssm.Ensemble(8, 64, seed=1)
     assert np.array_equal(R, g2.get_state()[0]) and np.array_equal(S, g2.get_state()[2])
