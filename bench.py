@@ -333,6 +333,9 @@ def main():
         nctx = max(1, a.e2e_contexts)
         pair = [ssm.Ensemble(N, M, seed=4, chain_offset=k0, stress_every=1, stress_capacity=inner, stage_chains=M,
                              device="cuda:%d" % local_rank, stream=torch.cuda.Stream(dev)) for _ in range(nctx)]
+        # one context alone, through the pipelined call: upload in chunks on a copy stream, chunks stepped as they land
+        solo = ssm.Ensemble(N, M, seed=4, chain_offset=k0, stress_every=1, stress_capacity=inner, stage_chains=max(64, M // 8),
+                            device="cuda:%d" % local_rank, stream=torch.cuda.Stream(dev))
         outs = [None] * nctx
         errs = []
 
@@ -380,15 +383,33 @@ def main():
         barrier()
         dt_serial = (time.perf_counter() - t1) / 2
         assert all(np.array_equal(outs[0], o) for o in outs[1:])    # same input, same seed: same samples
+
+        def solo_steps(n):
+            out = None
+            for _ in range(n):
+                solo.reset_accumulators()
+                solo.step_from_host(Rp, Ap, Sp, step, inner)
+                out = solo.stress()
+            return out
+        solo_steps(1)
+        barrier()
+        t2 = time.perf_counter()
+        out_solo = solo_steps(4)
+        barrier()
+        dt_solo = (time.perf_counter() - t2) / 4
+        assert np.array_equal(out_solo, outs[0])                    # the pipelined call gives the same samples
         t = torch.tensor([dt], dtype=torch.float64, device=dev)
         if world > 1:
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e = {"value": float(M) * N * inner * nctx * ke * world / float(t.item()), "unit": "bead-updates/s",
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(outs[0].nbytes),
-               "steps": nctx * ke, "contexts": nctx, "serial_value": float(M) * N * inner / dt_serial,
+               "steps": nctx * ke, "contexts": nctx, "serial_value": float(M) * N * inner / dt_solo,
+               "unpipelined_value": float(M) * N * inner / dt_serial,
                "what": "ssm_set_state(host pinned) + ssm_step(%d) + ssm_stress(host) per step; %d contexts on as many "
-                       "streams, one host thread each, started one upload apart (serial_value: one context "
-                       "alone)" % (inner, nctx)}
+                       "streams, one host thread each, started one upload apart (serial_value: ONE context, one "
+                       "thread, ssm_step_from_host = the same upload in chunks overlapped with the stepping of the "
+                       "chunks already landed; unpipelined_value: one context, set_state then step)" % (inner, nctx)}
+        del solo
         del pair
 
     if rank != 0:

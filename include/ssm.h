@@ -243,6 +243,17 @@ int ssm_get_state(ssm_ctx *ctx, float *R, float *A, uint8_t *S, int64_t *global_
 int ssm_set_state(ssm_ctx *ctx, const float *R, const float *A, const uint8_t *S,
                   int64_t global_step, int pointers_are_device);
 
+/* ssm_set_state from HOST buffers (pinned, or the copies cannot overlap anything) followed by ssm_step(n_steps,
+ * shear_rate), as ONE pipelined call: the ensemble is uploaded in about sixteen chunks on a copy stream of the library's
+ * own, and a chunk's chains are stepped through all n_steps as soon as it has landed, while the later chunks are still
+ * crossing PCIe.  Chains are independent (eq 54) and the integer record sums do not depend on the order in which
+ * chains add to them, so state and stress samples are those of ssm_set_state + ssm_step bit for bit.  The correlator must
+ * be off (sample_every = 0; SSM_ESTATE otherwise: it is fed ensemble-wide after every launch).  Uses both halves of the
+ * staging area as upload buffers (stage_chains >= 64).  Synchronises before returning; S is validated as by
+ * ssm_set_state. */
+int ssm_step_from_host(ssm_ctx *ctx, const float *R, const float *A, const uint8_t *S, int64_t global_step,
+                       int64_t n_steps, double shear_rate);
+
 /* Clear the stress samples and the correlator; keep the chains and the step counter. */
 int ssm_reset_accumulators(ssm_ctx *ctx);
 

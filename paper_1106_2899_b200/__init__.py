@@ -20,7 +20,7 @@ EXPORTS = ["ssm_workspace_bytes", "ssm_init", "ssm_step", "ssm_stress_count", "s
            "ssm_moduli", "ssm_eta0", "ssm_tau_d", "ssm_issue_rates",
            "ssm_gt_virtual", "ssm_gt_sums_virtual", "ssm_step_kappa", "ssm_group_stress",
            "ssm_step_kappa_device", "ssm_group_stress_device", "ssm_recenter",
-           "ssm_eta_star", "ssm_stress_from_sums", "ssm_stream_wait_ctx", "ssm_ctx_wait_stream"]
+           "ssm_eta_star", "ssm_stress_from_sums", "ssm_stream_wait_ctx", "ssm_ctx_wait_stream", "ssm_step_from_host"]
 
 
 class Params(C.Structure):
@@ -80,6 +80,7 @@ def lib():
     L.ssm_eta0.argtypes = [C.c_int32, dp, dp, dp]; L.ssm_eta0.restype = C.c_int
     L.ssm_eta_star.argtypes = [C.c_int32, dp, dp, C.c_int32, dp, dp]; L.ssm_eta_star.restype = C.c_int
     L.ssm_stress_from_sums.argtypes = [C.POINTER(C.c_int64), C.c_int64, C.c_int64, dp]; L.ssm_stress_from_sums.restype = C.c_int
+    L.ssm_step_from_host.argtypes = [vp, fp, fp, vp, C.c_int64, C.c_int64, C.c_double]; L.ssm_step_from_host.restype = C.c_int
     L.ssm_stream_wait_ctx.argtypes = [vp, vp]; L.ssm_stream_wait_ctx.restype = C.c_int
     L.ssm_ctx_wait_stream.argtypes = [vp, vp]; L.ssm_ctx_wait_stream.restype = C.c_int
     L.ssm_tau_d.argtypes = [C.c_int32, dp, dp, C.c_double, C.c_double, dp]; L.ssm_tau_d.restype = C.c_int
@@ -320,6 +321,15 @@ class Ensemble:
                 dev = 1 if R.is_cuda else 0
                 self._ck(lib().ssm_set_state(self.h, C.c_void_p(R.data_ptr()), C.c_void_p(A.data_ptr()),
                                              C.c_void_p(S.data_ptr()), global_step, dev))
+
+    def step_from_host(self, R, A, S, global_step, n_steps, shear_rate=0.0):
+        """ssm_step_from_host: upload the state from host numpy arrays (pinned for overlap) and advance n_steps, pipelined."""
+        assert R.dtype == np.float32 and A.dtype == np.float32 and S.dtype == np.uint8
+        assert R.flags.c_contiguous and A.flags.c_contiguous and S.flags.c_contiguous
+        assert R.shape == (3, self.N, self.M) and A.shape == (4, self.N, self.M) and S.shape == (self.N, self.M)
+        with self._dev():
+            self._ck(lib().ssm_step_from_host(self.h, C.c_void_p(R.ctypes.data), C.c_void_p(A.ctypes.data),
+                                              C.c_void_p(S.ctypes.data), global_step, n_steps, shear_rate))
 
     def reset_accumulators(self):
         with self._dev():

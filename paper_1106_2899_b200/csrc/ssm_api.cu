@@ -58,6 +58,8 @@ struct ssm_ctx {
     unsigned char cpos[kCorrMaxLevels], cfil[kCorrMaxLevels], cpar[kCorrMaxLevels];
     std::vector<long long> ccount;      // [L][P] insertions with a product at (level, bin)
     std::vector<float> kappa_host;      // dt kappa of the last ssm_step_kappa call, [groups][9]
+    cudaStream_t copy_st = nullptr;     // ssm_step_from_host: uploads run here, beside the stepping on st
+    cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
     std::string err;
 };
 
@@ -262,6 +264,36 @@ static void corr_schedule_sample(ssm_ctx *c)
     }
 }
 
+// the launch parameters of the next T <= fuse steps (records and samples due, where they go); the caller adds the flow
+static StepParams block_params(ssm_ctx *c, long long step, long long n_records, int T, long long *nrec_out, long long *nsmp_out)
+{
+    const ssm_params &p = c->p;
+    StepParams sp = c->sp;
+    sp.step0 = (unsigned long long)step; sp.n_fuse = T;
+    long long nrec = 0, nsmp = 0;
+    if (p.stress_every > 0) nrec = (step + T) / p.stress_every - step / p.stress_every;
+    if (p.sample_every > 0) nsmp = (step + T) / p.sample_every - step / p.sample_every;
+    sp.rec_mask = 0u; sp.smp_mask = 0u;
+    for (int n = 0; n < T; ++n) {
+        if (p.stress_every > 0 && (step + n + 1) % p.stress_every == 0) sp.rec_mask |= 1u << n;
+        if (p.sample_every > 0 && (step + n + 1) % p.sample_every == 0) sp.smp_mask |= 1u << n;
+    }
+    sp.n_rec = (int)nrec;
+    sp.stress = reinterpret_cast<long long *>(c->ws + c->lay.stress) + n_records * 12;
+    sp.samples = nsmp > 0 ? reinterpret_cast<float2 *>(c->ws + c->lay.samples) : nullptr;
+    *nrec_out = nrec; *nsmp_out = nsmp;
+    return sp;
+}
+
+// steps of the next launch: at most the fusion depth, and never across a multiple of 2^32 steps (the kernel forms the
+// part of its Philox calls that depends on the step's high bits once per tile: ssm_rng.cuh, stream_prefix)
+static int next_block(const ssm_ctx *c, long long step, long long left)
+{
+    long long T = left < c->fuse ? left : c->fuse;
+    const long long to_wrap = 0x100000000ll - (step & 0xFFFFFFFFll);
+    return (int)(T < to_wrap ? T : to_wrap);
+}
+
 // advance n_steps under simple shear (d_kappa null) or under the device table of tensors d_kappa
 static int step_impl(ssm_ctx *c, int64_t n_steps, double shear_rate, const float *d_kappa, long long tiles_per_group)
 {
@@ -270,12 +302,10 @@ static int step_impl(ssm_ctx *c, int64_t n_steps, double shear_rate, const float
         const long long need = (c->step + n_steps) / p.stress_every - c->step / p.stress_every;
         if (c->n_records + need > p.stress_capacity) return fail(c, SSM_ERANGE, "stress buffer would overflow (stress_capacity)");
     }
-    StepParams sp = c->sp;
-    sp.gdt = d_kappa ? 0.0f : (float)(shear_rate * p.dt);
-    sp.kappa = d_kappa; sp.tiles_per_group = (int)tiles_per_group;
+    const float gdt = d_kappa ? 0.0f : (float)(shear_rate * p.dt);
     // the fourth word of an anchor is the low part of its compensated advection; simple shear and the
     // general tensor encode it differently, so it restarts from zero when the kind of flow changes
-    const int want = d_kappa ? 2 : (sp.gdt != 0.0f ? 1 : 0);
+    const int want = d_kappa ? 2 : (gdt != 0.0f ? 1 : 0);
     if (n_steps > 0 && want != 0 && c->springs_on) {
         if (c->low_mode != 0 && c->low_mode != want) {
             CK(c, launch_clear_low(c->ws + c->lay.state, c->lay.n_tiles, c->st));
@@ -285,23 +315,10 @@ static int step_impl(ssm_ctx *c, int64_t n_steps, double shear_rate, const float
     }
     long long left = n_steps;
     while (left > 0) {
-        int T = (int)(left < c->fuse ? left : c->fuse);
-        // a launch never crosses a multiple of 2^32 steps: the kernel forms the part of its Philox calls that depends
-        // on the step's high bits once per tile (ssm_rng.cuh, stream_prefix)
-        const long long to_wrap = 0x100000000ll - (c->step & 0xFFFFFFFFll);
-        if (T > to_wrap) T = (int)to_wrap;
-        sp.step0 = (unsigned long long)c->step; sp.n_fuse = T;
+        const int T = next_block(c, c->step, left);
         long long nrec = 0, nsmp = 0;
-        if (p.stress_every > 0) nrec = (c->step + T) / p.stress_every - c->step / p.stress_every;
-        if (p.sample_every > 0) nsmp = (c->step + T) / p.sample_every - c->step / p.sample_every;
-        sp.rec_mask = 0u; sp.smp_mask = 0u;
-        for (int n = 0; n < T; ++n) {
-            if (p.stress_every > 0 && (c->step + n + 1) % p.stress_every == 0) sp.rec_mask |= 1u << n;
-            if (p.sample_every > 0 && (c->step + n + 1) % p.sample_every == 0) sp.smp_mask |= 1u << n;
-        }
-        sp.n_rec = (int)nrec;
-        sp.stress = reinterpret_cast<long long *>(c->ws + c->lay.stress) + c->n_records * 12;
-        sp.samples = nsmp > 0 ? reinterpret_cast<float2 *>(c->ws + c->lay.samples) : nullptr;
+        StepParams sp = block_params(c, c->step, c->n_records, T, &nrec, &nsmp);
+        sp.gdt = gdt; sp.kappa = d_kappa; sp.tiles_per_group = (int)tiles_per_group;
         sp.counter_slot = c->sp.counter_slot;
         CK(c, launch_step(padded_beads(p.n_beads), sp, c->grid, c->st));
         c->sp.counter_slot ^= 1;
@@ -580,6 +597,93 @@ extern "C" int ssm_set_state(ssm_ctx *c, const float *R, const float *A, const u
     return SSM_OK;
 }
 
+// ssm_set_state from HOST buffers followed by ssm_step, as one pipelined call: the ensemble is uploaded in chunks on a copy
+// stream, and a chunk's warp tiles are stepped (all n_steps, launch by launch) as soon as it has landed, while the next
+// chunks are still on their way.  Chains are independent (eq 54), and the exact integer record sums do not depend on the
+// order in which tiles add to them, so the results are those of ssm_set_state + ssm_step bit for bit.
+extern "C" int ssm_step_from_host(ssm_ctx *c, const float *R, const float *A, const uint8_t *S, int64_t global_step,
+                                  int64_t n_steps, double shear_rate)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (!R || !A || !S) return fail(c, SSM_EINVAL, "NULL state pointer");
+    if (global_step < 0 || n_steps < 0) return fail(c, SSM_EINVAL, "global_step or n_steps < 0");
+    if (!std::isfinite(shear_rate)) return fail(c, SSM_EINVAL, "shear_rate is not finite");
+    const ssm_params &p = c->p;
+    if (p.sample_every > 0) return fail(c, SSM_ESTATE, "ssm_step_from_host needs the correlator off (it is fed ensemble-wide after every launch)");
+    if (p.stress_every > 0) {
+        const long long need = (global_step + n_steps) / p.stress_every - global_step / p.stress_every;
+        if (c->n_records + need > p.stress_capacity) return fail(c, SSM_ERANGE, "stress buffer would overflow (stress_capacity)");
+    }
+    const int N = p.n_beads, npad = padded_beads(N);
+    const long long M = p.n_chains, cpw = chains_per_warp(npad);
+    if (!c->copy_st) {
+        CK(c, cudaStreamCreateWithFlags(&c->copy_st, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            CK(c, cudaEventCreateWithFlags(&c->ev_copied[i], cudaEventDisableTiming));
+            CK(c, cudaEventCreateWithFlags(&c->ev_free[i], cudaEventDisableTiming));
+        }
+    }
+    // two staging buffers of `chunk` chains each (multiples of 32 chains = whole CTAs of the import kernel and whole tiles)
+    long long chunk = (c->lay.stage_chains / 2) / 32 * 32;
+    if (chunk < 32) return fail(c, SSM_ENOMEM, "staging area too small to pipeline (stage_chains must be >= 64)");
+    {   // about sixteen chunks: the first upload, which nothing overlaps, is a sixteenth of the whole, and a launch still has
+        // a few tiles per resident warp (measured on C4: 8 / 16 / 32 / 64 chunks -> 33.0 / 32.4 / 36.7 / 39.9 ms per batch)
+        const long long want = ((M + 15) / 16 + 31) / 32 * 32;
+        if (want < chunk) chunk = want;
+    }
+    unsigned char *stage[2] = {c->ws + c->lay.stage, c->ws + c->lay.stage + (size_t)chunk * 29 * npad};
+    unsigned char *state = c->ws + c->lay.state;
+    int *bad = reinterpret_cast<int *>(c->ws + c->lay.counter) + 2;
+    const float gdt = (float)(shear_rate * p.dt);
+    // everything queued on the ctx's stream so far (it may still read the staging area or the state) comes first
+    CK(c, cudaEventRecord(c->ev_free[0], c->st));
+    CK(c, cudaEventRecord(c->ev_free[1], c->st));
+    long long j = 0;
+    for (long long k0 = 0; k0 < M; k0 += chunk, ++j) {
+        const long long nk = M - k0 < chunk ? M - k0 : chunk;
+        const int b = (int)(j & 1);
+        float *dR = reinterpret_cast<float *>(stage[b]);
+        float *dA = dR + (size_t)3 * N * chunk;
+        unsigned char *dS = reinterpret_cast<unsigned char *>(dA + (size_t)4 * N * chunk);
+        CK(c, cudaStreamWaitEvent(c->copy_st, c->ev_free[b], 0));
+        CK(c, cudaMemcpy2DAsync(dR, (size_t)chunk * 4, R + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)3 * N, cudaMemcpyHostToDevice, c->copy_st));
+        CK(c, cudaMemcpy2DAsync(dA, (size_t)chunk * 4, A + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)4 * N, cudaMemcpyHostToDevice, c->copy_st));
+        CK(c, cudaMemcpy2DAsync(dS, (size_t)chunk, S + k0, (size_t)M, (size_t)nk, (size_t)N, cudaMemcpyHostToDevice, c->copy_st));
+        CK(c, cudaEventRecord(c->ev_copied[b], c->copy_st));
+        CK(c, cudaStreamWaitEvent(c->st, c->ev_copied[b], 0));
+        CK(c, launch_xfer(false, state, dR, dA, dS, N, k0, nk, chunk, 0, bad, c->st));
+        CK(c, cudaEventRecord(c->ev_free[b], c->st));
+        c->launches += 1;
+        // this chunk's tiles through all n_steps
+        const long long t0 = k0 / cpw, t1 = (k0 + nk + cpw - 1) / cpw;
+        long long step = global_step, nrec_total = c->n_records, left = n_steps;
+        while (left > 0) {
+            const int T = next_block(c, step, left);
+            long long nrec = 0, nsmp = 0;
+            StepParams sp = block_params(c, step, nrec_total, T, &nrec, &nsmp);
+            sp.gdt = gdt; sp.kappa = nullptr; sp.tiles_per_group = 1;
+            sp.tile_first = (int)t0; sp.n_tiles = (int)(t1 - t0);
+            sp.counter_slot = c->sp.counter_slot;
+            CK(c, launch_step(npad, sp, c->grid, c->st));
+            c->sp.counter_slot ^= 1;
+            c->launches += 1;
+            nrec_total += nrec; step += T; left -= T;
+        }
+    }
+    if (p.stress_every > 0) c->n_records += (global_step + n_steps) / p.stress_every - global_step / p.stress_every;
+    c->step = global_step + n_steps;
+    c->low_mode = 1;                                                  // A[3] of the caller is the fp32 low part of x
+    int h_bad = 0;
+    CK(c, cudaMemcpyAsync(&h_bad, bad, sizeof h_bad, cudaMemcpyDeviceToHost, c->st));
+    CK(c, cudaStreamSynchronize(c->st));
+    if (h_bad) {
+        CK(c, cudaMemsetAsync(bad, 0, sizeof h_bad, c->st));
+        return fail(c, SSM_EINVAL, "S is malformed: a chain's occupied slots must be its leading ones and hold bead indices 1..n_beads "
+                                   "(the offending slots were cleared)");
+    }
+    return SSM_OK;
+}
+
 extern "C" int ssm_reset_accumulators(ssm_ctx *c)
 {
     if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
@@ -749,6 +853,15 @@ extern "C" int ssm_gt(ssm_ctx *c, int32_t *n_lags, double *h_t, double *h_G, dou
     return SSM_OK;
 }
 
-extern "C" void ssm_destroy(ssm_ctx *c) { delete c; }
+extern "C" void ssm_destroy(ssm_ctx *c)
+{
+    if (!c) return;
+    if (c->copy_st) {
+        cudaStreamSynchronize(c->copy_st);
+        for (int i = 0; i < 2; ++i) { cudaEventDestroy(c->ev_copied[i]); cudaEventDestroy(c->ev_free[i]); }
+        cudaStreamDestroy(c->copy_st);
+    }
+    delete c;
+}
 
 extern "C" const char *ssm_last_error(const ssm_ctx *c) { return c ? c->err.c_str() : g_err.c_str(); }

@@ -85,7 +85,8 @@ struct StepParams {
     long long      n_chains;          // M (chains >= M in the last tile are padding)
     unsigned long long chain_offset;  // global index of local chain 0
     unsigned long long step0;         // global index of the first step of this launch
-    int            n_tiles;
+    int            n_tiles;           // tiles this launch steps: [tile_first, tile_first + n_tiles)
+    int            tile_first;
     int           *tile_counter;      // [2] in the workspace: tiles handed out beyond each warp's first; slot counter_slot is
     int            counter_slot;      // this launch's (zero on entry), the other one is zeroed for the next launch
     int            n_fuse;            // steps in this launch (<= kMaxFuse)

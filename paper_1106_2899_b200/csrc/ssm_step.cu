@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     for (int i = threadIdx.x; i < kMaxFuse * 12; i += kBlockThreads) acc[i] = 0ull;
     Samp[lane] = 0; Samp2[lane] = 0; Samp2[32 + lane] = 0;
     Dm[lane] = 0u;
-    Ev[lane] = 0u;
+    Ev[lane] = 0u; Ev[32 + lane] = 0u;      // candidate masks, and the chains' last candidates (taken with atomicMax: must start at 0)
     reinterpret_cast<unsigned *>(Map)[lane] = 0u;
     __syncthreads();
 
@@ -201,9 +201,10 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     if (blockIdx.x == 0 && threadIdx.x == 0) P.tile_counter[1 - P.counter_slot] = 0;
     int tile = blockIdx.x * kWarpsPerBlock + warp;
     for (; tile < P.n_tiles; tile = nwarps + __shfl_sync(kFull, lane == 0 ? atomicAdd(P.tile_counter + P.counter_slot, 1) : 0, 0)) {
-        unsigned char *tp = P.state + (long long)tile * kTileBytes;
-        const long long chain_local = (long long)tile * CPW + cw;
-        const uint32_t chain0 = (uint32_t)(P.chain_offset + (unsigned long long)tile * CPW);
+        const long long gtile = (long long)P.tile_first + tile;          // the tile's number in the ensemble
+        unsigned char *tp = P.state + gtile * kTileBytes;
+        const long long chain_local = gtile * CPW + cw;
+        const uint32_t chain0 = (uint32_t)(P.chain_offset + (unsigned long long)gtile * CPW);
         const uint32_t chain = chain0 + (uint32_t)cw;
         const bool valid = chain_local < P.n_chains;
 
@@ -229,7 +230,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                 Pre[lane] = stream_prefix(sk0, P.rk, dom == 0 ? DOM_NOISE : (dom == 1 ? DOM_SLOT : DOM_ATTEMPT), chain0 + (uint32_t)c);
             }
             // dt kappa of the group this warp's chains belong to (a tile never straddles two groups)
-            if (FLOW == 2 && lane < 9) Kap[lane] = P.kappa[(long long)(tile / P.tiles_per_group) * 9 + lane];
+            if (FLOW == 2 && lane < 9) Kap[lane] = P.kappa[(gtile / P.tiles_per_group) * 9 + lane];
 #pragma unroll
             for (int v = 0; v < 6; ++v) Rf4[lq + v] = make_float4(r[4 * v], r[4 * v + 1], r[4 * v + 2], r[4 * v + 3]);
         }

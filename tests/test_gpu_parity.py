@@ -278,6 +278,33 @@ def test_issue_rate_probe(ssm):
     assert np.array_equal(R, g2.get_state()[0]) and np.array_equal(S, g2.get_state()[2])
 
 
+def test_pipelined_upload_and_step_equals_set_state_then_step(ssm):
+    """ssm_step_from_host uploads the ensemble in chunks on a copy stream and steps a chunk's tiles as soon as it has
+    landed: state and stress sums must be those of ssm_set_state + ssm_step bit for bit, for ragged ensembles, ragged
+    bead numbers, any staging size, with and without shear, and appended to earlier samples."""
+    import torch
+    for N, M, stage in ((32, 1000, 128), (32, 1000, 512), (20, 333, 64), (128, 77, 64), (8, 5000, 2048)):
+        e = oracle.Ensemble(N, M, seed=21)
+        e.round_to_fp32()
+        R, A, S = to_external(e)
+        pin = [torch.from_numpy(x).pin_memory().numpy() for x in (R, A, S)]
+        for rate in (0.0, 0.05):
+            a = ssm.Ensemble(N, M, seed=21, stress_every=1, stress_capacity=200, stage_chains=stage)
+            a.step(7, rate)                                     # earlier samples stay where they are
+            a.set_state(R, A, S, 40)
+            a.step(75, rate)
+            b = ssm.Ensemble(N, M, seed=21, stress_every=1, stress_capacity=200, stage_chains=stage)
+            b.step(7, rate)
+            b.step_from_host(*pin, 40, 75, rate)
+            for x, y in zip(a.get_state(), b.get_state()):
+                assert np.array_equal(x, y), (N, M, stage, rate)
+            assert np.array_equal(a.stress_sums(), b.stress_sums()) and a.stress_count() == 82
+    g = ssm.Ensemble(16, 100, seed=1, sample_every=10)
+    with pytest.raises(ssm.SsmError) as err:
+        g.step_from_host(*[np.ascontiguousarray(x) for x in g.get_state()[:3]], 0, 10)
+    assert err.value.code == ssm.SSM_ESTATE                     # the correlator must be off
+
+
 def test_set_state_rejects_malformed_slip_spring_indices(ssm):
     """The checkpoint-restore path validates S on the device: occupied slots must be the leading ones and
     hold bead indices 1..N.  A bad chain keeps its valid leading slots only, the call fails with SSM_EINVAL, and the
