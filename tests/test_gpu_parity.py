@@ -305,6 +305,35 @@ def test_pipelined_upload_and_step_equals_set_state_then_step(ssm):
     assert err.value.code == ssm.SSM_ESTATE                     # the correlator must be off
 
 
+def test_two_contexts_stepping_concurrently_give_the_same_samples(ssm):
+    """Two contexts on two streams, driven by two host threads, same seed and input: their kernels share the SMs, so a
+    CTA finds in shared memory whatever the other context's CTA left there.  Everything the step kernel reads must have
+    been written by it first (round 2 found the chains' last-candidate words read through atomicMax uninitialised this
+    way); the samples and states of the two must be identical, and equal to a context run alone."""
+    import threading
+    import torch
+    N, M, steps = 32, 200000, 64
+    ref = ssm.Ensemble(N, M, seed=9, stress_every=1, stress_capacity=steps)
+    ref.step(steps)
+    want = ref.stress_sums(); Rw = ref.get_state()
+    del ref
+    for _ in range(2):
+        ctx = [ssm.Ensemble(N, M, seed=9, stress_every=1, stress_capacity=steps, stream=torch.cuda.Stream()) for _ in range(2)]
+        def work(g):
+            for _ in range(steps // 16):
+                g.step(16)
+            g.synchronize()
+        th = [threading.Thread(target=work, args=(g,)) for g in ctx]
+        for t in th:
+            t.start()
+        for t in th:
+            t.join()
+        for g in ctx:
+            assert np.array_equal(g.stress_sums(), want)
+            for x, y in zip(g.get_state(), Rw):
+                assert np.array_equal(x, y)
+
+
 def test_set_state_rejects_malformed_slip_spring_indices(ssm):
     """The checkpoint-restore path validates S on the device: occupied slots must be the leading ones and
     hold bead indices 1..N.  A bad chain keeps its valid leading slots only, the call fails with SSM_EINVAL, and the
