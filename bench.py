@@ -210,6 +210,26 @@ def run_table1():
     print(json.dumps({"workload": "PAPER.md Table 1 (context)", "rows": rows}))
 
 
+def time_configs(ssm, torch):
+    """Rows of run_configs(): the C2 / C3 / C5 shapes, device-resident, CUDA events."""
+    cases = [("C2 equilibrium G(t)", dict(n_beads=16, n_chains=65536, stress_every=10, sample_every=10), 0.0, 6400),
+             ("C3 start-up shear", dict(n_beads=32, n_chains=262144, stress_every=10), 0.1, 2560),
+             ("C5 long chains, G(t)", dict(n_beads=128, n_chains=131072, dt=0.005, stress_every=10, sample_every=10), 0.0, 1280),
+             ("C5 long chains, steady shear", dict(n_beads=128, n_chains=131072, dt=0.005, stress_every=10), 1e-3, 1280)]
+    rows = []
+    for name, kw, rate, steps in cases:
+        g = ssm.Ensemble(seed=2, stress_capacity=steps // 5, **kw)
+        g.step(steps // 5, rate)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); g.step(steps, rate); e1.record(); torch.cuda.synchronize()
+        t = e0.elapsed_time(e1) * 1e-3
+        rows.append({"config": name, "n_beads": kw["n_beads"], "n_chains": kw["n_chains"], "shear_rate": rate, "steps": steps,
+                     "bead_updates_per_s": kw["n_beads"] * kw["n_chains"] * steps / t, "ms_per_32_steps": 1e3 * t / steps * 32})
+        del g
+    return rows
+
+
 def run_configs():
     """BASELINE.json configs[1], [2], [4] (C2, C3, C5 of SURVEY 8d) as they are run in production: same kernels as
     the bench line, their own shapes, sampling and flow; CUDA events around a few thousand steps after a warm-up.
@@ -454,6 +474,10 @@ def main():
         "paper_context": {"gpu_bead_updates_per_s": 7.3e8, "cpu_bead_updates_per_s": 2.5e6,
                           "hardware": "Tesla C1060 / Core 2 Duo E8500 1 thread (PAPER.md Table 1)"},
     }
+    if world == 1 and not a.no_e2e:
+        # context, not the metric: the other BASELINE.json shapes with the same kernels in the same run (clock record above)
+        del g
+        line["other_configs"] = time_configs(ssm, torch)
     if not a.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(N, a.cpu_seconds)
     print(json.dumps(line))
