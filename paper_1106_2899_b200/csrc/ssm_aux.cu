@@ -4,6 +4,8 @@
 // into the sums behind G(t) (eq 43).
 #include <cuda_runtime.h>
 
+#include <atomic>
+
 #include "ssm_common.h"
 #include "ssm_rng.cuh"
 
@@ -72,124 +74,267 @@ cudaError_t launch_init(const InitParams &p, cudaStream_t st)
 // State export / import between the tiled image and the external SoA layout of ssm.h.
 // rows 0..3N-1 of R, then 4N rows of A (x, y, z, low part of x), then N rows of S; chains
 // [k0, k0+nk), external element (row, k) at row*pitch + (k - k0).
-// A CTA owns 32 consecutive chains = G whole tiles and transposes them through an image of those
-// tiles in shared memory: the external rows are read / written 32 bytes (8 chains) per row and four
-// rows per warp request, the tiles 16 bytes per thread, so both sides of the copy move whole
-// sectors.  (One thread per element writing straight into the tiles, as at first, touched a 32-byte
-// sector per 4-byte word: 6.7 ms for the 1 GB of config 4 against the 17.5 ms of its PCIe copy.)  On import the CTA also
-// counts Z_k = number of occupied slots (they must be the leading ones).
+// A CTA owns 32 consecutive chains = G whole tiles and transposes them through shared memory, so that
+// both sides of the copy move whole lines: an external row is read / written by a warp, lane = chain
+// (128 contiguous bytes per request), the tiles 16 bytes per thread.  In between the 7N float rows sit
+// in a staging array [row][33] (element (row, chain) in bank (row + chain) mod 32: the row accesses
+// and the gathers / scatters of a tile word's four elements are both free of bank conflicts for
+// N = 8, 32, 64 and two- or four-way for 16 and 128) and S as bytes [chain][8G + 4] (an odd number of words
+// per chain: the row accesses, a byte per lane, and the 4-slot words of the tile side are both conflict-free).
+// The import brings its rows in with 4-byte asynchronous copies (cp.async), one row per warp instruction and all
+// 7N/8 rows of a warp in flight at once; the export's scattered side is its stores, which wait for nothing.
+// (History, config 4, 1.96 GB: one thread per element storing straight into the tiles touched a
+// 32-byte sector per word, 6.7 ms; an image of the tiles in shared memory with the external rows
+// moved as 32-byte pieces, 8 chains x 4 rows per warp request, import 0.48 ms = 62 % of the copy
+// bandwidth, export 0.57 ms; more of those loads in flight per thread changed nothing, whole-line
+// requests through registers took the export to 0.43 ms and left the import latency-bound at 0.59;
+// with the asynchronous copies it takes 0.40 ms.)
+// On import the CTA also counts Z_k = number of occupied slots (they must be the leading ones).
 // ---------------------------------------------------------------------------------------
-template <bool EXPORT>
-__global__ void __launch_bounds__(256, 6) ssm_xfer_kernel(unsigned char *state, float *R, float *A, unsigned char *S,
-                                                       int N, int NP, long long k0, long long nk, long long pitch, int hide_low,
-                                                       int *bad_state)
+constexpr int kXferPad = 33;
+__host__ __device__ constexpr int xfer_smem(int N, int NP) { return 7 * N * kXferPad * 4 + 32 * (NP + 4) + 128; }
+
+template <bool EXPORT, int G>
+__global__ void __launch_bounds__(256, G <= 4 ? 6 : (G == 8 ? 3 : 1))
+ssm_xfer_kernel(unsigned char *state, float *R, float *A, unsigned char *S, int N, long long k0, long long nk, long long pitch,
+                int hide_low, int *bad_state)
 {
-    extern __shared__ __align__(16) unsigned char img[];
-    const int G = NP / kBPL, cpw = 32 / G;
+    extern __shared__ __align__(16) unsigned char xs[];
+    constexpr int NP = kBPL * G, cpw = 32 / G;
+    constexpr int lg = G == 1 ? 0 : (G == 2 ? 1 : (G == 4 ? 2 : (G == 8 ? 3 : 4)));
+    constexpr int W16 = kTileBytes / 16, WR = (kTileA - kTileR) / 16, WA = (kTileS - kTileA) / 16, WS = (kTileZ - kTileS) / 16;
+    float *stg = reinterpret_cast<float *>(xs);                                  // [7N][33]: rows of R, then rows of A
+    constexpr int SST = NP + 4;
+    unsigned char *sS = xs + 7 * N * kXferPad * 4;                               // [32][SST]
+    int *sZ = reinterpret_cast<int *>(sS + 32 * SST);                            // [32]
     const long long cb = (k0 / 32 + blockIdx.x) * 32;           // first of this CTA's 32 chains
     const long long t0 = cb / cpw, t_last = (k0 + nk - 1) / cpw;
     const int nt = (int)(t_last - t0 + 1 < (long long)G ? t_last - t0 + 1 : (long long)G);    // tiles that exist
-    // an import that covers every byte the kernels read of these tiles needs no copy of the old image
+    // a CTA whose 32 chains are all in [k0, k0 + nk) writes its tiles whole; another leaves the rest of them as it is
     const bool full = cb >= k0 && cb + 32 <= k0 + nk;
-    uint4 *g4 = reinterpret_cast<uint4 *>(state + t0 * kTileBytes), *i4 = reinterpret_cast<uint4 *>(img);
-    const int n16 = nt * (kTileBytes / 16);
-    if (EXPORT || !full)
-        for (int i = threadIdx.x; i < n16; i += 256) i4[i] = g4[i];
-    else
-        for (int i = threadIdx.x; i < n16; i += 256) i4[i] = make_uint4(0u, 0u, 0u, 0u);     // the tiles' unused tail bytes
-    __syncthreads();
-    // Every thread moves one 16-byte word of the image (one float4 of a lane's beads, one anchor, four bytes of S)
-    // and gathers / scatters its four elements from / to four external rows; the lanes of a warp are laid so that
-    // the image side is (nearly) free of bank conflicts and an external request still covers whole 32-byte sectors
-    // (8 consecutive chains of a row).  Places and slots beyond N (N < 8G) are written as zero on import.
+    uint4 *g4 = reinterpret_cast<uint4 *>(state + t0 * kTileBytes);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int sh = __ffs(cpw) - 1, lg = 5 - sh;
-    // beads: unit (tile T, float4 v of the 6 a lane holds); lane = the lane of the step kernel, cw * G + g
-    for (int u = warp; u < nt * 6; u += 8) {
-        const int T = u / 6, v = u - 6 * T, cw = lane >> lg, g = lane & (G - 1);
-        const long long kk = cb + T * cpw + cw - k0;
-        if (kk < 0 || kk >= nk) continue;
-        float4 *p = reinterpret_cast<float4 *>(img + T * kTileBytes + kTileR) + v * 32 + lane;
-        SSM_ASSERT(T < nt && cw < cpw);
-        float w[4];
-        if (EXPORT) { const float4 t = *p; w[0] = t.x; w[1] = t.y; w[2] = t.z; w[3] = t.w; }
+    const long long kl = cb + lane - k0;                        // this lane's chain in the external rows
+    const bool in = kl >= 0 && kl < nk;
+    auto chain_in = [&](int c32) -> bool { const long long k = cb + c32 - k0; return k >= 0 && k < nk; };
+
+    // word wi of tile T: whose chain(s) it belongs to and where its elements sit in the staging arrays
+    // R word: float4 v of lane ln = cw G + g; element e is coordinate f % 3 of bead 8g + f / 3, f = 4v + e
+    // A word: anchor (cw, slot j), rows 3N + c N + j;  S word: 16 bytes of [cw][slot];  Z word: 4 chains
+    // The 16-byte words of a tile's R and A parts are moved in units of 32 (one per lane), 14 per tile: unit 0..5 =
+    // float4 v of every lane of the step kernel (lane cw G + g: element e is coordinate f % 3 of bead 8g + f / 3,
+    // f = 4v + e), unit 6..13 = 32 consecutive anchors (chain cw, slot j; rows 3N + c N + j).  Which unit a warp is at
+    // is the same for its lanes, so the index arithmetic runs on the uniform path and a lane adds its own part.
+    constexpr int LNP = lg + 3;
+    const int cwl = lane >> lg, gl = lane & (G - 1);
+    if (EXPORT) {
+        // ---- tiles -> staging (16 bytes per thread, coalesced), then staging -> rows
+        for (int u = warp; u < nt * 14; u += 8) {
+            const int T = u / 14, uu = u - 14 * T;
+            if (uu < 6) {
+                const uint4 t = g4[T * W16 + uu * 32 + lane];
+                const unsigned x[4] = {t.x, t.y, t.z, t.w};
+                float *sp = stg + (kBPL * gl) * kXferPad + T * cpw + cwl;
 #pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const int f = 4 * v + e, i = kBPL * g + f / 3, c = f % 3;
-            float *q = R + (long long)(c * N + i) * pitch + kk;
-            if (EXPORT) { if (i < N) *q = w[e]; } else w[e] = i < N ? *q : 0.0f;
-        }
-        if (!EXPORT) *p = make_float4(w[0], w[1], w[2], w[3]);
-    }
-    // anchors: unit (8 chains cg, 4 slots jb); lane = 4 * chain + slot
-    for (int u = warp; u < NP; u += 8) {
-        const int cl = (u & 3) * 8 + (lane >> 2), j = (u >> 2) * 4 + (lane & 3);
-        const long long kk = cb + cl - k0;
-        if (kk < 0 || kk >= nk) continue;
-        float4 *p = reinterpret_cast<float4 *>(img + (cl >> sh) * kTileBytes + kTileA) + (cl & (cpw - 1)) * NP + j;
-        SSM_ASSERT((cl >> sh) < nt && j < NP);
-        float w[4];
-        if (EXPORT) { const float4 t = *p; w[0] = t.x; w[1] = t.y; w[2] = t.z; w[3] = t.w; }
-        // (hide_low: the fourth word holds the packed low parts of ssm_step_kappa, not a float; export 0)
-        if (EXPORT && hide_low) w[3] = 0.0f;
+                for (int e = 0; e < 4; ++e) {
+                    const int f = 4 * uu + e, q = f / 3, c = f - 3 * q;
+                    if (kBPL * gl + q < N) sp[(c * N + q) * kXferPad] = __uint_as_float(x[e]);
+                }
+            } else {
+                const int ai = (uu - 6) * 32 + lane, cw = ai >> LNP, j = ai & (NP - 1);
+                const uint4 t = g4[T * W16 + WR + ai];
+                const unsigned x[4] = {t.x, t.y, t.z, hide_low ? 0u : t.w};
+                float *sp = stg + (3 * N + j) * kXferPad + T * cpw + cw;
+                if (j < N) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            float *q = A + (long long)(c * N + j) * pitch + kk;
-            if (EXPORT) { if (j < N) *q = w[c]; } else w[c] = j < N ? *q : 0.0f;
+                    for (int c = 0; c < 4; ++c) sp[c * N * kXferPad] = __uint_as_float(x[c]);
+                }
+            }
         }
-        if (!EXPORT) *p = make_float4(w[0], w[1], w[2], w[3]);
-    }
-    // bead indices: unit (8 chains, 4 groups of 4 slots); a thread packs the bytes of 4 consecutive slots
-    for (int u = warp; u < 4 * ((NP + 15) / 16); u += 8) {
-        const int cl = (u & 3) * 8 + (lane >> 2), j0 = ((u >> 2) * 4 + (lane & 3)) * 4;
-        const long long kk = cb + cl - k0;
-        if (kk < 0 || kk >= nk || j0 >= NP) continue;
-        unsigned *p = reinterpret_cast<unsigned *>(img + (cl >> sh) * kTileBytes + kTileS + (cl & (cpw - 1)) * NP + j0);
-        unsigned w = EXPORT ? *p : 0u;
+        for (int i = threadIdx.x; i < nt * WS; i += 256) {
+            const int T = i / WS, wi = i - T * WS;
+            const uint4 t = g4[T * W16 + WR + WA + wi];
+            const unsigned x[4] = {t.x, t.y, t.z, t.w};
 #pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            unsigned char *q = S + (long long)(j0 + e) * pitch + kk;
-            if (EXPORT) { if (j0 + e < N) *q = (unsigned char)(w >> (8 * e)); } else w |= (j0 + e < N ? (unsigned)*q : 0u) << (8 * e);
-        }
-        if (!EXPORT) *p = w;
-    }
-    const long long k = cb + lane;
-    const bool in = k >= k0 && k < k0 + nk;
-    if (!EXPORT) {
-        __syncthreads();
-        if (warp == 0 && in) {
-            // Z = the leading occupied slots.  A caller's S must hold bead indices 1..N there and 0 after
-            // them; anything else would send the step kernel's scatter outside the chain.  Such a chain keeps its
-            // valid leading slots only, the rest is cleared, and the flag makes ssm_set_state fail.
-            int Z = 0;
-            while (Z < N && img[off_S(lane, NP, Z)] != 0 && img[off_S(lane, NP, Z)] <= N) ++Z;
-            bool bad = false;
-            for (int j = Z; j < NP; ++j)
-                if (img[off_S(lane, NP, j)] != 0) { bad = true; img[off_S(lane, NP, j)] = 0; }
-            if (bad) atomicExch(bad_state, 1);
-            *reinterpret_cast<int *>(img + off_Z(lane, NP)) = Z;
+            for (int e = 0; e < 4; ++e) {
+                const int bi = wi * 16 + 4 * e, cw = bi >> LNP, j = bi & (NP - 1);
+                *reinterpret_cast<unsigned *>(sS + (T * cpw + cw) * SST + j) = x[e];
+            }
         }
         __syncthreads();
-        for (int i = threadIdx.x; i < n16; i += 256) g4[i] = i4[i];
+        if (in) {
+            {
+                float *row = R + (long long)warp * pitch + kl;
+                const float *sp = stg + warp * kXferPad + lane;
+                for (int r = warp; r < 3 * N; r += 8, row += 8 * pitch, sp += 8 * kXferPad) *row = *sp;
+            }
+            {
+                float *row = A + (long long)warp * pitch + kl;
+                const float *sp = stg + (3 * N + warp) * kXferPad + lane;
+                for (int r = warp; r < 4 * N; r += 8, row += 8 * pitch, sp += 8 * kXferPad) *row = *sp;
+            }
+            unsigned char *row = S + (long long)warp * pitch + kl;
+            for (int j = warp; j < N; j += 8, row += 8 * pitch) *row = sS[lane * SST + j];
+        }
+        return;
     }
+
+    // ---- import: rows -> staging, asynchronously (a row's 128 bytes per warp instruction, no register in between, so
+    // that a warp has all its 7N/8 rows in flight at once: the kernel is bound by the latency of these loads);
+    // a lane whose chain is outside [k0, k0 + nk) is filled with zero (source size 0)
+    // (hide_low is an export matter; the 4th row of A is taken as it comes)
+    {
+        const unsigned dst0 = (unsigned)__cvta_generic_to_shared(stg + lane);
+        const unsigned nbytes = in ? 4u : 0u;
+        const long long kls = in ? kl : 0;
+        {
+            const float *src = R + (long long)warp * pitch + kls;
+            unsigned dst = dst0 + (unsigned)(warp * kXferPad * 4);
+            for (int r = warp; r < 3 * N; r += 8, src += 8 * pitch, dst += 8 * kXferPad * 4)
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(nbytes) : "memory");
+        }
+        {
+            const float *src = A + (long long)warp * pitch + kls;
+            unsigned dst = dst0 + (unsigned)((3 * N + warp) * kXferPad * 4);
+            for (int r = warp; r < 4 * N; r += 8, src += 8 * pitch, dst += 8 * kXferPad * 4)
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(nbytes) : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
+#pragma unroll 4
+    for (int j = warp; j < NP; j += 8) sS[lane * SST + j] = in && j < N ? S[(long long)j * pitch + kl] : (unsigned char)0;
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncthreads();
+    // Z = the leading occupied slots.  A caller's S must hold bead indices 1..N there and 0 after
+    // them; anything else would send the step kernel's scatter outside the chain.  Such a chain keeps its
+    // valid leading slots only, the rest is cleared, and the flag makes ssm_set_state fail.
+    // Eight threads per chain, thread q looks at the slots [q NS, (q + 1) NS) of its chain.
+    {
+        constexpr int NS = NP >= 32 ? NP / 8 : 4, NQ = NP / NS;     // slots per thread, threads of a chain that have any
+        const int c32 = threadIdx.x >> 3, q = threadIdx.x & 7;
+        unsigned *sp = reinterpret_cast<unsigned *>(sS + c32 * SST) + q * (NS / 4);
+        unsigned wd[NS / 4];
+        int lead = 0;
+        bool run = q < NQ;
+#pragma unroll
+        for (int i = 0; i < NS / 4; ++i) {
+            wd[i] = q < NQ ? sp[i] : 0u;
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const unsigned by = (wd[i] >> (8 * e)) & 0xFFu;
+                run = run && by != 0u && by <= (unsigned)N;
+                lead += run ? 1 : 0;
+            }
+        }
+        // the chain's first thread whose slots are not all occupied
+        const unsigned fullmask = (__ballot_sync(0xffffffffu, run) >> (lane & 24)) & 0xFFu;
+        const int qs = __ffs(~fullmask) - 1;                                  // 0..8
+        const int lead_s = __shfl_sync(0xffffffffu, lead, (lane & 24) + (qs & 7));
+        const int Z = qs >= NQ ? NP : qs * NS + lead_s;
+        SSM_ASSERT(Z >= 0 && Z <= N);
+        // whatever sits at or after slot Z is cleared
+        bool bad = false;
+        if (q < NQ && q >= qs) {
+#pragma unroll
+            for (int i = 0; i < NS / 4; ++i) {
+                unsigned keep = 0u;
+#pragma unroll
+                for (int e = 0; e < 4; ++e)
+                    if (q * NS + 4 * i + e < Z) keep |= 0xFFu << (8 * e);
+                if (wd[i] & ~keep) { bad = true; sp[i] = wd[i] & keep; }
+            }
+        }
+        if (bad) atomicExch(bad_state, 1);
+        if (q == 0) sZ[c32] = Z;
+    }
+    __syncthreads();
+    // ---- staging -> tiles (16 bytes per thread, coalesced); beads and anchors: a word belongs to one chain
+    for (int u = warp; u < nt * 14; u += 8) {
+        const int T = u / 14, uu = u - 14 * T;
+        unsigned x[4] = {0u, 0u, 0u, 0u};
+        int c32;
+        uint4 *q;
+        if (uu < 6) {
+            c32 = T * cpw + cwl;
+            const float *sp = stg + (kBPL * gl) * kXferPad + c32;
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int f = 4 * uu + e, qd = f / 3, c = f - 3 * qd;
+                if (kBPL * gl + qd < N) x[e] = __float_as_uint(sp[(c * N + qd) * kXferPad]);
+            }
+            q = g4 + T * W16 + uu * 32 + lane;
+        } else {
+            const int ai = (uu - 6) * 32 + lane, cw = ai >> LNP, j = ai & (NP - 1);
+            c32 = T * cpw + cw;
+            const float *sp = stg + (3 * N + j) * kXferPad + c32;
+            if (j < N) {
+#pragma unroll
+                for (int c = 0; c < 4; ++c) x[c] = __float_as_uint(sp[c * N * kXferPad]);
+            }
+            q = g4 + T * W16 + WR + ai;
+        }
+        SSM_ASSERT(c32 < 32 && T < nt);
+        if (full || chain_in(c32)) *q = make_uint4(x[0], x[1], x[2], x[3]);
+    }
+    // bead indices (16 slots of one chain, or of two 8-bead chains) and Z (4 chains): a word may hold chains in and
+    // out of the range, so a CTA that is not whole blends with what the tile holds
+    for (int i = threadIdx.x; i < nt * (W16 - WR - WA); i += 256) {
+        const int T = i / (W16 - WR - WA), wi = i - T * (W16 - WR - WA);
+        unsigned x[4] = {0u, 0u, 0u, 0u}, keep[4] = {0u, 0u, 0u, 0u};              // keep: bits that stay as they are
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            if (wi >= WS) {
+                const int cw = (wi - WS) * 4 + e, c32 = T * cpw + cw;
+                if (cw >= cpw) continue;
+                if (full || chain_in(c32)) x[e] = (unsigned)sZ[c32]; else keep[e] = 0xFFFFFFFFu;
+            } else {
+                const int bi = wi * 16 + 4 * e, cw = bi >> LNP, j = bi & (NP - 1), c32 = T * cpw + cw;
+                SSM_ASSERT(cw < cpw && j + 3 < NP);
+                if (full || chain_in(c32)) x[e] = *reinterpret_cast<const unsigned *>(sS + c32 * SST + j); else keep[e] = 0xFFFFFFFFu;
+            }
+        }
+        uint4 *q = g4 + T * W16 + WR + WA + wi;
+        if (keep[0] | keep[1] | keep[2] | keep[3]) {
+            const uint4 o = *q;
+            x[0] |= o.x & keep[0]; x[1] |= o.y & keep[1]; x[2] |= o.z & keep[2]; x[3] |= o.w & keep[3];
+        }
+        *q = make_uint4(x[0], x[1], x[2], x[3]);
+    }
+}
+
+template <bool EXPORT, int G>
+static cudaError_t launch_xfer_g(unsigned grid, cudaStream_t st, unsigned char *state, float *R, float *A, unsigned char *S, int N,
+                                 long long k0, long long nk, long long pitch, int hide_low, int *bad_state)
+{
+    // the attribute belongs to the (function, device) pair: remember per device where it has been set
+    static std::atomic<unsigned long long> configured{0ull};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev >= 64 || !((configured.load(std::memory_order_relaxed) >> dev) & 1ull)) {
+        if ((e = cudaFuncSetAttribute(ssm_xfer_kernel<EXPORT, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, xfer_smem(kBPL * G, kBPL * G))) != cudaSuccess) return e;
+        if (dev < 64) configured.fetch_or(1ull << dev, std::memory_order_relaxed);
+    }
+    ssm_xfer_kernel<EXPORT, G><<<grid, 256, xfer_smem(N, kBPL * G), st>>>(state, R, A, S, N, k0, nk, pitch, hide_low, bad_state);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_xfer(bool do_export, unsigned char *state, float *R, float *A, unsigned char *S, int N,
                         long long k0, long long nk, long long pitch, int hide_low, int *bad_state, cudaStream_t st)
 {
     if (nk <= 0) return cudaSuccess;
-    const int NP = padded_beads(N);
-    const size_t smem = (size_t)(NP / kBPL) * kTileBytes;
     const unsigned grid = (unsigned)((k0 + nk - 1) / 32 - k0 / 32 + 1);
-    cudaError_t e;
-    if (do_export) {
-        if ((e = cudaFuncSetAttribute(ssm_xfer_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-        ssm_xfer_kernel<true><<<grid, 256, smem, st>>>(state, R, A, S, N, NP, k0, nk, pitch, hide_low, bad_state);
-    } else {
-        if ((e = cudaFuncSetAttribute(ssm_xfer_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-        ssm_xfer_kernel<false><<<grid, 256, smem, st>>>(state, R, A, S, N, NP, k0, nk, pitch, 0, bad_state);
+#define SSM_XFER(G) (do_export ? launch_xfer_g<true, G>(grid, st, state, R, A, S, N, k0, nk, pitch, hide_low, bad_state) \
+                               : launch_xfer_g<false, G>(grid, st, state, R, A, S, N, k0, nk, pitch, 0, bad_state))
+    switch (padded_beads(N)) {
+        case 8: return SSM_XFER(1);
+        case 16: return SSM_XFER(2);
+        case 32: return SSM_XFER(4);
+        case 64: return SSM_XFER(8);
+        case 128: return SSM_XFER(16);
     }
-    return cudaGetLastError();
+#undef SSM_XFER
+    return cudaErrorInvalidValue;
 }
 
 // ---------------------------------------------------------------------------------------
