@@ -129,25 +129,35 @@ ssm_xfer_kernel(unsigned char *state, float *R, float *A, unsigned char *S, int 
     const int cwl = lane >> lg, gl = lane & (G - 1);
     if (EXPORT) {
         // ---- tiles -> staging (16 bytes per thread, coalesced), then staging -> rows
-        for (int u = warp; u < nt * 14; u += 8) {
-            const int T = u / 14, uu = u - 14 * T;
-            if (uu < 6) {
-                const uint4 t = g4[T * W16 + uu * 32 + lane];
-                const unsigned x[4] = {t.x, t.y, t.z, t.w};
-                float *sp = stg + (kBPL * gl) * kXferPad + T * cpw + cwl;
+        // (two units per turn, both loads ahead of the stores: the loop waits for its loads)
+        for (int u0 = warp; u0 < nt * 14; u0 += 16) {
+            uint4 t[2];
+            int ai[2];
 #pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const int f = 4 * uu + e, q = f / 3, c = f - 3 * q;
-                    if (kBPL * gl + q < N) sp[(c * N + q) * kXferPad] = __uint_as_float(x[e]);
-                }
-            } else {
-                const int ai = (uu - 6) * 32 + lane, cw = ai >> LNP, j = ai & (NP - 1);
-                const uint4 t = g4[T * W16 + WR + ai];
-                const unsigned x[4] = {t.x, t.y, t.z, hide_low ? 0u : t.w};
-                float *sp = stg + (3 * N + j) * kXferPad + T * cpw + cw;
-                if (j < N) {
+            for (int h = 0; h < 2; ++h) {
+                const int u = u0 + 8 * h, T = u / 14, uu = u - 14 * T;
+                ai[h] = (uu - 6) * 32 + lane;
+                if (u < nt * 14) t[h] = g4[T * W16 + (uu < 6 ? uu * 32 + lane : WR + ai[h])];
+            }
 #pragma unroll
-                    for (int c = 0; c < 4; ++c) sp[c * N * kXferPad] = __uint_as_float(x[c]);
+            for (int h = 0; h < 2; ++h) {
+                const int u = u0 + 8 * h, T = u / 14, uu = u - 14 * T;
+                if (u >= nt * 14) continue;
+                const unsigned x[4] = {t[h].x, t[h].y, t[h].z, (uu >= 6 && hide_low) ? 0u : t[h].w};
+                if (uu < 6) {
+                    float *sp = stg + (kBPL * gl) * kXferPad + T * cpw + cwl;
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const int f = 4 * uu + e, q = f / 3, c = f - 3 * q;
+                        if (kBPL * gl + q < N) sp[(c * N + q) * kXferPad] = __uint_as_float(x[e]);
+                    }
+                } else {
+                    const int cw = ai[h] >> LNP, j = ai[h] & (NP - 1);
+                    float *sp = stg + (3 * N + j) * kXferPad + T * cpw + cw;
+                    if (j < N) {
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) sp[c * N * kXferPad] = __uint_as_float(x[c]);
+                    }
                 }
             }
         }
