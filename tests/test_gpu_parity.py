@@ -58,7 +58,7 @@ def test_state_import_export_every_shape_and_chunk(ssm):
     """a10: the import / export kernel moves 32 chains (G whole tiles) per CTA through an image of the tiles; chunks
     that start and end inside a tile, ragged bead numbers (N < 8G) and every G must give the same bytes back, and the
     import must count Z (read back as the mean of Z over all chains, exact in int64)."""
-    for N, M in ((8, 203), (16, 77), (20, 131), (32, 300), (80, 45), (128, 70)):
+    for N, M in ((3, 50), (8, 203), (16, 77), (20, 131), (32, 300), (64, 40), (80, 45), (100, 33), (128, 70)):
         e = oracle.Ensemble(N, M, seed=11)
         e.round_to_fp32()
         R, A, S = to_external(e)
