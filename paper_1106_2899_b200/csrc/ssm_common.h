@@ -64,8 +64,8 @@ constexpr int kSmEv = 12816;     // uint [64]   construction candidates [chain][
 constexpr int kSmSamp = 13072;   // int  [32]   per-chain fixed-point sum of d_x d_y over slip-springs (sample steps)
 constexpr int kSmKeys = 3840;    // uint [20]   the warp's copy of the Philox round keys (16-byte aligned)
 constexpr int kSmKap = 3920;     // float[9]   dt kappa of the warp's group of chains (general flow only), up to 3956
-constexpr int kSmPre = 3968;     // uint4[3][8] what rounds 1, 2 of Philox make of (domain, chain) for the NOISE, SLOT and ATTEMPT domains
-                                 //             (ssm_rng.cuh, stream_prefix), chains per warp <= 8 only; up to 4352
+constexpr int kSmPre = 3968;     // uint4[40]   what rounds 1, 2 of Philox make of (domain, chain) (ssm_rng.cuh, stream_prefix): [3][8] for the
+                                 //             NOISE, SLOT and ATTEMPT domains of up to 8 chains per warp, [2][16] (NOISE, SLOT) of 16; up to 4608
 constexpr int kSmSamp2 = 3584;   // int  [2][32] the same for d_y d_z and d_z d_x (isotropic correlator), in the spare kB after the mirror
 constexpr int kStageSteps = 8;   // recorded steps whose warp sums wait in kSmStage before they are added to the CTA sums
 constexpr int kSmStage = 13200;  // int  [8][12] warp sums of the last recorded steps (int32 fixed point)

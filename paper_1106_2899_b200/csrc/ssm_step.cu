@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     // constant offset from the warp's base register (a CTA-wide copy costs an address computation per call)
     const uint4 *Keys = reinterpret_cast<const uint4 *>(wb + kSmKeys);
     // the launch-constant part of the Philox calls of this tile's chains (ssm_rng.cuh, stream_prefix): [domain][chain]
-    constexpr bool PRE = CPW <= 8;
+    constexpr bool PRE = CPW <= 16, PRE_AT = CPW <= 8;      // the table holds 40 entries: three domains of 8 chains, or NOISE and SLOT of 16
     uint4 *Pre = reinterpret_cast<uint4 *>(wb + kSmPre);
     if (lane < 20) reinterpret_cast<unsigned *>(wb + kSmKeys)[lane] = P.rk[lane];
     for (int i = threadIdx.x; i < kMaxFuse * 12; i += kBlockThreads) acc[i] = 0ull;
@@ -224,7 +224,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
             for (int v = 0; v < 8; ++v) A4[v * 32 + lane] = gA[v * 32 + lane];
             reinterpret_cast<uint2 *>(Sb)[lane] = reinterpret_cast<const uint2 *>(tp + kTileS)[lane];
             Zs[lane] = reinterpret_cast<const int *>(tp + kTileZ)[lane];
-            if (PRE && lane < 3 * CPW) {
+            if (PRE && lane < (PRE_AT ? 3 : 2) * CPW) {
                 const StreamKey sk0 = make_stream(P.step0, P.rk);
                 const int dom = lane / CPW, c = lane - dom * CPW;
                 Pre[lane] = stream_prefix(sk0, P.rk, dom == 0 ? DOM_NOISE : (dom == 1 ? DOM_SLOT : DOM_ATTEMPT), chain0 + (uint32_t)c);
@@ -526,7 +526,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
                     SSM_ASSERT(K >= 0 && K <= NA && Z0 >= 0 && Z0 <= NA);
                     if (8 * l < K) {
                         uint32_t w[4];
-                        if (PRE) stream_call_pre(sk, Pre[2 * CPW + cw], (uint32_t)l, w, Keys);
+                        if (PRE_AT) stream_call_pre(sk, Pre[2 * CPW + cw], (uint32_t)l, w, Keys);
                         else stream_call<true>(sk, P.rk, DOM_ATTEMPT, chain, (uint32_t)l, w, Keys);
                         const int hmax = P.h_c2[K];
                         const unsigned m2 = __vminu2(__vminu2(w[0], w[1]), __vminu2(w[2], w[3]));
