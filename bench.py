@@ -429,6 +429,33 @@ def main():
                        "streams, one host thread each, started one upload apart (serial_value: ONE context, one "
                        "thread, ssm_step_from_host = the same upload in chunks overlapped with the stepping of the "
                        "chunks already landed; unpipelined_value: one context, set_state then step)" % (inner, nctx)}
+        # the state import / export kernel alone, full size, device pointers: CUDA events on the
+        # context's stream, median of 5; algorithmic bytes = the rows read / written + the tiles written / read
+        if rank == 0:
+            dRAS = [torch.from_numpy(x).to(dev) for x in (Rp, Ap, Sp)]
+            cpw = 256 // max(8, 1 << (N - 1).bit_length())          # chains per warp tile of 7552 bytes
+            tile_bytes = 7552 * ((M + cpw - 1) // cpw)
+            io_bytes = float(h2d + tile_bytes)
+            io = {}
+            for name, fn in (("import", lambda: pair[0].set_state(dRAS[0], dRAS[1], dRAS[2], step)),
+                             ("export", lambda: pair[0].get_state(dRAS[0], dRAS[1], dRAS[2]))):
+                fn()
+                ts = []
+                for _ in range(5):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    with torch.cuda.stream(pair[0].stream):
+                        e0.record()
+                        fn()
+                        e1.record()
+                    pair[0].stream.synchronize()
+                    ts.append(e0.elapsed_time(e1))
+                io[name + "_ms"] = sorted(ts)[2]
+                io[name + "_GBps"] = io_bytes / (sorted(ts)[2] * 1e-3) / 1e9
+            io["bytes"] = io_bytes
+            io["what"] = ("ssm_set_state / ssm_get_state with device pointers, %d chains (the import's time includes reading "
+                          "back its malformed-state flag)" % M)
+            e2e["state_io"] = io
+            del dRAS
         del solo
         del pair
 
@@ -438,6 +465,9 @@ def main():
         return
 
     peaks = measured_peaks()
+    if e2e is not None and "state_io" in e2e:
+        for name in ("import", "export"):
+            e2e["state_io"][name + "_frac_of_copy_peak"] = e2e["state_io"][name + "_GBps"] / peaks["hbm_gbs"]
     peak_alu = N_SM * SMSP_PER_SM * LANES * peaks["sm_max_mhz"] * 1e6 / 1e12      # T thread-instr/s
     per_launch_updates = float(M) * N * inner * K / max(launches, 1)
     achieved = I_ALG * per_launch_updates / (launch_ms * 1e-3) / 1e12
