@@ -107,6 +107,11 @@ ssm_xfer_kernel(unsigned char *state, float *R, float *A, unsigned char *S, int 
     constexpr int SST = NP + 4;
     unsigned char *sS = xs + 7 * N * kXferPad * 4;                               // [32][SST]
     int *sZ = reinterpret_cast<int *>(sS + 32 * SST);                            // [32]
+#ifdef SSM_CHECK
+    // poisoned shared memory in the checked build (see ssm_step.cu)
+    for (int i = threadIdx.x; i < xfer_smem(N, NP) / 4; i += 256) reinterpret_cast<unsigned *>(xs)[i] = 0xFFFFFFFFu;
+    __syncthreads();
+#endif
     const long long cb = (k0 / 32 + blockIdx.x) * 32;           // first of this CTA's 32 chains
     const long long t0 = cb / cpw, t_last = (k0 + nk - 1) / cpw;
     const int nt = (int)(t_last - t0 + 1 < (long long)G ? t_last - t0 + 1 : (long long)G);    // tiles that exist

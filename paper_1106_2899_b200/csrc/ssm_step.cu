@@ -102,6 +102,13 @@ __global__ void __launch_bounds__(kBlockThreads, 2) ssm_step_kernel(const __grid
     int4 *Stage4 = reinterpret_cast<int4 *>(wb + kSmStage);
     unsigned long long *acc = reinterpret_cast<unsigned long long *>(smem + kSmAcc);
 
+#ifdef SSM_CHECK
+    // the checked build starts from poisoned shared memory (all bits set: NaN as a float, -1 as an index), so that a
+    // read of a word nothing has written shows in the results (tests/test_gpu_sanitize.py compares them with the
+    // product build's bit for bit); stands in for compute-sanitizer's initcheck, which this pool does not run
+    for (int i = threadIdx.x; i < kSmStep / 4; i += kBlockThreads) reinterpret_cast<unsigned *>(smem)[i] = 0xFFFFFFFFu;
+    __syncthreads();
+#endif
     const BoxMuller bm_noise(P.bm_noise), bm_anchor(P.bm_anchor);
     // each warp keeps its own copy of the Philox round keys inside its region: their address is then a
     // constant offset from the warp's base register (a CTA-wide copy costs an address computation per call)

@@ -67,3 +67,53 @@ def test_every_kernel_once_with_device_assertions():
                         "-p", "no:cacheprovider"], cwd=root, env=env, capture_output=True, text=True)
     assert r.returncode == 0, r.stdout[-3000:] + r.stderr[-2000:]
     assert "4 passed" in r.stdout
+
+
+def _digest():
+    """Hashes of everything a set of small runs leaves behind (state, stress sums, correlator sums), over every G,
+    the three kinds of flow, a ragged bead number and the host / device state paths."""
+    import hashlib
+    import paper_1106_2899_b200 as ssm
+    out = []
+    kap = np.array([[0.0, 0.3, 0.0], [0.0, 0.0, 0.1], [0.05, 0.0, 0.0]])
+    for N, M, kw in ((8, 333, dict(sample_every=5, corr_levels=3, corr_components=3)), (16, 250, dict(k_attempts=1)),
+                     (20, 99, dict()), (32, 500, dict(sample_every=10, corr_levels=3)), (64, 60, dict()),
+                     (128, 40, dict(dt=0.005))):
+        g = ssm.Ensemble(N, M, seed=17, stress_every=1, stress_capacity=400, stage_chains=48, **kw)
+        g.step(70)
+        g.step(20, shear_rate=0.3)
+        g.step_kappa(20, kap)
+        R, A, S, step = g.get_state()
+        g.set_state(R, A, S, step)                               # through the import kernel and back into the run
+        g.step(40)
+        R, A, S, _ = g.get_state()
+        m = hashlib.sha1()
+        for x in (R, A, S, g.stress_sums()) + ((g.gt_sums()[0],) if "sample_every" in kw else ()):
+            m.update(np.ascontiguousarray(x).tobytes())
+        out.append(m.hexdigest()[:16])
+    return out
+
+
+def test_checked_build_from_poisoned_shared_memory_gives_the_same_bits():
+    """libssm_check.so fills the shared memory of the step and the import / export kernels with all-ones words before
+    they start (NaN as a float, -1 as an index): if any path read a word nothing had written, its results would
+    differ from the product build's.  They are compared bit for bit.  (Stands in for compute-sanitizer's initcheck,
+    which the B200 pool this was developed on does not run; profiles/r2_sanitizers.md.)"""
+    import json
+    import os
+    import subprocess
+    import sys
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    mine = _digest()
+    env = dict(os.environ, SSM_LIB="check")
+    code = ("import json, sys, importlib.util; sys.path.insert(0, %r); "
+            "sp = importlib.util.spec_from_file_location('sanitize_digest', %r); t = importlib.util.module_from_spec(sp); "
+            "sp.loader.exec_module(t); import paper_1106_2899_b200 as ssm; "
+            "assert ssm.lib()._name.endswith('libssm_check.so'), ssm.lib()._name; "
+            "print('DIGEST ' + json.dumps(t._digest()))" % (root, os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-c", code], cwd=root, env=env, capture_output=True, text=True)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-3000:]
+    theirs = json.loads([l for l in r.stdout.split("\n") if l.startswith("DIGEST ")][-1][7:])
+    assert mine == theirs
