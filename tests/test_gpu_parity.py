@@ -209,6 +209,25 @@ def test_split_runs_fusion_depth_and_ensemble_size_do_not_change_results(ssm):
     assert np.array_equal(R, R0[:, :, 128:192]) and np.array_equal(S, S0[:, 128:192])
 
 
+def test_results_do_not_depend_on_which_warp_runs_a_tile(ssm):
+    """a8: warps draw their tiles first come, first served and add fixed-point integers, so neither the number of CTAs
+    nor the order in which warps arrive may show in anything: one CTA (8 warps walk 500 tiles), three, and the default
+    grid give the same state, stress sums and correlator sums bit for bit; also under shear (compensated anchors)."""
+    N, M = 32, 4000
+    kw = dict(seed=33, stress_every=1, stress_capacity=200, sample_every=4, corr_levels=3)
+    outs = []
+    for blocks in (0, 1, 3):
+        g = ssm.Ensemble(N, M, **kw)
+        g.set_grid(blocks)
+        g.step(70)
+        g.step(30, shear_rate=0.2)
+        R, A, S, _ = g.get_state()
+        outs.append((R, A, S, g.stress_sums(), g.gt_sums()[0]))
+    for o in outs[1:]:
+        for x, y in zip(outs[0], o):
+            assert np.array_equal(x, y)
+
+
 @pytest.mark.parametrize("M,offset,comps", [(512, 0, 1), (500, 7, 1), (512, 0, 3), (500, 7, 3)])
 def test_correlator_matches_oracle_on_identical_trajectories(ssm, M, offset, comps):
     """Rouse limit (no forks): GPU multi-tau sums against the oracle's correlator fed by
