@@ -134,6 +134,26 @@ int ssm_group_stress(ssm_ctx *ctx, int64_t chains_per_group, double *h_out);
 int ssm_step_kappa_device(ssm_ctx *ctx, int64_t n_steps, int64_t chains_per_group, const double *d_kappa);
 int ssm_group_stress_device(ssm_ctx *ctx, int64_t chains_per_group, double *d_out);
 
+/* ssm_group_stress_device for callers that cannot give the library scratch memory.  Which callers: code that runs
+ * inside a host application that owns all of the GPU's memory through its own pool and passes a plug-in nothing but the
+ * buffers of its inputs and outputs (a raw cudaMalloc there fails, or takes memory the pool counts as its own); a
+ * time-critical coupling loop, where cudaMalloc / cudaFree would stall every stream of the device; and a caller whose
+ * workspace staging area -- where ssm_group_stress_device keeps its [groups][13] integer sums -- is in use by a state
+ * transfer queued on another stream.  Here those sums live in an array built into the library itself: 416 KiB of device
+ * memory that every GPU which loads libssm.so holds until the process ends.  Its size is fixed, so at most
+ * SSM_NOALLOC_MAX_GROUPS groups: SSM_ERANGE beyond that (take larger groups, or the _device call).
+ * Arguments and results are those of ssm_group_stress_device, bit for bit: d_out (device) [n_groups][13] double is
+ * written by kernels on the ctx's stream; no host synchronisation; nothing of the workspace but the chain state is read
+ * and nothing of it is written.  The call allocates and frees nothing.
+ *  - The GPU that holds the ctx's workspace must be the current device (SSM_EINVAL otherwise).
+ *  - The first call on each GPU looks up the array's device address (once per device, thread-safe); make that first call
+ *    before any stream capture begins.
+ *  - All calls on one GPU share the one array, which each call clears before use.  Calls queued on ONE stream are safe.
+ *    Calls whose GPU work can overlap (two ctxs on two streams of the same GPU, or two host threads) race on it and
+ *    return garbage: order them yourself, or use ssm_group_stress_device for all but one of them. */
+#define SSM_NOALLOC_MAX_GROUPS 4096
+int ssm_group_stress_noalloc(ssm_ctx *ctx, int64_t chains_per_group, double *d_out);
+
 /* Translate every chain so that its first bead is at the origin, anchors with it.  Nothing observable changes
  * (the model depends on R_i - R_j and R_S - A only: bonds, hop energies, both stresses); under a flow with a
  * stretching direction the chain's centre drifts as exp(kappa t), and a long run (steady elongation) has to call

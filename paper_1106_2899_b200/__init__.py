@@ -13,6 +13,7 @@ import numpy as np
 from . import build as _build
 
 SSM_OK, SSM_EINVAL, SSM_ENOMEM, SSM_ECUDA, SSM_ESTATE, SSM_ERANGE = 0, -1, -2, -3, -4, -5
+NOALLOC_MAX_GROUPS = 4096          # SSM_NOALLOC_MAX_GROUPS of include/ssm.h
 
 EXPORTS = ["ssm_workspace_bytes", "ssm_init", "ssm_step", "ssm_stress_count", "ssm_stress", "ssm_stress_sums",
            "ssm_stress_sums_device", "ssm_chain_stress", "ssm_gt", "ssm_gt_sums", "ssm_get_state", "ssm_set_state",
@@ -20,7 +21,8 @@ EXPORTS = ["ssm_workspace_bytes", "ssm_init", "ssm_step", "ssm_stress_count", "s
            "ssm_moduli", "ssm_eta0", "ssm_tau_d", "ssm_issue_rates",
            "ssm_gt_virtual", "ssm_gt_sums_virtual", "ssm_step_kappa", "ssm_group_stress",
            "ssm_step_kappa_device", "ssm_group_stress_device", "ssm_recenter",
-           "ssm_eta_star", "ssm_stress_from_sums", "ssm_stream_wait_ctx", "ssm_ctx_wait_stream", "ssm_step_from_host"]
+           "ssm_eta_star", "ssm_stress_from_sums", "ssm_stream_wait_ctx", "ssm_ctx_wait_stream", "ssm_step_from_host",
+           "ssm_group_stress_noalloc"]
 
 
 class Params(C.Structure):
@@ -75,6 +77,7 @@ def lib():
     L.ssm_group_stress.argtypes = [vp, C.c_int64, dp]; L.ssm_group_stress.restype = C.c_int
     L.ssm_step_kappa_device.argtypes = [vp, C.c_int64, C.c_int64, vp]; L.ssm_step_kappa_device.restype = C.c_int
     L.ssm_group_stress_device.argtypes = [vp, C.c_int64, vp]; L.ssm_group_stress_device.restype = C.c_int
+    L.ssm_group_stress_noalloc.argtypes = [vp, C.c_int64, vp]; L.ssm_group_stress_noalloc.restype = C.c_int
     L.ssm_recenter.argtypes = [vp]; L.ssm_recenter.restype = C.c_int
     L.ssm_moduli.argtypes = [C.c_int32, dp, dp, C.c_int32, dp, dp, dp]; L.ssm_moduli.restype = C.c_int
     L.ssm_eta0.argtypes = [C.c_int32, dp, dp, dp]; L.ssm_eta0.restype = C.c_int
@@ -214,6 +217,22 @@ class Ensemble:
         assert out.is_cuda and out.dtype == self._torch.float64 and out.is_contiguous() and out.numel() == ng * 13
         with self._torch.cuda.device(self.device):
             self._ck(lib().ssm_group_stress_device(self.h, cpg, C.c_void_p(out.data_ptr())))
+        return out
+
+    def group_stress_noalloc(self, chains_per_group=None, out=None):
+        """ssm_group_stress_noalloc: group_stress_device for callers that may not allocate device memory and have no
+        scratch to lend (a plug-in inside an application whose memory pool owns the GPU, a loop that cannot afford
+        cudaMalloc's device-wide stall).  The intermediate sums sit in a fixed array inside libssm.so, so at most
+        NOALLOC_MAX_GROUPS (4096) groups (SsmError SSM_ERANGE beyond), and calls whose GPU work overlaps race on it:
+        keep them on one stream.  Fills `out`, a CUDA float64 tensor [groups][13] that the CALLER passes (unlike
+        group_stress_device, this method does not create one: that would be an allocation); asynchronous."""
+        cpg = self.M if chains_per_group is None else min(int(chains_per_group), self.M)
+        ng = -(-self.M // cpg)
+        if out is None:
+            raise SsmError(SSM_EINVAL, "group_stress_noalloc: pass the output tensor (this call allocates nothing)")
+        assert out.is_cuda and out.dtype == self._torch.float64 and out.is_contiguous() and out.numel() == ng * 13
+        with self._torch.cuda.device(self.device):
+            self._ck(lib().ssm_group_stress_noalloc(self.h, cpg, C.c_void_p(out.data_ptr())))
         return out
 
     def recenter(self):

@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libssm.so")
 LIB_CHECK = os.path.join(_HERE, "libssm_check.so")       # the same sources with -DSSM_CHECK: device-side assertions on
-SOURCES = ["ssm_step.cu", "ssm_aux.cu", "ssm_api.cu", "ssm_rheo.cu"]
+SOURCES = ["ssm_step.cu", "ssm_aux.cu", "ssm_api.cu", "ssm_rheo.cu", "ssm_noalloc.cu"]
 STEP_G = [1, 2, 4, 8, 16]       # ssm_step.cu is also compiled once per G (-DSSM_G): the kernels of 8G bead places
 OBJ = os.path.join(_HERE, "build")
 HEADERS = ["ssm_common.h", "ssm_rng.cuh", os.path.join("..", "..", "include", "ssm.h")]

@@ -865,3 +865,16 @@ extern "C" void ssm_destroy(ssm_ctx *c)
 }
 
 extern "C" const char *ssm_last_error(const ssm_ctx *c) { return c ? c->err.c_str() : g_err.c_str(); }
+
+// ---------------------------------------------------------------------------------------
+// Access for the library's other translation units (ssm_noalloc.cu) to a ctx, whose layout stays private to this file.
+// ---------------------------------------------------------------------------------------
+namespace ssm {
+void ctx_view(const ssm_ctx *c, CtxView *v)
+{
+    v->state = c->ws + c->lay.state; v->n_beads = c->p.n_beads; v->n_chains = c->p.n_chains; v->cs = c->sp.cs;
+    v->stream = c->st;
+}
+int ctx_fail(ssm_ctx *c, int code, const char *msg) { return fail(c, code, msg); }
+void ctx_add_launches(ssm_ctx *c, int n) { c->launches += n; }
+}  // namespace ssm

@@ -142,6 +142,18 @@ struct CorrParams {
     unsigned char pos[kCorrMaxLevels], filled[kCorrMaxLevels], parity[kCorrMaxLevels];   // at launch start
 };
 
+// What an entry point defined outside ssm_api.cu (ssm_noalloc.cu) may see of a ctx, whose struct is private to
+// ssm_api.cu: the tiled state, the chain geometry, 3/N_s and the stream.  ctx_view fills it; ctx_fail records an
+// error text on the ctx (or on the thread when ctx is null) and returns the code; ctx_add_launches keeps
+// ssm_launch_count honest.
+struct CtxView {
+    const unsigned char *state;   // warp tiles (device)
+    int       n_beads;            // N
+    long long n_chains;           // M
+    float     cs;                 // 3/N_s (eq 76)
+    void     *stream;             // cudaStream_t
+};
+
 // address of bead coordinate / slot entry inside the tiled state (host and device)
 __host__ __device__ inline int padded_beads(int n) { int g = kBPL; while (g < n) g <<= 1; return g; }
 __host__ __device__ inline int chains_per_warp(int n_beads) { return 256 / n_beads; }
