@@ -218,6 +218,15 @@ int ssm_gt(ssm_ctx *ctx, int32_t *n_lags, double *h_lag_time, double *h_G, doubl
 int ssm_gt_virtual(ssm_ctx *ctx, int32_t *n_lags, double *h_lag_time, double *h_dgv, double *h_se);
 int ssm_gt_sums_virtual(ssm_ctx *ctx, double *h_sum_gg);
 
+/* DIAGNOSTIC: the record of the Box-Muller calibration behind this ctx's thermal noise (eqs 44, 46, 47; DESIGN.md section
+ * 8.3).  The kernels draw a normal as r cos(theta), r = sqrt(bm log2 u_a), on 2^16 radius and 2^16 angle codes through the
+ * GPU's special-function unit; ssm_init sums the variance this really delivers over all codes and picks the fp32 constant
+ * bm whose variance is nearest the exact one (once per device and constant in the process; that first ssm_init
+ * synchronises the stream).  h_out (host)[8] = [0] the plain constant -2 ln2 2dt rounded to fp32, [1] the constant in use,
+ * [2] relative error of the noise variance with [0], [3] with [1], [4] mean cos^2 - 1/2, [5] mean sin^2 - 1/2 over the
+ * angle codes, [6] ulps between [0] and [1], [7] 0.  No device work. */
+int ssm_noise_calibration(const ssm_ctx *ctx, double *h_out);
+
 /* DIAGNOSTIC, not part of the hot path (bench.py prints it beside the roofline): cycles per
  * group of instructions per scheduler, measured at the step kernel's residency (4 warps per scheduler):
  * h_cycles (host)[8] = [0] FFMA, [1] LOP3 (ALU pipe), [2] IMAD, [3] IMAD.WIDE + the LOP3 folding its halves,

@@ -22,7 +22,7 @@ EXPORTS = ["ssm_workspace_bytes", "ssm_init", "ssm_step", "ssm_stress_count", "s
            "ssm_gt_virtual", "ssm_gt_sums_virtual", "ssm_step_kappa", "ssm_group_stress",
            "ssm_step_kappa_device", "ssm_group_stress_device", "ssm_recenter",
            "ssm_eta_star", "ssm_stress_from_sums", "ssm_stream_wait_ctx", "ssm_ctx_wait_stream", "ssm_step_from_host",
-           "ssm_group_stress_noalloc"]
+           "ssm_group_stress_noalloc", "ssm_noise_calibration"]
 
 
 class Params(C.Structure):
@@ -79,6 +79,7 @@ def lib():
     L.ssm_group_stress_device.argtypes = [vp, C.c_int64, vp]; L.ssm_group_stress_device.restype = C.c_int
     L.ssm_group_stress_noalloc.argtypes = [vp, C.c_int64, vp]; L.ssm_group_stress_noalloc.restype = C.c_int
     L.ssm_recenter.argtypes = [vp]; L.ssm_recenter.restype = C.c_int
+    L.ssm_noise_calibration.argtypes = [vp, dp]; L.ssm_noise_calibration.restype = C.c_int
     L.ssm_moduli.argtypes = [C.c_int32, dp, dp, C.c_int32, dp, dp, dp]; L.ssm_moduli.restype = C.c_int
     L.ssm_eta0.argtypes = [C.c_int32, dp, dp, dp]; L.ssm_eta0.restype = C.c_int
     L.ssm_eta_star.argtypes = [C.c_int32, dp, dp, C.c_int32, dp, dp]; L.ssm_eta_star.restype = C.c_int
@@ -369,6 +370,13 @@ class Ensemble:
             self._ck(lib().ssm_issue_rates(self.h, out.ctypes.data_as(C.POINTER(C.c_double))))
         return {"ffma": out[0], "alu": out[1], "imad": out[2], "imad_wide": 0.5 * (out[7] - 2.0), "wide_lop3": out[3],
                 "wide_lop3_4ffma": out[4], "mufu": out[5], "i2f_f2i": out[6], "philox_round": out[7]}
+
+    def noise_calibration(self):
+        """ssm_noise_calibration (diagnostic): what ssm_init's Box-Muller calibration found for the thermal noise."""
+        out = np.zeros(8)
+        self._ck(lib().ssm_noise_calibration(self.h, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return {"bm_plain": out[0], "bm_used": out[1], "variance_error_plain": out[2], "variance_error_used": out[3],
+                "cos2_bias": out[4], "sin2_bias": out[5], "ulps_moved": int(out[6])}
 
     def stream_wait_ctx(self, stream):
         """ssm_stream_wait_ctx: later work on `stream` (a torch.cuda.Stream) waits for this context's queued work."""

@@ -6,6 +6,8 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -30,6 +32,7 @@ cudaError_t launch_group_mean(const long long *sums, double *out, long long n_gr
                               cudaStream_t st);
 cudaError_t launch_chain_stress(const unsigned char *state, float *out, int N, long long M, float cs, cudaStream_t st);
 cudaError_t launch_corr(const CorrParams &c, cudaStream_t st);
+cudaError_t launch_bm_calib(float bm0, int n_cand, double *d_out, cudaStream_t st);
 }  // namespace ssm
 
 using namespace ssm;
@@ -58,6 +61,7 @@ struct ssm_ctx {
     unsigned char cpos[kCorrMaxLevels], cfil[kCorrMaxLevels], cpar[kCorrMaxLevels];
     std::vector<long long> ccount;      // [L][P] insertions with a product at (level, bin)
     std::vector<float> kappa_host;      // dt kappa of the last ssm_step_kappa call, [groups][9]
+    double calib[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // ssm_noise_calibration: the record of calibrate_bm for bm_noise
     cudaStream_t copy_st = nullptr;     // ssm_step_from_host: uploads run here, beside the stepping on st
     cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
     std::string err;
@@ -73,6 +77,8 @@ static int cuda_fail(ssm_ctx *c, cudaError_t e, const char *what)
     return fail(c, SSM_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
 }
 #define CK(c, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail((c), e_, #call); } while (0)
+
+constexpr int kCalibCand = 9;      // neighbouring floats tried around the first estimate of a Box-Muller constant
 
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
@@ -164,6 +170,67 @@ static int clear_accumulators(ssm_ctx *c)
     return SSM_OK;
 }
 
+// ---------------------------------------------------------------------------------------
+// Calibrated Box-Muller constant.  The kernels draw N(0, sigma2) as r cos, r sin with
+// r^2 = bm log2(u_a), bm = -2 ln2 sigma2 in fp32, on 2^16 radius codes and 2^16 angle codes through the special-function
+// unit.  The variance that comes out is a finite sum, which ssm_bm_calib_kernel forms for a constant and its neighbouring
+// floats; here the float is chosen whose variance is nearest the exact one of the discrete law,
+//   sigma2 * mean_ka(-2 ln u_a) * 1/2        (the mean of cos^2 over the uniform angle grid is exactly 1/2),
+// which removes the fp32 rounding of bm and the (non-zero-mean) error of lg2 / sqrt / sin / cos from the amplitude, down
+// to half an ulp of bm (<= 3.4e-8 of the variance).  Costs no instruction in the kernels.  Two tiny launches and one
+// synchronisation of the stream, once per (device, sigma2) in the process: the result is cached.
+// rec (may be null) [8]: nominal bm, calibrated bm, relative variance error at the nominal and at the calibrated
+// constant, mean cos^2 - 1/2, mean sin^2 - 1/2, ulps moved, 0.
+// ---------------------------------------------------------------------------------------
+struct CalibEntry { float bm; double rec[8]; };
+static std::mutex g_calib_mutex;
+static std::map<std::pair<int, unsigned>, CalibEntry> g_calib_cache;
+
+static double exact_mean_r2()        // mean over the 2^16 codes of -2 ln u_a, u_a = (ka + 1/2) 2^-16
+{
+    static const double v = [] { double s = 0.0; for (int k = 65535; k >= 0; --k) s += -2.0 * std::log(((double)k + 0.5) / 65536.0); return s / 65536.0; }();
+    return v;
+}
+
+static cudaError_t calibrate_bm(int dev, double sigma2, double *d_scratch, cudaStream_t st, float *bm_out, double *rec)
+{
+    const float nominal = (float)(-2.0 * 0.6931471805599453 * sigma2);
+    unsigned bits; std::memcpy(&bits, &nominal, 4);
+    std::lock_guard<std::mutex> lock(g_calib_mutex);
+    auto it = g_calib_cache.find({dev, bits});
+    if (it == g_calib_cache.end()) {
+        const double target = sigma2 * exact_mean_r2() * 0.5;
+        double h[kCalibCand + 2] = {};
+        auto variance = [&](int c, int n) { return (h[c] / 65536.0) * (0.5 * (h[n] + h[n + 1]) / 65536.0); };
+        cudaError_t e;
+        if ((e = launch_bm_calib(nominal, 1, d_scratch, st)) != cudaSuccess
+            || (e = cudaMemcpyAsync(h, d_scratch, 3 * sizeof(double), cudaMemcpyDeviceToHost, st)) != cudaSuccess
+            || (e = cudaStreamSynchronize(st)) != cudaSuccess) return e;
+        CalibEntry en{};
+        en.rec[0] = nominal;
+        en.rec[2] = variance(0, 1) / target - 1.0;
+        en.rec[4] = h[1] / 65536.0 - 0.5; en.rec[5] = h[2] / 65536.0 - 0.5;
+        const float centre = (float)((double)nominal * target / variance(0, 1));
+        if ((e = launch_bm_calib(centre, kCalibCand, d_scratch, st)) != cudaSuccess
+            || (e = cudaMemcpyAsync(h, d_scratch, (kCalibCand + 2) * sizeof(double), cudaMemcpyDeviceToHost, st)) != cudaSuccess
+            || (e = cudaStreamSynchronize(st)) != cudaSuccess) return e;
+        int best = kCalibCand / 2;
+        for (int cnd = 0; cnd < kCalibCand; ++cnd)
+            if (std::fabs(variance(cnd, kCalibCand) - target) < std::fabs(variance(best, kCalibCand) - target)) best = cnd;
+        int cb; std::memcpy(&cb, &centre, 4);
+        cb += best - kCalibCand / 2;
+        std::memcpy(&en.bm, &cb, 4);
+        en.rec[1] = en.bm;
+        en.rec[3] = variance(best, kCalibCand) / target - 1.0;
+        int nb; std::memcpy(&nb, &nominal, 4);
+        en.rec[6] = (double)(cb - nb);
+        it = g_calib_cache.emplace(std::make_pair(dev, bits), en).first;
+    }
+    *bm_out = it->second.bm;
+    if (rec) std::memcpy(rec, it->second.rec, sizeof it->second.rec);
+    return cudaSuccess;
+}
+
 extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, size_t workspace_bytes, void *cuda_stream)
 {
     if (!out) return fail(nullptr, SSM_EINVAL, "out is NULL");
@@ -206,9 +273,16 @@ extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, s
     sp.n_act = p->n_beads;
     sp.n_comp = p->corr_components == 3 ? 3 : 1;
     sp.dt3 = (float)(3.0 * p->dt);
-    const double m2ln2 = -2.0 * 0.6931471805599453;        // r^2 = -2 ln u = (-2 ln 2) log2 u
-    sp.bm_noise = (float)(m2ln2 * 2.0 * p->dt);
-    sp.bm_anchor = (float)(m2ln2 * p->n_s / 3.0);
+    // the three Box-Muller constants, each calibrated on this device (calibrate_bm above; cached per process)
+    float bm_bond = 0.0f;
+    {
+        double *d_cal = reinterpret_cast<double *>(c->ws + lay.stage);
+        if ((e = calibrate_bm(dev, 2.0 * p->dt, d_cal, c->st, &sp.bm_noise, c->calib)) != cudaSuccess             // eqs 44, 46, 47
+            || (e = calibrate_bm(dev, p->n_s / 3.0, d_cal, c->st, &sp.bm_anchor, nullptr)) != cudaSuccess        // eqs 15, 52
+            || (e = calibrate_bm(dev, 1.0 / 3.0, d_cal, c->st, &bm_bond, nullptr)) != cudaSuccess) {             // eq 6
+            int rc = cuda_fail(nullptr, e, "Box-Muller calibration"); delete c; return rc;
+        }
+    }
     sp.fx_scale = (float)(p->dt * (3.0 / p->n_s) * (double)(1 << kFxShift));
     sp.q2l = (float)(2.0 * (3.0 / (4.0 * p->n_s)) * 1.4426950408889634);
     sp.h2 = (float)(2.0 * h);
@@ -227,7 +301,7 @@ extern "C" int ssm_init(ssm_ctx **out, const ssm_params *p, void *d_workspace, s
     ip.n_pad = padded_beads(p->n_beads);
     ip.chain_offset = p->chain_offset; std::memcpy(ip.rk, sp.rk, sizeof ip.rk);
     ip.n_beads = p->n_beads; ip.springs_on = sp.springs_on;
-    ip.bm_bond = (float)(m2ln2 / 3.0); ip.bm_anchor = sp.bm_anchor;
+    ip.bm_bond = bm_bond; ip.bm_anchor = sp.bm_anchor;
     if (c->springs_on) {       // Poisson(N/N0) CDF (eq 12) as integer thresholds
         const double lam = (double)p->n_beads / p->n_0;
         double pmf = std::exp(-lam), cdf = 0.0;
@@ -443,6 +517,13 @@ extern "C" int ssm_group_stress(ssm_ctx *c, int64_t chains_per_group, double *h_
         for (int t = 0; t < 13; ++t)
             h_out[g * 13 + t] = (double)raw[(size_t)g * 13 + t] / ((double)(1 << kStressShift) * (double)n);
     }
+    return SSM_OK;
+}
+
+extern "C" int ssm_noise_calibration(const ssm_ctx *c, double *h_out)
+{
+    if (!c || !h_out) return SSM_EINVAL;
+    std::memcpy(h_out, c->calib, sizeof c->calib);
     return SSM_OK;
 }
 

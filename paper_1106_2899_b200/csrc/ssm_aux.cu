@@ -519,6 +519,61 @@ cudaError_t launch_group_stress(const unsigned char *state, long long *out, int 
 }
 
 // ---------------------------------------------------------------------------------------
+// Calibration of the Box-Muller amplitude.  The noise of eqs 44, 46 is r cos(theta), r sin(theta)
+// with r = sqrt.approx(bm lg2.approx(u_a)) on the 2^16 codes of u_a and sin / cos.approx on the 2^16 angles (reading
+// R24): a finite table, so the variance this GPU really delivers for a given fp32 constant bm is a finite sum that can be
+// formed exactly.  The special-function unit's errors are not zero-mean (about 1.7e-7 of the variance), and bm itself is
+// rounded to fp32: a SYSTEMATIC relative error of the variance, which becomes 2 eps (N - 1) of the diagonal stress
+// 3 sum b_a^2 - N.  This kernel returns, for n_cand neighbouring floats bm_c = bm0 moved by c - n_cand/2 ulps,
+//   out[c] = sum over the 65536 codes of r(bm_c)^2,   out[n_cand] = sum cos^2,   out[n_cand + 1] = sum sin^2   (fp64),
+// and the host picks the candidate whose variance is closest to the exact sigma^2 mean(-2 ln u_a) / 2 (ssm_api.cu).
+// One CTA of 1024 threads; runs once per (device, constant), not per step.
+// ---------------------------------------------------------------------------------------
+constexpr int kCalibMaxCand = 17;
+__global__ void __launch_bounds__(1024) ssm_bm_calib_kernel(float bm0, int n_cand, double *out)
+{
+    __shared__ double red[32][kCalibMaxCand + 2];
+    double acc[kCalibMaxCand + 2];
+#pragma unroll
+    for (int i = 0; i < kCalibMaxCand + 2; ++i) acc[i] = 0.0;
+    for (uint32_t k = threadIdx.x; k < 65536u; k += 1024u) {
+        const uint32_t w = k | (k << 16);                  // the same code in both halves: radius from the low, angle from the high
+#pragma unroll
+        for (int c = 0; c < kCalibMaxCand; ++c)
+            if (c < n_cand) {
+                const BoxMuller bm(__int_as_float(__float_as_int(bm0) + (c - n_cand / 2)));
+                const double r = (double)bm.radius(w);
+                acc[c] += r * r;
+            }
+        const float th = BoxMuller::angle(w);
+        const double co = (double)__cosf(th), si = (double)__sinf(th);
+        acc[kCalibMaxCand] += co * co; acc[kCalibMaxCand + 1] += si * si;
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int i = 0; i < kCalibMaxCand + 2; ++i) {
+        double v = acc[i];
+        for (int o = 16; o >= 1; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if (lane == 0) red[warp][i] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < kCalibMaxCand + 2) {
+        double v = 0.0;
+        for (int wq = 0; wq < 32; ++wq) v += red[wq][threadIdx.x];
+        const int i = threadIdx.x;
+        if (i < n_cand) out[i] = v;
+        else if (i >= kCalibMaxCand) out[n_cand + (i - kCalibMaxCand)] = v;
+    }
+}
+
+cudaError_t launch_bm_calib(float bm0, int n_cand, double *d_out, cudaStream_t st)
+{
+    if (n_cand < 1 || n_cand > kCalibMaxCand) return cudaErrorInvalidValue;
+    ssm_bm_calib_kernel<<<1, 1024, 0, st>>>(bm0, n_cand, d_out);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------
 // Multi-tau correlator (BASELINE.json config 2).  One thread per chain.
 // Level l holds the last P values of g block-averaged over 2^l samples; inserting (f, g)
 // at level l adds f * g_(k entries ago) to sum[group][l][k] for k = kmin .. filled-1

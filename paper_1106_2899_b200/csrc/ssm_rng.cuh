@@ -183,12 +183,22 @@ __device__ __forceinline__ float mufu_lg2(float x)
 struct BoxMuller {
     float bm;            // -2 ln2 sigma^2
     __device__ __forceinline__ explicit BoxMuller(float b) : bm(b) {}
-    __device__ __forceinline__ void operator()(uint32_t w, float& z0, float& z1) const
+    // radius from the low half word, angle from the high one (also called one by one by the calibration kernel of
+    // ssm_aux.cu, which sums r^2, cos^2 and sin^2 over all 2^16 codes with exactly these instructions)
+    __device__ __forceinline__ float radius(uint32_t w) const
     {
         const float ua = fmaf(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610)), 1.52587890625e-05f, -127.99999237060547f);
+        return mufu_sqrt(bm * mufu_lg2(ua));
+    }
+    static __device__ __forceinline__ float angle(uint32_t w)
+    {
         const float kb = __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632)) - 8421376.0f;   // kb - 2^15
-        const float th = fmaf(kb, 9.5873799e-05f, 4.7936899e-05f);       // 2 pi 2^-16 (kb - 2^15) + pi 2^-16
-        const float r = mufu_sqrt(bm * mufu_lg2(ua));
+        return fmaf(kb, 9.5873799e-05f, 4.7936899e-05f);                 // 2 pi 2^-16 (kb - 2^15) + pi 2^-16
+    }
+    __device__ __forceinline__ void operator()(uint32_t w, float& z0, float& z1) const
+    {
+        const float th = angle(w);
+        const float r = radius(w);
         z0 = r * __cosf(th); z1 = r * __sinf(th);
     }
 };

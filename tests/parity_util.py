@@ -68,21 +68,18 @@ def compare_chain_stress_sums(e, g):
     cannot have forked yet: the mean over those chains of the oracle's per-chain sigma, sigma^(v) (eqs 16, 76) against
     the mean over the SAME chains of the GPU's ssm_chain_stress.
 
-    Tolerance: TOL relative, |d| <= TOL max(1, |sigma|), for the nine components that are plain sums.  The three
-    diagonal components of sigma are a DIFFERENCE, sigma_aa = 3 sum_bonds b_a^2 - N (eq 16): the bond virial is a sum
-    of N - 1 positive terms of order one and the exact constant N is subtracted from it.  The virial follows the
-    noise amplitude sqrt(2 dt) w, which the GPU forms with the special-function unit (lg2, sqrt: relative error up to
-    2^-22, not zero-mean) from fp32 constants (relative 2^-24): a systematic relative error eps of the amplitude is
-    2 eps of every b_a^2, i.e. 2 eps (N - 1) of sigma_aa, which no averaging over chains removes.  So those three are
-    bounded by TOL max(1, |sigma_aa|) + 2 x 2^-22 (N - 1) -- still 1e-5 of the virial itself at every N
-    (DESIGN.md section 8.3).  Returns (chains compared, worst ratio to the bound)."""
+    Tolerance: north_star's, TOL relative, |d| <= TOL max(1, |sigma|), on all twelve components.  (Until round 3 the
+    three diagonal components of sigma, 3 sum_bonds b_a^2 - N, needed 2 x 2^-22 (N - 1) more: the noise amplitude had a
+    systematic relative error of 1.4e-7 from the special-function unit and the fp32 constant, which the difference
+    with N magnifies.  ssm_init now calibrates that constant, and the worst ratio to the plain
+    bound measured over N = 8..128 and steps 1..2000 is 0.11.)  Returns (chains compared, worst ratio to the bound)."""
     cs = g.chain_stress()                                   # [12][M] of the GPU's current state
     ok = np.nonzero((e.first_fragile < 0) | (e.first_fragile >= e.step))[0]
     want = np.array([np.concatenate(e.chain_stress(int(k))) for k in ok]).mean(0)
     got = cs.T[ok].astype(np.float64).mean(0)
     bound = TOL * np.maximum(1.0, np.abs(want))
-    bound[:3] += 2.0 * 2.0 ** -22 * (e.N - 1)
     ratio = np.abs(got - want) / bound
+    print("stress sums over unforked chains: N=%d step=%d chains=%d |gpu - oracle| / bound = %s" % (e.N, e.step, len(ok), np.round(ratio, 2)))
     assert ratio.max() <= 1.0, ("stress summed over the %d unforked chains: |gpu - oracle| / bound = %s"
                                 % (len(ok), np.round(ratio, 2)))
     return len(ok), float(ratio.max())

@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 
 import oracle
-from parity_util import GUARD, TOL, close, compare_state, upload
+from parity_util import GUARD, TOL, close, compare_chain_stress_sums, compare_state, upload
 
 pytestmark = pytest.mark.gpu
 
@@ -34,7 +34,7 @@ def _min_unflagged(M, N, steps):
     return M * f - 4.0 * np.sqrt(M * f * (1.0 - f)) - 1.0
 
 
-@pytest.mark.parametrize("N,M,steps", [(8, 256, 1000), (32, 100, 1000), (128, 19, 200), (20, 100, 300), (80, 10, 200)])
+@pytest.mark.parametrize("N,M,steps", [(8, 256, 1000), (32, 100, 1000), (128, 160, 200), (20, 100, 300), (80, 100, 200)])
 def test_general_kappa_one_group(ssm, N, M, steps):
     """The flow itself amplifies every perturbation, rounding included, by |exp(kappa t)| (measured: 2e-5 at
     t = 10 under KAPPA, where positions have grown ninefold, against 2.4e-6 without flow), so the 1000-step runs
@@ -50,13 +50,17 @@ def test_general_kappa_one_group(ssm, N, M, steps):
         done = upto
         n, worst = compare_state(e, g)
         assert n >= _min_unflagged(M, N, upto), (upto, n)
+        compare_chain_stress_sums(e, g)                      # stress summed over the unforked chains, 1e-5, at every dump
     want, got = np.concatenate(wants), g.stress()
     first = e.first_fragile[e.first_fragile >= 0]
     clean = int(first.min()) if first.size else steps
-    # a mean over M chains of single-chain errors of about 2e-5 sqrt(N/8)
-    ok, w = close(got[:clean], want[:clean], max(TOL, 3e-5 * np.sqrt(N / 8.0) / np.sqrt(M)))
+    # the recorded ensemble stress at north_star's 1e-5 (M is large enough for the mean over chains to average the
+    # fp32 rounding of single chains below it)
+    ok, w = close(got[:clean], want[:clean], TOL)
+    print("kappa ensemble stress N=%d M=%d clean=%d worst/TOL=%.2f" % (N, M, clean, w / TOL))
     assert ok, "ensemble stress off by %.3g over the first %d steps" % (w, clean)
-    assert clean >= 3
+    assert clean >= 3 or M * N > 4000    # (with tens of thousands of hop decisions per step the first fragile one comes at once;
+                                         # the sums over the unforked chains above then carry the comparison)
 
 
 def test_simple_shear_through_the_tensor_equals_ssm_step(ssm):
@@ -98,7 +102,7 @@ def test_small_rates_do_not_stagnate(ssm):
 
 
 def test_groups_with_their_own_tensors_and_group_stress(ssm):
-    N, M, cpg, steps = 32, 96, 32, 200                       # 3 groups of 32 chains = 8 warp tiles each
+    N, M, cpg, steps = 32, 192, 64, 200                      # 3 groups of 64 chains = 8 warp tiles each
     kap = np.stack([KAPPA, np.zeros((3, 3)), -0.5 * KAPPA.T])
     e = oracle.Ensemble(N, M, seed=13)
     g = ssm.Ensemble(N, M, seed=13)
@@ -115,7 +119,7 @@ def test_groups_with_their_own_tensors_and_group_stress(ssm):
     Z = (S > 0).sum(0)
     for grp in range(3):
         sl = slice(grp * cpg, (grp + 1) * cpg)
-        assert np.allclose(got[grp, :12], per_chain[:, sl].astype(np.float64).mean(1), rtol=0, atol=2e-5)
+        assert np.allclose(got[grp, :12], per_chain[:, sl].astype(np.float64).mean(1), rtol=0, atol=TOL)
         assert abs(got[grp, 12] - Z[sl].mean()) < 1e-9
     # and against the oracle on the chains that cannot have forked
     ok = e.first_fragile < 0
@@ -123,13 +127,14 @@ def test_groups_with_their_own_tensors_and_group_stress(ssm):
         ks = [k for k in range(grp * cpg, (grp + 1) * cpg) if ok[k]]
         if len(ks) == cpg:
             want = np.mean([np.concatenate(e.chain_stress(k)) for k in ks], axis=0)
-            good, w = close(got[grp, :12], want, 2e-5)
+            good, w = close(got[grp, :12], want, TOL)
+            print("group %d stress vs oracle worst/TOL=%.2f" % (grp, w / TOL))
             assert good, (grp, w)
     # one group over everything, and a group size that does not divide M
     all1 = g.group_stress()
-    assert np.allclose(all1[0, :12], per_chain.astype(np.float64).mean(1), atol=2e-5)
-    g5 = g.group_stress(40)
-    assert g5.shape == (3, 13) and abs(g5[2, 12] - Z[80:].mean()) < 1e-9
+    assert np.allclose(all1[0, :12], per_chain.astype(np.float64).mean(1), atol=TOL)
+    g5 = g.group_stress(80)
+    assert g5.shape == (3, 13) and abs(g5[2, 12] - Z[160:].mean()) < 1e-9
 
 
 def test_device_variants_of_the_group_calls_equal_the_host_ones(ssm):
@@ -171,7 +176,7 @@ def test_split_calls_and_fusion_depth_do_not_change_results(ssm):
 
 # ----------------------------------------------------------------------------- any N (the paper's 10, 20, 40, 80)
 @pytest.mark.parametrize("N,M,steps", [(2, 70, 200), (3, 70, 200), (9, 50, 300), (10, 300, 1000), (20, 100, 1000),
-                                       (40, 50, 500), (80, 19, 200), (127, 9, 100)])
+                                       (40, 50, 500), (80, 100, 200), (127, 150, 100)])
 def test_bead_numbers_that_do_not_fill_the_lanes(ssm, N, M, steps):
     """The paper runs N = 10, 20, 40, 80 (Figs 1-6); a chain occupies 8, 16, 32, 64 or 128 bead places and the
     places beyond N are padding.  Device init (a0) and the step (a1-a8) against the oracle, as for the full sizes."""
@@ -189,13 +194,18 @@ def test_bead_numbers_that_do_not_fill_the_lanes(ssm, N, M, steps):
     assert n >= _min_unflagged(M, N, steps), n
     first = e.first_fragile[e.first_fragile >= 0]
     clean = int(first.min()) if first.size else steps
-    ok, w = close(g.stress()[:clean], want[:clean], max(TOL, 3e-5 * np.sqrt(max(N, 8) / 8.0) / np.sqrt(M)))
+    ok, w = close(g.stress()[:clean], want[:clean], TOL)
+    print("any-N ensemble stress N=%d M=%d clean=%d worst/TOL=%.2f" % (N, M, clean, w / TOL))
     assert ok, "ensemble stress off by %.3g over the first %d steps" % (w, clean)
-    # per-chain and per-group stresses of the final state on the chains that cannot have forked
+    # the stress summed over the chains that cannot have forked, final state, at 1e-5 (north_star's quantity) ...
+    compare_chain_stress_sums(e, g)
+    # ... and, as an extra, chain by chain: ONE chain's 3 sum b_a b_b carries the fp32 rounding of its N - 1 bonds with
+    # no averaging, 6 |b| delta_b sqrt(N - 1) with delta_b ~ 3e-6, above 1e-5 by construction
     cs = g.chain_stress()
     sel = e.first_fragile < 0
     want_c = np.array([np.concatenate(e.chain_stress(k)) for k in np.nonzero(sel)[0]])
     good, w = close(cs.T[sel], want_c, 2e-5 * np.sqrt(max(N, 8) / 8.0))
+    print("any-N per-chain stress N=%d worst/TOL=%.2f" % (N, w / TOL))
     assert good, w
     assert abs(g.group_stress()[0, 12] - e.Z.mean()) < (1e-9 if sel.all() else 1.0)
 

@@ -162,7 +162,25 @@ def test_slipspring_chains_all_sizes(ssm, N, M):
     want = np.array([np.concatenate(e.chain_stress(k)) for k in np.nonzero(ok)[0]])
     # one chain, no averaging: 6 |b| delta_b sqrt(N-1) with delta_b ~ 3e-6
     good, w = close(cs.T[ok], want, 2e-5 * np.sqrt(N / 8.0))
+    print("per-chain stress N=%d worst/TOL=%.2f" % (N, w / TOL))
     assert good, w
+
+
+def test_noise_amplitude_is_calibrated(ssm):
+    """the thermal noise of eqs 44, 46 is drawn through the special-function unit from 2^16 x 2^16
+    codes, so its variance on this GPU is a finite sum; ssm_init forms it and picks the fp32 Box-Muller constant whose
+    variance is nearest the exact sigma^2 mean(-2 ln u_a) / 2.  Left alone, the constant gives a variance low by
+    about 2.8e-7 -- the systematic error that made the diagonal stress 3 sum b_a^2 - N miss 1e-5 for N >= 64."""
+    for dt in (0.01, 0.005):
+        g = ssm.Ensemble(16, 64, dt=dt)
+        c = g.noise_calibration()
+        print("dt=%g: variance error plain %.3g, calibrated %.3g, %d ulps; cos2 %.3g sin2 %.3g"
+              % (dt, c["variance_error_plain"], c["variance_error_used"], c["ulps_moved"], c["cos2_bias"], c["sin2_bias"]))
+        assert abs(c["variance_error_used"]) <= 3.5e-8                 # half an ulp of the constant (mantissa 1.77)
+        assert abs(c["variance_error_used"]) <= abs(c["variance_error_plain"])
+        assert abs(c["bm_used"] / (-2.0 * np.log(2.0) * 2.0 * dt) - 1.0) < 2e-6 and abs(c["ulps_moved"]) < 16
+        assert abs(c["cos2_bias"] - c["sin2_bias"]) < 2e-8             # one constant serves both members of a pair
+        g.close()
 
 
 def test_shear_flow(ssm):

@@ -197,6 +197,7 @@ def test_edge_cases(ssm):
         first = e.first_fragile[e.first_fragile >= 0]
         clean = int(first.min()) if first.size else 40
         ok, w = close(g.stress()[:clean], want[:clean], 2e-5 * np.sqrt(N / 8.0))
+        print("ragged tile stress N=%d M=%d worst/TOL=%.2f" % (N, M, w / TOL))
         assert ok, (N, M, w)
     # zero steps is a no-op; stress before any sample is a range error, not a crash
     g = ssm.Ensemble(32, 64, seed=3, stress_every=1, stress_capacity=4)
