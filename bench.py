@@ -33,7 +33,7 @@ if ROOT not in sys.path:
 I_ALG = 95.0
 # of which 32 x 32 -> 64-bit multiplies (IMAD.WIDE) of Philox: 0.594 calls x 20.  On B200 each of them holds the issue
 # port for about three cycles beyond its own slot (other instructions do not overlap it: profiles/r2_issue_model.md);
-# ssm_issue_rates() measures that cost live for the rate-weighted fraction.
+# ssm_issue_rates8() measures that cost live for the rate-weighted fraction.
 I_ALG_WIDE = 0.59375 * 20.0
 N_SM, SMSP_PER_SM, LANES = 148, 4, 32
 
@@ -495,7 +495,7 @@ def main():
                      "rate_weighted": {"frac": weighted / peak_alu, "i_alg_issue_cycles_per_bead_update": i_alg_cycles,
                                        "measured_cycles_per_warp_instruction": rates,
                                        "how": "as frac, but the %.1f IMAD.WIDE of the algorithmic count are charged the "
-                                              "issue cycles ssm_issue_rates() measures for them on this GPU instead of 1"
+                                              "issue cycles ssm_issue_rates8() measures for them on this GPU instead of 1"
                                               % I_ALG_WIDE},
                      "peak_how": "148 SM x 4 SMSP x 32 lanes x %.0f MHz (sm_max_mhz, %s)" % (peaks["sm_max_mhz"], peaks["source"]),
                      "hbm": {"achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",

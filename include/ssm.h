@@ -232,8 +232,9 @@ int ssm_noise_calibration(const ssm_ctx *ctx, double *h_out);
  * h_cycles (host)[8] = [0] FFMA, [1] LOP3 (ALU pipe), [2] IMAD, [3] IMAD.WIDE + the LOP3 folding its halves,
  * [4] the same + 4 FFMA (they do not hide under the multiply: it holds the issue port), [5] MUFU, [6] I2FP + F2I,
  * [7] the instructions of one Philox round (2 multiplies, 2 LOP3).  Runs short kernels on the ctx's stream, uses the workspace's staging
- * area (nothing of the ensemble is touched) and synchronises. */
-int ssm_issue_rates(ssm_ctx *ctx, double *h_cycles);
+ * area (nothing of the ensemble is touched) and synchronises.  (The 8 in the name is the length of h_cycles: round 1's
+ * ssm_issue_rates wrote 4 doubles, and a caller built against it must fail to link rather than be overrun.) */
+int ssm_issue_rates8(ssm_ctx *ctx, double *h_cycles);
 
 /* Host post-processing of a tabulated G(t) (section 4.1); no device work, no ctx.
  * h_t[n_lags] strictly increasing lag times >= 0 (as ssm_gt returns them), h_G[n_lags].  All (host).
@@ -267,10 +268,20 @@ int ssm_gt_sums(ssm_ctx *ctx, double *h_sum, int64_t *h_count);
 int ssm_get_state(ssm_ctx *ctx, float *R, float *A, uint8_t *S, int64_t *global_step,
                   int pointers_are_device);
 /* ssm_set_state checks S on the device: a chain's occupied slots must be its leading ones and hold bead indices
- * 1..n_beads.  Otherwise it returns SSM_EINVAL; the chain then keeps its valid leading slots only (the state
- * stays safe to step).  It synchronises the stream (also with device pointers) to report that. */
+ * 1..n_beads.  A chain that breaks this keeps its valid leading slots only, so the state stays safe to step.
+ *  - HOST pointers: the call synchronises the stream (it has to, for the copies) and returns SSM_EINVAL for a malformed S.
+ *  - DEVICE pointers: the call is asynchronous -- one kernel on the ctx's stream, no host synchronisation -- so that a
+ *    device-resident loop (ssm_set_state, ssm_step_kappa_device, ssm_group_stress_device, ...) can be queued without the
+ *    host in it.  The verdict on S then waits on the device: ssm_state_status returns it.
+ * In both cases the ctx holds the imported state afterwards (offending slots cleared) and global_step is set, also when
+ * SSM_EINVAL is reported: the error says "this is not the state you meant", not "nothing happened".  Only a CUDA error
+ * half way (SSM_ECUDA) leaves the ensemble undefined; stepping is then refused (SSM_ESTATE) until a state is imported. */
 int ssm_set_state(ssm_ctx *ctx, const float *R, const float *A, const uint8_t *S,
                   int64_t global_step, int pointers_are_device);
+
+/* Synchronises the stream and returns SSM_EINVAL if a state imported since the last check had a malformed S (see
+ * ssm_set_state; the flag is cleared), SSM_ESTATE if an import failed half way, else SSM_OK. */
+int ssm_state_status(ssm_ctx *ctx);
 
 /* ssm_set_state from HOST buffers (pinned, or the copies cannot overlap anything) followed by ssm_step(n_steps,
  * shear_rate), as ONE pipelined call: the ensemble is uploaded in about sixteen chunks on a copy stream of the library's
@@ -279,7 +290,10 @@ int ssm_set_state(ssm_ctx *ctx, const float *R, const float *A, const uint8_t *S
  * chains add to them, so state and stress samples are those of ssm_set_state + ssm_step bit for bit.  The correlator must
  * be off (sample_every = 0; SSM_ESTATE otherwise: it is fed ensemble-wide after every launch).  Uses both halves of the
  * staging area as upload buffers (stage_chains >= 64).  Synchronises before returning; S is validated as by
- * ssm_set_state. */
+ * ssm_set_state: on SSM_EINVAL the offending slots were cleared, and the n_steps were run and recorded on that cleared
+ * state (chunks are stepped as they land, so the verdict on the last chunk comes after the first has been stepped).
+ * On a CUDA error both streams are drained before the call returns (no copy from R, A, S is left in flight), the step
+ * counter and the records stay as they were, and the ctx refuses to step (SSM_ESTATE) until a state is imported again. */
 int ssm_step_from_host(ssm_ctx *ctx, const float *R, const float *A, const uint8_t *S, int64_t global_step,
                        int64_t n_steps, double shear_rate);
 

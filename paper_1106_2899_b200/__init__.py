@@ -18,11 +18,11 @@ NOALLOC_MAX_GROUPS = 4096          # SSM_NOALLOC_MAX_GROUPS of include/ssm.h
 EXPORTS = ["ssm_workspace_bytes", "ssm_init", "ssm_step", "ssm_stress_count", "ssm_stress", "ssm_stress_sums",
            "ssm_stress_sums_device", "ssm_chain_stress", "ssm_gt", "ssm_gt_sums", "ssm_get_state", "ssm_set_state",
            "ssm_reset_accumulators", "ssm_launch_count", "ssm_set_fusion", "ssm_set_grid", "ssm_destroy", "ssm_last_error",
-           "ssm_moduli", "ssm_eta0", "ssm_tau_d", "ssm_issue_rates",
+           "ssm_moduli", "ssm_eta0", "ssm_tau_d", "ssm_issue_rates8",
            "ssm_gt_virtual", "ssm_gt_sums_virtual", "ssm_step_kappa", "ssm_group_stress",
            "ssm_step_kappa_device", "ssm_group_stress_device", "ssm_recenter",
            "ssm_eta_star", "ssm_stress_from_sums", "ssm_stream_wait_ctx", "ssm_ctx_wait_stream", "ssm_step_from_host",
-           "ssm_group_stress_noalloc", "ssm_noise_calibration"]
+           "ssm_group_stress_noalloc", "ssm_noise_calibration", "ssm_state_status"]
 
 
 class Params(C.Structure):
@@ -70,7 +70,8 @@ def lib():
     L.ssm_set_grid.argtypes = [vp, C.c_int32]; L.ssm_set_grid.restype = C.c_int
     L.ssm_destroy.argtypes = [vp]; L.ssm_destroy.restype = None
     L.ssm_last_error.argtypes = [vp]; L.ssm_last_error.restype = C.c_char_p
-    L.ssm_issue_rates.argtypes = [vp, dp]; L.ssm_issue_rates.restype = C.c_int
+    L.ssm_issue_rates8.argtypes = [vp, dp]; L.ssm_issue_rates8.restype = C.c_int
+    L.ssm_state_status.argtypes = [vp]; L.ssm_state_status.restype = C.c_int
     L.ssm_gt_virtual.argtypes = [vp, C.POINTER(C.c_int32), dp, dp, dp]; L.ssm_gt_virtual.restype = C.c_int
     L.ssm_gt_sums_virtual.argtypes = [vp, dp]; L.ssm_gt_sums_virtual.restype = C.c_int
     L.ssm_step_kappa.argtypes = [vp, C.c_int64, C.c_int64, dp]; L.ssm_step_kappa.restype = C.c_int
@@ -342,6 +343,12 @@ class Ensemble:
                 self._ck(lib().ssm_set_state(self.h, C.c_void_p(R.data_ptr()), C.c_void_p(A.data_ptr()),
                                              C.c_void_p(S.data_ptr()), global_step, dev))
 
+    def state_status(self):
+        """ssm_state_status: synchronises; raises SsmError(SSM_EINVAL) if a state imported from device pointers since the
+        last check had a malformed S."""
+        with self._dev():
+            self._ck(lib().ssm_state_status(self.h))
+
     def step_from_host(self, R, A, S, global_step, n_steps, shear_rate=0.0):
         """ssm_step_from_host: upload the state from host numpy arrays (pinned for overlap) and advance n_steps, pipelined."""
         assert R.dtype == np.float32 and A.dtype == np.float32 and S.dtype == np.uint8
@@ -362,12 +369,12 @@ class Ensemble:
         self._ck(lib().ssm_set_fusion(self.h, steps_per_launch))
 
     def issue_rates(self):
-        """ssm_issue_rates (diagnostic): cycles per instruction group per scheduler; imad_wide = the issue cycles one
+        """ssm_issue_rates8 (diagnostic): cycles per instruction group per scheduler; imad_wide = the issue cycles one
         32 x 32 -> 64-bit multiply occupies inside a Philox round (the round's cycles minus one slot for each of its
         two LOP3, halved)."""
         out = np.zeros(8)
         with self._dev():
-            self._ck(lib().ssm_issue_rates(self.h, out.ctypes.data_as(C.POINTER(C.c_double))))
+            self._ck(lib().ssm_issue_rates8(self.h, out.ctypes.data_as(C.POINTER(C.c_double))))
         return {"ffma": out[0], "alu": out[1], "imad": out[2], "imad_wide": 0.5 * (out[7] - 2.0), "wide_lop3": out[3],
                 "wide_lop3_4ffma": out[4], "mufu": out[5], "i2f_f2i": out[6], "philox_round": out[7]}
 

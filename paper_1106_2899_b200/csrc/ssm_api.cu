@@ -61,6 +61,7 @@ struct ssm_ctx {
     unsigned char cpos[kCorrMaxLevels], cfil[kCorrMaxLevels], cpar[kCorrMaxLevels];
     std::vector<long long> ccount;      // [L][P] insertions with a product at (level, bin)
     std::vector<float> kappa_host;      // dt kappa of the last ssm_step_kappa call, [groups][9]
+    bool state_valid = true;            // false after an import that failed half way (CUDA error): stepping is refused until a state is imported again
     double calib[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // ssm_noise_calibration: the record of calibrate_bm for bm_noise
     cudaStream_t copy_st = nullptr;     // ssm_step_from_host: uploads run here, beside the stepping on st
     cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
@@ -372,6 +373,7 @@ static int next_block(const ssm_ctx *c, long long step, long long left)
 static int step_impl(ssm_ctx *c, int64_t n_steps, double shear_rate, const float *d_kappa, long long tiles_per_group)
 {
     const ssm_params &p = c->p;
+    if (!c->state_valid) return fail(c, SSM_ESTATE, "a state import failed half way: import a state again before stepping");
     if (p.stress_every > 0) {
         const long long need = (c->step + n_steps) / p.stress_every - c->step / p.stress_every;
         if (c->n_records + need > p.stress_capacity) return fail(c, SSM_ERANGE, "stress buffer would overflow (stress_capacity)");
@@ -608,7 +610,7 @@ extern "C" int ssm_chain_stress(ssm_ctx *c, float *out, int dev)
     return SSM_OK;
 }
 
-static int xfer_state(ssm_ctx *c, bool do_export, float *R, float *A, uint8_t *S, int dev)
+static int xfer_state_impl(ssm_ctx *c, bool do_export, float *R, float *A, uint8_t *S, int dev)
 {
     const int N = c->p.n_beads; const long long M = c->p.n_chains;
     unsigned char *state = c->ws + c->lay.state;
@@ -649,6 +651,14 @@ static int xfer_state(ssm_ctx *c, bool do_export, float *R, float *A, uint8_t *S
     return SSM_OK;
 }
 
+// no return while copies from / to the caller's buffers are still in flight, also on failure
+static int xfer_state(ssm_ctx *c, bool do_export, float *R, float *A, uint8_t *S, int dev)
+{
+    const int rc = xfer_state_impl(c, do_export, R, A, S, dev);
+    if (rc != SSM_OK) cudaStreamSynchronize(c->st);
+    return rc;
+}
+
 extern "C" int ssm_get_state(ssm_ctx *c, float *R, float *A, uint8_t *S, int64_t *global_step, int dev)
 {
     if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
@@ -657,15 +667,9 @@ extern "C" int ssm_get_state(ssm_ctx *c, float *R, float *A, uint8_t *S, int64_t
     return xfer_state(c, true, R, A, S, dev);
 }
 
-extern "C" int ssm_set_state(ssm_ctx *c, const float *R, const float *A, const uint8_t *S, int64_t global_step, int dev)
+// read the "imported state was malformed" flag of the device and clear it; synchronises the stream
+static int check_state_flag(ssm_ctx *c)
 {
-    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
-    if (!R || !A || !S) return fail(c, SSM_EINVAL, "NULL state pointer");
-    if (global_step < 0) return fail(c, SSM_EINVAL, "global_step < 0");
-    int rc = xfer_state(c, false, const_cast<float *>(R), const_cast<float *>(A), const_cast<uint8_t *>(S), dev);
-    if (rc != SSM_OK) return rc;
-    c->step = global_step; c->low_mode = 1;                            // A[3] of the caller is the fp32 low part of x
-    // the import kernel flags a chain whose S is not "bead indices 1..N in the leading slots, 0 after them"
     int bad = 0;
     int *d_bad = reinterpret_cast<int *>(c->ws + c->lay.counter) + 2;
     CK(c, cudaMemcpyAsync(&bad, d_bad, sizeof bad, cudaMemcpyDeviceToHost, c->st));
@@ -676,6 +680,28 @@ extern "C" int ssm_set_state(ssm_ctx *c, const float *R, const float *A, const u
                                    "(the offending slots were cleared)");
     }
     return SSM_OK;
+}
+
+extern "C" int ssm_set_state(ssm_ctx *c, const float *R, const float *A, const uint8_t *S, int64_t global_step, int dev)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (!R || !A || !S) return fail(c, SSM_EINVAL, "NULL state pointer");
+    if (global_step < 0) return fail(c, SSM_EINVAL, "global_step < 0");
+    int rc = xfer_state(c, false, const_cast<float *>(R), const_cast<float *>(A), const_cast<uint8_t *>(S), dev);
+    if (rc != SSM_OK) { c->state_valid = false; return rc; }            // part of the ensemble may be new, part old
+    c->step = global_step; c->low_mode = 1;                            // A[3] of the caller is the fp32 low part of x
+    c->state_valid = true;
+    // the import kernel flags a chain whose S is not "bead indices 1..N in the leading slots, 0 after them".  With host
+    // pointers the call has synchronised anyway and reports it now; with device pointers it stays asynchronous and the
+    // flag waits on the device for ssm_state_status
+    return dev ? SSM_OK : check_state_flag(c);
+}
+
+extern "C" int ssm_state_status(ssm_ctx *c)
+{
+    if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
+    if (!c->state_valid) return fail(c, SSM_ESTATE, "a state import failed half way: import a state again");
+    return check_state_flag(c);
 }
 
 // ssm_set_state from HOST buffers followed by ssm_step, as one pipelined call: the ensemble is uploaded in chunks on a copy
@@ -716,9 +742,16 @@ extern "C" int ssm_step_from_host(ssm_ctx *c, const float *R, const float *A, co
     unsigned char *state = c->ws + c->lay.state;
     int *bad = reinterpret_cast<int *>(c->ws + c->lay.counter) + 2;
     const float gdt = (float)(shear_rate * p.dt);
+    // From here on copies from the caller's buffers and kernels are in flight on two streams.  A CUDA error must not
+    // return while they still are (the caller would free or reuse R, A, S under the DMA), and it leaves the ensemble
+    // part new, part old, some chunks stepped: both streams are drained, the step counter and the records stay as they
+    // were, and the ctx refuses to step until a state is imported again (SSM_ESTATE).
+#define CKQ(c, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { \
+        cudaStreamSynchronize((c)->copy_st); cudaStreamSynchronize((c)->st); (c)->state_valid = false; \
+        return cuda_fail((c), e_, #call); } } while (0)
     // everything queued on the ctx's stream so far (it may still read the staging area or the state) comes first
-    CK(c, cudaEventRecord(c->ev_free[0], c->st));
-    CK(c, cudaEventRecord(c->ev_free[1], c->st));
+    CKQ(c, cudaEventRecord(c->ev_free[0], c->st));
+    CKQ(c, cudaEventRecord(c->ev_free[1], c->st));
     long long j = 0;
     for (long long k0 = 0; k0 < M; k0 += chunk, ++j) {
         const long long nk = M - k0 < chunk ? M - k0 : chunk;
@@ -726,14 +759,14 @@ extern "C" int ssm_step_from_host(ssm_ctx *c, const float *R, const float *A, co
         float *dR = reinterpret_cast<float *>(stage[b]);
         float *dA = dR + (size_t)3 * N * chunk;
         unsigned char *dS = reinterpret_cast<unsigned char *>(dA + (size_t)4 * N * chunk);
-        CK(c, cudaStreamWaitEvent(c->copy_st, c->ev_free[b], 0));
-        CK(c, cudaMemcpy2DAsync(dR, (size_t)chunk * 4, R + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)3 * N, cudaMemcpyHostToDevice, c->copy_st));
-        CK(c, cudaMemcpy2DAsync(dA, (size_t)chunk * 4, A + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)4 * N, cudaMemcpyHostToDevice, c->copy_st));
-        CK(c, cudaMemcpy2DAsync(dS, (size_t)chunk, S + k0, (size_t)M, (size_t)nk, (size_t)N, cudaMemcpyHostToDevice, c->copy_st));
-        CK(c, cudaEventRecord(c->ev_copied[b], c->copy_st));
-        CK(c, cudaStreamWaitEvent(c->st, c->ev_copied[b], 0));
-        CK(c, launch_xfer(false, state, dR, dA, dS, N, k0, nk, chunk, 0, bad, c->st));
-        CK(c, cudaEventRecord(c->ev_free[b], c->st));
+        CKQ(c, cudaStreamWaitEvent(c->copy_st, c->ev_free[b], 0));
+        CKQ(c, cudaMemcpy2DAsync(dR, (size_t)chunk * 4, R + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)3 * N, cudaMemcpyHostToDevice, c->copy_st));
+        CKQ(c, cudaMemcpy2DAsync(dA, (size_t)chunk * 4, A + k0, (size_t)M * 4, (size_t)nk * 4, (size_t)4 * N, cudaMemcpyHostToDevice, c->copy_st));
+        CKQ(c, cudaMemcpy2DAsync(dS, (size_t)chunk, S + k0, (size_t)M, (size_t)nk, (size_t)N, cudaMemcpyHostToDevice, c->copy_st));
+        CKQ(c, cudaEventRecord(c->ev_copied[b], c->copy_st));
+        CKQ(c, cudaStreamWaitEvent(c->st, c->ev_copied[b], 0));
+        CKQ(c, launch_xfer(false, state, dR, dA, dS, N, k0, nk, chunk, 0, bad, c->st));
+        CKQ(c, cudaEventRecord(c->ev_free[b], c->st));
         c->launches += 1;
         // this chunk's tiles through all n_steps
         const long long t0 = k0 / cpw, t1 = (k0 + nk + cpw - 1) / cpw;
@@ -745,7 +778,7 @@ extern "C" int ssm_step_from_host(ssm_ctx *c, const float *R, const float *A, co
             sp.gdt = gdt; sp.kappa = nullptr; sp.tiles_per_group = 1;
             sp.tile_first = (int)t0; sp.n_tiles = (int)(t1 - t0);
             sp.counter_slot = c->sp.counter_slot;
-            CK(c, launch_step(npad, sp, c->grid, c->st));
+            CKQ(c, launch_step(npad, sp, c->grid, c->st));
             c->sp.counter_slot ^= 1;
             c->launches += 1;
             nrec_total += nrec; step += T; left -= T;
@@ -754,15 +787,9 @@ extern "C" int ssm_step_from_host(ssm_ctx *c, const float *R, const float *A, co
     if (p.stress_every > 0) c->n_records += (global_step + n_steps) / p.stress_every - global_step / p.stress_every;
     c->step = global_step + n_steps;
     c->low_mode = 1;                                                  // A[3] of the caller is the fp32 low part of x
-    int h_bad = 0;
-    CK(c, cudaMemcpyAsync(&h_bad, bad, sizeof h_bad, cudaMemcpyDeviceToHost, c->st));
-    CK(c, cudaStreamSynchronize(c->st));
-    if (h_bad) {
-        CK(c, cudaMemsetAsync(bad, 0, sizeof h_bad, c->st));
-        return fail(c, SSM_EINVAL, "S is malformed: a chain's occupied slots must be its leading ones and hold bead indices 1..n_beads "
-                                   "(the offending slots were cleared)");
-    }
-    return SSM_OK;
+    c->state_valid = true;
+    return check_state_flag(c);          // synchronises; SSM_EINVAL if some S was malformed (offending slots cleared, steps run)
+#undef CKQ
 }
 
 extern "C" int ssm_reset_accumulators(ssm_ctx *c)
@@ -779,7 +806,7 @@ extern "C" int ssm_set_fusion(ssm_ctx *c, int32_t t)
     return SSM_OK;
 }
 
-extern "C" int ssm_issue_rates(ssm_ctx *c, double *h_cycles)
+extern "C" int ssm_issue_rates8(ssm_ctx *c, double *h_cycles)
 {
     if (!c) return fail(nullptr, SSM_EINVAL, "ctx is NULL");
     if (!h_cycles) return fail(c, SSM_EINVAL, "h_cycles is NULL");

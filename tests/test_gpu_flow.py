@@ -137,6 +137,47 @@ def test_groups_with_their_own_tensors_and_group_stress(ssm):
     assert g5.shape == (3, 13) and abs(g5[2, 12] - Z[160:].mean()) < 1e-9
 
 
+def test_device_resident_loop_restores_a_state_without_the_host(ssm):
+    """ssm_set_state with device pointers is asynchronous: restore, micro steps and group stresses are queued behind a
+    busy stream and the calls return before the GPU reaches them; the verdict on a malformed S waits on the device
+    for ssm_state_status."""
+    import torch
+    N, M, cpg = 16, 256, 64
+    kap = np.stack([KAPPA, 0.5 * KAPPA, np.zeros((3, 3)), -KAPPA.T])
+    src = ssm.Ensemble(N, M, seed=5)
+    src.step(10)
+    R, A, S, step = src.get_state()
+    dR, dA, dS = (torch.tensor(x, device="cuda") for x in (R, A, S))
+    dk = torch.tensor(kap, dtype=torch.float64, device="cuda")
+    out = torch.empty((4, 13), dtype=torch.float64, device="cuda")
+    b = ssm.Ensemble(N, M, seed=5)
+    torch.cuda.synchronize()
+    torch.cuda._sleep(2_000_000_000)                       # about a second of GPU time ahead of the loop on its stream
+    b.set_state(dR, dA, dS, step)
+    b.step_kappa_device(20, dk, chains_per_group=cpg)
+    b.group_stress_device(cpg, out)
+    done = torch.cuda.Event(); done.record()
+    assert not done.query(), "the three calls blocked the host"
+    torch.cuda.synchronize()
+    b.state_status()                                       # well-formed: no error
+    a = ssm.Ensemble(N, M, seed=5)                         # the same through the host-pointer calls
+    a.set_state(R, A, S, step)
+    a.step_kappa(20, kap, chains_per_group=cpg)
+    assert np.array_equal(a.group_stress(cpg), out.cpu().numpy())
+    # a malformed S (an occupied slot after an empty one): the queue is not disturbed, the error is reported afterwards
+    Z = (S > 0).sum(0)
+    k = int(np.argmax(Z < N - 2))
+    S2 = S.copy(); S2[Z[k] + 1, k] = 3
+    b.set_state(dR, dA, torch.tensor(S2, device="cuda"), step)         # returns at once, no exception
+    b.step_kappa_device(20, dk, chains_per_group=cpg)
+    b.group_stress_device(cpg, out)
+    with pytest.raises(ssm.SsmError) as err:
+        b.state_status()
+    assert err.value.code == ssm.SSM_EINVAL
+    b.state_status()                                       # the flag was cleared by the report
+    assert np.array_equal(a.group_stress(cpg), out.cpu().numpy())      # the stray slot was dropped: same chains as before
+
+
 def test_device_variants_of_the_group_calls_equal_the_host_ones(ssm):
     """A coupling loop queued without the host in it: tensors from a CUDA tensor, group stresses into one."""
     import torch

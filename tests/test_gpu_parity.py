@@ -299,7 +299,7 @@ def test_device_view_of_the_stress_sums_is_what_the_exchange_reduces(ssm):
 
 
 def test_issue_rate_probe(ssm):
-    """ssm_issue_rates: FP32 issues once per cycle per scheduler, the ALU pipe (LOP3) and
+    """ssm_issue_rates8: FP32 issues once per cycle per scheduler, the ALU pipe (LOP3) and
     IMAD every second cycle, the special-function unit every eighth, and the 32 x 32 -> 64-bit multiply of Philox
     holds the issue port for about three cycles beyond its own -- FFMAs beside it do not hide."""
     g = ssm.Ensemble(8, 64, seed=1)
