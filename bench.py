@@ -210,50 +210,68 @@ def run_table1():
     print(json.dumps({"workload": "PAPER.md Table 1 (context)", "rows": rows}))
 
 
-def time_configs(ssm, torch):
-    """Rows of run_configs(): the C2 / C3 / C5 shapes, device-resident, CUDA events."""
-    cases = [("C2 equilibrium G(t)", dict(n_beads=16, n_chains=65536, stress_every=10, sample_every=10), 0.0, 6400),
-             ("C3 start-up shear", dict(n_beads=32, n_chains=262144, stress_every=10), 0.1, 2560),
-             ("C5 long chains, G(t)", dict(n_beads=128, n_chains=131072, dt=0.005, stress_every=10, sample_every=10), 0.0, 1280),
-             ("C5 long chains, steady shear", dict(n_beads=128, n_chains=131072, dt=0.005, stress_every=10), 1e-3, 1280)]
+# The other BASELINE.json shapes (C2, C3, C5 of SURVEY 8d): (name, Ensemble keywords, shear rate, timed steps)
+OTHER_CONFIGS = [
+    ("C2 equilibrium G(t)", dict(n_beads=16, n_chains=65536, stress_every=10, sample_every=10), 0.0, 6400),
+    ("C2 without the correlator", dict(n_beads=16, n_chains=65536, stress_every=10), 0.0, 6400),
+    ("C3 start-up shear", dict(n_beads=32, n_chains=262144, stress_every=10), 0.1, 2560),
+    ("C5 long chains, G(t)", dict(n_beads=128, n_chains=131072, dt=0.005, stress_every=10, sample_every=10), 0.0, 1280),
+    ("C5 long chains, steady shear", dict(n_beads=128, n_chains=131072, dt=0.005, stress_every=10), 1e-3, 1280)]
+
+
+def i_alg_config(stress_every, sample_every):
+    """Frozen algorithmic thread-instructions per bead-update of a configuration: the table behind
+    I_ALG = 95 is per bead and does not depend on N (noise, bead update, slot work and attempts scale with the beads at
+    <Z> = N/4, K = N - Z); what depends on the configuration is the stress work, done on recorded steps only -- bond
+    virial 6.0, ensemble reduction 4.5, slip-spring virial 7 x 1/4 = 1.75 per bead-update -- and the correlator's feed
+    (per-chain sigma_xy, sigma^(v)_xy and the level-0 products of ssm_corr_kernel: about 3 per bead-update of a sampled step)."""
+    rec = 6.0 + 4.5 + 1.75
+    v = I_ALG - rec + (rec / stress_every if stress_every > 0 else 0.0)
+    if sample_every > 0:
+        v += 3.0 / sample_every
+    return v
+
+
+def time_configs(ssm, torch, peak_alu=None):
+    """The C2 / C3 / C5 shapes as they are run in production: same kernels as the bench line, their own shapes, sampling
+    and flow, device-resident; CUDA events around a few thousand steps after a warm-up.  Context beside the bench line
+    (which is configs[3]); parity of these shapes is tests/test_gpu_configs.py.  With peak_alu (T thread-instr/s) every
+    row carries its own roofline fraction: i_alg_config() x bead-updates/s / peak (time = everything on the stream,
+    correlator launches included)."""
     rows = []
-    for name, kw, rate, steps in cases:
+    for name, kw, rate, steps in OTHER_CONFIGS:
         g = ssm.Ensemble(seed=2, stress_capacity=steps // 5, **kw)
         g.step(steps // 5, rate)
         torch.cuda.synchronize()
+        l0 = g.launch_count()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(); g.step(steps, rate); e1.record(); torch.cuda.synchronize()
         t = e0.elapsed_time(e1) * 1e-3
-        rows.append({"config": name, "n_beads": kw["n_beads"], "n_chains": kw["n_chains"], "shear_rate": rate, "steps": steps,
-                     "bead_updates_per_s": kw["n_beads"] * kw["n_chains"] * steps / t, "ms_per_32_steps": 1e3 * t / steps * 32})
+        rate_bu = kw["n_beads"] * kw["n_chains"] * steps / t
+        row = {"config": name, "n_beads": kw["n_beads"], "n_chains": kw["n_chains"], "shear_rate": rate, "steps": steps,
+               "seconds": t, "bead_updates_per_s": rate_bu, "ms_per_32_steps": 1e3 * t / steps * 32,
+               "launches": int(g.launch_count() - l0)}
+        if peak_alu:
+            ia = i_alg_config(kw.get("stress_every", 0), kw.get("sample_every", 0))
+            row["roofline"] = {"bound": "alu", "i_alg_per_bead_update": ia, "achieved": ia * rate_bu / 1e12, "peak": peak_alu,
+                               "unit": "T thread-instr/s", "frac": ia * rate_bu / 1e12 / peak_alu}
+        rows.append(row)
         del g
     return rows
 
 
 def run_configs():
-    """BASELINE.json configs[1], [2], [4] (C2, C3, C5 of SURVEY 8d) as they are run in production: same kernels as
-    the bench line, their own shapes, sampling and flow; CUDA events around a few thousand steps after a warm-up.
-    Context beside the bench line (which is configs[3]); parity of these shapes is tests/test_gpu_statistics.py."""
     import torch
     import paper_1106_2899_b200 as ssm
-    cases = [("C2 equilibrium G(t)", dict(n_beads=16, n_chains=65536, stress_every=10, sample_every=10), 0.0, 6400),
-             ("C2 without the correlator", dict(n_beads=16, n_chains=65536, stress_every=10), 0.0, 6400),
-             ("C3 start-up shear", dict(n_beads=32, n_chains=262144, stress_every=10), 0.1, 2560),
-             ("C5 long chains, G(t)", dict(n_beads=128, n_chains=131072, dt=0.005, stress_every=10, sample_every=10), 0.0, 1280),
-             ("C5 long chains, steady shear", dict(n_beads=128, n_chains=131072, dt=0.005, stress_every=10), 1e-3, 1280)]
-    rows = []
-    for name, kw, rate, steps in cases:
-        g = ssm.Ensemble(seed=2, stress_capacity=steps // 5, **kw)
-        g.step(steps // 5, rate)
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(); g.step(steps, rate); e1.record(); torch.cuda.synchronize()
-        t = e0.elapsed_time(e1) * 1e-3
-        rows.append({"config": name, "n_beads": kw["n_beads"], "n_chains": kw["n_chains"], "shear_rate": rate, "steps": steps,
-                     "seconds": t, "bead_updates_per_s": kw["n_beads"] * kw["n_chains"] * steps / t,
-                     "ms_per_32_steps": 1e3 * t / steps * 32})
-        del g
-    print(json.dumps({"workload": "BASELINE.json configs[1], [2], [4] (context)", "rows": rows}))
+    peaks = measured_peaks()
+    peak_alu = N_SM * SMSP_PER_SM * LANES * peaks["sm_max_mhz"] * 1e6 / 1e12
+    print(json.dumps({"workload": "BASELINE.json configs[1], [2], [4] (context)", "rows": time_configs(ssm, torch, peak_alu)}))
+
+
+def spawn_command(n_gpus, port, argv):
+    """The launcher line of `python bench.py --gpus N` run without one: the driver's own torchrun line."""
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(n_gpus),
+            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
 
 
 def main():
@@ -272,9 +290,7 @@ def main():
         import socket
         with socket.socket() as so:
             so.bind(("127.0.0.1", 0)); port = so.getsockname()[1]
-        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(a.gpus),
-               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
-        raise SystemExit(subprocess.call(cmd))
+        raise SystemExit(subprocess.call(spawn_command(a.gpus, port, sys.argv[1:])))
 
     import torch
     import torch.distributed as dist
@@ -404,31 +420,51 @@ def main():
         dt_serial = (time.perf_counter() - t1) / 2
         assert all(np.array_equal(outs[0], o) for o in outs[1:])    # same input, same seed: same samples
 
-        def solo_steps(n):
+        def solo_steps(n, bring_back=None):
             out = None
             for _ in range(n):
                 solo.reset_accumulators()
                 solo.step_from_host(Rp, Ap, Sp, step, inner)
                 out = solo.stress()
+                if bring_back is not None:                          # the checkpointing user's step: the state comes home too
+                    solo.get_state(*bring_back)
             return out
         solo_steps(1)
         barrier()
         t2 = time.perf_counter()
-        out_solo = solo_steps(4)
+        out_solo = solo_steps(ke)
         barrier()
-        dt_solo = (time.perf_counter() - t2) / 4
+        dt_solo = (time.perf_counter() - t2) / ke
         assert np.array_equal(out_solo, outs[0])                    # the pipelined call gives the same samples
-        t = torch.tensor([dt], dtype=torch.float64, device=dev)
+        # round trip: as above, and ssm_get_state brings the advanced state back into pinned host buffers every step
+        back_pin = [torch.empty_like(p_).pin_memory() for p_ in pin]
+        back = [p_.numpy() for p_ in back_pin]
+        solo_steps(1, back)
+        barrier()
+        t3 = time.perf_counter()
+        solo_steps(3, back)
+        barrier()
+        dt_round = (time.perf_counter() - t3) / 3
+        d2h_state = sum(x.nbytes for x in back)
+        t = torch.tensor([dt_solo, dt / (nctx * ke), dt_round], dtype=torch.float64, device=dev)
         if world > 1:
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e = {"value": float(M) * N * inner * nctx * ke * world / float(t.item()), "unit": "bead-updates/s",
+        per = float(M) * N * inner * world
+        e2e = {"value": per / float(t[0].item()), "unit": "bead-updates/s",
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(outs[0].nbytes),
-               "steps": nctx * ke, "contexts": nctx, "serial_value": float(M) * N * inner / dt_solo,
-               "unpipelined_value": float(M) * N * inner / dt_serial,
-               "what": "ssm_set_state(host pinned) + ssm_step(%d) + ssm_stress(host) per step; %d contexts on as many "
-                       "streams, one host thread each, started one upload apart (serial_value: ONE context, one "
-                       "thread, ssm_step_from_host = the same upload in chunks overlapped with the stepping of the "
-                       "chunks already landed; unpipelined_value: one context, set_state then step)" % (inner, nctx)}
+               "steps": ke, "contexts": 1, "pipelined_value": per / float(t[0].item()),
+               "two_context_value": per / float(t[1].item()),
+               "serial_value": float(M) * N * inner / dt_serial,
+               "round_trip": {"value": per / float(t[2].item()), "unit": "bead-updates/s", "h2d_bytes_per_step": int(h2d),
+                              "d2h_bytes_per_step": int(outs[0].nbytes + d2h_state), "steps": 3,
+                              "what": "as value, and ssm_get_state(host pinned) brings the advanced state back every step"},
+               "what": "value = pipelined_value: ONE context, one host thread, per step ssm_step_from_host(host pinned, %d time "
+                       "steps: the upload in chunks on a copy stream, chunks stepped as they land) + ssm_stress(host).  "
+                       "two_context_value: ssm_set_state(host pinned) + ssm_step + ssm_stress per step on %d contexts "
+                       "(streams, host threads, twice the device memory) started one upload apart; every context pays its "
+                       "own copies but they all upload the SAME input, so this is pipelining, not more distinct work.  "
+                       "serial_value: one context, ssm_set_state then ssm_step then ssm_stress, nothing overlapped "
+                       "(its meaning in BENCH_r01)." % (inner, nctx)}
         # the state import / export kernel alone, full size, device pointers: CUDA events on the
         # context's stream, median of 5; algorithmic bytes = the rows read / written + the tiles written / read
         if rank == 0:
@@ -452,8 +488,7 @@ def main():
                 io[name + "_ms"] = sorted(ts)[2]
                 io[name + "_GBps"] = io_bytes / (sorted(ts)[2] * 1e-3) / 1e9
             io["bytes"] = io_bytes
-            io["what"] = ("ssm_set_state / ssm_get_state with device pointers, %d chains (the import's time includes reading "
-                          "back its malformed-state flag)" % M)
+            io["what"] = "ssm_set_state / ssm_get_state with device pointers, %d chains (asynchronous calls, CUDA events on the ctx's stream)" % M
             e2e["state_io"] = io
             del dRAS
         del solo
@@ -507,7 +542,7 @@ def main():
     if world == 1 and not a.no_e2e:
         # context, not the metric: the other BASELINE.json shapes with the same kernels in the same run (clock record above)
         del g
-        line["other_configs"] = time_configs(ssm, torch)
+        line["other_configs"] = time_configs(ssm, torch, peak_alu)
     if not a.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(N, a.cpu_seconds)
     print(json.dumps(line))

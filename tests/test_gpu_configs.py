@@ -160,13 +160,25 @@ def test_c3_startup_shear_four_rates_full_size(ssm):
 
 def test_c5_long_chains_gt_and_shear(ssm):
     """configs[4]: 131,072 chains x N = 128 (16 lanes per chain: the shared-memory-resident kernel), dt = 0.005,
-    equilibrium G(t) through the 16 x 16 correlator, then steady shear at rate 1e-3.  2e5 steps each.  Oracle twin:
-    512 chains x 1e5 steps; under shear 16 blocks of 32 chains x 2e4 steps."""
+    equilibrium G(t) through the 16 x 16 correlator over the stated 1e6 steps (t = 5000 tau0), then shear at rate 1e-3
+    for another 1e6 steps: total strain 5, t = 5000 tau0 -- the longest relaxation time of N = 128 is about 1e4 tau0
+    (tau_d ~ (N - 1)^3.48), so eta+(t) is still growing towards eta0 (eqs 61, 62) and is checked against the
+    linear-response int_0^t G of the same run while the strain is small, and for how far it has come at the end.
+    Oracle twin: 512 chains x 1e5 steps; under shear 16 blocks of 32 chains x 2e4 steps."""
     N, M, dt = 128, 131072, 0.005
-    g = ssm.Ensemble(N, M, dt=dt, seed=5, stress_every=10, stress_capacity=20000, sample_every=10,
+    n_eq = 1000000
+    g = ssm.Ensemble(N, M, dt=dt, seed=5, stress_every=10, stress_capacity=100000, sample_every=10,
                      corr_levels=16, corr_bins=16, corr_groups=32)
-    g.step(200000)
+    g.step(n_eq)
     t_g, G_g, se_g = g.gt()
+    # 1e5 samples reach level 13 (12 insertions, bins 8..11): the deep levels hold what the schedule says they hold
+    assert len(t_g) >= 16 + 12 * 8 and t_g[-1] >= 8 * 2 ** 13 * 10 * dt
+    _, cnt = g.gt_sums()
+    for lev in range(16):
+        ins = (n_eq // 10) // 2 ** lev
+        for q in range(16):
+            want = max(0, ins - q) if (lev == 0 or q >= 8) else 0
+            assert cnt[:, lev, q].sum() == want * M, (lev, q)
     e = oracle.Ensemble(N, 512, dt=dt, seed=1005)
     corr = oracle.Correlator(512, levels=16, bins=16, groups=16)
     e.run(100000, sample_every=10, corr=corr, n_threads=NT)
@@ -182,8 +194,9 @@ def test_c5_long_chains_gt_and_shear(ssm):
     # ---- shear at 1e-3 from the equilibrated ensemble
     rate = 1e-3
     g.reset_accumulators()
-    g.step(200000, shear_rate=rate)
+    g.step(1000000, shear_rate=rate)
     eta_g = g.stress()[:, 3] / (N * rate)
+    assert eta_g.size == 100000
 
     def one(b):
         x = oracle.Ensemble(N, 32, dt=dt, seed=2005, chain_offset=32 * b)
@@ -196,7 +209,7 @@ def test_c5_long_chains_gt_and_shear(ssm):
     mo_b = mo.reshape(-1, k).mean(1); so_b = c.reshape(16, -1, k).mean(2).std(0, ddof=1) / 4.0
     mg_b = eta_g[: mo.size].reshape(-1, k).mean(1)
     zb = (mg_b - mo_b) / so_b
-    print("C5 shear 1e-3: eta+ (block means) GPU %s oracle %s; max |z| = %.2f; eta+ at t = 1000: %.2f"
+    print("C5 shear 1e-3: eta+ (block means) GPU %s oracle %s; max |z| = %.2f; last sample eta+(t = 5000) = %.2f"
           % (np.round(mg_b[[0, 4, 9, 19]], 2), np.round(mo_b[[0, 4, 9, 19]], 2), np.abs(zb).max(), eta_g[-1]))
     assert np.mean(np.abs(zb) < 3.0) >= 0.9 and np.abs(zb).max() < 5.0, zb
     # linear response while the strain is small (t <= 100: strain 0.1): eta+(t) = int_0^t G
@@ -207,6 +220,16 @@ def test_c5_long_chains_gt_and_shear(ssm):
     dev = np.abs(eta_g[sel].reshape(-1, 40).mean(1) / lr[sel].reshape(-1, 40).mean(1) - 1.0)
     print("C5 shear 1e-3: eta+ / int G - 1 over 20 < t <= 100 (means of 2 tau0): max %.3f" % dev.max())
     assert dev.max() < 0.08
+    # where the viscosity growth stands after 5000 tau0 (strain 5) against the linear-response integral of this run's own
+    # G(t) up to the same time and up to the correlator's longest lag.  Strain 5 at Wi = rate tau_d ~ 10 is beyond the
+    # linear regime: eta+ has to lie BELOW int_0^t G (shear thinning, Fig 5) and above its value at strain 1/2.
+    last = eta_g[-2000:].mean()                                        # mean over the last 100 tau0
+    at = lambda tt: eta_g[(t > tt - 50.0) & (t <= tt + 50.0)].mean()
+    grow = [at(500.0), at(1000.0), at(2000.0), at(3000.0), at(4000.0), last]
+    print("C5 shear 1e-3: eta+ at t = 500, 1000, 2000, 3000, 4000, 4950: %s; int_0^t G at t = 500, 1000, 2000: %s, over all lags "
+          "(to t = %.0f): %.1f" % (np.round(grow, 1), np.round(np.interp([500.0, 1000.0, 2000.0], t_g, cum), 1), t_g[-1], cum[-1]))
+    assert 0.0 < last < 1.05 * cum[-1]                                 # the shear envelope: eta+ stays below int G (no strain hardening in shear)
+    assert abs(at(500.0) / np.interp(500.0, t_g, cum) - 1.0) < 0.15    # strain 1/2: still close to linear response
 
 
 def test_sixteen_level_correlator_equals_the_oracle_on_identical_trajectories(ssm):

@@ -97,3 +97,23 @@ def test_two_rank_gloo_allreduce_reproduces_the_single_process_ensemble():
     e = oracle.Ensemble(N, M, seed=seed)
     ref = e.run(steps, stress_every=1)
     assert np.allclose(shard.stress_means(want, M), ref, atol=12 * 2.0 ** -19)
+
+
+def test_bench_refuses_a_world_size_other_than_gpus_and_builds_the_drivers_launch_line():
+    """bench.py --gpus N reports only when N ranks run: one rank must not stand in for an N-GPU measurement
+    (SURVEY 8e).  Without a launcher it starts the ranks itself with the driver's torchrun line."""
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0", MASTER_ADDR="127.0.0.1", MASTER_PORT="29511")
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "1"],
+                       env=env, capture_output=True, text=True, timeout=300)
+    assert r.returncode != 0
+    assert "--gpus 2 but the launcher started 1 rank" in r.stderr
+    assert not any(line.startswith("{") for line in r.stdout.splitlines())        # no JSON line from a wrong world
+    sys.path.insert(0, root)
+    import bench
+    cmd = bench.spawn_command(4, 29512, ["--gpus", "4", "--steps", "3"])
+    assert cmd[:10] == [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "4",
+                        "--master-addr", "127.0.0.1", "--master-port", "29512"]
+    assert cmd[10] == os.path.join(root, "bench.py") and cmd[11:] == ["--gpus", "4", "--steps", "3"]
