@@ -67,7 +67,7 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
 
 
-TRAFFIC_CSV = os.path.join("profiles", "r2_step_kernel_metrics.csv")
+TRAFFIC_CSV = os.path.join("profiles", "r3_step_kernel_metrics.csv")
 
 
 def ncu_traffic(n_beads, n_chains):
