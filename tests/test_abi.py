@@ -94,3 +94,15 @@ def test_null_ctx_calls_fail_cleanly():
     assert L.ssm_stress_count(None) == 0
     assert L.ssm_reset_accumulators(None) == m.SSM_EINVAL
     L.ssm_destroy(None)
+
+
+def test_round3_entry_points_check_their_arguments_without_a_gpu():
+    """NULL contexts and outputs are refused before any CUDA call (no device needed): the no-allocation group stress,
+    the deferred state verdict and the calibration record."""
+    L = m.lib()
+    assert L.ssm_group_stress_noalloc(None, 1, None) == m.SSM_EINVAL
+    assert L.ssm_state_status(None) == m.SSM_EINVAL
+    assert L.ssm_noise_calibration(None, None) == m.SSM_EINVAL
+    assert m.NOALLOC_MAX_GROUPS == 4096
+    text = open(os.path.join(ROOT, "include", "ssm.h")).read()
+    assert re.search(r"#define\s+SSM_NOALLOC_MAX_GROUPS\s+4096\b", text)      # header and binding state the same limit
